@@ -1,0 +1,290 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the batched MIG-day simulator (BASELINE.json metric: simulated job-events/s and
+day-episodes/s on B200, with the fraction of the kernel's roofline).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl ours|reference]
+  python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P bench.py --gpus N ...
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: mig_sim_reset + mig_sim_rollout of every
+environment of the workload for one simulated day (arrival generation, event loop, scheduling, repartitioning, energy /
+tardiness accounting, per-epoch records, totals).  Inputs are synthetic (recipes in DESIGN.md section 4).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# Algorithmic warp-instructions per job-event (DESIGN.md section 6 derives it by hand from what the method must do
+# per ARRIVE/COMPLETE at one warp per environment); the roofline numerator uses THIS, not the executed count, so that
+# instruction bloat cannot inflate the fraction.
+ALG_WARP_INSTR_PER_JOB_EVENT = 260.0
+CPU_SAMPLE_ENVS = 2048
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            out = ""
+        clocks, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                clocks.append(float(f[0])); mx = float(f[1])
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(clocks) if clocks else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(clocks)}
+
+
+# ------------------------------------------------------------------------------------------------ oracle arm
+def _oracle_chunk(args):
+    name, n_envs, lo, hi = args
+    from oracle import oracle as O
+    from paper_2606_25082_b200 import workloads as W
+    wl = W.CONFIGS[name](n_envs)
+    ph = O.ParamsHolder(wl.params)
+    qh = O.QNetHolder(wl.qnet) if wl.qnet is not None else None
+    ev = 0
+    for e in range(lo, hi):
+        r = O.rollout(ph, wl.seed, e, algo=int(wl.algo[e]), cfg0=int(wl.cfg0[e]), policy=wl.policy,
+                      table=None if wl.table is None else wl.table[e], qnet=qh, epsilon=wl.epsilon)
+        ev += int(r.totals["n_jobs"]) + int(r.totals["n_completed"]) + int(r.totals["n_dropped"])
+    return ev
+
+
+def time_oracle(name, n_envs, n_sample, pool, cores):
+    """One pass of the UNMODIFIED single-threaded oracle over the first n_sample envs, split statically over `cores` processes."""
+    bounds = [(name, n_envs, (n_sample * i) // cores, (n_sample * (i + 1)) // cores) for i in range(cores)]
+    t0 = time.perf_counter()
+    ev = sum(pool.map(_oracle_chunk, bounds))
+    dt = time.perf_counter() - t0
+    return ev, dt
+
+
+def run_reference(args):
+    import concurrent.futures as cf
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import build as obuild
+    obuild.build()
+    cores = os.cpu_count() or 1
+    n_envs = args.envs
+    n_sample = min(n_envs, CPU_SAMPLE_ENVS)
+    with cf.ProcessPoolExecutor(cores) as pool:
+        for _ in range(args.warmup):
+            time_oracle(args.workload, n_envs, min(n_sample, cores * 4), pool, cores)
+        ev_tot, t_tot = 0, 0.0
+        for _ in range(args.steps):
+            ev, dt = time_oracle(args.workload, n_envs, n_sample, pool, cores)
+            ev_tot += ev; t_tot += dt
+    value = ev_tot / t_tot
+    sample = "first %d of %d envs of %s per step, one simulated day each, env range split statically over %d processes" % (n_sample, n_envs, args.workload, cores)
+    line = {
+        "impl": "reference", "metric": "job_events_per_s", "value": value, "unit": "job-events/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int64", "data": "synthetic",
+        "config": {"workload": args.workload, "n_envs": n_envs, "sample": sample},
+        "day_episodes_per_s": n_sample * args.steps / t_tot,
+        "cpu_baseline": {"value": value, "unit": "job-events/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "job-events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ CUDA arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2606_25082_b200 import binding as B
+    from paper_2606_25082_b200 import workloads as W
+    import dataclasses
+
+    peaks, peak_src = _peaks()
+    n_envs = args.envs                                   # per GPU (weak scaling: every rank simulates a full batch)
+    wl = W.CONFIGS[args.workload](n_envs)
+    sp = dataclasses.replace(wl.params, env_offset=rank * n_envs)      # Philox keyed by global env id
+    sim = B.MigSim(sp, n_envs, wl.seed)
+    qnet = B.QNet(wl.qnet) if wl.qnet is not None else None
+    d_algo, d_cfg0 = torch.from_numpy(wl.algo).cuda(), torch.from_numpy(wl.cfg0).cuda()
+    d_table = None if wl.table is None else torch.from_numpy(wl.table).cuda()
+    recs, totals = sim.alloc_recs(), sim.alloc_totals()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one_step(episode, ev_pair=None):
+        sim.reset(episode, d_algo, d_cfg0)
+        if ev_pair:
+            ev_pair[0].record(stream)
+        sim.rollout(wl.policy, table=d_table, qnet=qnet, epsilon=wl.epsilon, recs_out=recs, totals_out=totals)
+        if ev_pair:
+            ev_pair[1].record(stream)
+
+    for w in range(args.warmup):
+        one_step(w)
+        flush.fill_(w & 0xFF)
+    barrier()
+    # ---- timed region: resident inputs --------------------------------------------------------------------------
+    sampler = ClockSampler(local) if rank == 0 else None
+    pairs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    job_events = torch.zeros(1, dtype=torch.int64, device="cuda")
+    launches0 = sim.launch_count()
+    e0.record(stream)
+    for k in range(args.steps):
+        one_step(args.warmup + k, pairs[k])
+        t = totals.view(torch.int32).view(n_envs, 20)
+        job_events += (t[:, 8].long() + t[:, 9].long() + t[:, 10].long()).sum()          # n_jobs + n_completed + n_dropped
+        flush.fill_(k & 0xFF)                                                              # L2 flush between iterations
+    e1.record(stream)
+    barrier()
+    launches = sim.launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    t_ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    ev_all = job_events.clone()
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(ev_all, op=dist.ReduceOp.SUM)
+    t_s = float(t_ms.item()) / 1e3
+    ev_total = int(ev_all.item())
+    kern_ms = statistics.mean(a.elapsed_time(b) for a, b in pairs)
+    ev_per_launch = int(job_events.item()) / args.steps
+    # ---- end to end: HOST buffers through the C ABI, copies inside the timed region ---------------------------------
+    h_tot = np.zeros(n_envs, dtype=B.TOTALS_DTYPE)
+    h_recs = np.zeros((sp.n_epochs + 1, n_envs), dtype=B.REC_DTYPE)
+    pin = [torch.from_numpy(a) for a in (wl.algo, wl.cfg0)] + ([torch.from_numpy(wl.table)] if wl.table is not None else [])
+    rt = torch.cuda.cudart()
+    for a in (h_tot, h_recs, wl.algo, wl.cfg0) + ((wl.table,) if wl.table is not None else ()):
+        rt.cudaHostRegister(a.ctypes.data, a.nbytes, 0)
+    sim.rollout_host(0, wl.algo, wl.cfg0, wl.policy, wl.table, qnet, wl.epsilon, h_recs, h_tot)     # warm
+    barrier()
+    t0 = time.perf_counter()
+    ev_e2e = 0
+    n_e2e = max(1, min(args.steps, 3))
+    for k in range(n_e2e):
+        sim.rollout_host(100 + k, wl.algo, wl.cfg0, wl.policy, wl.table, qnet, wl.epsilon, h_recs, h_tot)
+        ev_e2e += int(h_tot["n_jobs"].sum() + h_tot["n_completed"].sum() + h_tot["n_dropped"].sum())
+    torch.cuda.synchronize()
+    e2e_t = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+    e2e_ev = torch.tensor([ev_e2e], dtype=torch.int64, device="cuda")
+    if world > 1:
+        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(e2e_ev, op=dist.ReduceOp.SUM)
+    h2d = wl.algo.nbytes + wl.cfg0.nbytes + (wl.table.nbytes if wl.table is not None else 0)
+    d2h = h_tot.nbytes + h_recs.nbytes
+    # ---- roofline of the dominant kernel (sim_kernel): plain ALU / issue slots --------------------------------------
+    props = torch.cuda.get_device_properties(local)
+    sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    peak_gips = props.multi_processor_count * 4 * sm_mhz * 1e6 / 1e9             # G warp-instr/s: SMs x 4 schedulers x f_max
+    achieved_gips = ALG_WARP_INSTR_PER_JOB_EVENT * ev_per_launch / (kern_ms / 1e3) / 1e9
+    alg_bytes = n_envs * ((sp.n_epochs + 1) * 64 + 80 + 2 * 256)                  # records + totals + state header in/out
+    roofline = {"bound": "alu", "achieved": achieved_gips, "peak": peak_gips, "unit": "Gwarp-instr/s", "frac": achieved_gips / peak_gips,
+                "traffic": None, "kernel": "sim_kernel<false>", "kernel_ms": kern_ms,
+                "alg_warp_instr_per_job_event": ALG_WARP_INSTR_PER_JOB_EVENT, "peak_source": "%d SMs x 4 x %s sm_max_mhz %.0f" % (props.multi_processor_count, peak_src, sm_mhz),
+                "hbm_algorithmic_bytes_per_launch": alg_bytes, "hbm_gbs_at_that": alg_bytes / (kern_ms / 1e3) / 1e9,
+                "hbm_peak_gbs": peaks.get("hbm_gbs")}
+    line = None
+    if rank == 0:
+        import concurrent.futures as cf
+        cpu = None
+        if not args.no_cpu_baseline:
+            cores = os.cpu_count() or 1
+            n_sample = min(n_envs, CPU_SAMPLE_ENVS)
+            with cf.ProcessPoolExecutor(cores) as pool:
+                time_oracle(args.workload, n_envs, min(n_sample, cores * 2), pool, cores)
+                ev, dt = time_oracle(args.workload, n_envs, n_sample, pool, cores)
+            cpu = {"value": ev / dt, "unit": "job-events/s", "cores": cores, "kind": "oracle",
+                   "sample": "first %d of %d envs of %s, one simulated day each, split statically over %d processes (%.1f s wall)" % (n_sample, n_envs, args.workload, cores, dt)}
+        line = {
+            "metric": "job_events_per_s", "value": ev_total / t_s, "unit": "job-events/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * t_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+            "config": {"workload": args.workload, "n_envs_per_gpu": n_envs, "n_envs_total": n_envs * world, "policy": ["static", "table", "dqn"][wl.policy],
+                       "job_events_per_step": ev_total / args.steps, "l2": "flushed between iterations (256 MiB write)", "parallelism": "env-range sharding, no data-path collective"},
+            "day_episodes_per_s": n_envs * world * args.steps / t_s,
+            "e2e": {"value": float(e2e_ev.item()) / float(e2e_t.item()), "unit": "job-events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
+            "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+        }
+        print(json.dumps(line))
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--envs", type=int, default=0, help="environments per GPU (default: the workload's BASELINE size)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if not args.envs:
+        args.envs = {"C1": 1, "C2": 1024, "C3": 4096, "C4": 8192, "C5": 65536}[args.workload]
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

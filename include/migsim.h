@@ -1,0 +1,193 @@
+/*
+ * migsim.h -- C ABI of libmigsim.so: the batched MIG-day simulator for NVIDIA B200 (sm_100a).
+ *
+ * What it computes: thousands of independent environments, each one MIG-partitioned GPU simulated over one day
+ * (Lipe et al., "Energy Efficient Scheduling of AI/ML Workloads on Multi Instance GPUs with Dynamic
+ * Repartitioning", CCGrid 2025 -- "PAPER.md" below is the extracted text of that paper; Lnn are its lines):
+ *   problem statement, three sub-problems (partition, job priority, slice choice)
+ *   MIG configurations, slice sizes 1/2/3/4/7 over 7 slots                                PAPER.md:L71-90 (Fig. 1)
+ *   job model dur_js, elasticity families
+ *   tardiness l_j = max(c_j - d_j, 0)
+ *   ET metric (energy / tardiness scalarisation)
+ *   power as a function of active compute units
+ *   preemption points: every arrival and completion, all jobs re-evaluated
+ *   EDF-FS, EDF-SS, LLF, LALF
+ *   DQN: state, 12 actions (= target configuration), reward, repartition penalty
+ *   workload: non-homogeneous Poisson arrivals, day-time peak
+ * The exact readings of everything the paper leaves open are in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - plain C; every call returns 0 (MIG_OK) or a negative error code; never throws, never exits;
+ *     mig_last_error() returns a thread-local message for the last failing call.
+ *   - "host" pointers are read during the call and copied (the caller keeps ownership and may free them);
+ *     "dev" pointers are device memory OWNED BY THE CALLER (e.g. torch tensors), valid on the handle's device; the
+ *     library never allocates outputs.  NULL is allowed where stated.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls taking a stream are asynchronous on
+ *     it; create / destroy / debug_set_jobs / the *_host call synchronise.
+ *   - a handle is not thread-safe; there is no global state and NO CPU FALLBACK: without a CUDA device every
+ *     compute call fails with MIG_ECUDA.
+ *   - all simulated quantities are integers: seconds (int32), milliwatts (int32), millijoules and tardiness (int64).
+ *     The only floating point is the fp32 state vector, the reward and the Q-network.
+ */
+#ifndef MIGSIM_H_
+#define MIGSIM_H_
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MIG_OK 0
+#define MIG_EINVAL (-1) /* invalid argument / parameter table */
+#define MIG_ENOMEM (-2) /* host or device allocation failed */
+#define MIG_ECUDA (-3)  /* CUDA runtime error (message has the CUDA string) */
+#define MIG_ESTATE (-4) /* call not allowed in the handle's current state (e.g. a 25th step without reset) */
+
+#define MIG_SLOTS 7
+#define MIG_STATE_DIM 64
+#define MIG_MAX_CLASSES 16
+#define MIG_MAX_CONFIGS 16
+#define MIG_THR_BINS 1440
+#define MIG_MAX_JOBS (1u << 20) /* job ids are < 2^20 per env-day: generation stops after this many accepted jobs */
+
+/* scheduling algorithm per environment */
+enum { MIG_ALGO_EDF_FS = 0, MIG_ALGO_EDF_SS = 1, MIG_ALGO_LLF = 2, MIG_ALGO_LALF = 3 };
+/* repartitioning policy of mig_sim_rollout */
+enum { MIG_POLICY_STATIC = 0, MIG_POLICY_TABLE = 1, MIG_POLICY_DQN = 2 };
+/* per-environment status bits */
+#define MIG_ST_TRUNCATED 1u  /* t_limit_s reached with jobs still in the system */
+#define MIG_ST_BAD_ACTION 2u /* an action >= n_configs was treated as "stay" */
+/* event types of the trace */
+enum { MIG_EV_ARRIVE = 1, MIG_EV_DROP = 2, MIG_EV_START = 3, MIG_EV_PREEMPT = 4, MIG_EV_COMPLETE = 5, MIG_EV_CRIT = 6,
+       MIG_EV_SLICE_UP = 7, MIG_EV_REPART = 8 };
+
+/* Parameters of mig_sim_create: all pointers are HOST arrays, copied.  Slice-size index: 0..4 = 1g,2g,3g,4g,7g. */
+typedef struct {
+  uint32_t n_classes;           /* 1..16 job classes (PAPER.md:L98-102 elasticity families x duration mixes) */
+  uint32_t n_configs;           /* 1..16 MIG configurations (paper: the 12 of Fig. 1) */
+  const uint32_t *speed;        /* [n_classes][5] work units per second on 1g,2g,3g,4g,7g; >= 1.  dur_js = ceil(rem/speed) */
+  const int32_t *dur7_q;        /* [n_classes][65] quantile table of the duration on 7g in seconds; non-decreasing, >= 1 */
+  const uint32_t *class_cum;    /* [n_classes] cumulative class thresholds, non-decreasing; last = 0xFFFFFFFF */
+  const uint16_t *slack_q10;    /* [n_classes][2] lo,hi of the due-date slack multiplier in Q10 (lo <= hi) */
+  const uint8_t *size_at_slot;  /* [n_configs][7] size of the slice STARTING at slot p (1,2,3,4,7) or 0 */
+  const uint32_t *accept_thr;   /* [1440] per-minute thinning threshold lambda(t)/lambda_max * 2^32 (PAPER.md:L222 NHPP) */
+  int32_t curve_mw[8];          /* power vs number of busy compute units 0..7; may be all 0 */
+  int32_t p_idle_mw[5];         /* per-slice idle power by size index (BASELINE model); may be 0 */
+  int32_t p_busy_mw[5];         /* per-slice busy power by size index */
+  uint64_t gap_scale_q16;       /* round(2^16 ln2 / lambda_max): exponential gap = -log2(u) * this, in Q16 seconds */
+  int32_t day_s;                /* arrivals stop here (86400) */
+  int32_t epoch_s;              /* decision epoch length (3600) */
+  int32_t n_epochs;             /* epochs per day (24); day_s <= n_epochs * epoch_s */
+  int32_t t_limit_s;            /* hard horizon of the drain after the last epoch (> n_epochs * epoch_s) */
+  uint32_t cap;                 /* max jobs in system (waiting + running): 1..1024; arrivals beyond are dropped */
+  uint32_t job_limit;           /* 0 = none; else generation stops after this many accepted jobs */
+  int32_t repart_downtime_s;    /* new slices are down this long after a repartition (paper: 4 s, L214) */
+  int64_t repart_energy_mj;     /* fixed energy per repartition */
+  int32_t crit_laxity_s;        /* LLF/LALF critical-laxity threshold theta */
+  uint32_t crit_max;            /* max critical-laxity preemptions per job (paper: 3), <= 15 */
+  float w_energy, w_tardy;      /* reward weights: r = -(w_energy * dE + w_tardy * dT) */
+  uint32_t env_base;            /* global id of local env 0 (multi-GPU sharding: Philox is keyed by global env id) */
+} mig_params_t;
+
+/* One record per env per epoch (index n_epochs = the drain).  64 bytes. */
+typedef struct {
+  int64_t energy_mj;      /* energy integrated over the record's span, incl. the repartition energy */
+  int64_t tardiness_s;    /* sum of max(c_j - d_j, 0) over jobs completed in the span */
+  uint64_t trace_hash;    /* FNV-1a-64 of every event emitted so far (running value) */
+  int32_t busy_unit_s;    /* sum over time of busy compute units (utilisation) */
+  int32_t t_end;          /* simulation time at the end of the span */
+  uint32_t n_events;      /* trace events emitted in the span */
+  uint16_t n_arrived, n_completed, n_dropped, n_tardy, n_preempt, n_start, n_crit, n_sys_end;
+  uint8_t cfg;            /* configuration in force during the span (= the action taken) */
+  uint8_t repartitioned;  /* 1 if the epoch began with a repartition */
+  uint8_t status;         /* MIG_ST_* so far */
+  uint8_t n_running_end;
+  uint32_t n_sys_max;     /* max jobs in system during the span */
+  uint32_t pad_;
+} mig_epoch_rec_t;
+
+/* Per-env totals over the day + drain.  80 bytes. */
+typedef struct {
+  int64_t energy_mj, tardiness_s;
+  uint64_t trace_hash;
+  int64_t busy_unit_s;
+  uint32_t n_jobs, n_completed, n_dropped, n_tardy, n_preempt, n_start, n_crit, n_events, n_repart, n_sys_max;
+  int32_t t_end;
+  uint32_t status;
+} mig_totals_t;
+
+/* One trace event, 16 bytes.  slot = 0xFF when not applicable; job = 0xFFFFFFFF when none. */
+typedef struct { int32_t t; uint8_t type; uint8_t slot; uint16_t aux; uint32_t job; int32_t value; } mig_event_t;
+
+/* A scripted arrival (tests): arrival tick, class, duration on 7g in seconds, absolute due date. */
+typedef struct { int32_t arr; uint32_t cls; int32_t dur7; int32_t due; } mig_job_t;
+
+typedef struct mig_sim mig_sim_t;
+typedef struct mig_qnet mig_qnet_t;
+
+const char *mig_last_error(void);
+/* library / build identification, e.g. "migsim sm_100a <date>" */
+const char *mig_version(void);
+
+/* Creates a simulator of n_envs environments on the current CUDA device.  Validates every table (sizes in
+ * {0,1,2,3,4,7}, slices inside 7 slots and not overlapping, speed >= 1, monotone quantiles, cap in 1..1024, all
+ * derived quantities inside int32) -> MIG_EINVAL with a message.  seed is the Philox key. */
+int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n_envs, uint64_t seed);
+int mig_sim_destroy(mig_sim_t *s);
+
+/* Starts a new day: episode goes into the Philox counter (fresh arrivals per episode).  algo, cfg0: dev[n_envs].
+ * state_out: dev[n_envs][64] fp32 initial observation, or NULL. */
+int mig_sim_reset(mig_sim_t *s, uint32_t episode, const uint8_t *algo, const uint8_t *cfg0, float *state_out, void *stream);
+
+/* One decision epoch for every env: action = target configuration (== current: stay, no cost;
+ * >= n_configs: stay + MIG_ST_BAD_ACTION).  The last epoch also runs the drain.  Outputs (each dev[n_envs] or NULL):
+ * state_out [n_envs][64], reward_out, energy_mj_out / tardiness_s_out (this epoch, drain included on the last),
+ * rec_out (this epoch's record), drain_rec_out (written on the last epoch only).  MIG_ESTATE after n_epochs steps. */
+int mig_sim_step(mig_sim_t *s, const uint8_t *action, float *state_out, float *reward_out, int64_t *energy_mj_out,
+                 int64_t *tardiness_s_out, mig_epoch_rec_t *rec_out, mig_epoch_rec_t *drain_rec_out, void *stream);
+
+/* Runs every remaining epoch of the day with the policy evaluated on the device; equals the same number of
+ * mig_sim_step calls with the same actions.
+ *   STATIC: stay on the current configuration.   TABLE: table dev[n_envs][n_epochs][4] u8, action =
+ *   table[env][k][bucket], bucket by jobs in system (0 | <8 | <64 | else).   DQN: q + epsilon (eps-greedy from
+ *   Philox stream 2), one Q forward per epoch over the state batch (scratch owned by the handle).
+ * recs_out: dev[n_epochs+1][n_envs] or NULL.  totals_out: dev[n_envs] or NULL. */
+int mig_sim_rollout(mig_sim_t *s, int policy, const uint8_t *table, const mig_qnet_t *q, float epsilon,
+                    mig_epoch_rec_t *recs_out, mig_totals_t *totals_out, void *stream);
+
+/* Per-env totals so far: dev[n_envs]. */
+int mig_sim_totals(mig_sim_t *s, mig_totals_t *totals_out, void *stream);
+
+/* End-to-end convenience with HOST buffers: copies algo/cfg0/table (host[n_envs], host[n_envs][n_epochs][4] or NULL)
+ * to the device, reset(episode) + rollout, copies totals (host[n_envs]) and records (host[n_epochs+1][n_envs] or
+ * NULL) back, synchronises.  DQN policy allowed (q non-NULL). */
+int mig_sim_rollout_host(mig_sim_t *s, uint32_t episode, const uint8_t *algo, const uint8_t *cfg0, int policy,
+                         const uint8_t *table, const mig_qnet_t *q, float epsilon, mig_epoch_rec_t *recs_out,
+                         mig_totals_t *totals_out);
+
+/* Q-network MLP 64 -> H -> H -> n_actions, ReLU, fp32.  Host arrays, copied; W row-major [in][out].
+ * Every output is accumulated in ascending k with one fused multiply-add per term (bit-reproducible). H in {64,128,256}. */
+int mig_qnet_create(mig_qnet_t **out, const float *W1, const float *b1, const float *W2, const float *b2,
+                    const float *W3, const float *b3, uint32_t hidden, uint32_t n_actions);
+int mig_qnet_destroy(mig_qnet_t *q);
+/* state dev[B][64] -> q_out dev[B][n_actions] (or NULL), argmax_out dev[B] u8 lowest index on ties (or NULL). */
+int mig_q_eval(const mig_qnet_t *q, const float *state, uint32_t B, float *q_out, uint8_t *argmax_out, void *stream);
+
+/* Debug / parity: re-runs ONE env for a whole day from the last reset's (episode, algo, cfg0), recording every event.
+ * policy STATIC or TABLE (table as in rollout), or actions != NULL: dev[n_epochs] explicit action sequence.
+ * buf dev[cap_events]; n_out dev[1] = number of events emitted (may exceed cap_events; only the first are stored);
+ * totals_out dev[1] or NULL.  Does not touch the handle's per-env state. */
+int mig_sim_debug_trace(mig_sim_t *s, uint32_t env, int policy, const uint8_t *table, const uint8_t *actions,
+                        mig_event_t *buf, uint32_t cap_events, uint32_t *n_out, mig_totals_t *totals_out, void *stream);
+/* Scripted arrivals (host array, non-decreasing arr) replace the generator for every env; n = 0 restores it. */
+int mig_sim_debug_set_jobs(mig_sim_t *s, const mig_job_t *jobs, uint32_t n);
+/* The exact-division constants the kernels use for x / v (host helper, exposed for tests): x / v == v == 1 ? x :
+ * (umulhi(x, m) >> sh) for every 0 <= x < 2^31. */
+int mig_debug_div_magic(uint32_t v, uint32_t *m, uint32_t *sh);
+/* Number of kernel launches issued through this handle so far (bench.py's gpu_launches). */
+uint64_t mig_sim_launch_count(const mig_sim_t *s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,437 @@
+// migsim.cu -- host side of libmigsim.so: the C ABI of include/migsim.h (argument checking, table preparation, launches).
+// Every step of the simulated path runs in the kernels of sim_device.cuh / qnet_device.cuh; there is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "qnet_device.cuh"
+#include "sim_device.cuh"
+
+using namespace migsim;
+
+// ------------------------------------------------------------------------------------------------ errors
+static thread_local char g_err[512] = "";
+static int fail(int code, const char *fmt, ...) {
+  va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof(g_err), fmt, ap); va_end(ap);
+  return code;
+}
+#define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(MIG_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); } while (0)
+
+extern "C" const char *mig_last_error(void) { return g_err; }
+extern "C" const char *mig_version(void) { return "migsim 0.1 sm_100a (" __DATE__ ")"; }
+
+// ------------------------------------------------------------------------------------------------ handles
+struct mig_qnet {
+  float *d = nullptr;        // one allocation: W1 b1 W2 b2 W3 b3
+  const float *W1, *b1, *W2, *b2, *W3, *b3;
+  uint32_t H = 0, A = 0;
+  int device = 0;
+};
+
+struct mig_sim {
+  mig_params_t p;            // scalars (pointers inside are NOT kept)
+  uint32_t n_envs = 0; uint64_t seed = 0; uint32_t episode = 0;
+  int device = 0, n_sm = 0;
+  uint32_t smem_entries = 0; size_t smem_bytes = 0; int grid_max = 0;
+  DevTables *d_tab = nullptr;
+  uint32_t *d_hdr = nullptr; uint4 *d_jobtab = nullptr; uint4 *d_dbgtab = nullptr;
+  unsigned int *d_counter = nullptr;
+  uint8_t *d_algo = nullptr, *d_cfg0 = nullptr;      // copies of the last reset's arrays (debug_trace re-runs from them)
+  float *d_state = nullptr; uint8_t *d_action = nullptr;   // scratch of the DQN rollout
+  uint8_t *d_table = nullptr; size_t table_bytes = 0;      // staging of rollout_host
+  mig_epoch_rec_t *d_recs = nullptr; mig_totals_t *d_totals = nullptr;
+  mig_job_t *d_script = nullptr; uint32_t n_script = 0;
+  int epoch = -1;            // -1: never reset
+  uint64_t launches = 0;
+};
+
+// ------------------------------------------------------------------------------------------------ exact division constants
+// floor(x / v) == umulhi(x, m) >> sh for every 0 <= x < 2^31 (Granlund-Montgomery, N = 31): l = ceil(log2 v),
+// m = ceil(2^(31+l) / v) < 2^32, shift = l - 1.  v == 1 is flagged by sh = 32 (the quotient is x itself).
+extern "C" int mig_debug_div_magic(uint32_t v, uint32_t *m, uint32_t *sh) {
+  if (!m || !sh || v == 0) return fail(MIG_EINVAL, "div_magic: v must be >= 1");
+  if (v == 1) { *m = 0; *sh = 32; return MIG_OK; }
+  uint32_t l = 0;
+  while ((1ull << l) < v) ++l;                         // l = ceil(log2 v) >= 1
+  unsigned __int128 num = (unsigned __int128)1 << (31 + l);
+  unsigned __int128 q = (num + v - 1) / v;
+  *m = (uint32_t)q; *sh = l - 1;
+  return MIG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ create
+static int size_index(int g) { return g == 1 ? 0 : g == 2 ? 1 : g == 3 ? 2 : g == 4 ? 3 : g == 7 ? 4 : -1; }
+
+static int build_tables(const mig_params_t *p, DevTables *t) {
+  memset(t, 0, sizeof(*t));
+  if (!p->speed || !p->dur7_q || !p->class_cum || !p->slack_q10 || !p->size_at_slot || !p->accept_thr)
+    return fail(MIG_EINVAL, "create: a table pointer is NULL");
+  if (p->n_classes < 1 || p->n_classes > MIG_MAX_CLASSES) return fail(MIG_EINVAL, "create: n_classes %u not in 1..16", p->n_classes);
+  if (p->n_configs < 1 || p->n_configs > MIG_MAX_CONFIGS) return fail(MIG_EINVAL, "create: n_configs %u not in 1..16", p->n_configs);
+  if (p->cap < 1 || p->cap > 1024) return fail(MIG_EINVAL, "create: cap %u not in 1..1024", p->cap);
+  if (p->epoch_s < 1 || p->n_epochs < 1 || p->n_epochs > 255) return fail(MIG_EINVAL, "create: epoch_s / n_epochs out of range");
+  if (p->day_s < 0 || p->day_s > 86400) return fail(MIG_EINVAL, "create: day_s %d not in 0..86400 (one threshold per minute)", p->day_s);
+  long long day_end = (long long)p->epoch_s * p->n_epochs;
+  if (day_end > (1ll << 30) || p->day_s > day_end) return fail(MIG_EINVAL, "create: n_epochs * epoch_s must cover day_s and be <= 2^30");
+  if (p->t_limit_s <= day_end || p->t_limit_s > (1 << 30)) return fail(MIG_EINVAL, "create: t_limit_s must be in (n_epochs*epoch_s, 2^30]");
+  if (p->repart_downtime_s < 0 || p->repart_downtime_s > (1 << 24)) return fail(MIG_EINVAL, "create: repart_downtime_s out of range");
+  if (p->repart_energy_mj < 0 || p->repart_energy_mj > (1ll << 48)) return fail(MIG_EINVAL, "create: repart_energy_mj out of range");
+  if (p->crit_laxity_s < 0 || p->crit_laxity_s > (1 << 24)) return fail(MIG_EINVAL, "create: crit_laxity_s out of range");
+  if (p->crit_max > 15) return fail(MIG_EINVAL, "create: crit_max %u > 15", p->crit_max);
+  if (p->gap_scale_q16 == 0) return fail(MIG_EINVAL, "create: gap_scale_q16 must be > 0");
+  for (int i = 0; i < 8; ++i) if (p->curve_mw[i] < 0 || p->curve_mw[i] > (1 << 27)) return fail(MIG_EINVAL, "create: curve_mw[%d] out of [0, 2^27]", i);
+  for (int i = 0; i < 5; ++i)
+    if (p->p_idle_mw[i] < 0 || p->p_idle_mw[i] > (1 << 27) || p->p_busy_mw[i] < 0 || p->p_busy_mw[i] > (1 << 27))
+      return fail(MIG_EINVAL, "create: p_idle_mw / p_busy_mw[%d] out of [0, 2^27]", i);
+  static const int SIZES[5] = {1, 2, 3, 4, 7};
+  for (int i = 0; i < 8; ++i) t->curve[i] = p->curve_mw[i];
+  for (int i = 0; i < 5; ++i) { t->p_idle[SIZES[i]] = p->p_idle_mw[i]; t->p_busy[SIZES[i]] = p->p_busy_mw[i]; }
+  for (uint32_t c = 0; c < p->n_configs; ++c) {
+    uint32_t pack = 0; int covered_to = 0, n = 0;
+    for (int s = 0; s < MIG_SLOTS; ++s) {
+      int g = p->size_at_slot[c * 7 + s];
+      if (!g) continue;
+      if (size_index(g) < 0) return fail(MIG_EINVAL, "create: config %u slot %d: slice size %d not in {1,2,3,4,7}", c, s, g);
+      if (s < covered_to) return fail(MIG_EINVAL, "create: config %u: slices overlap at slot %d", c, s);
+      if (s + g > MIG_SLOTS) return fail(MIG_EINVAL, "create: config %u: slice at slot %d exceeds 7 slots", c, s);
+      covered_to = s + g; pack |= (uint32_t)g << (4 * s); ++n;
+    }
+    if (!n) return fail(MIG_EINVAL, "create: config %u has no slice", c);
+    t->cfg_pack[c] = pack;
+  }
+  for (uint32_t c = 0; c < p->n_classes; ++c) {
+    const int32_t *q = p->dur7_q + c * 65;
+    for (int i = 0; i < 65; ++i) {
+      if (q[i] < 1 || q[i] > (1 << 24)) return fail(MIG_EINVAL, "create: dur7_q[%u][%d] = %d not in 1..2^24", c, i, q[i]);
+      if (i && q[i] < q[i - 1]) return fail(MIG_EINVAL, "create: dur7_q[%u] not non-decreasing at %d", c, i);
+      t->dur7_q[c * 65 + i] = q[i];
+    }
+    uint32_t vmin = 0xFFFFFFFFu, vmax = 0;
+    for (int i = 0; i < 5; ++i) {
+      uint32_t v = p->speed[c * 5 + i];
+      if (v < 1 || v > (1u << 24)) return fail(MIG_EINVAL, "create: speed[%u][%d] = %u not in 1..2^24", c, i, v);
+      vmin = v < vmin ? v : vmin; vmax = v > vmax ? v : vmax;
+      uint32_t m, sh; mig_debug_div_magic(v, &m, &sh);
+      t->speed[c * 5 + i] = make_uint4(v, m, sh, 0);
+    }
+    unsigned long long work_max = (unsigned long long)q[64] * p->speed[c * 5 + 4];
+    if (work_max + vmax >= (1ull << 31)) return fail(MIG_EINVAL, "create: class %u: max work %llu + max speed exceeds int32", c, work_max);
+    if ((work_max + vmin - 1) / vmin >= (1ull << 28)) return fail(MIG_EINVAL, "create: class %u: longest duration exceeds 2^28 s", c);
+    if (c && p->class_cum[c] < p->class_cum[c - 1]) return fail(MIG_EINVAL, "create: class_cum not non-decreasing at %u", c);
+    t->class_cum[c] = p->class_cum[c];
+    uint32_t lo = p->slack_q10[c * 2], hi = p->slack_q10[c * 2 + 1];
+    if (lo > hi) return fail(MIG_EINVAL, "create: slack_q10[%u]: lo > hi", c);
+    t->slack_lo[c] = lo; t->slack_span[c] = hi - lo + 1;
+  }
+  if (p->class_cum[p->n_classes - 1] != 0xFFFFFFFFu) return fail(MIG_EINVAL, "create: class_cum[last] must be 0xFFFFFFFF");
+  for (int i = 0; i < MIG_THR_BINS; ++i) t->thr[i] = p->accept_thr[i];
+  for (int i = 0; i <= 256; ++i) t->logT[i] = (uint32_t)llround(16777216.0 * log2(1.0 + (double)i / 256.0));
+  return MIG_OK;
+}
+
+extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n_envs, uint64_t seed) {
+  if (!out || !p) return fail(MIG_EINVAL, "create: NULL argument");
+  *out = nullptr;
+  if (n_envs < 1 || n_envs > (1u << 24)) return fail(MIG_EINVAL, "create: n_envs %u not in 1..2^24", n_envs);
+  std::vector<DevTables> host(1);
+  int rc = build_tables(p, host.data());
+  if (rc) return rc;
+  int ndev = 0;
+  cudaError_t ce = cudaGetDeviceCount(&ndev);
+  if (ce != cudaSuccess || ndev == 0) return fail(MIG_ECUDA, "create: no CUDA device (%s); there is no CPU fallback", cudaGetErrorString(ce));
+  mig_sim *s = new (std::nothrow) mig_sim();
+  if (!s) return fail(MIG_ENOMEM, "create: host allocation failed");
+  s->p = *p;
+  s->p.speed = nullptr; s->p.dur7_q = nullptr; s->p.class_cum = nullptr; s->p.slack_q10 = nullptr; s->p.size_at_slot = nullptr; s->p.accept_thr = nullptr;
+  s->n_envs = n_envs; s->seed = seed;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&s->device) != cudaSuccess || cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) { delete s; return fail(MIG_ECUDA, "create: cannot query the device"); }
+  s->n_sm = prop.multiProcessorCount;
+  s->smem_entries = p->cap < 64 ? p->cap : 64;
+  s->smem_bytes = ((sizeof(HotTables) + 15) & ~(size_t)15) + (size_t)kWarpsPerCta * (WS_WORDS * 4 + (size_t)s->smem_entries * 16);
+  int occ = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sim_kernel<false>, kWarpsPerCta * 32, s->smem_bytes) != cudaSuccess || occ < 1) {
+    delete s; return fail(MIG_ECUDA, "create: the rollout kernel does not fit this device (%s)", cudaGetErrorString(cudaGetLastError()));
+  }
+  s->grid_max = occ * s->n_sm;
+  size_t n = n_envs;
+#define ALLOC(ptr, bytes) if (cudaMalloc((void **)&(ptr), (bytes)) != cudaSuccess) { cudaGetLastError(); mig_sim_destroy(s); return fail(MIG_ENOMEM, "create: cudaMalloc of %zu bytes failed", (size_t)(bytes)); }
+  ALLOC(s->d_tab, sizeof(DevTables));
+  ALLOC(s->d_hdr, n * kHeaderWords * 4);
+  ALLOC(s->d_jobtab, n * p->cap * sizeof(uint4));
+  ALLOC(s->d_dbgtab, (size_t)p->cap * sizeof(uint4));
+  ALLOC(s->d_counter, sizeof(unsigned int));
+  ALLOC(s->d_algo, n); ALLOC(s->d_cfg0, n);
+  ALLOC(s->d_state, n * MIG_STATE_DIM * sizeof(float));
+  ALLOC(s->d_action, n);
+#undef ALLOC
+  if (cudaMemcpy(s->d_tab, host.data(), sizeof(DevTables), cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemset(s->d_hdr, 0, n * kHeaderWords * 4) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) {
+    mig_sim_destroy(s); return fail(MIG_ECUDA, "create: table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+  }
+  *out = s;
+  return MIG_OK;
+}
+
+extern "C" int mig_sim_destroy(mig_sim_t *s) {
+  if (!s) return MIG_OK;
+  cudaDeviceSynchronize();
+  cudaFree(s->d_tab); cudaFree(s->d_hdr); cudaFree(s->d_jobtab); cudaFree(s->d_dbgtab); cudaFree(s->d_counter);
+  cudaFree(s->d_algo); cudaFree(s->d_cfg0); cudaFree(s->d_state); cudaFree(s->d_action); cudaFree(s->d_table);
+  cudaFree(s->d_recs); cudaFree(s->d_totals); cudaFree(s->d_script);
+  cudaGetLastError();
+  delete s;
+  return MIG_OK;
+}
+
+extern "C" uint64_t mig_sim_launch_count(const mig_sim_t *s) { return s ? s->launches : 0; }
+
+// ------------------------------------------------------------------------------------------------ launches
+static void base_args(const mig_sim *s, SimArgs &a) {
+  memset(&a, 0, sizeof(a));
+  const mig_params_t &p = s->p;
+  a.tab = s->d_tab; a.hdr = s->d_hdr; a.jobtab = s->d_jobtab; a.counter = s->d_counter;
+  a.n_envs = s->n_envs; a.env_first = 0;
+  a.n_classes = p.n_classes; a.n_configs = p.n_configs;
+  a.k0 = (uint32_t)s->seed; a.k1 = (uint32_t)(s->seed >> 32); a.episode = s->episode; a.env_base = p.env_base;
+  a.gap_scale = p.gap_scale_q16;
+  a.day_s = p.day_s; a.epoch_s = p.epoch_s; a.n_epochs = p.n_epochs; a.t_limit_s = p.t_limit_s;
+  a.cap = p.cap; a.job_limit = p.job_limit; a.smem_entries = s->smem_entries;
+  a.downtime_s = p.repart_downtime_s; a.repart_energy = p.repart_energy_mj;
+  a.theta = p.crit_laxity_s; a.crit_max = p.crit_max;
+  a.w_energy = p.w_energy; a.w_tardy = p.w_tardy;
+  a.algo = s->d_algo; a.cfg0 = s->d_cfg0;
+  a.script = s->n_script ? s->d_script : nullptr; a.n_script = s->n_script;
+  a.rec_stride = s->n_envs;
+}
+
+template <bool TRACE>
+static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
+  CU(cudaMemsetAsync(s->d_counter, 0, sizeof(unsigned int), st));
+  int ctas = (int)((a.n_envs + kWarpsPerCta - 1) / kWarpsPerCta);
+  if (ctas > s->grid_max) ctas = s->grid_max;
+  sim_kernel<TRACE><<<ctas, kWarpsPerCta * 32, s->smem_bytes, st>>>(a);
+  CU(cudaGetLastError());
+  s->launches++;
+  return MIG_OK;
+}
+
+extern "C" int mig_sim_reset(mig_sim_t *s, uint32_t episode, const uint8_t *algo, const uint8_t *cfg0, float *state_out, void *stream) {
+  if (!s || !algo || !cfg0) return fail(MIG_EINVAL, "reset: NULL argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  CU(cudaMemcpyAsync(s->d_algo, algo, s->n_envs, cudaMemcpyDeviceToDevice, st));
+  CU(cudaMemcpyAsync(s->d_cfg0, cfg0, s->n_envs, cudaMemcpyDeviceToDevice, st));
+  s->episode = episode;
+  SimArgs a; base_args(s, a);
+  a.from_init = 1; a.save = 1; a.n_steps = 0; a.state_out = state_out;
+  int rc = launch_sim<false>(s, a, st);
+  if (rc) return rc;
+  s->epoch = 0;
+  return MIG_OK;
+}
+
+extern "C" int mig_sim_step(mig_sim_t *s, const uint8_t *action, float *state_out, float *reward_out, int64_t *energy_mj_out,
+                            int64_t *tardiness_s_out, mig_epoch_rec_t *rec_out, mig_epoch_rec_t *drain_rec_out, void *stream) {
+  if (!s || !action) return fail(MIG_EINVAL, "step: NULL argument");
+  if (s->epoch < 0) return fail(MIG_ESTATE, "step: reset has not been called");
+  if (s->epoch >= s->p.n_epochs) return fail(MIG_ESTATE, "step: the day is over (%d epochs done); call reset", s->epoch);
+  SimArgs a; base_args(s, a);
+  a.save = 1; a.n_steps = 1; a.policy = 3;
+  a.actions = action; a.act_stride_env = 1; a.act_stride_k = 0;
+  a.state_out = state_out; a.reward_out = reward_out; a.energy_out = energy_mj_out; a.tard_out = tardiness_s_out;
+  a.recs = rec_out; a.rec_k0 = s->epoch; a.drain_rec = drain_rec_out;
+  int rc = launch_sim<false>(s, a, (cudaStream_t)stream);
+  if (rc) return rc;
+  s->epoch++;
+  return MIG_OK;
+}
+
+static int launch_qnet(const mig_qnet *q, QArgs &qa, cudaStream_t st) {
+  qa.W1 = q->W1; qa.b1 = q->b1; qa.W2 = q->W2; qa.b2 = q->b2; qa.W3 = q->W3; qa.b3 = q->b3; qa.H = q->H; qa.A = q->A;
+  size_t smem = (size_t)(MIG_STATE_DIM + 2 * q->H + q->A) * kQRows * sizeof(float);
+  static thread_local size_t attr_set = 0;
+  if (smem > 48 * 1024 && attr_set < smem) {
+    CU(cudaFuncSetAttribute(qnet_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_set = smem;
+  }
+  uint32_t blocks = (qa.B + kQRows - 1) / kQRows;
+  qnet_kernel<<<blocks, q->H, smem, st>>>(qa);
+  CU(cudaGetLastError());
+  return MIG_OK;
+}
+
+extern "C" int mig_sim_rollout(mig_sim_t *s, int policy, const uint8_t *table, const mig_qnet_t *q, float epsilon,
+                               mig_epoch_rec_t *recs_out, mig_totals_t *totals_out, void *stream) {
+  if (!s) return fail(MIG_EINVAL, "rollout: NULL handle");
+  if (s->epoch < 0) return fail(MIG_ESTATE, "rollout: reset has not been called");
+  if (s->epoch >= s->p.n_epochs) return fail(MIG_ESTATE, "rollout: the day is over; call reset");
+  if (policy != MIG_POLICY_STATIC && policy != MIG_POLICY_TABLE && policy != MIG_POLICY_DQN) return fail(MIG_EINVAL, "rollout: unknown policy %d", policy);
+  if (policy == MIG_POLICY_TABLE && !table) return fail(MIG_EINVAL, "rollout: TABLE policy needs a table");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int ne = s->p.n_epochs;
+  if (policy != MIG_POLICY_DQN) {
+    SimArgs a; base_args(s, a);
+    a.save = 1; a.n_steps = ne - s->epoch; a.policy = policy; a.table = table;
+    a.recs = recs_out; a.rec_k0 = 0; a.drain_rec = recs_out ? recs_out + (size_t)ne * s->n_envs : nullptr;
+    a.totals = totals_out;
+    int rc = launch_sim<false>(s, a, st);
+    if (rc) return rc;
+    s->epoch = ne;
+    return MIG_OK;
+  }
+  if (!q) return fail(MIG_EINVAL, "rollout: DQN policy needs a Q-network");
+  if (q->A != s->p.n_configs) return fail(MIG_EINVAL, "rollout: Q-network has %u actions, the simulator %u configurations", q->A, s->p.n_configs);
+  if (!(epsilon >= 0.0f) || epsilon > 1.0f) return fail(MIG_EINVAL, "rollout: epsilon must be in [0, 1]");
+  double et = (double)epsilon * 4294967296.0;
+  uint32_t eps_thr = et >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)llround(et);
+  {                                             // current observation into the handle's scratch
+    SimArgs a; base_args(s, a);
+    a.save = 0; a.n_steps = 0; a.state_out = s->d_state;
+    int rc = launch_sim<false>(s, a, st);
+    if (rc) return rc;
+  }
+  while (s->epoch < ne) {
+    QArgs qa; memset(&qa, 0, sizeof(qa));
+    qa.state = s->d_state; qa.B = s->n_envs; qa.action_out = s->d_action; qa.eps_thr = eps_thr;
+    qa.epoch = (uint32_t)s->epoch; qa.k0 = (uint32_t)s->seed; qa.k1 = (uint32_t)(s->seed >> 32); qa.episode = s->episode; qa.env_base = s->p.env_base;
+    int rc = launch_qnet(q, qa, st);
+    if (rc) return rc;
+    s->launches++;
+    SimArgs a; base_args(s, a);
+    a.save = 1; a.n_steps = 1; a.policy = 3;
+    a.actions = s->d_action; a.act_stride_env = 1; a.act_stride_k = 0;
+    a.state_out = s->d_state;
+    a.recs = recs_out; a.rec_k0 = 0; a.drain_rec = recs_out ? recs_out + (size_t)ne * s->n_envs : nullptr;
+    if (s->epoch == ne - 1) a.totals = totals_out;
+    rc = launch_sim<false>(s, a, st);
+    if (rc) return rc;
+    s->epoch++;
+  }
+  return MIG_OK;
+}
+
+extern "C" int mig_sim_totals(mig_sim_t *s, mig_totals_t *totals_out, void *stream) {
+  if (!s || !totals_out) return fail(MIG_EINVAL, "totals: NULL argument");
+  if (s->epoch < 0) return fail(MIG_ESTATE, "totals: reset has not been called");
+  SimArgs a; base_args(s, a);
+  a.save = 0; a.n_steps = 0; a.totals = totals_out;
+  return launch_sim<false>(s, a, (cudaStream_t)stream);
+}
+
+extern "C" int mig_sim_rollout_host(mig_sim_t *s, uint32_t episode, const uint8_t *algo, const uint8_t *cfg0, int policy,
+                                    const uint8_t *table, const mig_qnet_t *q, float epsilon, mig_epoch_rec_t *recs_out,
+                                    mig_totals_t *totals_out) {
+  if (!s || !algo || !cfg0 || !totals_out) return fail(MIG_EINVAL, "rollout_host: NULL argument");
+  const size_t n = s->n_envs, ne = (size_t)s->p.n_epochs;
+  if (!s->d_totals) { if (cudaMalloc((void **)&s->d_totals, n * sizeof(mig_totals_t)) != cudaSuccess) { cudaGetLastError(); return fail(MIG_ENOMEM, "rollout_host: cudaMalloc failed"); } }
+  if (recs_out && !s->d_recs) { if (cudaMalloc((void **)&s->d_recs, n * (ne + 1) * sizeof(mig_epoch_rec_t)) != cudaSuccess) { cudaGetLastError(); return fail(MIG_ENOMEM, "rollout_host: cudaMalloc failed"); } }
+  if (policy == MIG_POLICY_TABLE) {
+    if (!table) return fail(MIG_EINVAL, "rollout_host: TABLE policy needs a table");
+    size_t tb = n * ne * 4;
+    if (s->table_bytes < tb) { cudaFree(s->d_table); s->d_table = nullptr; if (cudaMalloc((void **)&s->d_table, tb) != cudaSuccess) { cudaGetLastError(); s->table_bytes = 0; return fail(MIG_ENOMEM, "rollout_host: cudaMalloc failed"); } s->table_bytes = tb; }
+    CU(cudaMemcpyAsync(s->d_table, table, tb, cudaMemcpyHostToDevice, 0));
+  }
+  // reset() copies device -> device from its arguments: stage the host arrays in the DQN action/state scratch first
+  uint8_t *stage_algo = s->d_action; uint8_t *stage_cfg = reinterpret_cast<uint8_t *>(s->d_state);
+  CU(cudaMemcpyAsync(stage_algo, algo, n, cudaMemcpyHostToDevice, 0));
+  CU(cudaMemcpyAsync(stage_cfg, cfg0, n, cudaMemcpyHostToDevice, 0));
+  int rc = mig_sim_reset(s, episode, stage_algo, stage_cfg, nullptr, nullptr);
+  if (rc) return rc;
+  rc = mig_sim_rollout(s, policy, s->d_table, q, epsilon, recs_out ? s->d_recs : nullptr, s->d_totals, nullptr);
+  if (rc) return rc;
+  CU(cudaMemcpyAsync(totals_out, s->d_totals, n * sizeof(mig_totals_t), cudaMemcpyDeviceToHost, 0));
+  if (recs_out) CU(cudaMemcpyAsync(recs_out, s->d_recs, n * (ne + 1) * sizeof(mig_epoch_rec_t), cudaMemcpyDeviceToHost, 0));
+  CU(cudaStreamSynchronize(0));
+  return MIG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ Q-network
+extern "C" int mig_qnet_create(mig_qnet_t **out, const float *W1, const float *b1, const float *W2, const float *b2,
+                               const float *W3, const float *b3, uint32_t hidden, uint32_t n_actions) {
+  if (!out || !W1 || !b1 || !W2 || !b2 || !W3 || !b3) return fail(MIG_EINVAL, "qnet_create: NULL argument");
+  *out = nullptr;
+  if (hidden < 32 || hidden > 256 || hidden % 32) return fail(MIG_EINVAL, "qnet_create: hidden %u must be a multiple of 32 in 32..256", hidden);
+  if (n_actions < 1 || n_actions > MIG_MAX_CONFIGS) return fail(MIG_EINVAL, "qnet_create: n_actions %u not in 1..16", n_actions);
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(MIG_ECUDA, "qnet_create: no CUDA device; there is no CPU fallback"); }
+  mig_qnet *q = new (std::nothrow) mig_qnet();
+  if (!q) return fail(MIG_ENOMEM, "qnet_create: host allocation failed");
+  const size_t H = hidden, A = n_actions;
+  const size_t sz[6] = {MIG_STATE_DIM * H, H, H * H, H, H * A, A};
+  const float *src[6] = {W1, b1, W2, b2, W3, b3};
+  size_t off[6], tot = 0;
+  for (int i = 0; i < 6; ++i) { off[i] = tot; tot += (sz[i] + 3) & ~(size_t)3; }
+  if (cudaMalloc((void **)&q->d, tot * sizeof(float)) != cudaSuccess) { cudaGetLastError(); delete q; return fail(MIG_ENOMEM, "qnet_create: cudaMalloc failed"); }
+  for (int i = 0; i < 6; ++i)
+    if (cudaMemcpy(q->d + off[i], src[i], sz[i] * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) { cudaFree(q->d); delete q; return fail(MIG_ECUDA, "qnet_create: upload failed"); }
+  q->W1 = q->d + off[0]; q->b1 = q->d + off[1]; q->W2 = q->d + off[2]; q->b2 = q->d + off[3]; q->W3 = q->d + off[4]; q->b3 = q->d + off[5];
+  q->H = hidden; q->A = n_actions;
+  cudaGetDevice(&q->device);
+  *out = q;
+  return MIG_OK;
+}
+
+extern "C" int mig_qnet_destroy(mig_qnet_t *q) {
+  if (!q) return MIG_OK;
+  cudaDeviceSynchronize(); cudaFree(q->d); cudaGetLastError();
+  delete q;
+  return MIG_OK;
+}
+
+extern "C" int mig_q_eval(const mig_qnet_t *q, const float *state, uint32_t B, float *q_out, uint8_t *argmax_out, void *stream) {
+  if (!q || !state) return fail(MIG_EINVAL, "q_eval: NULL argument");
+  if (B == 0) return MIG_OK;
+  QArgs qa; memset(&qa, 0, sizeof(qa));
+  qa.state = state; qa.B = B; qa.q_out = q_out; qa.argmax_out = argmax_out;
+  return launch_qnet(q, qa, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------------------------------------ debug / parity
+extern "C" int mig_sim_debug_trace(mig_sim_t *s, uint32_t env, int policy, const uint8_t *table, const uint8_t *actions,
+                                   mig_event_t *buf, uint32_t cap_events, uint32_t *n_out, mig_totals_t *totals_out, void *stream) {
+  if (!s || !n_out) return fail(MIG_EINVAL, "debug_trace: NULL argument");
+  if (s->epoch < 0) return fail(MIG_ESTATE, "debug_trace: reset has not been called");
+  if (env >= s->n_envs) return fail(MIG_EINVAL, "debug_trace: env %u out of range", env);
+  if (!actions && policy != MIG_POLICY_STATIC && policy != MIG_POLICY_TABLE) return fail(MIG_EINVAL, "debug_trace: policy must be STATIC or TABLE, or pass actions");
+  if (!actions && policy == MIG_POLICY_TABLE && !table) return fail(MIG_EINVAL, "debug_trace: TABLE policy needs a table");
+  SimArgs a; base_args(s, a);
+  a.n_envs = 1; a.env_first = env; a.tab_override = s->d_dbgtab;
+  a.from_init = 1; a.save = 0; a.n_steps = s->p.n_epochs;
+  if (actions) { a.policy = 3; a.actions = actions; a.act_stride_env = 0; a.act_stride_k = 1; }
+  else { a.policy = policy; a.table = table; }
+  a.trace = buf; a.trace_cap = buf ? cap_events : 0; a.trace_n = n_out; a.totals = totals_out;
+  return launch_sim<true>(s, a, (cudaStream_t)stream);
+}
+
+extern "C" int mig_sim_debug_set_jobs(mig_sim_t *s, const mig_job_t *jobs, uint32_t n) {
+  if (!s) return fail(MIG_EINVAL, "debug_set_jobs: NULL handle");
+  CU(cudaDeviceSynchronize());
+  cudaFree(s->d_script); s->d_script = nullptr; s->n_script = 0;
+  if (n == 0) return MIG_OK;
+  if (!jobs) return fail(MIG_EINVAL, "debug_set_jobs: NULL jobs");
+  if (n > MIG_MAX_JOBS) return fail(MIG_EINVAL, "debug_set_jobs: too many jobs");
+  std::vector<DevTables> host(1);
+  CU(cudaMemcpy(host.data(), s->d_tab, sizeof(DevTables), cudaMemcpyDeviceToHost));
+  for (uint32_t i = 0; i < n; ++i) {
+    const mig_job_t &j = jobs[i];
+    if (j.cls >= s->p.n_classes) return fail(MIG_EINVAL, "debug_set_jobs: job %u: class %u out of range", i, j.cls);
+    if (j.arr < 0 || j.arr > (1 << 30) || j.due < 0 || j.due > (1 << 30)) return fail(MIG_EINVAL, "debug_set_jobs: job %u: arr/due out of [0, 2^30]", i);
+    if (i && j.arr < jobs[i - 1].arr) return fail(MIG_EINVAL, "debug_set_jobs: arrivals must be non-decreasing (job %u)", i);
+    if (j.dur7 < 1 || j.dur7 > (1 << 24)) return fail(MIG_EINVAL, "debug_set_jobs: job %u: dur7 %d not in 1..2^24", i, j.dur7);
+    uint32_t vmin = 0xFFFFFFFFu, vmax = 0;
+    for (int k = 0; k < 5; ++k) { uint32_t v = host[0].speed[j.cls * 5 + k].x; vmin = v < vmin ? v : vmin; vmax = v > vmax ? v : vmax; }
+    unsigned long long work = (unsigned long long)j.dur7 * host[0].speed[j.cls * 5 + 4].x;
+    if (work + vmax >= (1ull << 31) || (work + vmin - 1) / vmin >= (1ull << 28))
+      return fail(MIG_EINVAL, "debug_set_jobs: job %u: work %llu out of the int32 / 2^28 s range", i, work);
+  }
+  if (cudaMalloc((void **)&s->d_script, (size_t)n * sizeof(mig_job_t)) != cudaSuccess) { cudaGetLastError(); return fail(MIG_ENOMEM, "debug_set_jobs: cudaMalloc failed"); }
+  CU(cudaMemcpy(s->d_script, jobs, (size_t)n * sizeof(mig_job_t), cudaMemcpyHostToDevice));
+  s->n_script = n;
+  return MIG_OK;
+}

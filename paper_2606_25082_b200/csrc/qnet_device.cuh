@@ -1,0 +1,115 @@
+// qnet_device.cuh -- batched Q-network forward, MLP 64 -> H -> H -> A, ReLU, fp32.
+//
+// Every output is accumulated as acc = b[n]; for k ascending: acc = fmaf(in[k], W[k][n], acc): one rounding per
+// term, fixed order, so the result is bit-identical to a sequential CPU fmaf loop.  That is why this is a CUDA-core
+// register-tiled kernel and not a tensor-core GEMM (split accumulation would change the argmax on near-ties and
+// fork the DQN-driven event trace).  One CTA = 32 batch rows, H threads; activations live in shared memory
+// k-major ([k][row]) so that one LDS.128 feeds four FFMAs; weights stream from L2 (334 KB, resident), coalesced.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "sim_common.h"
+
+namespace migsim {
+
+constexpr int kQRows = 32;
+
+struct QArgs {
+  const float *W1, *b1, *W2, *b2, *W3, *b3;
+  uint32_t H, A;
+  const float *state;   // [B][64]
+  uint32_t B;
+  float *q_out;         // [B][A] or NULL
+  uint8_t *argmax_out;  // [B] or NULL
+  // epsilon-greedy from Philox stream 2 (R2): action_out[B]
+  uint8_t *action_out;  // NULL = no policy
+  uint32_t eps_thr;     // explore iff w_explore < eps_thr = min(round(eps 2^32), 2^32 - 1)
+  uint32_t epoch, k0, k1, episode, env_base;
+};
+
+__device__ __forceinline__ uint4 philox_q(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  return make_uint4(c0, c1, c2, c3);
+}
+
+// one dense layer for the CTA's 32 rows: thread n computes column n for all rows.  in: [K][32] k-major, out: [H][32].
+template <bool RELU>
+__device__ __forceinline__ void q_layer(const float *__restrict__ W, const float *__restrict__ b, int K, int H,
+                                        const float *in, float *out, int n) {
+  float acc[kQRows];
+  const float bias = b[n];
+#pragma unroll
+  for (int r = 0; r < kQRows; ++r) acc[r] = bias;
+#pragma unroll 4
+  for (int k = 0; k < K; ++k) {
+    const float w = __ldg(&W[(size_t)k * H + n]);
+    const float4 *row = reinterpret_cast<const float4 *>(in + k * kQRows);
+#pragma unroll
+    for (int r4 = 0; r4 < kQRows / 4; ++r4) {
+      float4 x = row[r4];                                   // broadcast: every thread of the warp reads the same address
+      acc[4 * r4 + 0] = __fmaf_rn(x.x, w, acc[4 * r4 + 0]);
+      acc[4 * r4 + 1] = __fmaf_rn(x.y, w, acc[4 * r4 + 1]);
+      acc[4 * r4 + 2] = __fmaf_rn(x.z, w, acc[4 * r4 + 2]);
+      acc[4 * r4 + 3] = __fmaf_rn(x.w, w, acc[4 * r4 + 3]);
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < kQRows; ++r) {
+    float v = acc[r];
+    if (RELU) v = v > 0.0f ? v : 0.0f;
+    out[n * kQRows + r] = v;
+  }
+}
+
+__global__ void __launch_bounds__(256) qnet_kernel(const QArgs a) {
+  extern __shared__ __align__(16) float qsm[];
+  const int H = (int)a.H, A = (int)a.A;
+  float *x = qsm;                               // [64][32]
+  float *h1 = x + MIG_STATE_DIM * kQRows;       // [H][32]
+  float *h2 = h1 + H * kQRows;                  // [H][32]
+  float *qo = h2 + H * kQRows;                  // [A][32]
+  const int tid = threadIdx.x;
+  const uint32_t row0 = blockIdx.x * kQRows;
+  for (int i = tid; i < MIG_STATE_DIM * kQRows; i += blockDim.x) {   // coalesced read of [row][k], transposed store
+    int r = i / MIG_STATE_DIM, k = i % MIG_STATE_DIM;
+    uint32_t row = row0 + r;
+    x[k * kQRows + r] = row < a.B ? a.state[(size_t)row * MIG_STATE_DIM + k] : 0.0f;
+  }
+  __syncthreads();
+  q_layer<true>(a.W1, a.b1, MIG_STATE_DIM, H, x, h1, tid);
+  __syncthreads();
+  q_layer<true>(a.W2, a.b2, H, H, h1, h2, tid);
+  __syncthreads();
+  for (int o = tid; o < A * kQRows; o += blockDim.x) {                // output layer: (n, row) pairs
+    int n = o / kQRows, r = o % kQRows;
+    float acc = a.b3[n];
+    for (int k = 0; k < H; ++k) acc = __fmaf_rn(h2[k * kQRows + r], __ldg(&a.W3[(size_t)k * A + n]), acc);
+    qo[n * kQRows + r] = acc;
+  }
+  __syncthreads();
+  if (a.q_out)
+    for (int o = tid; o < A * kQRows; o += blockDim.x) {
+      int r = o / A, n = o % A;
+      if (row0 + r < a.B) a.q_out[(size_t)(row0 + r) * A + n] = qo[n * kQRows + r];
+    }
+  if (tid < kQRows && row0 + tid < a.B) {
+    const uint32_t row = row0 + tid;
+    int best = 0; float bv = qo[tid];
+    for (int n = 1; n < A; ++n) { float v = qo[n * kQRows + tid]; if (v > bv) { bv = v; best = n; } }   // lowest index on ties
+    if (a.argmax_out) a.argmax_out[row] = (uint8_t)best;
+    if (a.action_out) {
+      uint4 w = philox_q(a.epoch, 2u, a.env_base + row, a.episode, a.k0, a.k1);
+      bool explore = w.x < a.eps_thr;
+      a.action_out[row] = explore ? (uint8_t)(((unsigned long long)w.y * (unsigned long long)A) >> 32) : (uint8_t)best;
+    }
+  }
+}
+
+}  // namespace migsim

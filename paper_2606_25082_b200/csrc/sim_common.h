@@ -1,0 +1,62 @@
+// sim_common.h -- structures shared by the host API (migsim.cu) and the device code (sim_device.cuh).
+// Part of libmigsim.so (product path).  Nothing here is shared with oracle/.
+#pragma once
+#include <stdint.h>
+
+#include "../../include/migsim.h"
+
+namespace migsim {
+
+constexpr int kSlots = MIG_SLOTS;
+constexpr int kWarpsPerCta = 4;
+constexpr int kHeaderWords = 64;  // saved per-env header: 256 bytes
+
+// meta word of a job-table entry: id[0:20) | class[20:24) | crit_cnt[24:28) | slot+1 [28:31)
+constexpr uint32_t kIdMask = 0xFFFFFu;
+
+// Everything the kernels read that is a table (global memory, read-only, L1/L2 resident).
+struct DevTables {
+  uint4 speed[MIG_MAX_CLASSES * 5];         // {v, magic m, shift (>=32: v == 1), 0}: x / v = umulhi(x, m) >> sh
+  int32_t dur7_q[MIG_MAX_CLASSES * 65];
+  uint32_t class_cum[MIG_MAX_CLASSES];
+  uint32_t slack_lo[MIG_MAX_CLASSES], slack_span[MIG_MAX_CLASSES];  // lo, hi - lo + 1
+  uint32_t cfg_pack[MIG_MAX_CONFIGS];       // 7 nibbles: size of the slice starting at slot p
+  uint32_t thr[MIG_THR_BINS];
+  uint32_t logT[257];                        // round(2^24 log2(1 + i/256))
+  int32_t curve[8], p_idle[8], p_busy[8];    // p_idle/p_busy indexed by SIZE (0..7), not by size index
+};
+
+// Kernel arguments (by value, constant bank).
+struct SimArgs {
+  const DevTables *tab;
+  uint32_t *hdr;        // [n_envs][64] words
+  uint4 *jobtab;        // [n_envs][cap] entries {skey, meta, rem, due}
+  uint4 *tab_override;  // debug trace: overflow table for the single env (cap entries) instead of jobtab
+  unsigned int *counter;  // dynamic env counter (zeroed before the launch)
+  uint32_t n_envs, env_first;  // envs [env_first, env_first + n_envs) of the handle
+  uint32_t n_classes, n_configs;
+  uint32_t k0, k1, episode, env_base;  // Philox key, counter words
+  uint64_t gap_scale;
+  int32_t day_s, epoch_s, n_epochs, t_limit_s;
+  uint32_t cap, job_limit, smem_entries;
+  int32_t downtime_s; int64_t repart_energy;
+  int32_t theta; uint32_t crit_max;
+  float w_energy, w_tardy;
+  // what to do
+  int from_init;        // 1: initialise from algo/cfg0 (reset), 0: load the saved state
+  int save;             // 1: write the state back
+  int n_steps;          // epochs to run in this launch
+  int policy;           // 0 static, 1 table, 3 explicit actions
+  const uint8_t *algo, *cfg0;                        // from_init
+  const uint8_t *table;                              // [n_envs][n_epochs][4]
+  const uint8_t *actions; uint32_t act_stride_env, act_stride_k;   // action = actions[env * se + (k - k_first) * sk]
+  const mig_job_t *script; uint32_t n_script;
+  // outputs (NULL = skip)
+  float *state_out; float *reward_out; int64_t *energy_out; int64_t *tard_out;
+  mig_epoch_rec_t *recs; int32_t rec_k0; mig_epoch_rec_t *drain_rec;   // record of epoch k -> recs[(k - rec_k0) * n_envs_total + env]
+  uint32_t rec_stride;                               // n_envs_total
+  mig_totals_t *totals;
+  mig_event_t *trace; uint32_t trace_cap; uint32_t *trace_n;
+};
+
+}  // namespace migsim

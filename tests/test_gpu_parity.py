@@ -1,0 +1,353 @@
+"""GPU parity: the CUDA path (through the C ABI) vs the CPU oracle, element by element, on the same seeded inputs.
+
+Bar (north_star): BIT-EXACT on every event trace and integer objective component; the fp32 state vector is exact by
+construction (small integers times powers of two); Q-values and rewards are compared bit-for-bit as well (fixed-order
+fmaf / two products and an add), which is stricter than the 1e-4 relative tolerance north_star allows.
+"""
+import concurrent.futures as cf
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2606_25082_b200 import workloads as W
+import trace_check
+from util import CAP3, LINEAR, SUB05, golden, tiny_params
+
+pytestmark = pytest.mark.gpu
+
+B = None
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _binding():
+    global B
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_25082_b200 import binding
+    B = binding
+    yield
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+# ------------------------------------------------------------------------------------------------ oracle side
+def _oracle_env(args):
+    wl_name, n_envs, e, want_trace, overrides = args
+    wl = W.CONFIGS[wl_name](n_envs)
+    sp = wl.params
+    r = O.rollout(sp, wl.seed, e + sp.env_offset, algo=int(wl.algo[e]), cfg0=int(wl.cfg0[e]), policy=wl.policy,
+                  table=None if wl.table is None else wl.table[e], qnet=wl.qnet, epsilon=wl.epsilon,
+                  trace_cap=600000 if want_trace else 0, want_states=True)
+    return e, r.recs, r.totals, (r.trace if want_trace else None), r.states, r.actions, r.rewards
+
+
+def oracle_many(wl_name, n_envs, envs, want_trace=False):
+    args = [(wl_name, n_envs, int(e), want_trace, None) for e in envs]
+    workers = min(len(args), os.cpu_count() or 1)
+    if workers <= 1:
+        return [_oracle_env(a) for a in args]
+    with cf.ProcessPoolExecutor(workers) as ex:
+        return list(ex.map(_oracle_env, args, chunksize=max(1, len(args) // (4 * workers))))
+
+
+def gpu_rollout(wl, sim=None, qnet=None):
+    sim = sim or B.MigSim(wl.params, wl.n_envs, wl.seed)
+    recs, totals = sim.alloc_recs(), sim.alloc_totals()
+    sim.reset(0, dev(wl.algo), dev(wl.cfg0))
+    table = None if wl.table is None else dev(wl.table)
+    if wl.policy == W.POLICY_DQN and qnet is None:
+        qnet = B.QNet(wl.qnet)
+    sim.rollout(wl.policy, table=table, qnet=qnet, epsilon=wl.epsilon, recs_out=recs, totals_out=totals)
+    torch.cuda.synchronize()
+    return sim, B.recs_to_numpy(recs), B.totals_to_numpy(totals), table
+
+
+def assert_same_records(g_recs, g_tot, o_recs, o_tot, tag):
+    assert g_tot.tobytes() == o_tot.tobytes(), "%s totals differ:\n gpu %s\n orc %s" % (tag, g_tot, o_tot)
+    for k in range(len(o_recs)):
+        assert g_recs[k].tobytes() == o_recs[k].tobytes(), "%s record %d differs:\n gpu %s\n orc %s" % (tag, k, g_recs[k], o_recs[k])
+
+
+def compare_workload(name, n_envs, sample_envs, trace_envs):
+    wl = W.CONFIGS[name](n_envs)
+    sim, recs, totals, table = gpu_rollout(wl)
+    assert np.all(totals["status"] == 0)
+    res = oracle_many(name, n_envs, sample_envs)
+    for e, o_recs, o_tot, _, _, _, _ in res:
+        assert_same_records(recs[:, e], totals[e], o_recs, o_tot, "%s env %d" % (name, e))
+    # full event trace for a subset (DQN: replay the actions the rollout took = the records' cfg)
+    for e, o_recs, o_tot, o_trace, _, o_act, _ in oracle_many(name, n_envs, trace_envs, want_trace=True):
+        if wl.policy == W.POLICY_DQN:
+            ev, tot = sim.debug_trace(e, actions=dev(recs[:24, e]["cfg"].astype(np.uint8)))
+        else:
+            ev, tot = sim.debug_trace(e, policy=wl.policy, table=table)
+        assert len(ev) == len(o_trace), "%s env %d: %d events vs %d" % (name, e, len(ev), len(o_trace))
+        if ev.tobytes() != o_trace.tobytes():
+            i = int(np.nonzero(ev != o_trace)[0][0])
+            raise AssertionError("%s env %d: first differing event %d:\n gpu %s\n orc %s" % (name, e, i, ev[max(0, i - 3):i + 2], o_trace[max(0, i - 3):i + 2]))
+        assert tot.tobytes() == o_tot.tobytes()
+        trace_check.check_against_records(wl.params, int(wl.cfg0[e]), ev, recs[:, e], totals[e])
+    sim.close()
+    return totals
+
+
+# ------------------------------------------------------------------------------------------------ BASELINE configs
+def test_c1_full_trace():
+    compare_workload("C1", 1, [0], [0])
+
+
+def test_c2_all_envs_all_algorithms_all_configs():
+    tot = compare_workload("C2", 1024, range(1024), range(0, 1024, 16))
+    assert tot["n_jobs"].sum() > 1024 * 1900
+
+
+def test_c3_twice_daily_repartitioning():
+    tot = compare_workload("C3", 4096, range(0, 4096, 4), range(0, 4096, 64))
+    assert np.all(tot["n_repart"] == 2)
+
+
+def test_c4_dqn_driven():
+    tot = compare_workload("C4", 8192, range(0, 8192, 16), range(0, 8192, 128))
+    assert tot["n_repart"].mean() > 5
+
+
+def test_c5_full_size_sampled():
+    # BASELINE's full size in the launch configuration bench.py times; the oracle checks a sample one by one
+    tot = compare_workload("C5", 65536, range(0, 65536, 256), range(0, 65536, 4096))
+    # properties that hold at any size
+    assert np.all(tot["n_jobs"] == tot["n_completed"] + tot["n_dropped"])
+    assert abs(tot["n_jobs"].mean() - 8000) < 8000 * 0.01
+
+
+# ------------------------------------------------------------------------------------------------ hand-worked schedules on the GPU
+G = golden("handworked.json")
+
+
+def gpu_script(sp, rows, algo, cfg, n_envs=1, actions=None, cap_events=4096):
+    sim = B.MigSim(sp, n_envs, 0)
+    jobs = O.make_jobs(rows).astype(B.JOB_DTYPE)
+    sim.debug_set_jobs(jobs)
+    sim.reset(0, dev(np.full(n_envs, algo, np.uint8)), dev(np.full(n_envs, cfg, np.uint8)))
+    ev, tot = sim.debug_trace(0, actions=None if actions is None else dev(np.asarray(actions, np.uint8)), cap_events=cap_events)
+    sim.close()
+    return ev, tot
+
+
+@pytest.mark.parametrize("case,algos,speeds,kw", [
+    ("A", [0, 1, 2, 3], (LINEAR,), dict(crit_laxity_s=1)),
+    ("B", [0, 1], (LINEAR,), {}),
+    ("C", [0, 1], (LINEAR,), {}),
+    ("E", [0, 1, 2, 3], (LINEAR,), dict(crit_laxity_s=5, crit_max=3)),
+    ("F", [0, 2, 3], (LINEAR, SUB05), dict(crit_laxity_s=1)),
+    ("G", [0, 1, 2, 3], (CAP3,), {}),
+])
+def test_handworked_schedules_trace_equal(case, algos, speeds, kw):
+    g = G[case]
+    sp = tiny_params(speeds=speeds, **kw)
+    for algo in algos:
+        ev, tot = gpu_script(sp, g["jobs"], algo, g["cfg"])
+        r = O.rollout(sp, 0, 0, algo=algo, cfg0=g["cfg"], jobs=O.make_jobs(g["jobs"]), trace_cap=256)
+        assert ev.tobytes() == r.trace.tobytes(), (case, algo, ev, r.trace)
+        assert tot.tobytes() == r.totals.tobytes()
+
+
+def test_handworked_values_direct():
+    # the GPU against the hand-computed numbers themselves (not via the oracle)
+    g = G["B"]
+    sp = tiny_params()
+    for name, algo in (("EDF-FS", 0), ("EDF-SS", 1)):
+        ev, tot = gpu_script(sp, g["jobs"], algo, g["cfg"])
+        comp = {int(e["job"]): int(e["t"]) for e in ev if e["type"] == 5}
+        assert comp == {int(k): v for k, v in g[name]["completion"].items()}
+        assert int(tot["energy_mj"]) == g["idle_mw"] * 86400 + g[name]["dyn_energy_mj"]
+    g = G["D"]
+    sp = tiny_params(repart_downtime_s=g["downtime_s"], repart_energy_mj=g["repart_energy_mj"])
+    acts = [g["cfg0"]] + [g["action_epoch1"]] * 23
+    ev, tot = gpu_script(sp, g["jobs"], g["algo"], g["cfg0"], actions=acts)
+    comp = {int(e["job"]): int(e["t"]) for e in ev if e["type"] == 5}
+    assert comp == {int(k): v for k, v in g["completion"].items()}
+    assert int(tot["n_repart"]) == 1 and int(tot["tardiness_s"]) == 0
+    assert int(tot["energy_mj"]) == g["epoch0_energy_mj"] + g["epoch1_energy_mj"] + 22 * 85000 * 3600
+
+
+# ------------------------------------------------------------------------------------------------ step API, states, rewards
+@pytest.mark.parametrize("name,n", [("C3", 96), ("C4", 96), ("C2", 96)])
+def test_step_equals_rollout_and_oracle_states(name, n):
+    wl = W.CONFIGS[name](n)
+    res = {e: r for e, *r in oracle_many(name, n, range(n))}
+    sim = B.MigSim(wl.params, n, wl.seed)
+    state = sim.alloc_state()
+    sim.reset(0, dev(wl.algo), dev(wl.cfg0), state_out=state)
+    s0 = state.cpu().numpy()
+    for e in range(n):
+        assert np.array_equal(s0[e], res[e][3][0])
+    reward = torch.zeros(n, dtype=torch.float32, device="cuda")
+    dE = torch.zeros(n, dtype=torch.int64, device="cuda")
+    dT = torch.zeros(n, dtype=torch.int64, device="cuda")
+    rec = torch.zeros((n, 64), dtype=torch.uint8, device="cuda")
+    drain = torch.zeros((n, 64), dtype=torch.uint8, device="cuda")
+    for k in range(24):
+        act = np.array([res[e][4][k] for e in range(n)], dtype=np.uint8)       # the oracle's actions (teacher forcing)
+        sim.step(dev(act), state_out=state, reward_out=reward, energy_out=dE, tard_out=dT, rec_out=rec, drain_rec_out=drain)
+        torch.cuda.synchronize()
+        s, rw, recs = state.cpu().numpy(), reward.cpu().numpy(), B.recs_to_numpy(rec)
+        for e in range(n):
+            o_recs, o_tot, _, o_states, o_act, o_rew = res[e]
+            assert recs[e].tobytes() == o_recs[k].tobytes(), (name, e, k, recs[e], o_recs[k])
+            assert np.array_equal(s[e], o_states[k + 1]), (name, e, k, s[e], o_states[k + 1])
+            assert rw[e].tobytes() == np.float32(o_rew[k]).tobytes(), (name, e, k)
+            extra = int(o_recs[24]["energy_mj"]) if k == 23 else 0
+            assert int(dE[e]) == int(o_recs[k]["energy_mj"]) + extra
+    dr = B.recs_to_numpy(drain)
+    tot = sim.alloc_totals()
+    sim.totals(tot)
+    tot = B.totals_to_numpy(tot)
+    for e in range(n):
+        assert dr[e].tobytes() == res[e][0][24].tobytes()
+        assert tot[e].tobytes() == res[e][1].tobytes()
+    with pytest.raises(B.MigError) as ei:
+        sim.step(dev(np.zeros(n, np.uint8)))
+    assert ei.value.code == B.MIG_ESTATE
+    sim.close()
+
+
+def test_partial_steps_then_rollout():
+    wl = W.config_c3(64)
+    _, recs_ref, tot_ref, table = gpu_rollout(wl)
+    sim = B.MigSim(wl.params, 64, wl.seed)
+    sim.reset(0, dev(wl.algo), dev(wl.cfg0))
+    for k in range(7):
+        sim.step(dev(recs_ref[k]["cfg"].astype(np.uint8)))
+    recs, tot = sim.alloc_recs(), sim.alloc_totals()
+    sim.rollout(W.POLICY_TABLE, table=table, recs_out=recs, totals_out=tot)
+    torch.cuda.synchronize()
+    assert B.totals_to_numpy(tot).tobytes() == tot_ref.tobytes()
+    assert B.recs_to_numpy(recs)[7:].tobytes() == recs_ref[7:].tobytes()
+    sim.close()
+
+
+def test_rollout_host_matches_device_rollout():
+    for name, n in (("C3", 128), ("C4", 128)):
+        wl = W.CONFIGS[name](n)
+        _, recs_ref, tot_ref, _ = gpu_rollout(wl)
+        sim = B.MigSim(wl.params, n, wl.seed)
+        q = B.QNet(wl.qnet) if wl.qnet is not None else None
+        tot = np.zeros(n, dtype=B.TOTALS_DTYPE)
+        recs = np.zeros((25, n), dtype=B.REC_DTYPE)
+        sim.rollout_host(0, wl.algo, wl.cfg0, wl.policy, wl.table, q, wl.epsilon, recs, tot)
+        assert tot.tobytes() == tot_ref.tobytes() and recs.tobytes() == recs_ref.tobytes()
+        sim.close()
+
+
+def test_env_base_sharding_is_placement_invariant():
+    import dataclasses
+    wl = W.config_c3(64)
+    _, recs_ref, tot_ref, _ = gpu_rollout(wl)
+    for lo, hi in (W.shard_range(64, 0, 2), W.shard_range(64, 1, 2)):
+        sp = dataclasses.replace(wl.params, env_offset=lo)
+        sim = B.MigSim(sp, hi - lo, wl.seed)
+        recs, tot = sim.alloc_recs(), sim.alloc_totals()
+        sim.reset(0, dev(wl.algo[lo:hi]), dev(wl.cfg0[lo:hi]))
+        sim.rollout(wl.policy, table=dev(wl.table[lo:hi]), recs_out=recs, totals_out=tot)
+        torch.cuda.synchronize()
+        assert B.totals_to_numpy(tot).tobytes() == tot_ref[lo:hi].tobytes()
+        sim.close()
+
+
+# ------------------------------------------------------------------------------------------------ Q-network
+@pytest.mark.parametrize("B_", [1, 31, 32, 33, 1000, 8192])
+def test_q_eval_bit_exact(B_):
+    qw = W.make_qnet(7, 12)
+    q = B.QNet(qw)
+    rng = np.random.default_rng(B_)
+    x = rng.uniform(0, 4, size=(B_, 64)).astype(np.float32)
+    x[rng.uniform(size=x.shape) < 0.5] = 0.0
+    q_out = torch.zeros((B_, 12), dtype=torch.float32, device="cuda")
+    am = torch.zeros(B_, dtype=torch.uint8, device="cuda")
+    q.q_eval(dev(x), q_out, am)
+    torch.cuda.synchronize()
+    ref_q, ref_am = O.q_eval(qw, x)
+    assert q_out.cpu().numpy().tobytes() == ref_q.tobytes()
+    assert np.array_equal(am.cpu().numpy(), ref_am)
+    # and within north_star's 1e-4 relative of the float64 evaluation
+    ref64 = O.q_eval_f64(qw, x)
+    assert np.max(np.abs(q_out.cpu().numpy() - ref64) / np.maximum(np.abs(ref64), 1e-2)) < 1e-4
+
+
+def test_q_eval_small_hidden_and_ties():
+    qw = W.make_qnet(3, 5, hidden=64)
+    qw.W3[:] = 0; qw.b3[:] = [1, 7, 7, 7, 0]
+    q = B.QNet(qw)
+    x = np.random.default_rng(0).normal(size=(40, 64)).astype(np.float32)
+    am = torch.zeros(40, dtype=torch.uint8, device="cuda")
+    q.q_eval(dev(x), None, am)
+    assert np.all(am.cpu().numpy() == 1)
+
+
+# ------------------------------------------------------------------------------------------------ edge cases
+def test_queue_cap_overflows_shared_table_and_drops():
+    sp = tiny_params(cap=256)
+    rows = [(5, 0, 100, 100000)] * 300 + [(50000, 0, 7, 50100)] * 3
+    ev, tot = gpu_script(sp, rows, 0, 3)
+    r = O.rollout(sp, 0, 0, algo=0, cfg0=3, jobs=O.make_jobs(rows), trace_cap=4096)
+    assert int(tot["n_dropped"]) == 44 and int(tot["n_sys_max"]) == 256
+    assert ev.tobytes() == r.trace.tobytes() and tot.tobytes() == r.totals.tobytes()
+
+
+@pytest.mark.parametrize("algo", [0, 1, 2, 3])
+def test_long_queue_all_algorithms(algo):
+    # several hundred jobs in system (beyond the 64 entries kept in shared memory), all 4 algorithms, mixed classes
+    sp = tiny_params(speeds=(LINEAR, SUB05, CAP3), cap=1024, crit_laxity_s=30)
+    rng = np.random.default_rng(algo)
+    rows = sorted((int(rng.integers(0, 2000)), int(rng.integers(0, 3)), int(rng.integers(1, 10)), 0) for _ in range(700))
+    rows = [(a, c, d, a + int(rng.integers(1, 4000))) for (a, c, d, _) in rows]
+    ev, tot = gpu_script(sp, rows, algo, 5, cap_events=20000)
+    r = O.rollout(sp, 0, 0, algo=algo, cfg0=5, jobs=O.make_jobs(rows), trace_cap=20000)
+    assert int(tot["n_sys_max"]) > 200
+    assert len(ev) == len(r.trace)
+    assert ev.tobytes() == r.trace.tobytes() and tot.tobytes() == r.totals.tobytes()
+
+
+def test_truncation_bad_action_and_empty_day():
+    sp = tiny_params(t_limit_s=90000)
+    ev, tot = gpu_script(sp, [(0, 0, 10, 50)], 0, 0)       # dur7 limited by the class table (10 s): finishes
+    assert int(tot["status"]) == 0
+    import dataclasses
+    sp2 = dataclasses.replace(W.make_params([LINEAR], [W.dur_constant(100000)], [1], jobs_per_day=200, amplitude=0.0), t_limit_s=90000)
+    ev, tot = gpu_script(sp2, [(0, 0, 100000, 50)], 0, 0)
+    r = O.rollout(sp2, 0, 0, algo=0, cfg0=0, jobs=O.make_jobs([(0, 0, 100000, 50)]), trace_cap=100)
+    assert int(tot["status"]) & 1 and tot.tobytes() == r.totals.tobytes() and ev.tobytes() == r.trace.tobytes()
+    # bad action = stay + flag
+    ev, tot = gpu_script(sp, [(10, 0, 5, 100)], 0, 3, actions=[200] * 24)
+    assert int(tot["status"]) & 2 and int(tot["n_repart"]) == 0
+    # a day with no arrivals at all (thinning threshold 0 ... only w_accept == 0 passes)
+    sp3 = dataclasses.replace(W.config_c2(4).params, accept_thr=np.zeros(1440, np.uint32))
+    sim = B.MigSim(sp3, 4, 1)
+    tot = sim.alloc_totals()
+    sim.reset(0, dev(np.arange(4, dtype=np.uint8)), dev(np.array([0, 3, 6, 11], np.uint8)))
+    sim.rollout(W.POLICY_STATIC, totals_out=tot)
+    t = B.totals_to_numpy(tot)
+    assert np.all(t["n_jobs"] == 0) and np.all(t["n_events"] == 0) and np.all(t["t_end"] == 86400)
+    for e, cfg in enumerate([0, 3, 6, 11]):
+        idle = sum(int(sp3.p_idle_mw[W.SIZE_INDEX[int(g)]]) for g in sp3.size_at_slot[cfg] if g)
+        assert int(t[e]["energy_mj"]) == idle * 86400
+    sim.close()
+
+
+def test_episode_changes_the_day_and_reset_is_repeatable():
+    wl = W.config_c2(32)
+    sim = B.MigSim(wl.params, 32, wl.seed)
+    hashes = []
+    for ep in (0, 1, 0):
+        tot = sim.alloc_totals()
+        sim.reset(ep, dev(wl.algo), dev(wl.cfg0))
+        sim.rollout(W.POLICY_STATIC, totals_out=tot)
+        hashes.append(B.totals_to_numpy(tot)["trace_hash"].copy())
+    assert np.array_equal(hashes[0], hashes[2]) and not np.any(hashes[0] == hashes[1])
+    r = O.rollout(wl.params, wl.seed, 5, episode=1, algo=int(wl.algo[5]), cfg0=int(wl.cfg0[5]))
+    assert int(r.totals["trace_hash"]) == int(hashes[1][5])
+    sim.close()
