@@ -300,10 +300,11 @@ def test_queue_cap_overflows_shared_table_and_drops():
 
 @pytest.mark.parametrize("algo", [0, 1, 2, 3])
 def test_long_queue_all_algorithms(algo):
-    # several hundred jobs in system (beyond the 64 entries kept in shared memory), all 4 algorithms, mixed classes
+    # ~500 jobs in system (beyond the entries kept in shared memory), all 4 algorithms, mixed classes; the LLF / LALF
+    # runs also raise several hundred critical-laxity events
     sp = tiny_params(speeds=(LINEAR, SUB05, CAP3), cap=1024, crit_laxity_s=30)
     rng = np.random.default_rng(algo)
-    rows = sorted((int(rng.integers(0, 2000)), int(rng.integers(0, 3)), int(rng.integers(1, 10)), 0) for _ in range(700))
+    rows = sorted((int(rng.integers(0, 2000)), int(rng.integers(0, 3)), int(rng.integers(1, 30)), 0) for _ in range(700))
     rows = [(a, c, d, a + int(rng.integers(1, 4000))) for (a, c, d, _) in rows]
     ev, tot = gpu_script(sp, rows, algo, 5, cap_events=20000)
     r = O.rollout(sp, 0, 0, algo=algo, cfg0=5, jobs=O.make_jobs(rows), trace_cap=20000)
