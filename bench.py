@@ -157,7 +157,7 @@ def run_ours(args):
     n_envs = args.envs                                   # per GPU (weak scaling: every rank simulates a full batch)
     wl = W.CONFIGS[args.workload](n_envs)
     sp = dataclasses.replace(wl.params, env_offset=rank * n_envs)      # Philox keyed by global env id
-    sim = B.MigSim(sp, n_envs, wl.seed)
+    sim = B.MigSim(sp, n_envs, wl.seed, tile=args.tile)
     qnet = B.QNet(wl.qnet) if wl.qnet is not None else None
     d_algo, d_cfg0 = torch.from_numpy(wl.algo).cuda(), torch.from_numpy(wl.cfg0).cuda()
     d_table = None if wl.table is None else torch.from_numpy(wl.table).cuda()
@@ -256,7 +256,7 @@ def run_ours(args):
         line = {
             "metric": "job_events_per_s", "value": ev_total / t_s, "unit": "job-events/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
-            "config": {"workload": args.workload, "n_envs_per_gpu": n_envs, "n_envs_total": n_envs * world, "policy": ["static", "table", "dqn"][wl.policy],
+            "config": {"workload": args.workload, "n_envs_per_gpu": n_envs, "n_envs_total": n_envs * world, "policy": ["static", "table", "dqn"][wl.policy], "lanes_per_env": sim.get_tile(),
                        "job_events_per_step": ev_total / args.steps, "l2": "flushed between iterations (256 MiB write)", "parallelism": "env-range sharding, no data-path collective"},
             "day_episodes_per_s": n_envs * world * args.steps / t_s,
             "e2e": {"value": float(e2e_ev.item()) / float(e2e_t.item()), "unit": "job-events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
@@ -278,6 +278,7 @@ def main():
     ap.add_argument("--envs", type=int, default=0, help="environments per GPU (default: the workload's BASELINE size)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tile", type=int, default=0, choices=[0, 8, 16, 32], help="lanes per environment (0 = library default)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -184,6 +184,12 @@ int mig_sim_debug_set_jobs(mig_sim_t *s, const mig_job_t *jobs, uint32_t n);
 /* The exact-division constants the kernels use for x / v (host helper, exposed for tests): x / v == v == 1 ? x :
  * (umulhi(x, m) >> sh) for every 0 <= x < 2^31. */
 int mig_debug_div_magic(uint32_t v, uint32_t *m, uint32_t *sh);
+/* Lanes per environment of the rollout kernel: 8 (default; four environments per warp in lockstep -- the paper-shaped
+ * workloads keep about a dozen jobs in the system and a MIG GPU has 7 slots), 16, or 32 (one warp per environment, for
+ * workloads with hundreds of jobs in the system).  0 = default.  Results are identical for every value (tested); only
+ * the launch geometry and the shared-memory footprint change.  Allowed between any two calls; MIG_EINVAL otherwise. */
+int mig_sim_set_tile(mig_sim_t *s, int lanes_per_env);
+int mig_sim_get_tile(const mig_sim_t *s);
 /* Number of kernel launches issued through this handle so far (bench.py's gpu_launches). */
 uint64_t mig_sim_launch_count(const mig_sim_t *s);
 

@@ -33,7 +33,8 @@ assert EVENT_DTYPE.itemsize == 16 and REC_DTYPE.itemsize == 64 and TOTALS_DTYPE.
 EXPORTS = (
     "mig_last_error", "mig_version", "mig_sim_create", "mig_sim_destroy", "mig_sim_reset", "mig_sim_step",
     "mig_sim_rollout", "mig_sim_totals", "mig_sim_rollout_host", "mig_qnet_create", "mig_qnet_destroy", "mig_q_eval",
-    "mig_sim_debug_trace", "mig_sim_debug_set_jobs", "mig_debug_div_magic", "mig_sim_launch_count")
+    "mig_sim_debug_trace", "mig_sim_debug_set_jobs", "mig_debug_div_magic", "mig_sim_launch_count", "mig_sim_set_tile",
+    "mig_sim_get_tile")
 
 
 class MigError(RuntimeError):
@@ -84,6 +85,8 @@ def lib():
         L.mig_debug_div_magic.argtypes = [u32, C.POINTER(u32), C.POINTER(u32)]
         L.mig_sim_launch_count.argtypes = [vp]
         L.mig_sim_launch_count.restype = u64
+        L.mig_sim_set_tile.argtypes = [vp, i32]
+        L.mig_sim_get_tile.argtypes = [vp]
         _lib = L
     return _lib
 
@@ -169,7 +172,7 @@ class MigSim:
     """mig_sim_* calls on one handle.  Tensors are caller-owned CUDA tensors; nothing is allocated here except by
     the convenience helpers whose names start with ``alloc_``."""
 
-    def __init__(self, sp: SimParams, n_envs: int, seed: int):
+    def __init__(self, sp: SimParams, n_envs: int, seed: int, tile: int = 0):
         if not torch.cuda.is_available():
             raise MigError(MIG_ECUDA, "no CUDA device: the simulator has no CPU fallback")
         self.sp, self.n_envs, self.seed = sp, int(n_envs), int(seed)
@@ -177,6 +180,14 @@ class MigSim:
         ps, keep = _fill_params(sp)
         self.h = C.c_void_p()
         _check(lib().mig_sim_create(C.byref(self.h), C.byref(ps), self.n_envs, self.seed))
+        if tile:
+            self.set_tile(tile)
+
+    def set_tile(self, lanes_per_env: int):
+        _check(lib().mig_sim_set_tile(self.h, int(lanes_per_env)))
+
+    def get_tile(self) -> int:
+        return int(lib().mig_sim_get_tile(self.h))
 
     def close(self):
         if getattr(self, "h", None):

@@ -38,6 +38,7 @@ struct mig_sim {
   mig_params_t p;            // scalars (pointers inside are NOT kept)
   uint32_t n_envs = 0; uint64_t seed = 0; uint32_t episode = 0;
   int device = 0, n_sm = 0;
+  int tile = 8;              // lanes per environment (8, 16 or 32): 32 / tile environments per warp
   uint32_t smem_entries = 0; size_t smem_bytes = 0; int grid_max = 0;
   DevTables *d_tab = nullptr;
   uint32_t *d_hdr = nullptr; uint4 *d_jobtab = nullptr; uint4 *d_dbgtab = nullptr;
@@ -135,6 +136,45 @@ static int build_tables(const mig_params_t *p, DevTables *t) {
   return MIG_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ tile width
+constexpr int kDefaultTile = 8;
+
+template <bool TRACE>
+static const void *kernel_ptr(int tile) {
+  switch (tile) {
+    case 8: return (const void *)sim_kernel<8, TRACE>;
+    case 16: return (const void *)sim_kernel<16, TRACE>;
+    default: return (const void *)sim_kernel<32, TRACE>;
+  }
+}
+
+// shared-memory footprint and resident grid for `tile` lanes per environment
+static int configure_tile(mig_sim *s, int tile) {
+  if (tile != 8 && tile != 16 && tile != 32) return fail(MIG_EINVAL, "set_tile: lanes per environment must be 8, 16 or 32 (got %d)", tile);
+  const uint32_t cap8 = (s->p.cap + 7u) & ~7u;
+  const uint32_t entries = cap8 < 64u ? cap8 : 64u;
+  const size_t bytes = ((sizeof(HotTables) + 127) & ~(size_t)127) + (size_t)kWarpsPerCta * (32 / tile) * tile_smem_bytes(entries);
+  int occ = 0;
+  for (int trace = 0; trace < 2; ++trace) {
+    const void *k = trace ? kernel_ptr<true>(tile) : kernel_ptr<false>(tile);
+    if (bytes > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
+      return fail(MIG_ECUDA, "set_tile: %zu bytes of shared memory per CTA refused (%s)", bytes, cudaGetErrorString(cudaGetLastError()));
+    int o = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k, kWarpsPerCta * 32, bytes) != cudaSuccess || o < 1)
+      return fail(MIG_ECUDA, "set_tile: the rollout kernel does not fit this device (%s)", cudaGetErrorString(cudaGetLastError()));
+    if (!trace) occ = o;
+  }
+  s->tile = tile; s->smem_entries = entries; s->smem_bytes = bytes; s->grid_max = occ * s->n_sm;
+  return MIG_OK;
+}
+
+extern "C" int mig_sim_set_tile(mig_sim_t *s, int lanes_per_env) {
+  if (!s) return fail(MIG_EINVAL, "set_tile: NULL handle");
+  return configure_tile(s, lanes_per_env ? lanes_per_env : kDefaultTile);
+}
+
+extern "C" int mig_sim_get_tile(const mig_sim_t *s) { return s ? s->tile : 0; }
+
 extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n_envs, uint64_t seed) {
   if (!out || !p) return fail(MIG_EINVAL, "create: NULL argument");
   *out = nullptr;
@@ -153,13 +193,8 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
   cudaDeviceProp prop;
   if (cudaGetDevice(&s->device) != cudaSuccess || cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) { delete s; return fail(MIG_ECUDA, "create: cannot query the device"); }
   s->n_sm = prop.multiProcessorCount;
-  s->smem_entries = p->cap < 64 ? p->cap : 64;
-  s->smem_bytes = ((sizeof(HotTables) + 15) & ~(size_t)15) + (size_t)kWarpsPerCta * (WS_WORDS * 4 + (size_t)s->smem_entries * 16);
-  int occ = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sim_kernel<false>, kWarpsPerCta * 32, s->smem_bytes) != cudaSuccess || occ < 1) {
-    delete s; return fail(MIG_ECUDA, "create: the rollout kernel does not fit this device (%s)", cudaGetErrorString(cudaGetLastError()));
-  }
-  s->grid_max = occ * s->n_sm;
+  rc = configure_tile(s, kDefaultTile);
+  if (rc) { delete s; return rc; }
   size_t n = n_envs;
 #define ALLOC(ptr, bytes) if (cudaMalloc((void **)&(ptr), (bytes)) != cudaSuccess) { cudaGetLastError(); mig_sim_destroy(s); return fail(MIG_ENOMEM, "create: cudaMalloc of %zu bytes failed", (size_t)(bytes)); }
   ALLOC(s->d_tab, sizeof(DevTables));
@@ -214,9 +249,15 @@ static void base_args(const mig_sim *s, SimArgs &a) {
 template <bool TRACE>
 static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
   CU(cudaMemsetAsync(s->d_counter, 0, sizeof(unsigned int), st));
-  int ctas = (int)((a.n_envs + kWarpsPerCta - 1) / kWarpsPerCta);
+  const uint32_t envs_per_cta = (uint32_t)kWarpsPerCta * (32u / (uint32_t)s->tile);
+  int ctas = (int)((a.n_envs + envs_per_cta - 1) / envs_per_cta);
   if (ctas > s->grid_max) ctas = s->grid_max;
-  sim_kernel<TRACE><<<ctas, kWarpsPerCta * 32, s->smem_bytes, st>>>(a);
+  const dim3 grid((unsigned)ctas), block(kWarpsPerCta * 32);
+  switch (s->tile) {
+    case 8: sim_kernel<8, TRACE><<<grid, block, s->smem_bytes, st>>>(a); break;
+    case 16: sim_kernel<16, TRACE><<<grid, block, s->smem_bytes, st>>>(a); break;
+    default: sim_kernel<32, TRACE><<<grid, block, s->smem_bytes, st>>>(a); break;
+  }
   CU(cudaGetLastError());
   s->launches++;
   return MIG_OK;
