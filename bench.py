@@ -278,7 +278,7 @@ def main():
     ap.add_argument("--envs", type=int, default=0, help="environments per GPU (default: the workload's BASELINE size)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--tile", type=int, default=0, choices=[0, 8, 16, 32], help="lanes per environment (0 = library default)")
+    ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 8, 16, 32], help="lanes per environment (0 = library default)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -168,6 +168,10 @@ class QNet:
     __del__ = close
 
 
+# lanes per environment passed to mig_sim_set_tile by MigSim() when its `tile` argument is 0 (0 = the library's choice)
+DEFAULT_TILE = 0
+
+
 class MigSim:
     """mig_sim_* calls on one handle.  Tensors are caller-owned CUDA tensors; nothing is allocated here except by
     the convenience helpers whose names start with ``alloc_``."""
@@ -180,6 +184,7 @@ class MigSim:
         ps, keep = _fill_params(sp)
         self.h = C.c_void_p()
         _check(lib().mig_sim_create(C.byref(self.h), C.byref(ps), self.n_envs, self.seed))
+        tile = tile or DEFAULT_TILE
         if tile:
             self.set_tile(tile)
 

@@ -12,6 +12,7 @@
 
 #include "qnet_device.cuh"
 #include "sim_device.cuh"
+#include "sim_thread.cuh"
 
 using namespace migsim;
 
@@ -41,7 +42,7 @@ struct mig_sim {
   int tile = 8;              // lanes per environment (8, 16 or 32): 32 / tile environments per warp
   uint32_t smem_entries = 0; size_t smem_bytes = 0; int grid_max = 0;
   DevTables *d_tab = nullptr;
-  uint32_t *d_hdr = nullptr; uint4 *d_jobtab = nullptr; uint4 *d_dbgtab = nullptr;
+  uint32_t *d_hdr = nullptr; uint4 *d_jobtab = nullptr; uint4 *d_dbgtab = nullptr; uint32_t *d_dbghdr = nullptr;
   unsigned int *d_counter = nullptr;
   uint8_t *d_algo = nullptr, *d_cfg0 = nullptr;      // copies of the last reset's arrays (debug_trace re-runs from them)
   float *d_state = nullptr; uint8_t *d_action = nullptr;   // scratch of the DQN rollout
@@ -105,6 +106,14 @@ static int build_tables(const mig_params_t *p, DevTables *t) {
     }
     if (!n) return fail(MIG_EINVAL, "create: config %u has no slice", c);
     t->cfg_pack[c] = pack;
+    uint32_t ranks = 0, slot_of = 0; int pidle = 0;           // tie rule of reading #4: smaller size, then lower slot
+    for (int s = 0; s < MIG_SLOTS; ++s) {
+      int g = (pack >> (4 * s)) & 15, r = 0;
+      if (!g) continue;
+      for (int q = 0; q < MIG_SLOTS; ++q) { int h = (pack >> (4 * q)) & 15; if (h && (h < g || (h == g && q < s))) ++r; }
+      ranks |= (uint32_t)r << (4 * s); slot_of |= (uint32_t)s << (4 * r); pidle += t->p_idle[g];
+    }
+    t->cfg_rank[c] = ranks; t->cfg_slot_of[c] = slot_of; t->cfg_pidle[c] = pidle;
   }
   for (uint32_t c = 0; c < p->n_classes; ++c) {
     const int32_t *q = p->dur7_q + c * 65;
@@ -142,28 +151,39 @@ constexpr int kDefaultTile = 8;
 template <bool TRACE>
 static const void *kernel_ptr(int tile) {
   switch (tile) {
+    case 1: return (const void *)sim_thread_kernel<kThreadCta, TRACE>;
     case 8: return (const void *)sim_kernel<8, TRACE>;
     case 16: return (const void *)sim_kernel<16, TRACE>;
     default: return (const void *)sim_kernel<32, TRACE>;
   }
 }
 
-// shared-memory footprint and resident grid for `tile` lanes per environment
+// shared-memory footprint and resident grid for `tile` lanes per environment (1 = one thread per environment)
 static int configure_tile(mig_sim *s, int tile) {
-  if (tile != 8 && tile != 16 && tile != 32) return fail(MIG_EINVAL, "set_tile: lanes per environment must be 8, 16 or 32 (got %d)", tile);
-  const uint32_t cap8 = (s->p.cap + 7u) & ~7u;
-  const uint32_t entries = cap8 < 64u ? cap8 : 64u;
-  const size_t bytes = ((sizeof(HotTables) + 127) & ~(size_t)127) + (size_t)kWarpsPerCta * (32 / tile) * tile_smem_bytes(entries);
+  if (tile != 1 && tile != 8 && tile != 16 && tile != 32) return fail(MIG_EINVAL, "set_tile: lanes per environment must be 1, 8, 16 or 32 (got %d)", tile);
+  const uint32_t cap4 = (s->p.cap + 3u) & ~3u, cap8 = (s->p.cap + 7u) & ~7u;
+  uint32_t entries; size_t bytes; int threads;
+  if (tile == 1) {
+    // 16 entries in shared memory per environment: 448 B per thread, 7 CTAs of 64 threads per SM = 448 resident
+    // environments per SM (66 304 per B200: BASELINE C5's 65 536 run as ONE resident wave)
+    entries = cap4 < 16u ? cap4 : 16u; threads = kThreadCta;
+    bytes = thread_smem_bytes(entries, kThreadCta);
+  } else {
+    entries = cap8 < 64u ? cap8 : 64u; threads = kWarpsPerCta * 32;
+    bytes = ((sizeof(HotTables) + 127) & ~(size_t)127) + (size_t)kWarpsPerCta * (32 / tile) * tile_smem_bytes(entries);
+  }
   int occ = 0;
   for (int trace = 0; trace < 2; ++trace) {
     const void *k = trace ? kernel_ptr<true>(tile) : kernel_ptr<false>(tile);
     if (bytes > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
       return fail(MIG_ECUDA, "set_tile: %zu bytes of shared memory per CTA refused (%s)", bytes, cudaGetErrorString(cudaGetLastError()));
+    if (tile == 1) cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     int o = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k, kWarpsPerCta * 32, bytes) != cudaSuccess || o < 1)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k, threads, bytes) != cudaSuccess || o < 1)
       return fail(MIG_ECUDA, "set_tile: the rollout kernel does not fit this device (%s)", cudaGetErrorString(cudaGetLastError()));
     if (!trace) occ = o;
   }
+  if ((tile == 1) != (s->tile == 1)) s->epoch = -1;      // the saved per-env state has another layout: reset first
   s->tile = tile; s->smem_entries = entries; s->smem_bytes = bytes; s->grid_max = occ * s->n_sm;
   return MIG_OK;
 }
@@ -201,6 +221,7 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
   ALLOC(s->d_hdr, n * kHeaderWords * 4);
   ALLOC(s->d_jobtab, n * p->cap * sizeof(uint4));
   ALLOC(s->d_dbgtab, (size_t)p->cap * sizeof(uint4));
+  ALLOC(s->d_dbghdr, kHeaderWords * 4);
   ALLOC(s->d_counter, sizeof(unsigned int));
   ALLOC(s->d_algo, n); ALLOC(s->d_cfg0, n);
   ALLOC(s->d_state, n * MIG_STATE_DIM * sizeof(float));
@@ -217,7 +238,7 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
 extern "C" int mig_sim_destroy(mig_sim_t *s) {
   if (!s) return MIG_OK;
   cudaDeviceSynchronize();
-  cudaFree(s->d_tab); cudaFree(s->d_hdr); cudaFree(s->d_jobtab); cudaFree(s->d_dbgtab); cudaFree(s->d_counter);
+  cudaFree(s->d_tab); cudaFree(s->d_hdr); cudaFree(s->d_jobtab); cudaFree(s->d_dbgtab); cudaFree(s->d_dbghdr); cudaFree(s->d_counter);
   cudaFree(s->d_algo); cudaFree(s->d_cfg0); cudaFree(s->d_state); cudaFree(s->d_action); cudaFree(s->d_table);
   cudaFree(s->d_recs); cudaFree(s->d_totals); cudaFree(s->d_script);
   cudaGetLastError();
@@ -248,6 +269,13 @@ static void base_args(const mig_sim *s, SimArgs &a) {
 
 template <bool TRACE>
 static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
+  if (s->tile == 1) {                                     // one thread per environment, one CTA per 64 environments
+    const dim3 grid((a.n_envs + kThreadCta - 1) / kThreadCta), block(kThreadCta);
+    sim_thread_kernel<kThreadCta, TRACE><<<grid, block, s->smem_bytes, st>>>(a);
+    CU(cudaGetLastError());
+    s->launches++;
+    return MIG_OK;
+  }
   CU(cudaMemsetAsync(s->d_counter, 0, sizeof(unsigned int), st));
   const uint32_t envs_per_cta = (uint32_t)kWarpsPerCta * (32u / (uint32_t)s->tile);
   int ctas = (int)((a.n_envs + envs_per_cta - 1) / envs_per_cta);
@@ -442,7 +470,7 @@ extern "C" int mig_sim_debug_trace(mig_sim_t *s, uint32_t env, int policy, const
   if (!actions && policy != MIG_POLICY_STATIC && policy != MIG_POLICY_TABLE) return fail(MIG_EINVAL, "debug_trace: policy must be STATIC or TABLE, or pass actions");
   if (!actions && policy == MIG_POLICY_TABLE && !table) return fail(MIG_EINVAL, "debug_trace: TABLE policy needs a table");
   SimArgs a; base_args(s, a);
-  a.n_envs = 1; a.env_first = env; a.tab_override = s->d_dbgtab;
+  a.n_envs = 1; a.env_first = env; a.tab_override = s->d_dbgtab; a.hdr_override = s->d_dbghdr;
   a.from_init = 1; a.save = 0; a.n_steps = s->p.n_epochs;
   if (actions) { a.policy = 3; a.actions = actions; a.act_stride_env = 0; a.act_stride_k = 1; }
   else { a.policy = policy; a.table = table; }

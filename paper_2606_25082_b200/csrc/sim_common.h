@@ -21,6 +21,9 @@ struct DevTables {
   uint32_t class_cum[MIG_MAX_CLASSES];
   uint32_t slack_lo[MIG_MAX_CLASSES], slack_span[MIG_MAX_CLASSES];  // lo, hi - lo + 1
   uint32_t cfg_pack[MIG_MAX_CONFIGS];       // 7 nibbles: size of the slice starting at slot p
+  uint32_t cfg_rank[MIG_MAX_CONFIGS];       // nibble p: rank of that slice among the configuration's in (size, slot) order
+  uint32_t cfg_slot_of[MIG_MAX_CONFIGS];    // nibble r: start slot of the slice of rank r
+  int32_t cfg_pidle[MIG_MAX_CONFIGS];       // sum of p_idle over the configuration's slices
   uint32_t thr[MIG_THR_BINS];
   uint32_t logT[257];                        // round(2^24 log2(1 + i/256))
   int32_t curve[8], p_idle[8], p_busy[8];    // p_idle/p_busy indexed by SIZE (0..7), not by size index
@@ -32,6 +35,7 @@ struct SimArgs {
   uint32_t *hdr;        // [n_envs][64] words
   uint4 *jobtab;        // [n_envs][cap] entries {skey, meta, rem, due}
   uint4 *tab_override;  // debug trace: overflow table for the single env (cap entries) instead of jobtab
+  uint32_t *hdr_override;  // debug trace: scratch header for the single env (thread-per-env kernel keeps running totals there)
   unsigned int *counter;  // dynamic env counter (zeroed before the launch)
   uint32_t n_envs, env_first;  // envs [env_first, env_first + n_envs) of the handle
   uint32_t n_classes, n_configs;

@@ -21,13 +21,16 @@ pytestmark = pytest.mark.gpu
 B = None
 
 
-@pytest.fixture(scope="module", autouse=True)
-def _binding():
+# every test runs on both rollout kernels: 8-lane warp tiles and one thread per environment (mig_sim_set_tile)
+@pytest.fixture(scope="module", autouse=True, params=[8, 1], ids=["tile8", "thread"])
+def _binding(request):
     global B
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
     from paper_2606_25082_b200 import binding
     B = binding
+    B.DEFAULT_TILE = request.param
     yield
+    B.DEFAULT_TILE = 0
 
 
 def dev(a):
@@ -45,7 +48,17 @@ def _oracle_env(args):
     return e, r.recs, r.totals, (r.trace if want_trace else None), r.states, r.actions, r.rewards
 
 
+_ORACLE_CACHE = {}
+
+
 def oracle_many(wl_name, n_envs, envs, want_trace=False):
+    key = (wl_name, n_envs, tuple(int(e) for e in envs), want_trace)          # the oracle's answers serve both kernels
+    if key not in _ORACLE_CACHE:
+        _ORACLE_CACHE[key] = _oracle_many(wl_name, n_envs, envs, want_trace)
+    return _ORACLE_CACHE[key]
+
+
+def _oracle_many(wl_name, n_envs, envs, want_trace=False):
     args = [(wl_name, n_envs, int(e), want_trace, None) for e in envs]
     workers = min(len(args), os.cpu_count() or 1)
     if workers <= 1:
@@ -256,6 +269,33 @@ def test_env_base_sharding_is_placement_invariant():
         torch.cuda.synchronize()
         assert B.totals_to_numpy(tot).tobytes() == tot_ref[lo:hi].tobytes()
         sim.close()
+
+
+@pytest.mark.parametrize("tile", [1, 16, 32])
+def test_every_tile_width_gives_the_same_records(tile):
+    for name, n in (("C2", 200), ("C3", 200)):
+        wl = W.CONFIGS[name](n)
+        _, recs_ref, tot_ref, _ = gpu_rollout(wl, sim=B.MigSim(wl.params, n, wl.seed, tile=8))
+        sim = B.MigSim(wl.params, n, wl.seed, tile=tile)
+        assert sim.get_tile() == tile
+        _, recs, tot, _ = gpu_rollout(wl, sim=sim)
+        assert tot.tobytes() == tot_ref.tobytes() and recs.tobytes() == recs_ref.tobytes()
+        sim.close()
+
+
+def test_set_tile_between_kernel_families_needs_a_reset():
+    wl = W.config_c3(32)
+    sim = B.MigSim(wl.params, 32, wl.seed, tile=8)
+    sim.reset(0, dev(wl.algo), dev(wl.cfg0))
+    sim.set_tile(16)                                        # same saved-state layout: allowed mid-day
+    sim.step(dev(wl.cfg0))
+    sim.set_tile(1)                                         # another layout: the day must be restarted
+    with pytest.raises(B.MigError) as ei:
+        sim.step(dev(wl.cfg0))
+    assert ei.value.code == B.MIG_ESTATE
+    with pytest.raises(B.MigError):
+        sim.set_tile(4)
+    sim.close()
 
 
 # ------------------------------------------------------------------------------------------------ Q-network
