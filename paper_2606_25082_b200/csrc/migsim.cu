@@ -164,9 +164,9 @@ static int configure_tile(mig_sim *s, int tile) {
   const uint32_t cap4 = (s->p.cap + 3u) & ~3u, cap8 = (s->p.cap + 7u) & ~7u;
   uint32_t entries; size_t bytes; int threads;
   if (tile == 1) {
-    // 16 entries in shared memory per environment: 448 B per thread, 7 CTAs of 64 threads per SM = 448 resident
+    // 12 heap entries in shared memory per environment: 456 B per thread, 7 CTAs of 64 threads per SM = 448 resident
     // environments per SM (66 304 per B200: BASELINE C5's 65 536 run as ONE resident wave)
-    entries = cap4 < 16u ? cap4 : 16u; threads = kThreadCta;
+    entries = cap4 < 12u ? cap4 : 12u; threads = kThreadCta;
     bytes = thread_smem_bytes(entries, kThreadCta);
   } else {
     entries = cap8 < 64u ? cap8 : 64u; threads = kWarpsPerCta * 32;
@@ -219,8 +219,8 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
 #define ALLOC(ptr, bytes) if (cudaMalloc((void **)&(ptr), (bytes)) != cudaSuccess) { cudaGetLastError(); mig_sim_destroy(s); return fail(MIG_ENOMEM, "create: cudaMalloc of %zu bytes failed", (size_t)(bytes)); }
   ALLOC(s->d_tab, sizeof(DevTables));
   ALLOC(s->d_hdr, n * kHeaderWords * 4);
-  ALLOC(s->d_jobtab, n * p->cap * sizeof(uint4));
-  ALLOC(s->d_dbgtab, (size_t)p->cap * sizeof(uint4));
+  ALLOC(s->d_jobtab, n * (p->cap + kThreadTabExtra) * sizeof(uint4));
+  ALLOC(s->d_dbgtab, (size_t)(p->cap + kThreadTabExtra) * sizeof(uint4));
   ALLOC(s->d_dbghdr, kHeaderWords * 4);
   ALLOC(s->d_counter, sizeof(unsigned int));
   ALLOC(s->d_algo, n); ALLOC(s->d_cfg0, n);

@@ -8,29 +8,34 @@
 // environments to fill the machine (one resident wave = 148 SMs x 448 threads = 66 304 environments), which is what
 // the heavy batches (BASELINE C5: 65 536) have; small batches stay on the 8-lane tiles.
 //
-// Per-thread data lives in shared memory, interleaved by thread (word w of thread tid at base[w * NT + tid], so every
-// access of a warp is bank-conflict-free whatever index each lane uses):
-//   * slice table: table position and speed of the running job, up_at, per slot;
-//   * job table {skey, meta | rem, due} (16 B / job), first `smem_entries` entries, overflow in global memory;
-//   * the counters of the current record span and the reschedule's assignment scratch.
-// Scalars (time, hash, energy, generator, look-ahead arrival) live in registers.  The results are bit-identical to the
-// tile kernels and to the oracle (tests/test_gpu_parity.py); no code is shared with oracle/.
+// Data structures are chosen so that no step scans the queue (a lane with a 300-job queue would otherwise hold its 31
+// neighbours for the length of its scan):
+//   * RUNNING jobs live in the slice table: slot p holds {skey, meta, rem, due} and the speed of the job running there;
+//   * WAITING jobs live in a binary min-heap on (skey, id) of the same 16-byte records: the reschedule's "all jobs in
+//     priority order" is a merge of the <= 7 running jobs with successive heap minima, O(K log n);
+//     EDF keys never change and LLF / LALF keys change only while a job runs, so the heap order stays valid (a
+//     repartition, which changes every laxity, rebuilds it).
+// Per-thread data is in shared memory, interleaved by thread (row r of thread tid at base[r * NT + tid]: every access
+// of a warp is bank-conflict-free whatever index each lane uses); heap entries beyond `smem_entries` are in global
+// memory.  Scalars (time, hash, energy, generator, look-ahead arrival) live in registers.  The results are bit-identical
+// to the tile kernels and to the oracle (tests/test_gpu_parity.py); no code is shared with oracle/.
 #pragma once
 #include "sim_device.cuh"
 
 namespace migsim {
 
-constexpr int kThreadCta = 64;   // threads (= environments) per CTA of the thread-per-environment kernel
+constexpr int kThreadCta = 64;        // threads (= environments) per CTA of the thread-per-environment kernel
+constexpr int kThreadTabExtra = 8;    // job-table entries per env beyond cap: the slice table's save area
 
-// per-thread 32-bit words ahead of the job table
-enum { TW_POS = 0 /* 7: table index of the running job */, TW_V = 7 /* 7: its speed on the slice */, TW_UPAT = 14 /* 7 */,
-       TW_CNT = 21 /* C_COUNT = 10 */, TW_SCR = 31 /* 16: assignment scratch / class counters */, TW_FIXED = 48 };
-enum { SCR_ASG = 0 /* 7 */, SCR_R = 8 /* 7 */ };
+// per-thread rows of 8 bytes (uint2): slice records, pick staging, then the heap; rows of 4 bytes follow
+enum { T2_SLKM = 0 /* 7: {skey, meta} of the job running on slot p */, T2_SLRD = 7 /* 7: {rem, due}; a DOWN slice keeps up_at in .x */,
+       T2_STG = 14 /* 7: {meta | slot << 28 | moved << 31, rem} of pick k */, T2_HEAP = 21 };
+enum { T1_V = 0 /* 7: speed of the running job */, T1_STGDUE = 7 /* 7 */, T1_CNT = 14 /* C_COUNT = 10 */, T1_WORDS = 24 };
 
 // saved per-env header of this kernel (kHeaderWords words); the running totals H1_TOT / H1_CNT live here all the time
-enum { H1_UPAT = 0 /* 7 */, H1_T = 7, H1_PK, H1_NSYS, H1_HLO, H1_HHI, H1_GK, H1_GT_LO, H1_GT_HI, H1_GDONE, H1_NACC, H1_ISCRIPT,
-       H1_DROPS, H1_MASKS /* busy | down << 8 | fsz << 16 */, H1_TOT = 20 /* 6 */, H1_LOOKV = 26, H1_LOOKTICK, H1_LOOKCLS, H1_LOOKWORK,
-       H1_LOOKDUE, H1_LOOKID, H1_POS = 32 /* 7 */, H1_CNT = 48 /* 10 */ };
+enum { H1_T = 0, H1_PK, H1_NSYS, H1_NWAIT, H1_HLO, H1_HHI, H1_GK, H1_GT_LO, H1_GT_HI, H1_GDONE, H1_NACC, H1_ISCRIPT,
+       H1_DROPS, H1_MASKS /* busy | down << 8 */, H1_TOT = 20 /* 6 */, H1_LOOKV = 26, H1_LOOKTICK, H1_LOOKCLS, H1_LOOKWORK,
+       H1_LOOKDUE, H1_LOOKID, H1_CNT = 48 /* 10 */ };
 
 struct HotTablesT {              // per CTA, shared memory
   HotTables h;
@@ -41,7 +46,7 @@ struct HotTablesT {              // per CTA, shared memory
 };
 
 __host__ __device__ constexpr size_t thread_smem_bytes(uint32_t smem_entries, int nt) {
-  return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * (TW_FIXED + 4 * (size_t)smem_entries) * 4;
+  return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * ((T2_HEAP + 2 * (size_t)smem_entries) * 8 + T1_WORDS * 4);
 }
 
 template <int NT, bool TRACE>
@@ -49,91 +54,83 @@ struct EnvT {
   // ------------------------------------------------------------------ environment state
   const SimArgs &a;
   const HotTablesT &hot;
-  uint32_t *const fx;      // fixed words: fx[w * NT]
-  uint2 *const tb;         // job table: {skey, meta} at tb[(2 * i) * NT], {rem, due} at tb[(2 * i + 1) * NT]
-  uint4 *gtab;             // overflow part (and save area) in global memory, same entry index
+  uint2 *const r2;         // 8-byte rows: r2[row * NT]
+  uint32_t *const r1;      // 4-byte rows: r1[row * NT]
+  uint4 *gtab;             // heap overflow (entry index i >= S) and save area in global memory
   uint32_t *hdr;           // this env's saved header (running totals are kept there)
-  const uint32_t S;        // entries held in shared memory
+  const uint32_t S;        // heap entries held in shared memory
   uint32_t env_g;
-  int t, t_end, epoch, cfg, algo; uint32_t status, n_sys, cfg_sizes, cfg_rank, slice_mask;
+  int t, t_end, epoch, cfg, algo; uint32_t status, n_sys, n_wait, cfg_sizes, cfg_rank, slice_mask;
   uint32_t h_lo, h_hi;
   long long e_ep, tard_ep, busy_ep;
   int P, U, next_crit, next_done, next_up, repartitioned;
   uint32_t busy_mask, down_mask;
-  uint32_t fsz;            // entries [0, fsz) of the job table are sorted by (key, id) and precede every other entry
   uint32_t g_k, g_done, n_accepted; unsigned long long g_T;
   int look_valid, look_tick, look_work, look_due; uint32_t look_cls, look_id;
   uint32_t n_trace, i_script, n_events;
 
-  __device__ __forceinline__ EnvT(const SimArgs &a_, const HotTablesT &h_, uint32_t *fx_, uint2 *tb_)
-      : a(a_), hot(h_), fx(fx_), tb(tb_), S(a_.smem_entries) {}
+  __device__ __forceinline__ EnvT(const SimArgs &a_, const HotTablesT &h_, uint2 *r2_, uint32_t *r1_)
+      : a(a_), hot(h_), r2(r2_), r1(r1_), S(a_.smem_entries) {}
 
-  // ------------------------------------------------------------------ job table access
-  __device__ __forceinline__ uint2 ld_km(uint32_t i) const {
-    return i < S ? tb[(2 * i) * NT] : *reinterpret_cast<const uint2 *>(&gtab[i]);
-  }
-  __device__ __forceinline__ uint2 ld_rd(uint32_t i) const {
-    return i < S ? tb[(2 * i + 1) * NT] : *(reinterpret_cast<const uint2 *>(&gtab[i]) + 1);
-  }
-  __device__ __forceinline__ void st_entry(uint32_t i, uint2 km, uint2 rd) {
-    if (i < S) { tb[(2 * i) * NT] = km; tb[(2 * i + 1) * NT] = rd; } else gtab[i] = make_uint4(km.x, km.y, rd.x, rd.y);
-  }
-  // word w of entry i: 0 skey, 1 meta, 2 rem, 3 due
-  __device__ __forceinline__ uint32_t *entry_word(uint32_t i, int w) {
-    if (i < S) return reinterpret_cast<uint32_t *>(&tb[(2 * i + (w >> 1)) * NT]) + (w & 1);
-    return reinterpret_cast<uint32_t *>(&gtab[i]) + w;
-  }
-  __device__ __forceinline__ uint32_t &F(int w) { return fx[w * NT]; }
-  __device__ __forceinline__ void count(int c, uint32_t n) { fx[(TW_CNT + c) * NT] += n; }
+  __device__ __forceinline__ uint2 &R2(int row) { return r2[row * NT]; }
+  __device__ __forceinline__ uint32_t &R1(int row) { return r1[row * NT]; }
+  __device__ __forceinline__ void count(int c, uint32_t n) { r1[(T1_CNT + c) * NT] += n; }
 
-  // ------------------------------------------------------------------ sorted front of the job table
-  // The reschedule needs the K <= 7 first jobs in (key, id) order.  Instead of K scans over the whole table, entries
-  // [0, fsz), fsz <= kFront, are kept sorted and not larger than any other entry; the rest is unordered.  Arrivals are
-  // sifted in, completions shift the front up, and a single pass over the rest refills the front when it runs short
-  // (EDF keys never change; LLF / LALF keys of running jobs do, so those algorithms rebuild the front every time).
-  static constexpr uint32_t kFront = 8;
+  // ------------------------------------------------------------------ the waiting heap: entry i = {skey, meta}, {rem, due}
+  // One access path for both homes of an entry: a generic pointer to its {skey, meta} pair and the distance (in uint2)
+  // to its {rem, due} pair -- the next interleaved row in shared memory, the next 8 bytes in global memory.
+  __device__ __forceinline__ uint2 *ent(uint32_t i, uint32_t &step) const {
+    const bool in_smem = i < S;
+    step = in_smem ? (uint32_t)NT : 1u;
+    return in_smem ? &r2[(T2_HEAP + 2 * i) * NT] : reinterpret_cast<uint2 *>(gtab + i);
+  }
+  __device__ __forceinline__ uint2 ld_km(uint32_t i) const { uint32_t st; return *ent(i, st); }
+  __device__ __forceinline__ uint2 ld_rd(uint32_t i) const { uint32_t st; const uint2 *p = ent(i, st); return p[st]; }
+  __device__ __forceinline__ void ld_entry(uint32_t i, uint2 &km, uint2 &rd) const { uint32_t st; const uint2 *p = ent(i, st); km = p[0]; rd = p[st]; }
+  __device__ __forceinline__ void st_entry(uint32_t i, uint2 km, uint2 rd) { uint32_t st; uint2 *p = ent(i, st); p[0] = km; p[st] = rd; }
+  __device__ __forceinline__ void st_km(uint32_t i, uint2 km) { uint32_t st; *ent(i, st) = km; }
   static __device__ __forceinline__ bool before(uint2 x, uint2 y) {          // (key, id) order; ties -> lower id (reading #5)
     return (int)x.x < (int)y.x || (x.x == y.x && (x.y & kIdMask) < (y.y & kIdMask));
   }
-  // store an entry at `dst`; the slice running it follows
-  __device__ __forceinline__ void put(uint32_t dst, uint2 km, uint2 rd) {
-    st_entry(dst, km, rd);
-    const uint32_t sl = (km.y >> 28) & 7u;
-    if (sl) F(TW_POS + sl - 1) = dst;
-  }
-  // entries [0, len) are sorted and position len is free: place the entry so that [0, len] is sorted
-  __device__ __forceinline__ void sift(uint32_t len, uint2 km, uint2 rd) {
-    uint32_t j = len;
-    while (j > 0) {
-      const uint2 q = ld_km(j - 1);
-      if (!before(km, q)) break;
-      put(j, q, ld_rd(j - 1));
-      --j;
+  __device__ __forceinline__ void heap_push(uint2 km, uint2 rd) {
+    uint32_t i = n_wait;
+    n_wait = i + 1;
+    while (i > 0) {
+      const uint32_t par = (i - 1) >> 1;
+      uint2 qk, qr;
+      ld_entry(par, qk, qr);
+      if (!before(km, qk)) break;
+      st_entry(i, qk, qr);
+      i = par;
     }
-    put(j, km, rd);
+    st_entry(i, km, rd);
   }
-  __device__ __forceinline__ void insert_entry(uint2 km, uint2 rd) {
-    const bool in_front = (fsz == n_sys && fsz < kFront) || (fsz > 0 && before(km, ld_km(fsz - 1)));
-    if (!in_front) put(n_sys, km, rd);
-    else if (fsz == kFront) { put(n_sys, ld_km(kFront - 1), ld_rd(kFront - 1)); sift(kFront - 1, km, rd); }
-    else { if (fsz < n_sys) put(n_sys, ld_km(fsz), ld_rd(fsz)); sift(fsz, km, rd); fsz++; }
-    n_sys++;
-  }
-  // make [0, min(kFront, n_sys)) the smallest entries, sorted: grow the front over what follows it, then one pass over the rest
-  __device__ __forceinline__ void refill_front() {
-    const uint32_t tgt = min(kFront, n_sys);
-    while (fsz < tgt) { sift(fsz, ld_km(fsz), ld_rd(fsz)); fsz++; }
-    if (n_sys <= kFront) return;
-    uint2 worst = ld_km(kFront - 1);
-    for (uint32_t i = kFront; i < n_sys; ++i) {
-      const uint2 km = ld_km(i);
-      if (before(km, worst)) {
-        const uint2 rd = ld_rd(i);
-        put(i, worst, ld_rd(kFront - 1));
-        sift(kFront - 1, km, rd);
-        worst = ld_km(kFront - 1);
+  // place {km, rd} at the hole i of a heap of n entries, sifting it down
+  __device__ __forceinline__ void sift_down(uint32_t i, uint32_t n, uint2 km, uint2 rd) {
+    for (;;) {
+      uint32_t c = 2 * i + 1;
+      if (c >= n) break;
+      uint2 kc, rc;
+      ld_entry(c, kc, rc);
+      if (c + 1 < n) {
+        uint2 k2, r2_;
+        ld_entry(c + 1, k2, r2_);
+        if (before(k2, kc)) { kc = k2; rc = r2_; ++c; }
       }
+      if (!before(kc, km)) break;
+      st_entry(i, kc, rc);
+      i = c;
     }
+    st_entry(i, km, rd);
+  }
+  // removes entry 0.  (The last entry is read before n_wait is touched: ptxas 12.9 was seen to address it through the
+  // register of n_wait after that register had been reassigned.)
+  __device__ __forceinline__ void heap_pop() {
+    uint2 km, rd;
+    ld_entry(n_wait - 1, km, rd);
+    const uint32_t n = n_wait - 1;
+    if (n) sift_down(0, n, km, rd);
+    n_wait = n;
   }
 
   // ------------------------------------------------------------------ trace
@@ -217,29 +214,30 @@ struct EnvT {
     const uint32_t limit = a.job_limit ? min(a.job_limit, MIG_MAX_JOBS) : MIG_MAX_JOBS;
     if (n_accepted >= limit) return;
     const DevTables *tb_ = a.tab;
-    while (!g_done) {
-      const uint32_t k = g_k++;
-      const uint4 w = philox4x32_10(k, 0u, env_g, a.episode, a.k0, a.k1);    // stream 0: gap, accept, class, slack
+    uint4 w; unsigned long long tick; uint32_t k;
+    for (;;) {                                                                // thinning: draw candidates until one is accepted
+      if (g_done) return;
+      k = g_k++;
+      w = philox4x32_10(k, 0u, env_g, a.episode, a.k0, a.k1);                // stream 0: gap, accept, class, slack
       g_T += ((unsigned long long)neglog2_q24(w.x) * a.gap_scale) >> 24;
-      const unsigned long long tick = g_T >> 16;
-      if (tick >= (unsigned long long)a.day_s) { g_done = 1; break; }         // arrivals stop at the end of the day
-      if (w.y > __ldg(&tb_->thr[(uint32_t)tick / 60u])) continue;              // Lewis-Shedler thinning
-      uint32_t c = 0;
-      for (uint32_t i = 0; i + 1 < a.n_classes; ++i) c += (w.z > __ldg(&tb_->class_cum[i])) ? 1u : 0u;
-      const uint4 wd = philox4x32_10(k, 1u, env_g, a.episode, a.k0, a.k1);   // stream 1: duration
-      const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
-      const int q0 = __ldg(&tb_->dur7_q[c * 65 + qi]), q1 = __ldg(&tb_->dur7_q[c * 65 + qi + 1]);
-      const int dur7 = q0 + (int)(((long long)(q1 - q0) * (long long)f) >> 10);
-      const uint32_t slack = __ldg(&tb_->slack_lo[c]) + __umulhi(w.w, __ldg(&tb_->slack_span[c]));
-      unsigned long long rel = ((unsigned long long)(uint32_t)dur7 * slack) >> 10;
-      if (rel < 1) rel = 1;
-      look_tick = (int)tick; look_cls = c;
-      look_work = (int)((uint32_t)dur7 * hot.h.speed[c * 5 + 4].x);
-      look_due = (int)((long long)tick + (long long)rel);
-      look_id = n_accepted++;
-      look_valid = 1;
-      break;
+      tick = g_T >> 16;
+      if (tick >= (unsigned long long)a.day_s) { g_done = 1; return; }        // arrivals stop at the end of the day
+      if (w.y <= __ldg(&tb_->thr[(uint32_t)tick / 60u])) break;               // Lewis-Shedler thinning
     }
+    uint32_t c = 0;
+    for (uint32_t i = 0; i + 1 < a.n_classes; ++i) c += (w.z > __ldg(&tb_->class_cum[i])) ? 1u : 0u;
+    const uint4 wd = philox4x32_10(k, 1u, env_g, a.episode, a.k0, a.k1);     // stream 1: duration
+    const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
+    const int q0 = __ldg(&tb_->dur7_q[c * 65 + qi]), q1 = __ldg(&tb_->dur7_q[c * 65 + qi + 1]);
+    const int dur7 = q0 + (int)(((long long)(q1 - q0) * (long long)f) >> 10);
+    const uint32_t slack = __ldg(&tb_->slack_lo[c]) + __umulhi(w.w, __ldg(&tb_->slack_span[c]));
+    unsigned long long rel = ((unsigned long long)(uint32_t)dur7 * slack) >> 10;
+    if (rel < 1) rel = 1;
+    look_tick = (int)tick; look_cls = c;
+    look_work = (int)((uint32_t)dur7 * hot.h.speed[c * 5 + 4].x);
+    look_due = (int)((long long)tick + (long long)rel);
+    look_id = n_accepted++;
+    look_valid = 1;
   }
 
   // ------------------------------------------------------------------ reschedule
@@ -247,34 +245,43 @@ struct EnvT {
   __device__ __forceinline__ void compute_next_crit() {
     int best = MIG_INF;
     if (algo >= MIG_ALGO_LLF)
-      for (uint32_t i = 0; i < n_sys; ++i) {
+      for (uint32_t i = 0; i < n_wait; ++i) {
         const uint2 e = ld_km(i);
         const int tc = (int)e.x - a.theta;
-        const bool waiting = ((e.y >> 28) & 7u) == 0u;
-        if (waiting && ((e.y >> 24) & 15u) < a.crit_max && tc > t) best = min(best, tc);
+        if (((e.y >> 24) & 15u) < a.crit_max && tc > t) best = min(best, tc);
       }
     next_crit = best;
   }
 
-  // every job in the system is re-evaluated: the K = min(up slices, jobs) first jobs in (key, id) order pick a slice each
+  // Every job in the system is re-evaluated: in (key, id) order, while an up slice is left, each job picks a slice by its
+  // rule.  The order is produced by merging the running jobs (slice table) with successive minima of the waiting heap.
   __device__ __forceinline__ void reschedule() {
     if (algo >= MIG_ALGO_LLF)                       // the keys of running jobs move with their remaining work
       for (uint32_t m = busy_mask; m; m &= m - 1) {
-        const uint32_t pos = F(TW_POS + __ffs((int)m) - 1);
-        const uint2 km = ld_km(pos), rdv = ld_rd(pos);
-        *entry_word(pos, 0) = (uint32_t)skey_of((int)rdv.y, (int)rdv.x, (km.y >> 20) & 15u);
+        const int p = __ffs((int)m) - 1;
+        const uint2 km = R2(T2_SLKM + p), rdv = R2(T2_SLRD + p);
+        R2(T2_SLKM + p).x = (uint32_t)skey_of((int)rdv.y, (int)rdv.x, (km.y >> 20) & 15u);
       }
-    const uint32_t up = slice_mask & ~down_mask;    // every UP slice, occupied or not
-    uint32_t avail = up;
-    const int K = (int)min((uint32_t)__popc(up), n_sys);
-    if (algo >= MIG_ALGO_LLF) fsz = 0;
-    if (fsz < (uint32_t)K) refill_front();
-    uint32_t keep = 0;
-    for (int k = 0; k < K; ++k) {                   // entry k is the k-th job in (key, id) order
-      const uint32_t bmeta = ld_km((uint32_t)k).y;
-      const uint2 rdv = ld_rd((uint32_t)k);
+    uint32_t avail = slice_mask & ~down_mask;       // every UP slice, occupied or not
+    uint32_t rmask = busy_mask;                     // running jobs not picked yet
+    uint32_t keep = 0, nb = 0; int K = 0, nd = MIG_INF, u = 0, pd = 0;
+    while (avail != 0u) {
+      // --- next job in (key, id) order: the first of the unpicked running jobs, or the heap's minimum
+      uint2 bkm = make_uint2(0x7FFFFFFFu, 0xFFFFFFFFu); int bp = -1;
+      for (uint32_t m = rmask; m; m &= m - 1) {
+        const int p = __ffs((int)m) - 1;
+        const uint2 km = R2(T2_SLKM + p);
+        if (bp < 0 || before(km, bkm)) { bkm = km; bp = p; }
+      }
+      uint2 rdv;
+      if (n_wait) {
+        const uint2 wk = ld_km(0);
+        if (bp < 0 || before(wk, bkm)) { bkm = wk; bp = 7; }
+      }
+      if (bp < 0) break;                                                  // nobody left
+      if (bp == 7) { rdv = ld_rd(0); heap_pop(); } else { rdv = R2(T2_SLRD + bp); rmask &= ~(1u << bp); }
       const int rem = (int)rdv.x, slack = (int)rdv.y - t;
-      const uint32_t cls = (bmeta >> 20) & 15u;
+      const uint32_t cls = (bkm.y >> 20) & 15u;
       // --- slice choice: one composite key per rule, (r, rank) is unique per slice
       int fsb = MIG_INF, ssb = -1;
       for (uint32_t m = avail; m; m &= m - 1) {
@@ -288,11 +295,14 @@ struct EnvT {
       const int pick = use_ss ? ssb : fsb;
       const int rk = use_ss ? 7 - (pick & 7) : (pick & 7);
       const int s = (int)((hot.cfg_slot_of[cfg] >> (4 * rk)) & 7u);
+      const int g = size_at(s);
       avail &= ~(1u << s);
-      const bool moved = ((bmeta >> 28) & 7u) != (uint32_t)(s + 1);
+      nb |= 1u << s; nd = min(nd, t + (pick >> 3)); u += g; pd += hot.h.p_busy[g] - hot.h.p_idle[g];
+      const bool moved = bp != s;
       if (!moved) keep |= 1u << s;
-      F(TW_SCR + SCR_ASG + k) = (uint32_t)s | (moved ? 0x8000u : 0u);
-      F(TW_SCR + SCR_R + k) = (uint32_t)(pick >> 3);
+      R2(T2_STG + K) = make_uint2((bkm.y & 0x0FFFFFFFu) | ((uint32_t)s << 28) | (moved ? 0x80000000u : 0u), rdv.x);
+      R1(T1_STGDUE + K) = rdv.y;
+      ++K;
     }
     // --- diff against the previous assignment: PREEMPT ascending old slot, START in priority order
     const uint32_t pm = busy_mask & ~keep;
@@ -300,26 +310,23 @@ struct EnvT {
       count(C_PREEMPT, __popc(pm));
       for (uint32_t m = pm; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
-        const uint32_t pos = F(TW_POS + p);
-        const uint2 km = ld_km(pos), rdv = ld_rd(pos);
-        emit(MIG_EV_PREEMPT, p, (uint32_t)size_at(p), km.y & kIdMask, (int)rdv.x);
-        *entry_word(pos, 1) = km.y & ~(7u << 28);
+        emit(MIG_EV_PREEMPT, p, (uint32_t)size_at(p), R2(T2_SLKM + p).y & kIdMask, (int)R2(T2_SLRD + p).x);
+      }
+      for (uint32_t m = rmask; m; m &= m - 1) {                           // running jobs that lost their slice wait again
+        const int p = __ffs((int)m) - 1;
+        heap_push(R2(T2_SLKM + p), R2(T2_SLRD + p));
       }
     }
-    uint32_t nb = 0; int nd = MIG_INF, u = 0, pd = 0, n_start = 0;
+    int n_start = 0;
     for (int k = 0; k < K; ++k) {
-      const uint32_t w = F(TW_SCR + SCR_ASG + k);
-      const int r = (int)F(TW_SCR + SCR_R + k);
-      const int s = (int)(w & 7u);
-      const int g = size_at(s);
-      nb |= 1u << s; nd = min(nd, t + r); u += g; pd += hot.h.p_busy[g] - hot.h.p_idle[g];
-      if (w & 0x8000u) {
-        const uint32_t pos = (uint32_t)k;
-        const uint2 km = ld_km(pos), rdv = ld_rd(pos);
-        emit(MIG_EV_START, s, (uint32_t)g, km.y & kIdMask, (int)rdv.x);
-        *entry_word(pos, 1) = (km.y & ~(7u << 28)) | ((uint32_t)(s + 1) << 28);
-        F(TW_POS + s) = pos;
-        F(TW_V + s) = speed_of((km.y >> 20) & 15u, g).x;
+      const uint2 st = R2(T2_STG + k);
+      if (st.x & 0x80000000u) {
+        const int s = (int)((st.x >> 28) & 7u), g = size_at(s);
+        const uint32_t meta = st.x & 0x0FFFFFFFu, due = R1(T1_STGDUE + k);
+        emit(MIG_EV_START, s, (uint32_t)g, meta & kIdMask, (int)st.y);
+        R2(T2_SLKM + s) = make_uint2(due, meta);                          // EDF key = due; LLF / LALF keys are refreshed on use
+        R2(T2_SLRD + s) = make_uint2(st.y, due);
+        R1(T1_V + s) = speed_of((meta >> 20) & 15u, g).x;
         ++n_start;
       }
     }
@@ -327,18 +334,6 @@ struct EnvT {
     busy_mask = nb; next_done = nd;
     U = u; P = hot.cfg_pidle[cfg] + pd + hot.h.curve[u & 7];
     compute_next_crit();
-  }
-
-  // remove entry `pos`: the sorted front closes up, the hole is filled with the last entry
-  __device__ __forceinline__ void remove_entry(uint32_t pos) {
-    uint32_t hole = pos;
-    if (pos < fsz) {
-      for (uint32_t j = pos; j + 1 < fsz; ++j) put(j, ld_km(j + 1), ld_rd(j + 1));
-      hole = --fsz;
-    }
-    const uint32_t last = n_sys - 1;
-    if (hole != last) put(hole, ld_km(last), ld_rd(last));
-    n_sys = last;
   }
 
   // ------------------------------------------------------------------ event loop
@@ -355,30 +350,27 @@ struct EnvT {
     if (dt)
       for (uint32_t m = busy_mask; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
-        uint32_t *rp = entry_word(F(TW_POS + p), 2);
-        const int rem = (int)*rp - dt * (int)F(TW_V + p);
-        *rp = (uint32_t)rem;
+        const int rem = (int)R2(T2_SLRD + p).x - dt * (int)R1(T1_V + p);
+        R2(T2_SLRD + p).x = (uint32_t)rem;
         if (rem <= 0) done |= 1u << p;
       }
     bool happened = false;
     for (; done; done &= done - 1) {                                  // (i) completions, ascending slot
       const int p = __ffs((int)done) - 1;
-      const uint32_t pos = F(TW_POS + p);
-      const uint32_t id = ld_km(pos).y & kIdMask;
-      const int tard = max(t - (int)ld_rd(pos).y, 0);                 // l_j = max(c_j - d_j, 0)
-      emit(MIG_EV_COMPLETE, p, (uint32_t)size_at(p), id, tard);
+      const int tard = max(t - (int)R2(T2_SLRD + p).y, 0);            // l_j = max(c_j - d_j, 0)
+      emit(MIG_EV_COMPLETE, p, (uint32_t)size_at(p), R2(T2_SLKM + p).y & kIdMask, tard);
       tard_ep += tard;
       count(C_COMPLETED, 1u);
       if (tard > 0) count(C_TARDY, 1u);
       busy_mask &= ~(1u << p);
-      remove_entry(pos);
+      n_sys--;
       happened = true;
     }
     if (next_up == t) {                                               // (ii) slices coming up, ascending slot
       int nu = MIG_INF;
       for (uint32_t m = down_mask; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
-        const int up = (int)F(TW_UPAT + p);
+        const int up = (int)R2(T2_SLRD + p).x;
         if (up == t) { emit(MIG_EV_SLICE_UP, p, (uint32_t)size_at(p), MIG_NOJOB, 0); down_mask &= ~(1u << p); happened = true; }
         else nu = min(nu, up);
       }
@@ -390,9 +382,10 @@ struct EnvT {
       count(C_ARRIVED, 1u);
       if (drop) count(C_DROPPED, 1u);
       else {
-        insert_entry(make_uint2((uint32_t)skey_of(look_due, look_work, look_cls), look_id | (look_cls << 20)),
-                     make_uint2((uint32_t)look_work, (uint32_t)look_due));
-        if (n_sys > F(TW_CNT + C_SYSMAX)) F(TW_CNT + C_SYSMAX) = n_sys;
+        heap_push(make_uint2((uint32_t)skey_of(look_due, look_work, look_cls), look_id | (look_cls << 20)),
+                  make_uint2((uint32_t)look_work, (uint32_t)look_due));
+        n_sys++;
+        if (n_sys > R1(T1_CNT + C_SYSMAX)) R1(T1_CNT + C_SYSMAX) = n_sys;
       }
       emit(drop ? MIG_EV_DROP : MIG_EV_ARRIVE, 0xFF, look_cls, look_id, look_due);
       happened = true;
@@ -401,16 +394,16 @@ struct EnvT {
     if (next_crit == t) {                                             // (iv) critical laxity, ascending id
       int last_id = -1;
       for (;;) {
-        uint32_t bid = 0xFFFFFFFFu, bi = 0, bmeta = 0;
-        for (uint32_t i = 0; i < n_sys; ++i) {                        // jobs present before this tick's arrivals (reading #23)
+        uint32_t bid = 0xFFFFFFFFu, bi = 0; uint2 bkm = make_uint2(0u, 0u);
+        for (uint32_t i = 0; i < n_wait; ++i) {                       // jobs present before this tick's arrivals (reading #23)
           const uint2 e = ld_km(i);
           const uint32_t id = e.y & kIdMask;
-          const bool q = id < first_new && ((e.y >> 28) & 7u) == 0u && ((e.y >> 24) & 15u) < a.crit_max && (int)e.x - a.theta == t && (int)id > last_id;
-          if (q && id < bid) { bid = id; bi = i; bmeta = e.y; }
+          const bool q = id < first_new && ((e.y >> 24) & 15u) < a.crit_max && (int)e.x - a.theta == t && (int)id > last_id;
+          if (q && id < bid) { bid = id; bi = i; bkm = e; }
         }
         if (bid == 0xFFFFFFFFu) break;
-        const uint32_t cc = ((bmeta >> 24) & 15u) + 1u;
-        *entry_word(bi, 1) = (bmeta & ~(15u << 24)) | (cc << 24);
+        const uint32_t cc = ((bkm.y >> 24) & 15u) + 1u;
+        st_km(bi, make_uint2(bkm.x, (bkm.y & ~(15u << 24)) | (cc << 24)));
         emit(MIG_EV_CRIT, 0xFF, cc, bid, (int)ld_rd(bi).y);
         count(C_CRIT, 1u);
         last_id = (int)bid;
@@ -434,10 +427,11 @@ struct EnvT {
       count(C_PREEMPT, __popc(pm));
       for (uint32_t m = pm; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
-        const uint32_t pos = F(TW_POS + p);
-        const uint2 km = ld_km(pos);
-        emit(MIG_EV_PREEMPT, p, (uint32_t)size_at(p), km.y & kIdMask, (int)ld_rd(pos).x);
-        *entry_word(pos, 1) = km.y & ~(7u << 28);
+        emit(MIG_EV_PREEMPT, p, (uint32_t)size_at(p), R2(T2_SLKM + p).y & kIdMask, (int)R2(T2_SLRD + p).x);
+      }
+      for (uint32_t m = pm; m; m &= m - 1) {                  // (LLF / LALF keys are recomputed below)
+        const int p = __ffs((int)m) - 1;
+        heap_push(R2(T2_SLKM + p), R2(T2_SLRD + p));
       }
       busy_mask &= ~pm;
     }
@@ -447,20 +441,22 @@ struct EnvT {
     if (a.downtime_s > 0)
       for (uint32_t m = changed & slice_mask; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
-        F(TW_UPAT + p) = (uint32_t)(t + a.downtime_s);
+        R2(T2_SLRD + p).x = (uint32_t)(t + a.downtime_s);
         down_mask |= 1u << p;
       }
     int nu = MIG_INF;
-    for (uint32_t m = down_mask; m; m &= m - 1) nu = min(nu, (int)F(TW_UPAT + __ffs((int)m) - 1));
+    for (uint32_t m = down_mask; m; m &= m - 1) nu = min(nu, (int)R2(T2_SLRD + __ffs((int)m) - 1).x);
     next_up = nu;
     e_ep += a.repart_energy; repartitioned = 1;
     count(C_REPART, 1u);
     emit(MIG_EV_REPART, 0xFF, ((uint32_t)old << 8) | action, MIG_NOJOB, 0);
-    if (algo >= MIG_ALGO_LLF)                                 // laxity keys are measured against the configuration
-      for (uint32_t i = 0; i < n_sys; ++i) {
+    if (algo >= MIG_ALGO_LLF && n_wait) {                     // laxity keys are measured against the configuration: re-key, re-heap
+      for (uint32_t i = 0; i < n_wait; ++i) {
         const uint2 km = ld_km(i), rdv = ld_rd(i);
-        *entry_word(i, 0) = (uint32_t)skey_of((int)rdv.y, (int)rdv.x, (km.y >> 20) & 15u);
+        st_km(i, make_uint2((uint32_t)skey_of((int)rdv.y, (int)rdv.x, (km.y >> 20) & 15u), km.y));
       }
+      for (uint32_t i = n_wait / 2; i-- > 0;) sift_down(i, n_wait, ld_km(i), ld_rd(i));
+    }
     reschedule();
   }
 
@@ -468,7 +464,7 @@ struct EnvT {
   __device__ __forceinline__ void begin_span() {
     e_ep = 0; tard_ep = 0; busy_ep = 0; n_events = 0;
 #pragma unroll
-    for (int i = 0; i < C_COUNT; ++i) F(TW_CNT + i) = (i == C_SYSMAX) ? n_sys : 0u;
+    for (int i = 0; i < C_COUNT; ++i) R1(T1_CNT + i) = (i == C_SYSMAX) ? n_sys : 0u;
     repartitioned = 0;
   }
 
@@ -476,7 +472,7 @@ struct EnvT {
   __device__ __forceinline__ void close_record(mig_epoch_rec_t *r) {
     uint32_t c[C_COUNT];
 #pragma unroll
-    for (int i = 0; i < C_COUNT; ++i) c[i] = F(TW_CNT + i);
+    for (int i = 0; i < C_COUNT; ++i) c[i] = R1(T1_CNT + i);
     c[C_EVENTS] = n_events;
 #pragma unroll
     for (int i = 0; i < C_COUNT; ++i) hdr[H1_CNT + i] = (i == C_SYSMAX) ? max(hdr[H1_CNT + i], c[i]) : hdr[H1_CNT + i] + c[i];
@@ -504,19 +500,16 @@ struct EnvT {
   }
 
   // ------------------------------------------------------------------ state vector
+  // job j of the system, running ones first: j < 7 = slot j (valid if busy), j >= 7 = heap entry j - 7
+  __device__ __forceinline__ bool job_at(uint32_t j, uint2 &km, uint2 &rd) {
+    if (j < 7u) { if (!((busy_mask >> j) & 1u)) return false; km = R2(T2_SLKM + (int)j); rd = R2(T2_SLRD + (int)j); return true; }
+    km = ld_km(j - 7u); rd = ld_rd(j - 7u); return true;
+  }
   __device__ __forceinline__ void observe(float *out) {
     float4 *o4 = reinterpret_cast<float4 *>(out);
 #pragma unroll
-    for (int w = 0; w < 16; ++w) F(TW_SCR + w) = 0u;
-    for (uint32_t i = 0; i < n_sys; ++i) {                     // waiting jobs per class
-      const uint32_t m = ld_km(i).y;
-      if (((m >> 28) & 7u) == 0u) F(TW_SCR + (int)((m >> 20) & 15u)) += 1u;
-    }
-#pragma unroll
-    for (int w = 0; w < 4; ++w)
-      o4[w] = make_float4((float)F(TW_SCR + 4 * w), (float)F(TW_SCR + 4 * w + 1), (float)F(TW_SCR + 4 * w + 2), (float)F(TW_SCR + 4 * w + 3));
-#pragma unroll
-    for (int w = 4; w < 16; ++w) o4[w] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    for (int w = 0; w < 16; ++w) o4[w] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    for (uint32_t i = 0; i < n_wait; ++i) out[(ld_km(i).y >> 20) & 15u] += 1.0f;        // waiting jobs per class (small integers: exact)
     const int n_run = __popc(busy_mask);
     for (uint32_t m = slice_mask; m; m &= m - 1) {
       const int p = __ffs((int)m) - 1, g = size_at(p);
@@ -525,22 +518,23 @@ struct EnvT {
       out[23 + p] = (float)g * 0.125f;
     }
     out[30 + (t / 3600) % 24] = 1.0f;
-    out[54] = (float)(n_sys - (uint32_t)n_run) * (1.0f / 64.0f);
+    out[54] = (float)n_wait * (1.0f / 64.0f);
     out[55] = (float)n_run * 0.125f;
     out[62] = (float)hdr[H1_DROPS] * (1.0f / 64.0f);
     out[63] = 1.0f;
     int pk = (int)0x80000000; uint32_t pid = 0;
     for (int m = 0; m < 3 && (uint32_t)m < n_sys; ++m) {        // first m = 3 jobs in (due, id) order
-      int bk = MIG_INF; uint32_t bid = 0xFFFFFFFFu, bi = 0;
-      for (uint32_t i = 0; i < n_sys; ++i) {
-        const int due = (int)ld_rd(i).y; const uint32_t id = ld_km(i).y & kIdMask;
+      int bk = MIG_INF; uint32_t bid = 0xFFFFFFFFu; uint2 bkm = make_uint2(0u, 0u), brd = bkm;
+      for (uint32_t j = 0; j < 7u + n_wait; ++j) {
+        uint2 km, rdv;
+        if (!job_at(j, km, rdv)) continue;
+        const int due = (int)rdv.y; const uint32_t id = km.y & kIdMask;
         const bool beyond = due > pk || (due == pk && id > pid);
         const bool better = due < bk || (due == bk && id < bid);
-        if (beyond && better) { bk = due; bid = id; bi = i; }
+        if (beyond && better) { bk = due; bid = id; bkm = km; brd = rdv; }
       }
-      const uint2 km = ld_km(bi), rdv = ld_rd(bi);
-      const int d = max(-32768, min(32767, (int)rdv.y - t));
-      const int mean = min(rd_cfg((int)rdv.x, (km.y >> 20) & 15u, true), 32767);
+      const int d = max(-32768, min(32767, (int)brd.y - t));
+      const int mean = min(rd_cfg((int)brd.x, (bkm.y >> 20) & 15u, true), 32767);
       out[56 + m] = (float)d * (1.0f / 4096.0f);
       out[59 + m] = (float)mean * (1.0f / 4096.0f);
       pk = bk; pid = bid;
@@ -549,12 +543,12 @@ struct EnvT {
 
   // ------------------------------------------------------------------ init / load / save
   __device__ __forceinline__ void init(uint32_t env_local) {
-    algo = a.algo[env_local] & 3; t = 0; epoch = 0; status = 0; n_sys = 0;
+    algo = a.algo[env_local] & 3; t = 0; epoch = 0; status = 0; n_sys = 0; n_wait = 0;
     h_lo = 0x84222325u; h_hi = 0xcbf29ce4u;                   // FNV-1a-64 offset basis
     uint32_t c0 = a.cfg0[env_local];
     if (c0 >= a.n_configs) { c0 = 0; status |= MIG_ST_BAD_ACTION; }
     set_cfg_tables((int)c0);
-    busy_mask = 0; down_mask = 0; fsz = 0; next_done = MIG_INF; next_up = MIG_INF; next_crit = MIG_INF;
+    busy_mask = 0; down_mask = 0; next_done = MIG_INF; next_up = MIG_INF; next_crit = MIG_INF;
     g_k = 0; g_T = 0; g_done = 0; n_accepted = 0;
     look_valid = 0; look_tick = 0; look_work = 0; look_due = 0; look_cls = 0; look_id = 0;
     n_trace = 0; i_script = 0;
@@ -565,17 +559,17 @@ struct EnvT {
   }
 
   __device__ __forceinline__ void save() {
-#pragma unroll
-    for (int p = 0; p < kSlots; ++p) { hdr[H1_UPAT + p] = F(TW_UPAT + p); hdr[H1_POS + p] = F(TW_POS + p); }
     hdr[H1_T] = (uint32_t)t;
     hdr[H1_PK] = (uint32_t)epoch | ((uint32_t)cfg << 8) | ((uint32_t)algo << 16) | (status << 24);
-    hdr[H1_NSYS] = n_sys; hdr[H1_HLO] = h_lo; hdr[H1_HHI] = h_hi;
+    hdr[H1_NSYS] = n_sys; hdr[H1_NWAIT] = n_wait; hdr[H1_HLO] = h_lo; hdr[H1_HHI] = h_hi;
     hdr[H1_GK] = g_k; hdr[H1_GT_LO] = (uint32_t)g_T; hdr[H1_GT_HI] = (uint32_t)(g_T >> 32); hdr[H1_GDONE] = g_done;
-    hdr[H1_NACC] = n_accepted; hdr[H1_ISCRIPT] = i_script; hdr[H1_MASKS] = busy_mask | (down_mask << 8) | (fsz << 16);
+    hdr[H1_NACC] = n_accepted; hdr[H1_ISCRIPT] = i_script; hdr[H1_MASKS] = busy_mask | (down_mask << 8);
     hdr[H1_LOOKV] = (uint32_t)look_valid; hdr[H1_LOOKTICK] = (uint32_t)look_tick; hdr[H1_LOOKCLS] = look_cls;
     hdr[H1_LOOKWORK] = (uint32_t)look_work; hdr[H1_LOOKDUE] = (uint32_t)look_due; hdr[H1_LOOKID] = look_id;
-    const uint32_t ns = min(n_sys, S);
-    for (uint32_t i = 0; i < ns; ++i) { const uint2 km = tb[(2 * i) * NT], rdv = tb[(2 * i + 1) * NT]; gtab[i] = make_uint4(km.x, km.y, rdv.x, rdv.y); }
+#pragma unroll
+    for (int p = 0; p < kSlots; ++p) { const uint2 km = R2(T2_SLKM + p), rdv = R2(T2_SLRD + p); gtab[a.cap + p] = make_uint4(km.x, km.y, rdv.x, rdv.y); }
+    const uint32_t ns = min(n_wait, S);
+    for (uint32_t i = 0; i < ns; ++i) { const uint2 km = ld_km(i), rdv = ld_rd(i); gtab[i] = make_uint4(km.x, km.y, rdv.x, rdv.y); }
   }
 
   __device__ __forceinline__ void load() {
@@ -583,24 +577,24 @@ struct EnvT {
     const uint32_t pk = hdr[H1_PK];
     epoch = pk & 0xFF; algo = (pk >> 16) & 0xFF; status = pk >> 24;
     set_cfg_tables((int)((pk >> 8) & 0xFF));
-    n_sys = hdr[H1_NSYS]; h_lo = hdr[H1_HLO]; h_hi = hdr[H1_HHI];
+    n_sys = hdr[H1_NSYS]; n_wait = hdr[H1_NWAIT]; h_lo = hdr[H1_HLO]; h_hi = hdr[H1_HHI];
     g_k = hdr[H1_GK]; g_T = (unsigned long long)hdr[H1_GT_LO] | ((unsigned long long)hdr[H1_GT_HI] << 32); g_done = hdr[H1_GDONE];
     n_accepted = hdr[H1_NACC]; i_script = hdr[H1_ISCRIPT];
-    busy_mask = hdr[H1_MASKS] & 0x7Fu; down_mask = (hdr[H1_MASKS] >> 8) & 0x7Fu; fsz = hdr[H1_MASKS] >> 16;
+    busy_mask = hdr[H1_MASKS] & 0x7Fu; down_mask = (hdr[H1_MASKS] >> 8) & 0x7Fu;
     look_valid = (int)hdr[H1_LOOKV]; look_tick = (int)hdr[H1_LOOKTICK]; look_cls = hdr[H1_LOOKCLS];
     look_work = (int)hdr[H1_LOOKWORK]; look_due = (int)hdr[H1_LOOKDUE]; look_id = hdr[H1_LOOKID];
-    const uint32_t ns = min(n_sys, S);
-    for (uint32_t i = 0; i < ns; ++i) { const uint4 e = gtab[i]; tb[(2 * i) * NT] = make_uint2(e.x, e.y); tb[(2 * i + 1) * NT] = make_uint2(e.z, e.w); }
+    const uint32_t ns = min(n_wait, S);
+    for (uint32_t i = 0; i < ns; ++i) { const uint4 e = gtab[i]; st_entry(i, make_uint2(e.x, e.y), make_uint2(e.z, e.w)); }
     int nd = MIG_INF, nu = MIG_INF;
 #pragma unroll
     for (int p = 0; p < kSlots; ++p) {
-      F(TW_UPAT + p) = hdr[H1_UPAT + p]; F(TW_POS + p) = hdr[H1_POS + p];
-      if ((down_mask >> p) & 1u) nu = min(nu, (int)hdr[H1_UPAT + p]);
+      const uint4 e = gtab[a.cap + p];
+      R2(T2_SLKM + p) = make_uint2(e.x, e.y); R2(T2_SLRD + p) = make_uint2(e.z, e.w);
+      if ((down_mask >> p) & 1u) nu = min(nu, (int)e.z);
       if ((busy_mask >> p) & 1u) {                            // running job: t + ceil(rem / v) never drifts
-        const uint32_t pos = hdr[H1_POS + p];
-        const uint4 sp = speed_of((ld_km(pos).y >> 20) & 15u, size_at(p));
-        F(TW_V + p) = sp.x;
-        nd = min(nd, t + rd_magic((int)ld_rd(pos).x, sp));
+        const uint4 sp = speed_of((e.y >> 20) & 15u, size_at(p));
+        R1(T1_V + p) = sp.x;
+        nd = min(nd, t + rd_magic((int)e.z, sp));
       }
     }
     next_done = nd; next_up = nu;
@@ -636,7 +630,7 @@ struct EnvT {
       // ---- the span is over
       dE += e_ep; dT += tard_ep;
       if (!drain) {
-        hdr[H1_DROPS] = F(TW_CNT + C_DROPPED);
+        hdr[H1_DROPS] = R1(T1_CNT + C_DROPPED);
         close_record(a.recs ? a.recs + (size_t)(epoch - a.rec_k0) * a.rec_stride + out_i : nullptr);
         if (epoch == a.n_epochs - 1) {                        // 4. drain (reading #11): energy stops at the last completion
           drain = true; begin_span(); t_end = a.t_limit_s;
@@ -674,12 +668,13 @@ __global__ void __launch_bounds__(NT) sim_thread_kernel(const SimArgs a) {
   __syncthreads();
   const uint32_t li = blockIdx.x * NT + threadIdx.x;            // index inside this launch's env range
   if (li >= a.n_envs) return;
-  uint32_t *fx = reinterpret_cast<uint32_t *>(smem_raw + ((sizeof(HotTablesT) + 127) & ~(size_t)127)) + threadIdx.x;
-  uint2 *tbl = reinterpret_cast<uint2 *>(fx - threadIdx.x + TW_FIXED * NT) + threadIdx.x;
-  EnvT<NT, TRACE> e(a, hot, fx, tbl);
+  unsigned char *base = smem_raw + ((sizeof(HotTablesT) + 127) & ~(size_t)127);
+  uint2 *r2 = reinterpret_cast<uint2 *>(base) + threadIdx.x;
+  uint32_t *r1 = reinterpret_cast<uint32_t *>(base + (size_t)NT * (T2_HEAP + 2 * (size_t)a.smem_entries) * 8) + threadIdx.x;
+  EnvT<NT, TRACE> e(a, hot, r2, r1);
   const uint32_t env = a.env_first + li;
   e.env_g = a.env_base + env;
-  e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * a.cap;
+  e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * (a.cap + kThreadTabExtra);
   e.hdr = a.hdr_override ? a.hdr_override : a.hdr + (size_t)env * kHeaderWords;
   if (a.from_init) e.init(env); else e.load();
   e.run(li, env);
