@@ -29,12 +29,12 @@ constexpr int kThreadTabExtra = 8;    // job-table entries per env beyond cap: t
 
 // per-thread rows of 8 bytes (uint2): slice records, pick staging, then the heap; rows of 4 bytes follow
 enum { T2_SLKM = 0 /* 7: {skey, meta} of the job running on slot p */, T2_SLRD = 7 /* 7: {rem, due}; a DOWN slice keeps up_at in .x */,
-       T2_STG = 14 /* 7: {meta | slot << 28 | moved << 31, rem} of pick k */, T2_HEAP = 21 };
+       T2_STG = 14 /* 7: {meta | slot | moved << 3, rem} of pick k */, T2_HEAP = 21 };
 enum { T1_V = 0 /* 7: speed of the running job */, T1_STGDUE = 7 /* 7 */, T1_CNT = 14 /* C_COUNT = 10 */, T1_WORDS = 24 };
 
 // saved per-env header of this kernel (kHeaderWords words); the running totals H1_TOT / H1_CNT live here all the time
 enum { H1_T = 0, H1_PK, H1_NSYS, H1_NWAIT, H1_HLO, H1_HHI, H1_GK, H1_GT_LO, H1_GT_HI, H1_GDONE, H1_NACC, H1_ISCRIPT,
-       H1_DROPS, H1_MASKS /* busy | down << 8 */, H1_TOT = 20 /* 6 */, H1_LOOKV = 26, H1_LOOKTICK, H1_LOOKCLS, H1_LOOKWORK,
+       H1_DROPS, H1_MASKS /* busy | down << 8 */, H1_ORDER, H1_TOT = 20 /* 6 */, H1_LOOKV = 26, H1_LOOKTICK, H1_LOOKCLS, H1_LOOKWORK,
        H1_LOOKDUE, H1_LOOKID, H1_CNT = 48 /* 10 */ };
 
 struct HotTablesT {              // per CTA, shared memory
@@ -43,6 +43,7 @@ struct HotTablesT {              // per CTA, shared memory
   uint32_t cfg_slot_of[MIG_MAX_CONFIGS];  // nibble r: start slot of the slice of rank r
   int32_t cfg_pidle[MIG_MAX_CONFIGS];     // sum of p_idle over the slices of the configuration
   uint32_t logT[257];
+  uint32_t class_cum[MIG_MAX_CLASSES];    // padded with 0xFFFFFFFF beyond n_classes
 };
 
 __host__ __device__ constexpr size_t thread_smem_bytes(uint32_t smem_entries, int nt) {
@@ -65,6 +66,7 @@ struct EnvT {
   long long e_ep, tard_ep, busy_ep;
   int P, U, next_crit, next_done, next_up, repartitioned;
   uint32_t busy_mask, down_mask;
+  uint32_t run_order;      // nibble k: slot of the k-th running job in (key, id) order at the last reschedule, 0xF = end
   uint32_t g_k, g_done, n_accepted; unsigned long long g_T;
   int look_valid, look_tick, look_work, look_due; uint32_t look_cls, look_id;
   uint32_t n_trace, i_script, n_events;
@@ -89,36 +91,42 @@ struct EnvT {
   __device__ __forceinline__ void ld_entry(uint32_t i, uint2 &km, uint2 &rd) const { uint32_t st; const uint2 *p = ent(i, st); km = p[0]; rd = p[st]; }
   __device__ __forceinline__ void st_entry(uint32_t i, uint2 km, uint2 rd) { uint32_t st; uint2 *p = ent(i, st); p[0] = km; p[st] = rd; }
   __device__ __forceinline__ void st_km(uint32_t i, uint2 km) { uint32_t st; *ent(i, st) = km; }
-  static __device__ __forceinline__ bool before(uint2 x, uint2 y) {          // (key, id) order; ties -> lower id (reading #5)
-    return (int)x.x < (int)y.x || (x.x == y.x && (x.y & kIdMask) < (y.y & kIdMask));
-  }
+  // meta word of this kernel's records: id[12:32) | class[8:12) | crit_cnt[4:8) | 4 scratch bits.  With the id on top,
+  // (skey, meta) compared as ONE signed 64-bit number is the (key, id) order (ties -> lower id, reading #5; ids are unique).
+  static __device__ __forceinline__ uint32_t m_id(uint32_t m) { return m >> 12; }
+  static __device__ __forceinline__ uint32_t m_cls(uint32_t m) { return (m >> 8) & 15u; }
+  static __device__ __forceinline__ uint32_t m_crit(uint32_t m) { return (m >> 4) & 15u; }
+  static __device__ __forceinline__ long long ord(uint2 x) { return (long long)(((unsigned long long)x.x << 32) | x.y); }
+  static __device__ __forceinline__ bool before(uint2 x, uint2 y) { return ord(x) < ord(y); }
   __device__ __forceinline__ void heap_push(uint2 km, uint2 rd) {
     uint32_t i = n_wait;
     n_wait = i + 1;
+    const long long o = ord(km);
     while (i > 0) {
       const uint32_t par = (i - 1) >> 1;
-      uint2 qk, qr;
-      ld_entry(par, qk, qr);
-      if (!before(km, qk)) break;
-      st_entry(i, qk, qr);
+      uint32_t st; uint2 *q = ent(par, st);
+      const uint2 qk = q[0];
+      if (o >= ord(qk)) break;
+      st_entry(i, qk, q[st]);
       i = par;
     }
     st_entry(i, km, rd);
   }
   // place {km, rd} at the hole i of a heap of n entries, sifting it down
   __device__ __forceinline__ void sift_down(uint32_t i, uint32_t n, uint2 km, uint2 rd) {
+    const long long o = ord(km);
     for (;;) {
       uint32_t c = 2 * i + 1;
       if (c >= n) break;
-      uint2 kc, rc;
-      ld_entry(c, kc, rc);
+      uint32_t st; uint2 *q = ent(c, st);
+      uint2 kc = q[0];
       if (c + 1 < n) {
-        uint2 k2, r2_;
-        ld_entry(c + 1, k2, r2_);
-        if (before(k2, kc)) { kc = k2; rc = r2_; ++c; }
+        uint32_t st2; uint2 *q2 = ent(c + 1, st2);
+        const uint2 k2 = q2[0];
+        if (ord(k2) < ord(kc)) { kc = k2; q = q2; st = st2; ++c; }
       }
-      if (!before(kc, km)) break;
-      st_entry(i, kc, rc);
+      if (ord(kc) >= o) break;
+      st_entry(i, kc, q[st]);
       i = c;
     }
     st_entry(i, km, rd);
@@ -225,7 +233,8 @@ struct EnvT {
       if (w.y <= __ldg(&tb_->thr[(uint32_t)tick / 60u])) break;               // Lewis-Shedler thinning
     }
     uint32_t c = 0;
-    for (uint32_t i = 0; i + 1 < a.n_classes; ++i) c += (w.z > __ldg(&tb_->class_cum[i])) ? 1u : 0u;
+#pragma unroll
+    for (int i = 0; i < MIG_MAX_CLASSES - 1; ++i) c += (w.z > hot.class_cum[i]) ? 1u : 0u;    // first c with w.z <= cum[c]
     const uint4 wd = philox4x32_10(k, 1u, env_g, a.episode, a.k0, a.k1);     // stream 1: duration
     const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
     const int q0 = __ldg(&tb_->dur7_q[c * 65 + qi]), q1 = __ldg(&tb_->dur7_q[c * 65 + qi + 1]);
@@ -248,7 +257,7 @@ struct EnvT {
       for (uint32_t i = 0; i < n_wait; ++i) {
         const uint2 e = ld_km(i);
         const int tc = (int)e.x - a.theta;
-        if (((e.y >> 24) & 15u) < a.crit_max && tc > t) best = min(best, tc);
+        if (m_crit(e.y) < a.crit_max && tc > t) best = min(best, tc);
       }
     next_crit = best;
   }
@@ -260,18 +269,24 @@ struct EnvT {
       for (uint32_t m = busy_mask; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
         const uint2 km = R2(T2_SLKM + p), rdv = R2(T2_SLRD + p);
-        R2(T2_SLKM + p).x = (uint32_t)skey_of((int)rdv.y, (int)rdv.x, (km.y >> 20) & 15u);
+        R2(T2_SLKM + p).x = (uint32_t)skey_of((int)rdv.y, (int)rdv.x, m_cls(km.y));
       }
     uint32_t avail = slice_mask & ~down_mask;       // every UP slice, occupied or not
     uint32_t rmask = busy_mask;                     // running jobs not picked yet
     uint32_t keep = 0, nb = 0; int K = 0, nd = MIG_INF, u = 0, pd = 0;
+    uint32_t ro = run_order | 0xF0000000u, new_order = 0xFFFFFFFFu;
     while (avail != 0u) {
       // --- next job in (key, id) order: the first of the unpicked running jobs, or the heap's minimum
       uint2 bkm = make_uint2(0x7FFFFFFFu, 0xFFFFFFFFu); int bp = -1;
-      for (uint32_t m = rmask; m; m &= m - 1) {
-        const int p = __ffs((int)m) - 1;
-        const uint2 km = R2(T2_SLKM + p);
-        if (bp < 0 || before(km, bkm)) { bkm = km; bp = p; }
+      if (algo < MIG_ALGO_LLF) {                    // EDF keys are static: the running jobs are still in last time's order
+        while ((ro & 15u) != 15u && !((rmask >> (ro & 15u)) & 1u)) ro >>= 4;
+        if ((ro & 15u) != 15u) { bp = (int)(ro & 15u); bkm = R2(T2_SLKM + bp); }
+      } else {
+        for (uint32_t m = rmask; m; m &= m - 1) {
+          const int p = __ffs((int)m) - 1;
+          const uint2 km = R2(T2_SLKM + p);
+          if (bp < 0 || before(km, bkm)) { bkm = km; bp = p; }
+        }
       }
       uint2 rdv;
       if (n_wait) {
@@ -279,9 +294,9 @@ struct EnvT {
         if (bp < 0 || before(wk, bkm)) { bkm = wk; bp = 7; }
       }
       if (bp < 0) break;                                                  // nobody left
-      if (bp == 7) { rdv = ld_rd(0); heap_pop(); } else { rdv = R2(T2_SLRD + bp); rmask &= ~(1u << bp); }
+      if (bp == 7) { rdv = ld_rd(0); heap_pop(); } else { rdv = R2(T2_SLRD + bp); rmask &= ~(1u << bp); ro >>= 4; }
       const int rem = (int)rdv.x, slack = (int)rdv.y - t;
-      const uint32_t cls = (bkm.y >> 20) & 15u;
+      const uint32_t cls = m_cls(bkm.y);
       // --- slice choice: one composite key per rule, (r, rank) is unique per slice
       int fsb = MIG_INF, ssb = -1;
       for (uint32_t m = avail; m; m &= m - 1) {
@@ -300,8 +315,9 @@ struct EnvT {
       nb |= 1u << s; nd = min(nd, t + (pick >> 3)); u += g; pd += hot.h.p_busy[g] - hot.h.p_idle[g];
       const bool moved = bp != s;
       if (!moved) keep |= 1u << s;
-      R2(T2_STG + K) = make_uint2((bkm.y & 0x0FFFFFFFu) | ((uint32_t)s << 28) | (moved ? 0x80000000u : 0u), rdv.x);
+      R2(T2_STG + K) = make_uint2((bkm.y & ~15u) | (uint32_t)s | (moved ? 8u : 0u), rdv.x);
       R1(T1_STGDUE + K) = rdv.y;
+      new_order = (new_order & ~(15u << (4 * K))) | ((uint32_t)s << (4 * K));
       ++K;
     }
     // --- diff against the previous assignment: PREEMPT ascending old slot, START in priority order
@@ -310,7 +326,7 @@ struct EnvT {
       count(C_PREEMPT, __popc(pm));
       for (uint32_t m = pm; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
-        emit(MIG_EV_PREEMPT, p, (uint32_t)size_at(p), R2(T2_SLKM + p).y & kIdMask, (int)R2(T2_SLRD + p).x);
+        emit(MIG_EV_PREEMPT, p, (uint32_t)size_at(p), m_id(R2(T2_SLKM + p).y), (int)R2(T2_SLRD + p).x);
       }
       for (uint32_t m = rmask; m; m &= m - 1) {                           // running jobs that lost their slice wait again
         const int p = __ffs((int)m) - 1;
@@ -320,18 +336,18 @@ struct EnvT {
     int n_start = 0;
     for (int k = 0; k < K; ++k) {
       const uint2 st = R2(T2_STG + k);
-      if (st.x & 0x80000000u) {
-        const int s = (int)((st.x >> 28) & 7u), g = size_at(s);
-        const uint32_t meta = st.x & 0x0FFFFFFFu, due = R1(T1_STGDUE + k);
-        emit(MIG_EV_START, s, (uint32_t)g, meta & kIdMask, (int)st.y);
+      if (st.x & 8u) {
+        const int s = (int)(st.x & 7u), g = size_at(s);
+        const uint32_t meta = st.x & ~15u, due = R1(T1_STGDUE + k);
+        emit(MIG_EV_START, s, (uint32_t)g, m_id(meta), (int)st.y);
         R2(T2_SLKM + s) = make_uint2(due, meta);                          // EDF key = due; LLF / LALF keys are refreshed on use
         R2(T2_SLRD + s) = make_uint2(st.y, due);
-        R1(T1_V + s) = speed_of((meta >> 20) & 15u, g).x;
+        R1(T1_V + s) = speed_of(m_cls(meta), g).x;
         ++n_start;
       }
     }
     if (n_start) count(C_START, (uint32_t)n_start);
-    busy_mask = nb; next_done = nd;
+    busy_mask = nb; next_done = nd; run_order = new_order;
     U = u; P = hot.cfg_pidle[cfg] + pd + hot.h.curve[u & 7];
     compute_next_crit();
   }
@@ -358,7 +374,7 @@ struct EnvT {
     for (; done; done &= done - 1) {                                  // (i) completions, ascending slot
       const int p = __ffs((int)done) - 1;
       const int tard = max(t - (int)R2(T2_SLRD + p).y, 0);            // l_j = max(c_j - d_j, 0)
-      emit(MIG_EV_COMPLETE, p, (uint32_t)size_at(p), R2(T2_SLKM + p).y & kIdMask, tard);
+      emit(MIG_EV_COMPLETE, p, (uint32_t)size_at(p), m_id(R2(T2_SLKM + p).y), tard);
       tard_ep += tard;
       count(C_COMPLETED, 1u);
       if (tard > 0) count(C_TARDY, 1u);
@@ -382,7 +398,7 @@ struct EnvT {
       count(C_ARRIVED, 1u);
       if (drop) count(C_DROPPED, 1u);
       else {
-        heap_push(make_uint2((uint32_t)skey_of(look_due, look_work, look_cls), look_id | (look_cls << 20)),
+        heap_push(make_uint2((uint32_t)skey_of(look_due, look_work, look_cls), (look_id << 12) | (look_cls << 8)),
                   make_uint2((uint32_t)look_work, (uint32_t)look_due));
         n_sys++;
         if (n_sys > R1(T1_CNT + C_SYSMAX)) R1(T1_CNT + C_SYSMAX) = n_sys;
@@ -397,13 +413,13 @@ struct EnvT {
         uint32_t bid = 0xFFFFFFFFu, bi = 0; uint2 bkm = make_uint2(0u, 0u);
         for (uint32_t i = 0; i < n_wait; ++i) {                       // jobs present before this tick's arrivals (reading #23)
           const uint2 e = ld_km(i);
-          const uint32_t id = e.y & kIdMask;
-          const bool q = id < first_new && ((e.y >> 24) & 15u) < a.crit_max && (int)e.x - a.theta == t && (int)id > last_id;
+          const uint32_t id = m_id(e.y);
+          const bool q = id < first_new && m_crit(e.y) < a.crit_max && (int)e.x - a.theta == t && (int)id > last_id;
           if (q && id < bid) { bid = id; bi = i; bkm = e; }
         }
         if (bid == 0xFFFFFFFFu) break;
-        const uint32_t cc = ((bkm.y >> 24) & 15u) + 1u;
-        st_km(bi, make_uint2(bkm.x, (bkm.y & ~(15u << 24)) | (cc << 24)));
+        const uint32_t cc = m_crit(bkm.y) + 1u;
+        st_km(bi, make_uint2(bkm.x, (bkm.y & ~(15u << 4)) | (cc << 4)));
         emit(MIG_EV_CRIT, 0xFF, cc, bid, (int)ld_rd(bi).y);
         count(C_CRIT, 1u);
         last_id = (int)bid;
@@ -427,7 +443,7 @@ struct EnvT {
       count(C_PREEMPT, __popc(pm));
       for (uint32_t m = pm; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
-        emit(MIG_EV_PREEMPT, p, (uint32_t)size_at(p), R2(T2_SLKM + p).y & kIdMask, (int)R2(T2_SLRD + p).x);
+        emit(MIG_EV_PREEMPT, p, (uint32_t)size_at(p), m_id(R2(T2_SLKM + p).y), (int)R2(T2_SLRD + p).x);
       }
       for (uint32_t m = pm; m; m &= m - 1) {                  // (LLF / LALF keys are recomputed below)
         const int p = __ffs((int)m) - 1;
@@ -453,7 +469,7 @@ struct EnvT {
     if (algo >= MIG_ALGO_LLF && n_wait) {                     // laxity keys are measured against the configuration: re-key, re-heap
       for (uint32_t i = 0; i < n_wait; ++i) {
         const uint2 km = ld_km(i), rdv = ld_rd(i);
-        st_km(i, make_uint2((uint32_t)skey_of((int)rdv.y, (int)rdv.x, (km.y >> 20) & 15u), km.y));
+        st_km(i, make_uint2((uint32_t)skey_of((int)rdv.y, (int)rdv.x, m_cls(km.y)), km.y));
       }
       for (uint32_t i = n_wait / 2; i-- > 0;) sift_down(i, n_wait, ld_km(i), ld_rd(i));
     }
@@ -509,7 +525,7 @@ struct EnvT {
     float4 *o4 = reinterpret_cast<float4 *>(out);
 #pragma unroll
     for (int w = 0; w < 16; ++w) o4[w] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-    for (uint32_t i = 0; i < n_wait; ++i) out[(ld_km(i).y >> 20) & 15u] += 1.0f;        // waiting jobs per class (small integers: exact)
+    for (uint32_t i = 0; i < n_wait; ++i) out[m_cls(ld_km(i).y)] += 1.0f;        // waiting jobs per class (small integers: exact)
     const int n_run = __popc(busy_mask);
     for (uint32_t m = slice_mask; m; m &= m - 1) {
       const int p = __ffs((int)m) - 1, g = size_at(p);
@@ -528,13 +544,13 @@ struct EnvT {
       for (uint32_t j = 0; j < 7u + n_wait; ++j) {
         uint2 km, rdv;
         if (!job_at(j, km, rdv)) continue;
-        const int due = (int)rdv.y; const uint32_t id = km.y & kIdMask;
+        const int due = (int)rdv.y; const uint32_t id = m_id(km.y);
         const bool beyond = due > pk || (due == pk && id > pid);
         const bool better = due < bk || (due == bk && id < bid);
         if (beyond && better) { bk = due; bid = id; bkm = km; brd = rdv; }
       }
       const int d = max(-32768, min(32767, (int)brd.y - t));
-      const int mean = min(rd_cfg((int)brd.x, (bkm.y >> 20) & 15u, true), 32767);
+      const int mean = min(rd_cfg((int)brd.x, m_cls(bkm.y), true), 32767);
       out[56 + m] = (float)d * (1.0f / 4096.0f);
       out[59 + m] = (float)mean * (1.0f / 4096.0f);
       pk = bk; pid = bid;
@@ -548,7 +564,7 @@ struct EnvT {
     uint32_t c0 = a.cfg0[env_local];
     if (c0 >= a.n_configs) { c0 = 0; status |= MIG_ST_BAD_ACTION; }
     set_cfg_tables((int)c0);
-    busy_mask = 0; down_mask = 0; next_done = MIG_INF; next_up = MIG_INF; next_crit = MIG_INF;
+    busy_mask = 0; down_mask = 0; run_order = 0xFFFFFFFFu; next_done = MIG_INF; next_up = MIG_INF; next_crit = MIG_INF;
     g_k = 0; g_T = 0; g_done = 0; n_accepted = 0;
     look_valid = 0; look_tick = 0; look_work = 0; look_due = 0; look_cls = 0; look_id = 0;
     n_trace = 0; i_script = 0;
@@ -563,7 +579,7 @@ struct EnvT {
     hdr[H1_PK] = (uint32_t)epoch | ((uint32_t)cfg << 8) | ((uint32_t)algo << 16) | (status << 24);
     hdr[H1_NSYS] = n_sys; hdr[H1_NWAIT] = n_wait; hdr[H1_HLO] = h_lo; hdr[H1_HHI] = h_hi;
     hdr[H1_GK] = g_k; hdr[H1_GT_LO] = (uint32_t)g_T; hdr[H1_GT_HI] = (uint32_t)(g_T >> 32); hdr[H1_GDONE] = g_done;
-    hdr[H1_NACC] = n_accepted; hdr[H1_ISCRIPT] = i_script; hdr[H1_MASKS] = busy_mask | (down_mask << 8);
+    hdr[H1_NACC] = n_accepted; hdr[H1_ISCRIPT] = i_script; hdr[H1_MASKS] = busy_mask | (down_mask << 8); hdr[H1_ORDER] = run_order;
     hdr[H1_LOOKV] = (uint32_t)look_valid; hdr[H1_LOOKTICK] = (uint32_t)look_tick; hdr[H1_LOOKCLS] = look_cls;
     hdr[H1_LOOKWORK] = (uint32_t)look_work; hdr[H1_LOOKDUE] = (uint32_t)look_due; hdr[H1_LOOKID] = look_id;
 #pragma unroll
@@ -580,7 +596,7 @@ struct EnvT {
     n_sys = hdr[H1_NSYS]; n_wait = hdr[H1_NWAIT]; h_lo = hdr[H1_HLO]; h_hi = hdr[H1_HHI];
     g_k = hdr[H1_GK]; g_T = (unsigned long long)hdr[H1_GT_LO] | ((unsigned long long)hdr[H1_GT_HI] << 32); g_done = hdr[H1_GDONE];
     n_accepted = hdr[H1_NACC]; i_script = hdr[H1_ISCRIPT];
-    busy_mask = hdr[H1_MASKS] & 0x7Fu; down_mask = (hdr[H1_MASKS] >> 8) & 0x7Fu;
+    busy_mask = hdr[H1_MASKS] & 0x7Fu; down_mask = (hdr[H1_MASKS] >> 8) & 0x7Fu; run_order = hdr[H1_ORDER];
     look_valid = (int)hdr[H1_LOOKV]; look_tick = (int)hdr[H1_LOOKTICK]; look_cls = hdr[H1_LOOKCLS];
     look_work = (int)hdr[H1_LOOKWORK]; look_due = (int)hdr[H1_LOOKDUE]; look_id = hdr[H1_LOOKID];
     const uint32_t ns = min(n_wait, S);
@@ -592,7 +608,7 @@ struct EnvT {
       R2(T2_SLKM + p) = make_uint2(e.x, e.y); R2(T2_SLRD + p) = make_uint2(e.z, e.w);
       if ((down_mask >> p) & 1u) nu = min(nu, (int)e.z);
       if ((busy_mask >> p) & 1u) {                            // running job: t + ceil(rem / v) never drifts
-        const uint4 sp = speed_of((e.y >> 20) & 15u, size_at(p));
+        const uint4 sp = speed_of(m_cls(e.y), size_at(p));
         R1(T1_V + p) = sp.x;
         nd = min(nd, t + rd_magic((int)e.z, sp));
       }
@@ -664,6 +680,7 @@ __global__ void __launch_bounds__(NT) sim_thread_kernel(const SimArgs a) {
     }
     if (threadIdx.x < 8) { hot.h.curve[threadIdx.x] = tb->curve[threadIdx.x]; hot.h.p_idle[threadIdx.x] = tb->p_idle[threadIdx.x]; hot.h.p_busy[threadIdx.x] = tb->p_busy[threadIdx.x]; }
     for (int i = threadIdx.x; i < 257; i += NT) hot.logT[i] = tb->logT[i];
+    if (threadIdx.x < MIG_MAX_CLASSES) hot.class_cum[threadIdx.x] = threadIdx.x < a.n_classes ? tb->class_cum[threadIdx.x] : 0xFFFFFFFFu;
   }
   __syncthreads();
   const uint32_t li = blockIdx.x * NT + threadIdx.x;            // index inside this launch's env range
