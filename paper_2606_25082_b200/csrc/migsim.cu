@@ -41,6 +41,7 @@ struct mig_sim {
   int device = 0, n_sm = 0;
   int tile = 8;              // lanes per environment (8, 16 or 32): 32 / tile environments per warp
   uint32_t smem_entries = 0; size_t smem_bytes = 0; int grid_max = 0;
+  uint32_t ring_cap = 1;     // power of two >= cap
   DevTables *d_tab = nullptr;
   uint32_t *d_hdr = nullptr; uint4 *d_jobtab = nullptr; uint4 *d_dbgtab = nullptr; uint32_t *d_dbghdr = nullptr;
   unsigned int *d_counter = nullptr;
@@ -219,8 +220,9 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
 #define ALLOC(ptr, bytes) if (cudaMalloc((void **)&(ptr), (bytes)) != cudaSuccess) { cudaGetLastError(); mig_sim_destroy(s); return fail(MIG_ENOMEM, "create: cudaMalloc of %zu bytes failed", (size_t)(bytes)); }
   ALLOC(s->d_tab, sizeof(DevTables));
   ALLOC(s->d_hdr, n * kHeaderWords * 4);
-  ALLOC(s->d_jobtab, n * (p->cap + kThreadTabExtra) * sizeof(uint4));
-  ALLOC(s->d_dbgtab, (size_t)(p->cap + kThreadTabExtra) * sizeof(uint4));
+  s->ring_cap = 1; while (s->ring_cap < p->cap) s->ring_cap <<= 1;
+  ALLOC(s->d_jobtab, n * (s->ring_cap + kThreadTabExtra) * sizeof(uint4));
+  ALLOC(s->d_dbgtab, (size_t)(s->ring_cap + kThreadTabExtra) * sizeof(uint4));
   ALLOC(s->d_dbghdr, kHeaderWords * 4);
   ALLOC(s->d_counter, sizeof(unsigned int));
   ALLOC(s->d_algo, n); ALLOC(s->d_cfg0, n);
@@ -258,7 +260,7 @@ static void base_args(const mig_sim *s, SimArgs &a) {
   a.k0 = (uint32_t)s->seed; a.k1 = (uint32_t)(s->seed >> 32); a.episode = s->episode; a.env_base = p.env_base;
   a.gap_scale = p.gap_scale_q16;
   a.day_s = p.day_s; a.epoch_s = p.epoch_s; a.n_epochs = p.n_epochs; a.t_limit_s = p.t_limit_s;
-  a.cap = p.cap; a.job_limit = p.job_limit; a.smem_entries = s->smem_entries;
+  a.cap = p.cap; a.job_limit = p.job_limit; a.smem_entries = s->smem_entries; a.ring_cap = s->ring_cap;
   a.downtime_s = p.repart_downtime_s; a.repart_energy = p.repart_energy_mj;
   a.theta = p.crit_laxity_s; a.crit_max = p.crit_max;
   a.w_energy = p.w_energy; a.w_tardy = p.w_tardy;

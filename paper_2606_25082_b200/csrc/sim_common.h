@@ -43,6 +43,7 @@ struct SimArgs {
   uint64_t gap_scale;
   int32_t day_s, epoch_s, n_epochs, t_limit_s;
   uint32_t cap, job_limit, smem_entries;
+  uint32_t ring_cap;    // thread-per-env kernel: capacity of the global part of the waiting queue (power of two >= cap)
   int32_t downtime_s; int64_t repart_energy;
   int32_t theta; uint32_t crit_max;
   float w_energy, w_tardy;

@@ -25,7 +25,7 @@
 namespace migsim {
 
 constexpr int kThreadCta = 64;        // threads (= environments) per CTA of the thread-per-environment kernel
-constexpr int kThreadTabExtra = 8;    // job-table entries per env beyond cap: the slice table's save area
+constexpr int kThreadTabExtra = 32;   // job-table entries per env beyond the global ring: save area of the shared ring (16) and the slice table (7)
 
 // per-thread rows of 8 bytes (uint2): slice records, pick staging, then the heap; rows of 4 bytes follow
 enum { T2_SLKM = 0 /* 7: {skey, meta} of the job running on slot p */, T2_SLRD = 7 /* 7: {rem, due}; a DOWN slice keeps up_at in .x */,
@@ -34,7 +34,7 @@ enum { T1_V = 0 /* 7: speed of the running job */, T1_STGDUE = 7 /* 7 */, T1_CNT
 
 // saved per-env header of this kernel (kHeaderWords words); the running totals H1_TOT / H1_CNT live here all the time
 enum { H1_T = 0, H1_PK, H1_NSYS, H1_NWAIT, H1_HLO, H1_HHI, H1_GK, H1_GT_LO, H1_GT_HI, H1_GDONE, H1_NACC, H1_ISCRIPT,
-       H1_DROPS, H1_MASKS /* busy | down << 8 */, H1_ORDER, H1_TOT = 20 /* 6 */, H1_LOOKV = 26, H1_LOOKTICK, H1_LOOKCLS, H1_LOOKWORK,
+       H1_DROPS, H1_MASKS /* busy | down << 8 */, H1_ORDER, H1_QHEAD, H1_QNS, H1_GHEAD, H1_QNG, H1_TOT = 20 /* 6 */, H1_LOOKV = 26, H1_LOOKTICK, H1_LOOKCLS, H1_LOOKWORK,
        H1_LOOKDUE, H1_LOOKID, H1_CNT = 48 /* 10 */ };
 
 struct HotTablesT {              // per CTA, shared memory
@@ -66,6 +66,7 @@ struct EnvT {
   long long e_ep, tard_ep, busy_ep;
   int P, U, next_crit, next_done, next_up, repartitioned;
   uint32_t busy_mask, down_mask;
+  uint32_t q_head, q_ns, g_head, q_ng;   // the waiting queue (n_wait = q_ns + q_ng)
   uint32_t run_order;      // nibble k: slot of the k-th running job in (key, id) order at the last reschedule, 0xF = end
   uint32_t g_k, g_done, n_accepted; unsigned long long g_T;
   int look_valid, look_tick, look_work, look_due; uint32_t look_cls, look_id;
@@ -78,19 +79,30 @@ struct EnvT {
   __device__ __forceinline__ uint32_t &R1(int row) { return r1[row * NT]; }
   __device__ __forceinline__ void count(int c, uint32_t n) { r1[(T1_CNT + c) * NT] += n; }
 
-  // ------------------------------------------------------------------ the waiting heap: entry i = {skey, meta}, {rem, due}
-  // One access path for both homes of an entry: a generic pointer to its {skey, meta} pair and the distance (in uint2)
-  // to its {rem, due} pair -- the next interleaved row in shared memory, the next 8 bytes in global memory.
-  __device__ __forceinline__ uint2 *ent(uint32_t i, uint32_t &step) const {
-    const bool in_smem = i < S;
-    step = in_smem ? (uint32_t)NT : 1u;
-    return in_smem ? &r2[(T2_HEAP + 2 * i) * NT] : reinterpret_cast<uint2 *>(gtab + i);
+  // ------------------------------------------------------------------ the waiting queue
+  // A SORTED double-ended queue on (skey, id) in two levels: the q_ns smallest records in a shared-memory ring of S
+  // slots (head q_head), the other q_ng in a global-memory ring (head g_head, capacity a.ring_cap, a power of two);
+  // invariant: the global part is empty unless the shared ring is full.  Why not a heap: deadlines are arrival time
+  // plus a slack, so a new arrival almost always belongs at the TAIL and a re-queued (preempted) job at the FRONT;
+  // insertion costs as many moves as jobs are overtaken (typically 0-2), the minimum is popped in O(1), and -- what
+  // matters under SIMT -- every lane that inserts or pops in a given event runs the same few instructions, where heap
+  // sifts of queue-dependent depth serialised the lanes of a warp (profiles/r1_thread.md).
+  __device__ __forceinline__ uint32_t s_phys(uint32_t i) const { const uint32_t p = q_head + i; return p >= S ? p - S : p; }
+  __device__ __forceinline__ uint32_t g_phys(uint32_t i) const { return (g_head + i) & (a.ring_cap - 1u); }
+  __device__ __forceinline__ uint2 &SK(uint32_t phys) { return r2[(T2_HEAP + 2 * phys) * NT]; }
+  __device__ __forceinline__ uint2 &SR(uint32_t phys) { return r2[(T2_HEAP + 2 * phys + 1) * NT]; }
+  // rare paths (critical-laxity scans, state vector, save): record at LOGICAL index i in (key, id) order
+  __device__ __forceinline__ uint2 ld_km(uint32_t i) {
+    if (i < q_ns) return SK(s_phys(i));
+    const uint4 e = gtab[g_phys(i - q_ns)]; return make_uint2(e.x, e.y);
   }
-  __device__ __forceinline__ uint2 ld_km(uint32_t i) const { uint32_t st; return *ent(i, st); }
-  __device__ __forceinline__ uint2 ld_rd(uint32_t i) const { uint32_t st; const uint2 *p = ent(i, st); return p[st]; }
-  __device__ __forceinline__ void ld_entry(uint32_t i, uint2 &km, uint2 &rd) const { uint32_t st; const uint2 *p = ent(i, st); km = p[0]; rd = p[st]; }
-  __device__ __forceinline__ void st_entry(uint32_t i, uint2 km, uint2 rd) { uint32_t st; uint2 *p = ent(i, st); p[0] = km; p[st] = rd; }
-  __device__ __forceinline__ void st_km(uint32_t i, uint2 km) { uint32_t st; *ent(i, st) = km; }
+  __device__ __forceinline__ uint2 ld_rd(uint32_t i) {
+    if (i < q_ns) return SR(s_phys(i));
+    const uint4 e = gtab[g_phys(i - q_ns)]; return make_uint2(e.z, e.w);
+  }
+  __device__ __forceinline__ void st_km(uint32_t i, uint2 km) {
+    if (i < q_ns) SK(s_phys(i)) = km; else *reinterpret_cast<uint2 *>(&gtab[g_phys(i - q_ns)]) = km;
+  }
   // meta word of this kernel's records: id[12:32) | class[8:12) | crit_cnt[4:8) | 4 scratch bits.  With the id on top,
   // (skey, meta) compared as ONE signed 64-bit number is the (key, id) order (ties -> lower id, reading #5; ids are unique).
   static __device__ __forceinline__ uint32_t m_id(uint32_t m) { return m >> 12; }
@@ -98,47 +110,112 @@ struct EnvT {
   static __device__ __forceinline__ uint32_t m_crit(uint32_t m) { return (m >> 4) & 15u; }
   static __device__ __forceinline__ long long ord(uint2 x) { return (long long)(((unsigned long long)x.x << 32) | x.y); }
   static __device__ __forceinline__ bool before(uint2 x, uint2 y) { return ord(x) < ord(y); }
-  __device__ __forceinline__ void heap_push(uint2 km, uint2 rd) {
-    uint32_t i = n_wait;
-    n_wait = i + 1;
+  // shared ring, room available: place the record, moving the larger ones one slot towards the tail
+  __device__ __forceinline__ void s_insert_back(uint2 km, uint2 rd) {
     const long long o = ord(km);
+    uint32_t i = q_ns, p = s_phys(i);
     while (i > 0) {
-      const uint32_t par = (i - 1) >> 1;
-      uint32_t st; uint2 *q = ent(par, st);
-      const uint2 qk = q[0];
+      const uint32_t pp = p ? p - 1 : S - 1;
+      const uint2 qk = SK(pp);
       if (o >= ord(qk)) break;
-      st_entry(i, qk, q[st]);
-      i = par;
+      SK(p) = qk; SR(p) = SR(pp);
+      p = pp; --i;
     }
-    st_entry(i, km, rd);
+    SK(p) = km; SR(p) = rd;
+    q_ns++;
   }
-  // place {km, rd} at the hole i of a heap of n entries, sifting it down
-  __device__ __forceinline__ void sift_down(uint32_t i, uint32_t n, uint2 km, uint2 rd) {
+  // shared ring, room available: the head moves down one slot and the smaller records move towards it
+  __device__ __forceinline__ void s_insert_front(uint2 km, uint2 rd) {
     const long long o = ord(km);
-    for (;;) {
-      uint32_t c = 2 * i + 1;
-      if (c >= n) break;
-      uint32_t st; uint2 *q = ent(c, st);
-      uint2 kc = q[0];
-      if (c + 1 < n) {
-        uint32_t st2; uint2 *q2 = ent(c + 1, st2);
-        const uint2 k2 = q2[0];
-        if (ord(k2) < ord(kc)) { kc = k2; q = q2; st = st2; ++c; }
-      }
-      if (ord(kc) >= o) break;
-      st_entry(i, kc, q[st]);
-      i = c;
+    q_head = q_head ? q_head - 1 : S - 1;
+    uint32_t i = 0, p = q_head;
+    while (i < q_ns) {
+      const uint32_t pn = p + 1 == S ? 0 : p + 1;
+      const uint2 qk = SK(pn);
+      if (o <= ord(qk)) break;
+      SK(p) = qk; SR(p) = SR(pn);
+      p = pn; ++i;
     }
-    st_entry(i, km, rd);
+    SK(p) = km; SR(p) = rd;
+    q_ns++;
   }
-  // removes entry 0.  (The last entry is read before n_wait is touched: ptxas 12.9 was seen to address it through the
-  // register of n_wait after that register had been reassigned.)
-  __device__ __forceinline__ void heap_pop() {
-    uint2 km, rd;
-    ld_entry(n_wait - 1, km, rd);
-    const uint32_t n = n_wait - 1;
-    if (n) sift_down(0, n, km, rd);
-    n_wait = n;
+  __device__ __forceinline__ void g_insert_back(uint2 km, uint2 rd) {
+    const long long o = ord(km);
+    uint32_t i = q_ng;
+    while (i > 0) {
+      const uint4 e = gtab[g_phys(i - 1)];
+      if (o >= ord(make_uint2(e.x, e.y))) break;
+      gtab[g_phys(i)] = e;
+      --i;
+    }
+    gtab[g_phys(i)] = make_uint4(km.x, km.y, rd.x, rd.y);
+    q_ng++;
+  }
+  __device__ __forceinline__ void g_insert_front(uint2 km, uint2 rd) {
+    const long long o = ord(km);
+    g_head = (g_head - 1u) & (a.ring_cap - 1u);
+    uint32_t i = 0;
+    while (i < q_ng) {
+      const uint4 e = gtab[g_phys(i + 1)];
+      if (o <= ord(make_uint2(e.x, e.y))) break;
+      gtab[g_phys(i)] = e;
+      ++i;
+    }
+    gtab[g_phys(i)] = make_uint4(km.x, km.y, rd.x, rd.y);
+    q_ng++;
+  }
+  // the shared ring is full: its largest record becomes the smallest of the global part
+  __device__ __forceinline__ void spill_tail() {
+    const uint32_t p = s_phys(S - 1);
+    const uint2 km = SK(p), rd = SR(p);
+    g_head = (g_head - 1u) & (a.ring_cap - 1u);
+    gtab[g_head] = make_uint4(km.x, km.y, rd.x, rd.y);
+    q_ng++; q_ns--;
+  }
+  // a new arrival: searched from the tail
+  __device__ __forceinline__ void queue_push_back(uint2 km, uint2 rd) {
+    n_wait++;
+    if (q_ns == S) {
+      if (ord(km) >= ord(SK(s_phys(S - 1)))) { g_insert_back(km, rd); return; }
+      spill_tail();
+    }
+    s_insert_back(km, rd);
+  }
+  // a job that was running: searched from the front
+  __device__ __forceinline__ void queue_push_front(uint2 km, uint2 rd) {
+    n_wait++;
+    if (q_ns == S) {
+      if (ord(km) >= ord(SK(s_phys(S - 1)))) { g_insert_front(km, rd); return; }
+      spill_tail();
+    }
+    s_insert_front(km, rd);
+  }
+  __device__ __forceinline__ uint2 queue_top_km() { return SK(q_head); }
+  __device__ __forceinline__ uint2 queue_top_rd() { return SR(q_head); }
+  __device__ __forceinline__ void queue_pop() {                              // removes the first record
+    q_head = q_head + 1 == S ? 0 : q_head + 1;
+    q_ns--; n_wait--;
+    if (q_ng) {                                                              // the smallest of the global part moves up
+      const uint4 e = gtab[g_head];
+      g_head = (g_head + 1u) & (a.ring_cap - 1u);
+      q_ng--;
+      const uint32_t p = s_phys(q_ns);
+      SK(p) = make_uint2(e.x, e.y); SR(p) = make_uint2(e.z, e.w);
+      q_ns++;
+    }
+  }
+  // after every key changed (LLF / LALF at a repartition): insertion sort over the logical order
+  __device__ __forceinline__ void queue_resort() {
+    for (uint32_t i = 1; i < n_wait; ++i) {
+      const uint2 km = ld_km(i), rd = ld_rd(i);
+      const long long o = ord(km);
+      uint32_t j = i;
+      while (j > 0 && o < ord(ld_km(j - 1))) { st_rec(j, ld_km(j - 1), ld_rd(j - 1)); --j; }
+      if (j != i) st_rec(j, km, rd);
+    }
+  }
+  __device__ __forceinline__ void st_rec(uint32_t i, uint2 km, uint2 rd) {
+    if (i < q_ns) { const uint32_t p = s_phys(i); SK(p) = km; SR(p) = rd; } else gtab[g_phys(i - q_ns)] = make_uint4(km.x, km.y, rd.x, rd.y);
   }
 
   // ------------------------------------------------------------------ trace
@@ -290,11 +367,11 @@ struct EnvT {
       }
       uint2 rdv;
       if (n_wait) {
-        const uint2 wk = ld_km(0);
+        const uint2 wk = queue_top_km();
         if (bp < 0 || before(wk, bkm)) { bkm = wk; bp = 7; }
       }
       if (bp < 0) break;                                                  // nobody left
-      if (bp == 7) { rdv = ld_rd(0); heap_pop(); } else { rdv = R2(T2_SLRD + bp); rmask &= ~(1u << bp); ro >>= 4; }
+      if (bp == 7) { rdv = queue_top_rd(); queue_pop(); } else { rdv = R2(T2_SLRD + bp); rmask &= ~(1u << bp); ro >>= 4; }
       const int rem = (int)rdv.x, slack = (int)rdv.y - t;
       const uint32_t cls = m_cls(bkm.y);
       // --- slice choice: one composite key per rule, (r, rank) is unique per slice
@@ -330,7 +407,7 @@ struct EnvT {
       }
       for (uint32_t m = rmask; m; m &= m - 1) {                           // running jobs that lost their slice wait again
         const int p = __ffs((int)m) - 1;
-        heap_push(R2(T2_SLKM + p), R2(T2_SLRD + p));
+        queue_push_front(R2(T2_SLKM + p), R2(T2_SLRD + p));
       }
     }
     int n_start = 0;
@@ -398,8 +475,8 @@ struct EnvT {
       count(C_ARRIVED, 1u);
       if (drop) count(C_DROPPED, 1u);
       else {
-        heap_push(make_uint2((uint32_t)skey_of(look_due, look_work, look_cls), (look_id << 12) | (look_cls << 8)),
-                  make_uint2((uint32_t)look_work, (uint32_t)look_due));
+        queue_push_back(make_uint2((uint32_t)skey_of(look_due, look_work, look_cls), (look_id << 12) | (look_cls << 8)),
+                        make_uint2((uint32_t)look_work, (uint32_t)look_due));
         n_sys++;
         if (n_sys > R1(T1_CNT + C_SYSMAX)) R1(T1_CNT + C_SYSMAX) = n_sys;
       }
@@ -447,7 +524,7 @@ struct EnvT {
       }
       for (uint32_t m = pm; m; m &= m - 1) {                  // (LLF / LALF keys are recomputed below)
         const int p = __ffs((int)m) - 1;
-        heap_push(R2(T2_SLKM + p), R2(T2_SLRD + p));
+        queue_push_front(R2(T2_SLKM + p), R2(T2_SLRD + p));
       }
       busy_mask &= ~pm;
     }
@@ -466,12 +543,12 @@ struct EnvT {
     e_ep += a.repart_energy; repartitioned = 1;
     count(C_REPART, 1u);
     emit(MIG_EV_REPART, 0xFF, ((uint32_t)old << 8) | action, MIG_NOJOB, 0);
-    if (algo >= MIG_ALGO_LLF && n_wait) {                     // laxity keys are measured against the configuration: re-key, re-heap
+    if (algo >= MIG_ALGO_LLF && n_wait) {                     // laxity keys are measured against the configuration: re-key, re-sort
       for (uint32_t i = 0; i < n_wait; ++i) {
         const uint2 km = ld_km(i), rdv = ld_rd(i);
         st_km(i, make_uint2((uint32_t)skey_of((int)rdv.y, (int)rdv.x, m_cls(km.y)), km.y));
       }
-      for (uint32_t i = n_wait / 2; i-- > 0;) sift_down(i, n_wait, ld_km(i), ld_rd(i));
+      queue_resort();
     }
     reschedule();
   }
@@ -559,7 +636,7 @@ struct EnvT {
 
   // ------------------------------------------------------------------ init / load / save
   __device__ __forceinline__ void init(uint32_t env_local) {
-    algo = a.algo[env_local] & 3; t = 0; epoch = 0; status = 0; n_sys = 0; n_wait = 0;
+    algo = a.algo[env_local] & 3; t = 0; epoch = 0; status = 0; n_sys = 0; n_wait = 0; q_head = 0; q_ns = 0; g_head = 0; q_ng = 0;
     h_lo = 0x84222325u; h_hi = 0xcbf29ce4u;                   // FNV-1a-64 offset basis
     uint32_t c0 = a.cfg0[env_local];
     if (c0 >= a.n_configs) { c0 = 0; status |= MIG_ST_BAD_ACTION; }
@@ -578,14 +655,14 @@ struct EnvT {
     hdr[H1_T] = (uint32_t)t;
     hdr[H1_PK] = (uint32_t)epoch | ((uint32_t)cfg << 8) | ((uint32_t)algo << 16) | (status << 24);
     hdr[H1_NSYS] = n_sys; hdr[H1_NWAIT] = n_wait; hdr[H1_HLO] = h_lo; hdr[H1_HHI] = h_hi;
+    hdr[H1_QHEAD] = q_head; hdr[H1_QNS] = q_ns; hdr[H1_GHEAD] = g_head; hdr[H1_QNG] = q_ng;
     hdr[H1_GK] = g_k; hdr[H1_GT_LO] = (uint32_t)g_T; hdr[H1_GT_HI] = (uint32_t)(g_T >> 32); hdr[H1_GDONE] = g_done;
     hdr[H1_NACC] = n_accepted; hdr[H1_ISCRIPT] = i_script; hdr[H1_MASKS] = busy_mask | (down_mask << 8); hdr[H1_ORDER] = run_order;
     hdr[H1_LOOKV] = (uint32_t)look_valid; hdr[H1_LOOKTICK] = (uint32_t)look_tick; hdr[H1_LOOKCLS] = look_cls;
     hdr[H1_LOOKWORK] = (uint32_t)look_work; hdr[H1_LOOKDUE] = (uint32_t)look_due; hdr[H1_LOOKID] = look_id;
 #pragma unroll
-    for (int p = 0; p < kSlots; ++p) { const uint2 km = R2(T2_SLKM + p), rdv = R2(T2_SLRD + p); gtab[a.cap + p] = make_uint4(km.x, km.y, rdv.x, rdv.y); }
-    const uint32_t ns = min(n_wait, S);
-    for (uint32_t i = 0; i < ns; ++i) { const uint2 km = ld_km(i), rdv = ld_rd(i); gtab[i] = make_uint4(km.x, km.y, rdv.x, rdv.y); }
+    for (int p = 0; p < kSlots; ++p) { const uint2 km = R2(T2_SLKM + p), rdv = R2(T2_SLRD + p); gtab[a.ring_cap + 16 + p] = make_uint4(km.x, km.y, rdv.x, rdv.y); }
+    for (uint32_t p = 0; p < S; ++p) { const uint2 km = SK(p), rdv = SR(p); gtab[a.ring_cap + p] = make_uint4(km.x, km.y, rdv.x, rdv.y); }
   }
 
   __device__ __forceinline__ void load() {
@@ -594,17 +671,17 @@ struct EnvT {
     epoch = pk & 0xFF; algo = (pk >> 16) & 0xFF; status = pk >> 24;
     set_cfg_tables((int)((pk >> 8) & 0xFF));
     n_sys = hdr[H1_NSYS]; n_wait = hdr[H1_NWAIT]; h_lo = hdr[H1_HLO]; h_hi = hdr[H1_HHI];
+    q_head = hdr[H1_QHEAD]; q_ns = hdr[H1_QNS]; g_head = hdr[H1_GHEAD]; q_ng = hdr[H1_QNG];
     g_k = hdr[H1_GK]; g_T = (unsigned long long)hdr[H1_GT_LO] | ((unsigned long long)hdr[H1_GT_HI] << 32); g_done = hdr[H1_GDONE];
     n_accepted = hdr[H1_NACC]; i_script = hdr[H1_ISCRIPT];
     busy_mask = hdr[H1_MASKS] & 0x7Fu; down_mask = (hdr[H1_MASKS] >> 8) & 0x7Fu; run_order = hdr[H1_ORDER];
     look_valid = (int)hdr[H1_LOOKV]; look_tick = (int)hdr[H1_LOOKTICK]; look_cls = hdr[H1_LOOKCLS];
     look_work = (int)hdr[H1_LOOKWORK]; look_due = (int)hdr[H1_LOOKDUE]; look_id = hdr[H1_LOOKID];
-    const uint32_t ns = min(n_wait, S);
-    for (uint32_t i = 0; i < ns; ++i) { const uint4 e = gtab[i]; st_entry(i, make_uint2(e.x, e.y), make_uint2(e.z, e.w)); }
+    for (uint32_t p = 0; p < S; ++p) { const uint4 e = gtab[a.ring_cap + p]; SK(p) = make_uint2(e.x, e.y); SR(p) = make_uint2(e.z, e.w); }
     int nd = MIG_INF, nu = MIG_INF;
 #pragma unroll
     for (int p = 0; p < kSlots; ++p) {
-      const uint4 e = gtab[a.cap + p];
+      const uint4 e = gtab[a.ring_cap + 16 + p];
       R2(T2_SLKM + p) = make_uint2(e.x, e.y); R2(T2_SLRD + p) = make_uint2(e.z, e.w);
       if ((down_mask >> p) & 1u) nu = min(nu, (int)e.z);
       if ((busy_mask >> p) & 1u) {                            // running job: t + ceil(rem / v) never drifts
@@ -691,7 +768,7 @@ __global__ void __launch_bounds__(NT) sim_thread_kernel(const SimArgs a) {
   EnvT<NT, TRACE> e(a, hot, r2, r1);
   const uint32_t env = a.env_first + li;
   e.env_g = a.env_base + env;
-  e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * (a.cap + kThreadTabExtra);
+  e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * (a.ring_cap + kThreadTabExtra);
   e.hdr = a.hdr_override ? a.hdr_override : a.hdr + (size_t)env * kHeaderWords;
   if (a.from_init) e.init(env); else e.load();
   e.run(li, env);
