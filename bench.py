@@ -178,21 +178,26 @@ def run_ours(args):
         if ev_pair:
             ev_pair[1].record(stream)
 
-    for w in range(args.warmup):
+    def count_events():                                                                      # n_jobs + n_completed + n_dropped
+        t = totals.view(torch.int32).view(n_envs, 20)
+        return (t[:, 8].long() + t[:, 9].long() + t[:, 10].long()).sum()
+
+    job_events = torch.zeros(1, dtype=torch.int64, device="cuda")
+    for w in range(args.warmup):                                                             # the same work as a timed step
         one_step(w)
+        job_events += count_events()
         flush.fill_(w & 0xFF)
     barrier()
     # ---- timed region: resident inputs --------------------------------------------------------------------------
     sampler = ClockSampler(local) if rank == 0 else None
     pairs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    job_events = torch.zeros(1, dtype=torch.int64, device="cuda")
+    job_events.zero_()
     launches0 = sim.launch_count()
     e0.record(stream)
     for k in range(args.steps):
         one_step(args.warmup + k, pairs[k])
-        t = totals.view(torch.int32).view(n_envs, 20)
-        job_events += (t[:, 8].long() + t[:, 9].long() + t[:, 10].long()).sum()          # n_jobs + n_completed + n_dropped
+        job_events += count_events()
         flush.fill_(k & 0xFF)                                                              # L2 flush between iterations
     e1.record(stream)
     barrier()

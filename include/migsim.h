@@ -189,6 +189,13 @@ int mig_debug_div_magic(uint32_t v, uint32_t *m, uint32_t *sh);
  * workloads with hundreds of jobs in the system).  0 = default.  Results are identical for every value (tested); only
  * the launch geometry and the shared-memory footprint change.  Allowed between any two calls; MIG_EINVAL otherwise. */
 int mig_sim_set_tile(mig_sim_t *s, int lanes_per_env);
+/* Thread-per-environment kernel only: capacity (records of 16 bytes per environment) of the arrival lists that a launch
+ * fills, in one loop that all lanes of a warp run in step, before it simulates (the arrival process does
+ * not depend on the schedule).  Default: the expected number of accepted arrivals per day + 8 sigma, computed from
+ * accept_thr and gap_scale_q16 (C5: 8 784 records = 140 KB per environment).  0 = draw arrivals inside the event loop
+ * (no global buffer).  A list that fills up is refilled when it runs empty, so ANY capacity >= 1 gives the same results
+ * (tested); memory is allocated at the next launch (inline generation if it does not fit).  Allowed between any two calls. */
+int mig_sim_set_arrival_buffer(mig_sim_t *s, uint32_t entries_per_env);
 int mig_sim_get_tile(const mig_sim_t *s);
 /* Number of kernel launches issued through this handle so far (bench.py's gpu_launches). */
 uint64_t mig_sim_launch_count(const mig_sim_t *s);

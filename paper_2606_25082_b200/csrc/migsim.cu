@@ -42,6 +42,8 @@ struct mig_sim {
   int tile = 8;              // lanes per environment (8, 16 or 32): 32 / tile environments per warp
   uint32_t smem_entries = 0; size_t smem_bytes = 0; int grid_max = 0;
   uint32_t ring_cap = 1;     // power of two >= cap
+  uint4 *d_arr = nullptr; uint32_t arr_cap = 0;      // thread-per-env kernel: pre-generated arrival lists (allocated on first use)
+  uint32_t arr_want = 0;     // entries per env wanted (0 = generate inline)
   DevTables *d_tab = nullptr;
   uint32_t *d_hdr = nullptr; uint4 *d_jobtab = nullptr; uint4 *d_dbgtab = nullptr; uint32_t *d_dbghdr = nullptr;
   unsigned int *d_counter = nullptr;
@@ -196,6 +198,13 @@ extern "C" int mig_sim_set_tile(mig_sim_t *s, int lanes_per_env) {
 
 extern "C" int mig_sim_get_tile(const mig_sim_t *s) { return s ? s->tile : 0; }
 
+extern "C" int mig_sim_set_arrival_buffer(mig_sim_t *s, uint32_t entries_per_env) {
+  if (!s) return fail(MIG_EINVAL, "set_arrival_buffer: NULL handle");
+  if (entries_per_env > MIG_MAX_JOBS) return fail(MIG_EINVAL, "set_arrival_buffer: more than %u entries per environment", MIG_MAX_JOBS);
+  s->arr_want = entries_per_env;
+  return MIG_OK;
+}
+
 extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n_envs, uint64_t seed) {
   if (!out || !p) return fail(MIG_EINVAL, "create: NULL argument");
   *out = nullptr;
@@ -221,6 +230,15 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
   ALLOC(s->d_tab, sizeof(DevTables));
   ALLOC(s->d_hdr, n * kHeaderWords * 4);
   s->ring_cap = 1; while (s->ring_cap < p->cap) s->ring_cap <<= 1;
+  {                                                       // expected accepted arrivals per day (+ 8 sigma): capacity of an arrival list
+    const double lam_max = 65536.0 * 0.6931471805599453 / (double)p->gap_scale_q16;     // candidates per second
+    double acc = 0.0;
+    for (int m = 0; m < MIG_THR_BINS && m * 60 < p->day_s; ++m) acc += ((double)p->accept_thr[m] + 1.0) / 4294967296.0 * lam_max * (double)((p->day_s - m * 60) < 60 ? (p->day_s - m * 60) : 60);
+    double want = acc + 8.0 * sqrt(acc + 1.0) + 64.0;
+    if (p->job_limit && want > (double)p->job_limit + 1.0) want = (double)p->job_limit + 1.0;
+    if (want > (double)MIG_MAX_JOBS) want = (double)MIG_MAX_JOBS;
+    s->arr_want = ((uint32_t)want + 7u) & ~7u;
+  }
   ALLOC(s->d_jobtab, n * (s->ring_cap + kThreadTabExtra) * sizeof(uint4));
   ALLOC(s->d_dbgtab, (size_t)(s->ring_cap + kThreadTabExtra) * sizeof(uint4));
   ALLOC(s->d_dbghdr, kHeaderWords * 4);
@@ -242,7 +260,7 @@ extern "C" int mig_sim_destroy(mig_sim_t *s) {
   cudaDeviceSynchronize();
   cudaFree(s->d_tab); cudaFree(s->d_hdr); cudaFree(s->d_jobtab); cudaFree(s->d_dbgtab); cudaFree(s->d_dbghdr); cudaFree(s->d_counter);
   cudaFree(s->d_algo); cudaFree(s->d_cfg0); cudaFree(s->d_state); cudaFree(s->d_action); cudaFree(s->d_table);
-  cudaFree(s->d_recs); cudaFree(s->d_totals); cudaFree(s->d_script);
+  cudaFree(s->d_recs); cudaFree(s->d_totals); cudaFree(s->d_script); cudaFree(s->d_arr);
   cudaGetLastError();
   delete s;
   return MIG_OK;
@@ -272,8 +290,19 @@ static void base_args(const mig_sim *s, SimArgs &a) {
 template <bool TRACE>
 static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
   if (s->tile == 1) {                                     // one thread per environment, one CTA per 64 environments
-    const dim3 grid((a.n_envs + kThreadCta - 1) / kThreadCta), block(kThreadCta);
-    sim_thread_kernel<kThreadCta, TRACE><<<grid, block, s->smem_bytes, st>>>(a);
+    if (s->arr_want && a.n_steps > 0 && !a.script) {      // arrival lists: allocated on first use; inline generation if they do not fit
+      if (s->d_arr && s->arr_cap != s->arr_want) { CU(cudaStreamSynchronize(st)); cudaFree(s->d_arr); s->d_arr = nullptr; s->arr_cap = 0; }
+      if (!s->d_arr) {
+        size_t free_b = 0, total_b = 0;
+        const size_t need = (size_t)s->n_envs * s->arr_want * sizeof(uint4);
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need <= free_b / 2 && cudaMalloc((void **)&s->d_arr, need) == cudaSuccess) s->arr_cap = s->arr_want;
+        else { cudaGetLastError(); s->d_arr = nullptr; s->arr_cap = 0; s->arr_want = 0; }
+      }
+    }
+    SimArgs b = a;
+    b.arr = s->arr_want ? s->d_arr : nullptr; b.arr_cap = s->arr_cap;
+    const dim3 grid((b.n_envs + kThreadCta - 1) / kThreadCta), block(kThreadCta);
+    sim_thread_kernel<kThreadCta, TRACE><<<grid, block, s->smem_bytes, st>>>(b);
     CU(cudaGetLastError());
     s->launches++;
     return MIG_OK;

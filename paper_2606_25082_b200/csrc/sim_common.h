@@ -56,6 +56,7 @@ struct SimArgs {
   const uint8_t *table;                              // [n_envs][n_epochs][4]
   const uint8_t *actions; uint32_t act_stride_env, act_stride_k;   // action = actions[env * se + (k - k_first) * sk]
   const mig_job_t *script; uint32_t n_script;
+  uint4 *arr; uint32_t arr_cap;                      // thread-per-env kernel: pre-generated arrival lists [n_envs][arr_cap] {tick, class, work, due}, or NULL
   // outputs (NULL = skip)
   float *state_out; float *reward_out; int64_t *energy_out; int64_t *tard_out;
   mig_epoch_rec_t *recs; int32_t rec_k0; mig_epoch_rec_t *drain_rec;   // record of epoch k -> recs[(k - rec_k0) * n_envs_total + env]

@@ -71,6 +71,8 @@ struct EnvT {
   uint32_t g_k, g_done, n_accepted; unsigned long long g_T;
   int look_valid, look_tick, look_work, look_due; uint32_t look_cls, look_id;
   uint32_t n_trace, i_script, n_events;
+  uint4 *arr;              // this env's arrival list (NULL: generate inline)
+  uint32_t a_head, a_count, a_id0, a_more; int a_horizon;
 
   __device__ __forceinline__ EnvT(const SimArgs &a_, const HotTablesT &h_, uint2 *r2_, uint32_t *r1_)
       : a(a_), hot(h_), r2(r2_), r1(r1_), S(a_.smem_entries) {}
@@ -284,7 +286,54 @@ struct EnvT {
     return ((uint32_t)(1 + lz) << 24) - L;
   }
 
-  // advance the look-ahead to the next accepted arrival (or none): sequential thinning, one candidate per trip
+  // class, work and due date of the accepted candidate k (R5): {tick, class, work, due}
+  __device__ __forceinline__ uint4 job_attributes(uint32_t k, uint4 w, uint32_t tick) const {
+    const DevTables *tb_ = a.tab;
+    uint32_t c = 0;
+#pragma unroll
+    for (int i = 0; i < MIG_MAX_CLASSES - 1; ++i) c += (w.z > hot.class_cum[i]) ? 1u : 0u;    // first c with w.z <= cum[c]
+    const uint4 wd = philox4x32_10(k, 1u, env_g, a.episode, a.k0, a.k1);     // stream 1: duration
+    const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
+    const int q0 = __ldg(&tb_->dur7_q[c * 65 + qi]), q1 = __ldg(&tb_->dur7_q[c * 65 + qi + 1]);
+    const int dur7 = q0 + (int)(((long long)(q1 - q0) * (long long)f) >> 10);
+    const uint32_t slack = __ldg(&tb_->slack_lo[c]) + __umulhi(w.w, __ldg(&tb_->slack_span[c]));
+    unsigned long long rel = ((unsigned long long)(uint32_t)dur7 * slack) >> 10;
+    if (rel < 1) rel = 1;
+    return make_uint4(tick, c, (uint32_t)dur7 * hot.h.speed[c * 5 + 4].x, (uint32_t)((long long)tick + (long long)rel));
+  }
+  __device__ __forceinline__ uint32_t job_limit() const { return a.job_limit ? min(a.job_limit, MIG_MAX_JOBS) : MIG_MAX_JOBS; }
+
+  // Pre-generation (a.arr != NULL): at the start of a launch every lane draws ALL candidates up to the launch's horizon,
+  // one candidate per trip of ONE loop -- every lane of the warp executes the same instructions (the thinning loop of
+  // the inline generator below runs a lane-dependent number of trips per arrival) -- and appends the accepted ones to
+  // its arrival list in global memory, from which the event loop then reads its look-ahead.  A candidate beyond the
+  // horizon or the list's capacity is NOT committed (g_k, g_T stay before it), so generation resumes exactly there.
+  __device__ __forceinline__ void fill_arrivals() {
+    a_head = 0; a_count = 0; a_more = 0;
+    a_id0 = n_accepted;
+    if (look_valid) {                               // a look-ahead carried over from a launch of the inline generator
+      arr[0] = make_uint4((uint32_t)look_tick, look_cls, (uint32_t)look_work, (uint32_t)look_due);
+      a_id0 = look_id; a_count = 1; look_valid = 0;
+    }
+    const uint32_t limit = job_limit();
+    const DevTables *tb_ = a.tab;
+    while (!g_done && n_accepted < limit) {
+      const uint32_t k = g_k;
+      const uint4 w = philox4x32_10(k, 0u, env_g, a.episode, a.k0, a.k1);    // stream 0: gap, accept, class, slack
+      const unsigned long long T = g_T + (((unsigned long long)neglog2_q24(w.x) * a.gap_scale) >> 24);
+      const unsigned long long tick = T >> 16;
+      if (tick >= (unsigned long long)a.day_s) { g_done = 1; break; }         // arrivals stop at the end of the day
+      if (tick > (unsigned long long)a_horizon) break;
+      if (a_count == a.arr_cap) { a_more = 1; break; }
+      g_k = k + 1; g_T = T;
+      if (w.y <= __ldg(&tb_->thr[(uint32_t)tick / 60u])) {                    // Lewis-Shedler thinning
+        arr[a_count++] = job_attributes(k, w, (uint32_t)tick);
+        n_accepted++;
+      }
+    }
+  }
+
+  // advance the look-ahead to the next accepted arrival (or none)
   __device__ __forceinline__ void gen_next() {
     look_valid = 0;
     if (a.script) {                                                           // scripted arrivals (tests), kernel-uniform branch
@@ -296,11 +345,22 @@ struct EnvT {
       }
       return;
     }
-    const uint32_t limit = a.job_limit ? min(a.job_limit, MIG_MAX_JOBS) : MIG_MAX_JOBS;
-    if (n_accepted >= limit) return;
+    if (arr) {                                                                // pre-generated list (kernel-uniform branch)
+      if (a_head == a_count) {
+        if (!a_more) return;
+        fill_arrivals();                                                      // the list was full: next stretch (rare)
+        if (a_count == 0) return;
+      }
+      const uint4 e = arr[a_head];
+      look_tick = (int)e.x; look_cls = e.y; look_work = (int)e.z; look_due = (int)e.w;
+      look_id = a_id0 + a_head++;
+      look_valid = 1;
+      return;
+    }
+    if (n_accepted >= job_limit()) return;
     const DevTables *tb_ = a.tab;
     uint4 w; unsigned long long tick; uint32_t k;
-    for (;;) {                                                                // thinning: draw candidates until one is accepted
+    for (;;) {                                                                // inline: draw candidates until one is accepted
       if (g_done) return;
       k = g_k++;
       w = philox4x32_10(k, 0u, env_g, a.episode, a.k0, a.k1);                // stream 0: gap, accept, class, slack
@@ -309,19 +369,8 @@ struct EnvT {
       if (tick >= (unsigned long long)a.day_s) { g_done = 1; return; }        // arrivals stop at the end of the day
       if (w.y <= __ldg(&tb_->thr[(uint32_t)tick / 60u])) break;               // Lewis-Shedler thinning
     }
-    uint32_t c = 0;
-#pragma unroll
-    for (int i = 0; i < MIG_MAX_CLASSES - 1; ++i) c += (w.z > hot.class_cum[i]) ? 1u : 0u;    // first c with w.z <= cum[c]
-    const uint4 wd = philox4x32_10(k, 1u, env_g, a.episode, a.k0, a.k1);     // stream 1: duration
-    const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
-    const int q0 = __ldg(&tb_->dur7_q[c * 65 + qi]), q1 = __ldg(&tb_->dur7_q[c * 65 + qi + 1]);
-    const int dur7 = q0 + (int)(((long long)(q1 - q0) * (long long)f) >> 10);
-    const uint32_t slack = __ldg(&tb_->slack_lo[c]) + __umulhi(w.w, __ldg(&tb_->slack_span[c]));
-    unsigned long long rel = ((unsigned long long)(uint32_t)dur7 * slack) >> 10;
-    if (rel < 1) rel = 1;
-    look_tick = (int)tick; look_cls = c;
-    look_work = (int)((uint32_t)dur7 * hot.h.speed[c * 5 + 4].x);
-    look_due = (int)((long long)tick + (long long)rel);
+    const uint4 e = job_attributes(k, w, (uint32_t)tick);
+    look_tick = (int)e.x; look_cls = e.y; look_work = (int)e.z; look_due = (int)e.w;
     look_id = n_accepted++;
     look_valid = 1;
   }
@@ -648,7 +697,6 @@ struct EnvT {
     for (int w = H1_DROPS; w < kHeaderWords; ++w) hdr[w] = 0u;      // running totals, drops
     begin_span();
     update_power();
-    gen_next();
   }
 
   __device__ __forceinline__ void save() {
@@ -746,7 +794,7 @@ struct EnvT {
 };
 
 template <int NT, bool TRACE>
-__global__ void __launch_bounds__(NT) sim_thread_kernel(const SimArgs a) {
+__global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   HotTablesT &hot = *reinterpret_cast<HotTablesT *>(smem_raw);
   {
@@ -770,7 +818,16 @@ __global__ void __launch_bounds__(NT) sim_thread_kernel(const SimArgs a) {
   e.env_g = a.env_base + env;
   e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * (a.ring_cap + kThreadTabExtra);
   e.hdr = a.hdr_override ? a.hdr_override : a.hdr + (size_t)env * kHeaderWords;
+  e.arr = (a.arr && !a.script) ? a.arr + (size_t)env * a.arr_cap : nullptr;
+  e.a_head = 0; e.a_count = 0; e.a_id0 = 0; e.a_more = 0;
   if (a.from_init) e.init(env); else e.load();
+  if (a.n_steps > 0 && e.epoch < a.n_epochs) {
+    if (e.arr) {                                                // arrivals up to the end of the last epoch of this launch
+      e.a_horizon = min(e.epoch + a.n_steps, a.n_epochs) * a.epoch_s;
+      e.fill_arrivals();
+      e.gen_next();
+    } else if (!e.look_valid) e.gen_next();                     // prime the inline generator's look-ahead
+  }
   e.run(li, env);
   if (a.state_out) e.observe(a.state_out + (size_t)(TRACE ? 0u : env) * MIG_STATE_DIM);
   if (a.totals) e.store_totals(a.totals + (TRACE ? 0u : env));   // totals so far (hash and t are live values)

@@ -283,6 +283,27 @@ def test_every_tile_width_gives_the_same_records(tile):
         sim.close()
 
 
+@pytest.mark.parametrize("entries", [0, 1, 7, 100])
+def test_thread_kernel_arrival_lists_of_any_capacity_give_the_same_day(entries):
+    # 0 = arrivals drawn inside the event loop; 1, 7, 100 = lists that fill up and are refilled many times a day
+    for name, n in (("C3", 96), ("C4", 64)):
+        wl = W.CONFIGS[name](n)
+        _, recs_ref, tot_ref, _ = gpu_rollout(wl, sim=B.MigSim(wl.params, n, wl.seed, tile=1))
+        sim = B.MigSim(wl.params, n, wl.seed, tile=1)
+        sim.set_arrival_buffer(entries)
+        _, recs, tot, _ = gpu_rollout(wl, sim=sim)
+        assert tot.tobytes() == tot_ref.tobytes() and recs.tobytes() == recs_ref.tobytes()
+        # step by step, switching the generator between epochs
+        sim.reset(0, dev(wl.algo), dev(wl.cfg0))
+        rec = torch.zeros((n, 64), dtype=torch.uint8, device="cuda")
+        for k in range(24):
+            sim.set_arrival_buffer(entries if k % 2 else (0 if entries else 50))
+            sim.step(dev(recs_ref[k]["cfg"].astype(np.uint8)), rec_out=rec)
+            torch.cuda.synchronize()
+            assert B.recs_to_numpy(rec).tobytes() == recs_ref[k].tobytes(), (name, entries, k)
+        sim.close()
+
+
 def test_set_tile_between_kernel_families_needs_a_reset():
     wl = W.config_c3(32)
     sim = B.MigSim(wl.params, 32, wl.seed, tile=8)
