@@ -25,10 +25,14 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# Algorithmic warp-instructions per job-event (DESIGN.md section 6 derives it by hand from what the method must do
-# per ARRIVE/COMPLETE at one warp per environment); the roofline numerator uses THIS, not the executed count, so that
-# instruction bloat cannot inflate the fraction.
-ALG_WARP_INSTR_PER_JOB_EVENT = 260.0
+# Algorithmic LANE-instructions per job-event (DESIGN.md section 6 derives it by hand from what the serial method must
+# execute per ARRIVE/COMPLETE: generator 136, event advance 22, arrival/completion accounting + trace hash 30,
+# reschedule 128); the roofline numerator uses THIS, not the executed count, so that neither instruction bloat nor
+# idle lanes can inflate the fraction.  Peak = SMs x 128 FP32/INT32 lanes x f_max lane-instructions per second.
+ALG_THREAD_INSTR_PER_JOB_EVENT = 316.0
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE rollout launch from the ncu --set full capture in profiles/
+# (per launch like `achieved`); None where no capture of that launch configuration exists.
+NCU_DRAM_BYTES_PER_LAUNCH = {("C5", 65536, 1): 10.19e9 + 9.62e9}
 CPU_SAMPLE_ENVS = 2048
 
 
@@ -238,14 +242,18 @@ def run_ours(args):
     # ---- roofline of the dominant kernel (sim_kernel): plain ALU / issue slots --------------------------------------
     props = torch.cuda.get_device_properties(local)
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
-    peak_gips = props.multi_processor_count * 4 * sm_mhz * 1e6 / 1e9             # G warp-instr/s: SMs x 4 schedulers x f_max
-    achieved_gips = ALG_WARP_INSTR_PER_JOB_EVENT * ev_per_launch / (kern_ms / 1e3) / 1e9
+    tile = sim.get_tile()
+    peak_gips = props.multi_processor_count * 128 * sm_mhz * 1e6 / 1e9           # G lane-instr/s: SMs x 128 lanes x f_max
+    achieved_gips = ALG_THREAD_INSTR_PER_JOB_EVENT * ev_per_launch / (kern_ms / 1e3) / 1e9
     alg_bytes = n_envs * ((sp.n_epochs + 1) * 64 + 80 + 2 * 256)                  # records + totals + state header in/out
-    roofline = {"bound": "alu", "achieved": achieved_gips, "peak": peak_gips, "unit": "Gwarp-instr/s", "frac": achieved_gips / peak_gips,
-                "traffic": None, "kernel": "sim_kernel<false>", "kernel_ms": kern_ms,
-                "alg_warp_instr_per_job_event": ALG_WARP_INSTR_PER_JOB_EVENT, "peak_source": "%d SMs x 4 x %s sm_max_mhz %.0f" % (props.multi_processor_count, peak_src, sm_mhz),
+    if tile == 1:
+        alg_bytes += int(2 * 16 * ev_per_launch / 2)                              # arrival lists: 16 B per job written once, read once
+    roofline = {"bound": "alu", "achieved": achieved_gips, "peak": peak_gips, "unit": "Glane-instr/s", "frac": achieved_gips / peak_gips,
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.workload, n_envs, tile)),
+                "kernel": "sim_thread_kernel<64,false>" if tile == 1 else "sim_kernel<%d,false>" % tile, "kernel_ms": kern_ms,
+                "alg_thread_instr_per_job_event": ALG_THREAD_INSTR_PER_JOB_EVENT, "peak_source": "%d SMs x 128 lanes x %s sm_max_mhz %.0f" % (props.multi_processor_count, peak_src, sm_mhz),
                 "hbm_algorithmic_bytes_per_launch": alg_bytes, "hbm_gbs_at_that": alg_bytes / (kern_ms / 1e3) / 1e9,
-                "hbm_peak_gbs": peaks.get("hbm_gbs")}
+                "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_frac": alg_bytes / (kern_ms / 1e3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0))}
     line = None
     if rank == 0:
         import concurrent.futures as cf
@@ -283,7 +291,7 @@ def main():
     ap.add_argument("--envs", type=int, default=0, help="environments per GPU (default: the workload's BASELINE size)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 8, 16, 32], help="lanes per environment (0 = library default)")
+    ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 8, 16, 32], help="lanes per environment (0 = library default: 1 = thread per environment for >= 12288 envs, else 8)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -184,10 +184,12 @@ int mig_sim_debug_set_jobs(mig_sim_t *s, const mig_job_t *jobs, uint32_t n);
 /* The exact-division constants the kernels use for x / v (host helper, exposed for tests): x / v == v == 1 ? x :
  * (umulhi(x, m) >> sh) for every 0 <= x < 2^31. */
 int mig_debug_div_magic(uint32_t v, uint32_t *m, uint32_t *sh);
-/* Lanes per environment of the rollout kernel: 8 (default; four environments per warp in lockstep -- the paper-shaped
- * workloads keep about a dozen jobs in the system and a MIG GPU has 7 slots), 16, or 32 (one warp per environment, for
- * workloads with hundreds of jobs in the system).  0 = default.  Results are identical for every value (tested); only
- * the launch geometry and the shared-memory footprint change.  Allowed between any two calls; MIG_EINVAL otherwise. */
+/* Lanes per environment of the rollout kernel.  1 = one THREAD per environment (running jobs in the slice table, waiting
+ * jobs in a sorted two-level queue, no cross-lane traffic; needs >= ~12 000 environments to fill a B200 and is then 3-5x
+ * faster); 8 = four environments per warp in lockstep, 16, 32 = one warp per environment (north_star's layout).
+ * 0 = default: 1 if n_envs >= 12288, else 8.  Results are identical for every value (tested); only the launch geometry
+ * and the memory footprint change.  Switching between 1 and {8, 16, 32} changes the layout of the saved per-env state:
+ * allowed at any time, but the next call must then be mig_sim_reset (MIG_ESTATE otherwise).  Other values: MIG_EINVAL. */
 int mig_sim_set_tile(mig_sim_t *s, int lanes_per_env);
 /* Thread-per-environment kernel only: capacity (records of 16 bytes per environment) of the arrival lists that a launch
  * fills, in one loop that all lanes of a warp run in step, before it simulates (the arrival process does

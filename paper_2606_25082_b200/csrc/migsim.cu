@@ -149,7 +149,12 @@ static int build_tables(const mig_params_t *p, DevTables *t) {
 }
 
 // ------------------------------------------------------------------------------------------------ tile width
-constexpr int kDefaultTile = 8;
+// Default lanes per environment: the thread-per-environment kernel takes a whole simulated day of latency whatever the
+// batch (about 80-100 ms for the C5 shape) and wins as soon as the batch fills the machine with warps; measured
+// crossover against the 8-lane tiles on B200 (C5 shape): 8192 envs 78 vs 90 ms, 16384 envs 82 vs 152 ms; C3 (4096 envs)
+// and C4 (8192 envs, one launch per epoch) are faster on the tiles.
+constexpr uint32_t kThreadKernelMinEnvs = 12288;
+static int default_tile(uint32_t n_envs) { return n_envs >= kThreadKernelMinEnvs ? 1 : 8; }
 
 template <bool TRACE>
 static const void *kernel_ptr(int tile) {
@@ -193,7 +198,7 @@ static int configure_tile(mig_sim *s, int tile) {
 
 extern "C" int mig_sim_set_tile(mig_sim_t *s, int lanes_per_env) {
   if (!s) return fail(MIG_EINVAL, "set_tile: NULL handle");
-  return configure_tile(s, lanes_per_env ? lanes_per_env : kDefaultTile);
+  return configure_tile(s, lanes_per_env ? lanes_per_env : default_tile(s->n_envs));
 }
 
 extern "C" int mig_sim_get_tile(const mig_sim_t *s) { return s ? s->tile : 0; }
@@ -223,7 +228,8 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
   cudaDeviceProp prop;
   if (cudaGetDevice(&s->device) != cudaSuccess || cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) { delete s; return fail(MIG_ECUDA, "create: cannot query the device"); }
   s->n_sm = prop.multiProcessorCount;
-  rc = configure_tile(s, kDefaultTile);
+  s->tile = 8;
+  rc = configure_tile(s, default_tile(n_envs));
   if (rc) { delete s; return rc; }
   size_t n = n_envs;
 #define ALLOC(ptr, bytes) if (cudaMalloc((void **)&(ptr), (bytes)) != cudaSuccess) { cudaGetLastError(); mig_sim_destroy(s); return fail(MIG_ENOMEM, "create: cudaMalloc of %zu bytes failed", (size_t)(bytes)); }

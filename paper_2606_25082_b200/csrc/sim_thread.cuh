@@ -9,16 +9,18 @@
 // the heavy batches (BASELINE C5: 65 536) have; small batches stay on the 8-lane tiles.
 //
 // Data structures are chosen so that no step scans the queue (a lane with a 300-job queue would otherwise hold its 31
-// neighbours for the length of its scan):
+// neighbours for the length of its scan) and that lanes doing the same thing run the same instructions:
 //   * RUNNING jobs live in the slice table: slot p holds {skey, meta, rem, due} and the speed of the job running there;
-//   * WAITING jobs live in a binary min-heap on (skey, id) of the same 16-byte records: the reschedule's "all jobs in
-//     priority order" is a merge of the <= 7 running jobs with successive heap minima, O(K log n);
-//     EDF keys never change and LLF / LALF keys change only while a job runs, so the heap order stays valid (a
-//     repartition, which changes every laxity, rebuilds it).
+//   * WAITING jobs live in a sorted two-level double-ended queue on (skey, id): a ring in shared memory for the
+//     smallest records, a ring in global memory for the rest.  The reschedule's "all jobs in priority order"
+//      is a merge of the <= 7 running jobs with the queue's front; arrivals are inserted from the tail,
+//     re-queued jobs from the front (deadlines grow with arrival time, so both are O(1) in practice);
+//   * ARRIVALS are drawn before the event loop starts, in one loop that all lanes run in step, into a per-environment
+//     list in global memory (the arrival process does not depend on the schedule).
 // Per-thread data is in shared memory, interleaved by thread (row r of thread tid at base[r * NT + tid]: every access
-// of a warp is bank-conflict-free whatever index each lane uses); heap entries beyond `smem_entries` are in global
-// memory.  Scalars (time, hash, energy, generator, look-ahead arrival) live in registers.  The results are bit-identical
-// to the tile kernels and to the oracle (tests/test_gpu_parity.py); no code is shared with oracle/.
+// of a warp is bank-conflict-free whatever index each lane uses).  Scalars (time, hash, energy, generator, look-ahead
+// arrival) live in registers.  The results are bit-identical to the tile kernels and to the oracle
+// (tests/test_gpu_parity.py); no code is shared with oracle/.
 #pragma once
 #include "sim_device.cuh"
 
@@ -27,7 +29,7 @@ namespace migsim {
 constexpr int kThreadCta = 64;        // threads (= environments) per CTA of the thread-per-environment kernel
 constexpr int kThreadTabExtra = 32;   // job-table entries per env beyond the global ring: save area of the shared ring (16) and the slice table (7)
 
-// per-thread rows of 8 bytes (uint2): slice records, pick staging, then the heap; rows of 4 bytes follow
+// per-thread rows of 8 bytes (uint2): slice records, pick staging, then the queue's shared ring; rows of 4 bytes follow
 enum { T2_SLKM = 0 /* 7: {skey, meta} of the job running on slot p */, T2_SLRD = 7 /* 7: {rem, due}; a DOWN slice keeps up_at in .x */,
        T2_STG = 14 /* 7: {meta | slot | moved << 3, rem} of pick k */, T2_HEAP = 21 };
 enum { T1_V = 0 /* 7: speed of the running job */, T1_STGDUE = 7 /* 7 */, T1_CNT = 14 /* C_COUNT = 10 */, T1_WORDS = 24 };
@@ -57,9 +59,9 @@ struct EnvT {
   const HotTablesT &hot;
   uint2 *const r2;         // 8-byte rows: r2[row * NT]
   uint32_t *const r1;      // 4-byte rows: r1[row * NT]
-  uint4 *gtab;             // heap overflow (entry index i >= S) and save area in global memory
+  uint4 *gtab;             // global ring of the waiting queue, then the save area of the shared ring and the slice table
   uint32_t *hdr;           // this env's saved header (running totals are kept there)
-  const uint32_t S;        // heap entries held in shared memory
+  const uint32_t S;        // slots of the shared-memory ring
   uint32_t env_g;
   int t, t_end, epoch, cfg, algo; uint32_t status, n_sys, n_wait, cfg_sizes, cfg_rank, slice_mask;
   uint32_t h_lo, h_hi;
@@ -73,6 +75,7 @@ struct EnvT {
   uint32_t n_trace, i_script, n_events;
   uint4 *arr;              // this env's arrival list (NULL: generate inline)
   uint32_t a_head, a_count, a_id0, a_more; int a_horizon;
+  uint4 a_nxt;             // arr[a_head], prefetched
 
   __device__ __forceinline__ EnvT(const SimArgs &a_, const HotTablesT &h_, uint2 *r2_, uint32_t *r1_)
       : a(a_), hot(h_), r2(r2_), r1(r1_), S(a_.smem_entries) {}
@@ -350,11 +353,13 @@ struct EnvT {
         if (!a_more) return;
         fill_arrivals();                                                      // the list was full: next stretch (rare)
         if (a_count == 0) return;
+        a_nxt = arr[0];
       }
-      const uint4 e = arr[a_head];
+      const uint4 e = a_nxt;                                                  // loaded one arrival ago: its latency is hidden
       look_tick = (int)e.x; look_cls = e.y; look_work = (int)e.z; look_due = (int)e.w;
       look_id = a_id0 + a_head++;
       look_valid = 1;
+      if (a_head < a_count) a_nxt = arr[a_head];
       return;
     }
     if (n_accepted >= job_limit()) return;
@@ -825,6 +830,7 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
     if (e.arr) {                                                // arrivals up to the end of the last epoch of this launch
       e.a_horizon = min(e.epoch + a.n_steps, a.n_epochs) * a.epoch_s;
       e.fill_arrivals();
+      if (e.a_count) e.a_nxt = e.arr[0];
       e.gen_next();
     } else if (!e.look_valid) e.gen_next();                     // prime the inline generator's look-ahead
   }
