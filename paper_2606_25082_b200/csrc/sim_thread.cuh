@@ -330,7 +330,7 @@ struct EnvT {
       if (a_count == a.arr_cap) { a_more = 1; break; }
       g_k = k + 1; g_T = T;
       if (w.y <= __ldg(&tb_->thr[(uint32_t)tick / 60u])) {                    // Lewis-Shedler thinning
-        arr[a_count++] = job_attributes(k, w, (uint32_t)tick);
+        __stcg(&arr[a_count++], job_attributes(k, w, (uint32_t)tick));       // streamed: keep L1 for the tables
         n_accepted++;
       }
     }
@@ -353,13 +353,16 @@ struct EnvT {
         if (!a_more) return;
         fill_arrivals();                                                      // the list was full: next stretch (rare)
         if (a_count == 0) return;
-        a_nxt = arr[0];
+        a_nxt = __ldcg(&arr[0]);
       }
       const uint4 e = a_nxt;                                                  // loaded one arrival ago: its latency is hidden
       look_tick = (int)e.x; look_cls = e.y; look_work = (int)e.z; look_due = (int)e.w;
       look_id = a_id0 + a_head++;
       look_valid = 1;
-      if (a_head < a_count) a_nxt = arr[a_head];
+      if (a_head < a_count) {
+        a_nxt = __ldcg(&arr[a_head]);
+        if ((a_head & 7u) == 0u && a_head + 8u < a_count) asm volatile("prefetch.global.L2 [%0];" ::"l"(arr + a_head + 8));   // next 128-byte line
+      }
       return;
     }
     if (n_accepted >= job_limit()) return;
@@ -830,7 +833,7 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
     if (e.arr) {                                                // arrivals up to the end of the last epoch of this launch
       e.a_horizon = min(e.epoch + a.n_steps, a.n_epochs) * a.epoch_s;
       e.fill_arrivals();
-      if (e.a_count) e.a_nxt = e.arr[0];
+      if (e.a_count) e.a_nxt = __ldcg(&e.arr[0]);
       e.gen_next();
     } else if (!e.look_valid) e.gen_next();                     // prime the inline generator's look-ahead
   }

@@ -271,6 +271,52 @@ def test_env_base_sharding_is_placement_invariant():
         sim.close()
 
 
+def _oracle_custom(args):
+    sp, seed, e, algo, cfg0, table = args
+    r = O.rollout(sp, seed, e, algo=algo, cfg0=cfg0, policy=W.POLICY_TABLE, table=table, trace_cap=400000, want_states=True)
+    return e, r.recs, r.totals, r.trace, r.states
+
+
+@pytest.mark.parametrize("downtime,theta", [(60, 60), (0, 5), (1800, 600)])
+def test_hourly_random_repartitions_all_algorithms(downtime, theta):
+    # every env repartitions to a random configuration every hour (a different one per load bucket), algorithms cycle
+    # over EDF-FS / EDF-SS / LLF / LALF: repartition with requeue, downtime, re-keyed laxities and critical-laxity events
+    import dataclasses
+    n = 64
+    base = W.config_c3(n)
+    sp = dataclasses.replace(base.params, repart_downtime_s=downtime, crit_laxity_s=theta)
+    rng = np.random.default_rng(downtime + theta)
+    table = rng.integers(0, 12, size=(n, 24, 4)).astype(np.uint8)
+    algo = (np.arange(n) % 4).astype(np.uint8)
+    cfg0 = rng.integers(0, 12, size=n).astype(np.uint8)
+    sim = B.MigSim(sp, n, 77)
+    recs, tot = sim.alloc_recs(), sim.alloc_totals()
+    state = sim.alloc_state()
+    d_table = dev(table)
+    sim.reset(0, dev(algo), dev(cfg0))
+    sim.rollout(W.POLICY_TABLE, table=d_table, recs_out=recs, totals_out=tot)
+    sim.totals(tot)
+    torch.cuda.synchronize()
+    g_recs, g_tot = B.recs_to_numpy(recs), B.totals_to_numpy(tot)
+    with cf.ProcessPoolExecutor(min(n, os.cpu_count() or 1)) as ex:
+        res = list(ex.map(_oracle_custom, [(sp, 77, e, int(algo[e]), int(cfg0[e]), table[e]) for e in range(n)]))
+    assert g_tot["n_repart"].min() > 10 and (theta > 60 or g_tot["n_crit"][2::4].sum() > 0)
+    for e, o_recs, o_tot, o_trace, o_states in res:
+        assert_same_records(g_recs[:, e], g_tot[e], o_recs, o_tot, "env %d algo %d" % (e, algo[e]))
+    for e, o_recs, o_tot, o_trace, o_states in res[:16]:
+        ev, t1 = sim.debug_trace(e, policy=W.POLICY_TABLE, table=d_table, cap_events=400000)
+        assert len(ev) == len(o_trace) and ev.tobytes() == o_trace.tobytes(), "env %d" % e
+    # the same day step by step with the actions the rollout took: states after every epoch
+    sim.reset(0, dev(algo), dev(cfg0), state_out=state)
+    for k in range(24):
+        sim.step(dev(g_recs[k]["cfg"].astype(np.uint8)), state_out=state)
+        torch.cuda.synchronize()
+        s_k = state.cpu().numpy()
+        for e, o_recs, o_tot, o_trace, o_states in res:
+            assert np.array_equal(s_k[e], o_states[k + 1]), (e, k)
+    sim.close()
+
+
 @pytest.mark.parametrize("tile", [1, 16, 32])
 def test_every_tile_width_gives_the_same_records(tile):
     for name, n in (("C2", 200), ("C3", 200)):
