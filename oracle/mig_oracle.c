@@ -297,10 +297,73 @@ static int pick_slice(const orc_env_t *e, const job_t *j, const int *avail)
   return pick_fastest(e, j, avail);
 }
 
+/* slowest slice of the set `ok` on which j completes by its due date (ties -> smaller size, lower slot), or NO_SLOT */
+static int pick_slowest_on_time(const orc_env_t *e, const job_t *j, const int *ok)
+{
+  int best = NO_SLOT; int32_t br = 0;
+  for (int p = 0; p < ORC_SLOTS; ++p) {
+    if (!ok[p]) continue;
+    int32_t r = rd(e, j, e->sl[p].size);
+    if ((int64_t)e->t + r > (int64_t)j->due) continue;
+    if (best == NO_SLOT || r > br || (r == br && e->sl[p].size < e->sl[best].size)) { best = p; br = r; }
+  }
+  return best;
+}
+
+/* EDF-SS with RESTRICTED preemption ("a variant that only preempts jobs in cases that directly
+ * prevent the jobs from missing their deadlines"; the paper gives no more than this sentence -- the rule below is
+ * DESIGN.md reading #26).  Running jobs keep their slices.  The waiting jobs are visited in (due, id) order; job j
+ *   (a) takes the slowest FREE up slice on which it finishes on time (the SS rule, L175); otherwise
+ *   (b) if it would finish on time on an OCCUPIED up slice whose job has a later (due, id), it takes the slowest such
+ *       slice: that job is preempted (PREEMPT, then START of j) and waits again -- it is visited later in this pass;
+ *   (c) otherwise, if a free up slice is left, it takes the fastest one (it is late anyway: EDF-SS's fallback, L175);
+ *   (d) otherwise it waits.
+ * Events are emitted in that order, as they happen. */
+static void reschedule_restricted(orc_env_t *e)
+{
+  uint32_t n = e->n_sys;
+  char *seen = (char *)calloc(n ? n : 1, 1);
+  for (;;) {
+    int best = -1;                            /* jobs[] is in id order: strict '<' keeps the lowest id on ties */
+    for (uint32_t i = 0; i < n; ++i) {
+      if (e->jobs[i].slot != NO_SLOT || seen[i]) continue;
+      if (best < 0 || e->jobs[i].due < e->jobs[best].due) best = (int)i;
+    }
+    if (best < 0) break;
+    seen[best] = 1;
+    job_t *j = &e->jobs[best];
+    int fr[ORC_SLOTS], oc[ORC_SLOTS], any_free = 0;
+    for (int p = 0; p < ORC_SLOTS; ++p) {
+      int up = e->sl[p].size && !e->sl[p].down;
+      fr[p] = up && e->sl[p].job == NONE_JOB; any_free |= fr[p];
+      oc[p] = 0;
+      if (up && e->sl[p].job != NONE_JOB) {
+        const job_t *r = find_job(e, e->sl[p].job);
+        oc[p] = r->due > j->due || (r->due == j->due && r->id > j->id);
+      }
+    }
+    int p = pick_slowest_on_time(e, j, fr);                                   /* (a) */
+    if (p == NO_SLOT) {
+      p = pick_slowest_on_time(e, j, oc);                                     /* (b) */
+      if (p != NO_SLOT) {
+        job_t *r = find_job(e, e->sl[p].job);
+        emit(e, ORC_EV_PREEMPT, p, (uint32_t)e->sl[p].size, r->id, r->rem); e->ep.n_preempt++; e->tot.n_preempt++;
+        r->slot = NO_SLOT; e->sl[p].job = NONE_JOB;
+      } else if (any_free) p = pick_fastest(e, j, fr);                        /* (c) */
+    }
+    if (p == NO_SLOT) continue;                                               /* (d) */
+    emit(e, ORC_EV_START, p, (uint32_t)e->sl[p].size, j->id, j->rem); e->ep.n_start++; e->tot.n_start++;
+    j->slot = p; e->sl[p].job = j->id;
+  }
+  for (uint32_t i = 0; i < n; ++i) e->jobs[i].t_crit = -1;
+  free(seen);
+}
+
 /* "all jobs currently in the system (either actively running ... or waiting in the queue) are
  * re-evaluated for job prioritization and slice allocation.  Any job can be preempted." */
 static void reschedule(orc_env_t *e)
 {
+  if (e->algo == ORC_ALGO_EDF_SS_R) { reschedule_restricted(e); return; }
   uint32_t n = e->n_sys;
   int avail[ORC_SLOTS]; int navail = 0;
   for (int p = 0; p < ORC_SLOTS; ++p) { avail[p] = (e->sl[p].size && !e->sl[p].down); navail += avail[p]; }

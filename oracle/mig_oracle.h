@@ -33,7 +33,8 @@ extern "C" {
 enum { ORC_EV_ARRIVE = 1, ORC_EV_DROP = 2, ORC_EV_START = 3, ORC_EV_PREEMPT = 4, ORC_EV_COMPLETE = 5,
        ORC_EV_CRIT = 6, ORC_EV_SLICE_UP = 7, ORC_EV_REPART = 8 };
 
-enum { ORC_ALGO_EDF_FS = 0, ORC_ALGO_EDF_SS = 1, ORC_ALGO_LLF = 2, ORC_ALGO_LALF = 3 };
+enum { ORC_ALGO_EDF_FS = 0, ORC_ALGO_EDF_SS = 1, ORC_ALGO_LLF = 2, ORC_ALGO_LALF = 3,
+       ORC_ALGO_EDF_SS_R = 4 /* EDF-SS with restricted preemption */ };
 enum { ORC_POLICY_STATIC = 0, ORC_POLICY_TABLE = 1, ORC_POLICY_DQN = 2 };
 
 typedef struct {

@@ -157,6 +157,32 @@ def test_G_tie_between_equally_fast_slices_takes_smaller(algo):
     assert completions(r.trace) == {0: g["completion"]}
 
 
+def test_H_restricted_preemption_evicts_only_to_save_a_deadline():
+    g = G["H"]
+    sp = tiny_params()
+    r = run(sp, g["jobs"], g["algo"], g["cfg"])
+    assert completions(r.trace) == as_int_keys(g["completion"])
+    assert events_at(r.trace, 10) == [tuple(e) for e in g["events_at_10"]]
+    assert events_at(r.trace, 12) == [tuple(e) for e in g["events_at_12"]]
+    assert [int(e["value"]) for e in r.trace if e["t"] == 12 and e["type"] == 4] == g["preempt_values_at_12"]
+    assert int(r.totals["n_preempt"]) == g["n_preempt"] and int(r.totals["tardiness_s"]) == g["tardiness_s"]
+    assert int(r.totals["energy_mj"]) == g["idle_mw"] * 86400 + g["dyn_energy_mj"]
+    assert cfg_idle_mw(sp, g["cfg"]) == g["idle_mw"]
+    # the unrestricted algorithm swaps the two running jobs at t = 10 ("switching two jobs between
+    # different slices that might not result in any energy consumption or tardiness differences")
+    u = run(sp, g["jobs"], ALGO["EDF-SS"], g["cfg"])
+    assert int(u.totals["n_preempt"]) == g["n_preempt_unrestricted"] and int(u.totals["tardiness_s"]) == 0
+
+
+def test_I_restricted_preemption_fallback_wait_and_no_eviction_of_earlier_deadlines():
+    g = G["I"]
+    r = run(tiny_params(), g["jobs"], g["algo"], g["cfg"])
+    assert completions(r.trace) == as_int_keys(g["completion"])
+    for t in (5, 6, 11, 175):
+        assert events_at(r.trace, t) == [tuple(e) for e in g["events_at_%d" % t]], t
+    assert int(r.totals["n_preempt"]) == g["n_preempt"] and int(r.totals["tardiness_s"]) == g["tardiness_s"]
+
+
 def test_speed_tables_match_survey_values():
     assert LINEAR == [120, 240, 360, 480, 840]
     assert SUB05 == [317, 449, 550, 635, 840]

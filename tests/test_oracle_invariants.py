@@ -61,6 +61,66 @@ def test_invariants_on_baseline_workloads(name, n_env):
             assert np.float32(r.rewards[k]) == np.float32(ref)
 
 
+def _restricted_day(e, cfg, table=None):
+    wl = W.config_c3(8)
+    r = O.rollout(wl.params, 11, e, algo=4, cfg0=cfg, policy=W.POLICY_STATIC if table is None else W.POLICY_TABLE, table=table,
+                  trace_cap=200000)
+    assert int(r.totals["status"]) == 0
+    trace_check.check_against_records(wl.params, cfg, r.trace, r.recs, r.totals)
+    return wl.params, r
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 6, 9, 11])
+def test_restricted_preemption_properties(cfg):
+    """PAPER.md:L198-204, reading #26, checked on the trace alone: (1) a job is never moved between slices while it
+    runs; (2) outside a repartition every PREEMPT is followed at once by the START, on the same slice, of a job with
+    an earlier (due, id) that completes there by its due date; (3) far fewer preemptions than unrestricted EDF-SS
+    (the paper reports 63-99 % fewer, Fig. 4) at a similar tardiness."""
+    sp, r = _restricted_day(3, cfg)
+    tr = r.trace
+    due, cls, where = {}, {}, {}
+    speed = np.asarray(sp.speed).reshape(-1, 5)
+    n_evict = 0
+    for i, ev in enumerate(tr):
+        ty, job, slot, t = int(ev["type"]), int(ev["job"]), int(ev["slot"]), int(ev["t"])
+        if ty == 1:
+            due[job], cls[job] = int(ev["value"]), int(ev["aux"])
+        elif ty == 3:
+            assert job not in where, "a running job was started again without a PREEMPT"
+            where[job] = slot
+        elif ty == 5:
+            del where[job]
+        elif ty == 4:
+            assert where.pop(job) == slot
+            nxt = tr[i + 1]
+            assert int(nxt["type"]) == 3 and int(nxt["slot"]) == slot and int(nxt["t"]) == t
+            j2 = int(nxt["job"])
+            assert (due[j2], j2) < (due[job], job)
+            v = int(speed[cls[j2]][W.SIZE_INDEX[int(nxt["aux"])]])
+            assert t + -(-int(nxt["value"]) // v) <= due[j2], "the evicting job does not make its deadline there"
+            n_evict += 1
+    u = O.rollout(sp, 11, 3, algo=1, cfg0=cfg)
+    assert int(r.totals["n_preempt"]) == n_evict
+    assert n_evict <= 0.4 * int(u.totals["n_preempt"])
+    assert int(r.totals["n_completed"]) == int(u.totals["n_completed"])
+
+
+def test_restricted_preemption_equals_edf_ss_when_nothing_ever_waits():
+    # sparse arrivals (no two jobs overlap): both variants place every job on the slowest slice that meets its deadline
+    sp = tiny_params()
+    rows = [(1000 * i, 0, 5 + i % 7, 1000 * i + 40 + 13 * (i % 5)) for i in range(60)]
+    a = O.rollout(sp, 0, 0, algo=4, cfg0=2, jobs=O.make_jobs(rows), trace_cap=1024)
+    b = O.rollout(sp, 0, 0, algo=1, cfg0=2, jobs=O.make_jobs(rows), trace_cap=1024)
+    assert a.trace.tobytes() == b.trace.tobytes() and a.totals.tobytes() == b.totals.tobytes()
+
+
+def test_restricted_preemption_with_repartitions_keeps_the_invariants():
+    rng = np.random.default_rng(5)
+    table = rng.integers(0, 12, size=(24, 4)).astype(np.uint8)
+    sp, r = _restricted_day(1, 4, table=table)
+    assert int(r.totals["n_repart"]) > 10 and int(r.totals["n_jobs"]) == int(r.totals["n_completed"]) + int(r.totals["n_dropped"])
+
+
 @pytest.mark.parametrize("cfg", [0, 4])
 def test_uniform_slice_configs_make_variants_coincide(cfg):
     # PAPER.md:L236: "configurations 1 and 5 ... the EDF variants produce the same value, as do the LLF variants"
