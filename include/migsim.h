@@ -51,7 +51,12 @@ extern "C" {
 #define MIG_MAX_JOBS (1u << 20) /* job ids are < 2^20 per env-day: generation stops after this many accepted jobs */
 
 /* scheduling algorithm per environment */
-enum { MIG_ALGO_EDF_FS = 0, MIG_ALGO_EDF_SS = 1, MIG_ALGO_LLF = 2, MIG_ALGO_LALF = 3 };
+enum { MIG_ALGO_EDF_FS = 0, MIG_ALGO_EDF_SS = 1, MIG_ALGO_LLF = 2, MIG_ALGO_LALF = 3,
+       /* EDF-SS with restricted preemption (the variant the paper's repartitioning runs on): running jobs
+        * keep their slices; waiting jobs in (due, id) order take the slowest free slice on which they finish on time, else
+        * evict a job with a later (due, id) from the slowest occupied slice on which they would, else take the fastest
+        * free slice, else wait (reading #26) */
+       MIG_ALGO_EDF_SS_R = 4 };
 /* repartitioning policy of mig_sim_rollout */
 enum { MIG_POLICY_STATIC = 0, MIG_POLICY_TABLE = 1, MIG_POLICY_DQN = 2 };
 /* per-environment status bits */

@@ -215,8 +215,9 @@ struct Env {
     }
     return mean ? sum / n : best;
   }
+  __device__ __forceinline__ bool is_lax() const { return (algo & ~1) == MIG_ALGO_LLF; }      // LLF or LALF
   __device__ __forceinline__ int skey_of(int due, int rem, uint32_t cls) const {
-    if (algo < MIG_ALGO_LLF) return due;                                  // EDF: deadline
+    if (!is_lax()) return due;                                  // EDF: deadline
     return due - rd_cfg(rem, cls, algo == MIG_ALGO_LALF);                 // laxity + t (t is common to all jobs)
   }
 
@@ -327,7 +328,7 @@ struct Env {
   // ------------------------------------------------------------------ reschedule
   // critical-laxity events (LLF / LALF): earliest t_crit = skey - theta > t over waiting jobs
   __device__ __forceinline__ void compute_next_crit(bool go) {
-    const bool lax = go && algo >= MIG_ALGO_LLF;
+    const bool lax = go && is_lax();
     if (!MIG_ANY(lax)) { if (go) next_crit = MIG_INF; return; }
     int best = MIG_INF;
     if (lax)
@@ -341,11 +342,86 @@ struct Env {
     if (go) next_crit = best;
   }
 
+  // EDF-SS with RESTRICTED preemption (reading #26).  Running jobs keep their slices; the
+  // waiting jobs are visited in (due, id) order (one tile argmin per visit, "beyond the previous one"): (a) slowest FREE
+  // slice on which the job is on time, else (b) slowest OCCUPIED slice on which it is on time among those whose job has
+  // a later (due, id): that job is preempted and waits again (it is visited later in the same pass), else (c) fastest
+  // free slice, else (d) it waits.  The visit stops when nothing is free and no running job has a later deadline.
+  __device__ __forceinline__ void reschedule_restricted(bool go) {
+    int pk = (int)0x80000000; uint32_t pid = 0;
+    bool open = go;
+    for (;;) {
+      const bool up = sl_size != 0 && !sl_down;
+      const bool any_free = T::tballot(open && up && sl_pos < 0, gshift) != 0u;
+      const int max_due = T::tmax((up && sl_pos >= 0) ? rj_due : (int)0x80000000);
+      int bk = MIG_INF; uint32_t bid = 0xFFFFFFFFu; int bi = -1;
+      if (open)
+        for (uint32_t i = gl; i < n_sys; i += G) {
+          uint2 e = ld_km(i);
+          int key = (int)e.x; uint32_t id = e.y & kIdMask;
+          bool waiting = ((e.y >> 28) & 7u) == 0u;
+          bool beyond = key > pk || (key == pk && id > pid);
+          bool better = key < bk || (key == bk && id < bid);
+          if (waiting && beyond && better) { bk = key; bid = id; bi = (int)i; }
+        }
+      const int mk = T::tmin(bk);
+      bool cand = bi >= 0 && bk == mk;
+      uint32_t cm = T::tballot(cand, gshift);
+      if (MIG_ANY((cm & (cm - 1)) != 0u)) {                             // equal deadlines on several lanes: lowest id first
+        uint32_t mid = T::tminu(cand ? bid : 0xFFFFFFFFu);
+        cm = T::tballot(cand && bid == mid, gshift);
+      }
+      open = open && cm != 0u && (any_free || mk <= max_due);           // (a deadline equal to max_due may still win on id)
+      if (!MIG_ANY(open)) break;
+      const int wl = __ffs((int)cm) - 1;
+      const uint32_t b = (uint32_t)T::tshfl(bi, wl);
+      uint2 km = make_uint2(0u, 0u), rdv = make_uint2(1u, 0u);
+      if (open) { km = ld_km(b); rdv = ld_rd(b); }
+      const uint32_t cls = (km.y >> 20) & 15u, id = km.y & kIdMask;
+      const int rem = (int)rdv.x, due = (int)rdv.y;
+      int r = MIG_INF >> 3;
+      if (open && up) r = rd_magic(rem, hot.speed[cls * 5 + sidx_of(sl_size)]);
+      const bool on_time = r <= due - t;
+      const bool is_free = open && up && sl_pos < 0;
+      const bool later = open && up && sl_pos >= 0 && (rj_due > due || (rj_due == due && rj_id > id));
+      const int ssf = (is_free && on_time) ? ((r << 3) | (7 - sl_rank)) : -1;
+      const int sso = (later && on_time) ? ((r << 3) | (7 - sl_rank)) : -1;
+      const int fsf = is_free ? ((r << 3) | sl_rank) : MIG_INF;
+      const int ssfb = T::tmax(ssf), ssob = T::tmax(sso), fsfb = T::tmin(fsf);
+      const int mode = ssfb >= 0 ? 0 : (ssob >= 0 ? 1 : (fsfb != MIG_INF ? 2 : 3));
+      const bool mine = mode == 0 ? (ssf >= 0 && ssf == ssfb) : (mode == 1 ? (sso >= 0 && sso == ssob) : (mode == 2 && fsf == fsfb));
+      const int s = __ffs((int)T::tballot(open && mine, gshift)) - 1;
+      if (open) { pk = mk; pid = id; }
+      const bool ev = open && mode == 1, st = open && mode != 3;
+      const uint32_t vid = T::tshfl(rj_id, s & (G - 1)); const int vrem = T::tshfl(rj_rem, s & (G - 1));
+      emit(ev, MIG_EV_PREEMPT, s, (uint32_t)size_at(s), vid, vrem);
+      count<C_PREEMPT>(ev ? 1u : 0u);
+      if (ev && gl == s) *entry_word((uint32_t)sl_pos, 1) &= ~(7u << 28);          // the evicted job waits again
+      __syncwarp();
+      emit(st, MIG_EV_START, s, (uint32_t)size_at(s), id, rem);
+      count<C_START>(st ? 1u : 0u);
+      if (st && gl == s) {
+        *entry_word(b, 1) = (km.y & ~(7u << 28)) | ((uint32_t)(s + 1) << 28);
+        sl_pos = (int)b; rj_id = id; rj_rem = rem; rj_due = due;
+        rj_v = hot.speed[cls * 5 + sidx_of(sl_size)].x;
+        rj_ctime = t + r;
+      }
+      __syncwarp();
+    }
+    update_power(go);
+    if (go) next_crit = MIG_INF;
+  }
+
   // tiles with go re-evaluate every job in the system; the others only keep the warp's instruction stream company
   __device__ __forceinline__ void reschedule(bool go) {
+    if (MIG_ANY(go && algo == MIG_ALGO_EDF_SS_R)) {          // (environments of a warp may run different algorithms)
+      reschedule_restricted(go && algo == MIG_ALGO_EDF_SS_R);
+      go = go && algo != MIG_ALGO_EDF_SS_R;
+      if (!MIG_ANY(go)) return;
+    }
     const bool busy = sl_pos >= 0;
-    if (MIG_ANY(go && algo >= MIG_ALGO_LLF)) {   // the keys of running jobs move with their remaining work
-      if (go && algo >= MIG_ALGO_LLF && busy)
+    if (MIG_ANY(go && is_lax())) {   // the keys of running jobs move with their remaining work
+      if (go && is_lax() && busy)
         *entry_word((uint32_t)sl_pos, 0) = (uint32_t)skey_of(rj_due, rj_rem, (ld_km((uint32_t)sl_pos).y >> 20) & 15u);
       __syncwarp();
     }
@@ -574,7 +650,7 @@ struct Env {
     count<C_REPART>(rp ? 1u : 0u);
     emit(rp, MIG_EV_REPART, 0xFF, ((uint32_t)old << 8) | action, MIG_NOJOB, 0);
     __syncwarp();
-    if (rp && algo >= MIG_ALGO_LLF)                           // laxity keys are measured against the configuration
+    if (rp && is_lax())                           // laxity keys are measured against the configuration
       for (uint32_t i = gl; i < n_sys; i += G) {
         uint2 km = ld_km(i), rdv = ld_rd(i);
         *entry_word(i, 0) = (uint32_t)skey_of((int)rdv.y, (int)rdv.x, (km.y >> 20) & 15u);
@@ -714,7 +790,7 @@ struct Env {
   }
 
   __device__ __forceinline__ void init(uint32_t env_local) {
-    algo = a.algo[env_local] & 3; t = 0; epoch = 0; status = 0; n_sys = 0;
+    algo = a.algo[env_local]; if (algo > MIG_ALGO_EDF_SS_R) algo &= 3; t = 0; epoch = 0; status = 0; n_sys = 0;
     h_lo = 0x84222325u; h_hi = 0xcbf29ce4u;                   // FNV-1a-64 offset basis
     uint32_t c0 = a.cfg0[env_local];
     if (c0 >= a.n_configs) { c0 = 0; status |= MIG_ST_BAD_ACTION; }

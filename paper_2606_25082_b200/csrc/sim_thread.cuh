@@ -255,8 +255,9 @@ struct EnvT {
     }
     return mean ? sum / n : best;
   }
+  __device__ __forceinline__ bool is_lax() const { return (algo & ~1) == MIG_ALGO_LLF; }      // LLF or LALF
   __device__ __forceinline__ int skey_of(int due, int rem, uint32_t cls) const {
-    if (algo < MIG_ALGO_LLF) return due;                                  // EDF: deadline
+    if (!is_lax()) return due;                                  // EDF: deadline
     return due - rd_cfg(rem, cls, algo == MIG_ALGO_LALF);                 // laxity + t (t is common to all jobs)
   }
 
@@ -387,7 +388,7 @@ struct EnvT {
   // critical-laxity events (LLF / LALF): earliest t_crit = skey - theta > t over waiting jobs
   __device__ __forceinline__ void compute_next_crit() {
     int best = MIG_INF;
-    if (algo >= MIG_ALGO_LLF)
+    if (is_lax())
       for (uint32_t i = 0; i < n_wait; ++i) {
         const uint2 e = ld_km(i);
         const int tc = (int)e.x - a.theta;
@@ -396,10 +397,75 @@ struct EnvT {
     next_crit = best;
   }
 
+  // remove the record at logical index i: the records before it move up one slot, then the front is dropped
+  __device__ __forceinline__ void queue_remove_at(uint32_t i) {
+    for (uint32_t k = i; k > 0; --k) st_rec(k, ld_km(k - 1), ld_rd(k - 1));
+    queue_pop();
+  }
+
+  // EDF-SS with RESTRICTED preemption (reading #26).  Running jobs keep their slices; the
+  // waiting jobs are visited in (due, id) order = queue order: (a) slowest FREE slice on which the job is on time, else
+  // (b) slowest OCCUPIED slice on which it is on time among those whose job has a later (due, id): that job is preempted
+  // and waits again (it is visited later in the same pass), else (c) fastest free slice, else (d) it waits.
+  __device__ __forceinline__ void reschedule_restricted() {
+    const uint32_t up = slice_mask & ~down_mask;
+    uint32_t free_m = up & ~busy_mask;
+    long long maxrun = (long long)0x8000000000000000ll;      // largest (due, id) among the running jobs
+    for (uint32_t m = busy_mask; m; m &= m - 1) maxrun = max(maxrun, ord(R2(T2_SLKM + __ffs((int)m) - 1)));
+    uint32_t i = 0; int n_start = 0, n_pre = 0;
+    while (i < n_wait) {
+      const uint2 km = ld_km(i), rdv = ld_rd(i);
+      if (free_m == 0u && ord(km) > maxrun) break;            // nobody from here on can start (the queue is sorted)
+      const int rem = (int)rdv.x, slack = (int)rdv.y - t;
+      const uint32_t cls = m_cls(km.y);
+      int ssf = -1, fsf = MIG_INF, sso = -1;
+      for (uint32_t m = up; m; m &= m - 1) {
+        const int p = __ffs((int)m) - 1;
+        const int r = rd_magic(rem, speed_of(cls, size_at(p)));
+        const int rk = (int)((cfg_rank >> (4 * p)) & 7u);
+        if ((free_m >> p) & 1u) {
+          fsf = min(fsf, (r << 3) | rk);
+          if (r <= slack) ssf = max(ssf, (r << 3) | (7 - rk));
+        } else if (r <= slack && before(km, R2(T2_SLKM + p))) sso = max(sso, (r << 3) | (7 - rk));
+      }
+      int rk; bool evict = false;
+      if (ssf >= 0) rk = 7 - (ssf & 7);                                      // (a)
+      else if (sso >= 0) { rk = 7 - (sso & 7); evict = true; }                // (b)
+      else if (free_m) rk = fsf & 7;                                          // (c)
+      else { ++i; continue; }                                                 // (d)
+      const int s = (int)((hot.cfg_slot_of[cfg] >> (4 * rk)) & 7u), g = size_at(s);
+      if (i) queue_remove_at(i); else queue_pop();
+      if (evict) {
+        const uint2 vk = R2(T2_SLKM + s), vr = R2(T2_SLRD + s);
+        emit(MIG_EV_PREEMPT, s, (uint32_t)g, m_id(vk.y), (int)vr.x);
+        queue_push_front(vk, vr);                                            // its key is later than km: index >= i
+        ++n_pre;
+      }
+      emit(MIG_EV_START, s, (uint32_t)g, m_id(km.y), rem);
+      R2(T2_SLKM + s) = make_uint2(rdv.y, km.y & ~15u);
+      R2(T2_SLRD + s) = rdv;
+      R1(T1_V + s) = speed_of(cls, g).x;
+      busy_mask |= 1u << s; free_m &= ~(1u << s);
+      ++n_start;
+      if (evict) { maxrun = (long long)0x8000000000000000ll; for (uint32_t m = busy_mask; m; m &= m - 1) maxrun = max(maxrun, ord(R2(T2_SLKM + __ffs((int)m) - 1))); }
+      else maxrun = max(maxrun, ord(make_uint2(rdv.y, km.y & ~15u)));
+    }
+    if (n_pre) count(C_PREEMPT, (uint32_t)n_pre);
+    if (n_start) count(C_START, (uint32_t)n_start);
+    int nd = MIG_INF;
+    for (uint32_t m = busy_mask; m; m &= m - 1) {              // completion times never drift: t + ceil(rem / v)
+      const int p = __ffs((int)m) - 1;
+      nd = min(nd, t + rd_magic((int)R2(T2_SLRD + p).x, speed_of(m_cls(R2(T2_SLKM + p).y), size_at(p))));
+    }
+    next_done = nd; next_crit = MIG_INF;
+    update_power();
+  }
+
   // Every job in the system is re-evaluated: in (key, id) order, while an up slice is left, each job picks a slice by its
   // rule.  The order is produced by merging the running jobs (slice table) with successive minima of the waiting heap.
   __device__ __forceinline__ void reschedule() {
-    if (algo >= MIG_ALGO_LLF)                       // the keys of running jobs move with their remaining work
+    if (algo == MIG_ALGO_EDF_SS_R) { reschedule_restricted(); return; }
+    if (is_lax())                       // the keys of running jobs move with their remaining work
       for (uint32_t m = busy_mask; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
         const uint2 km = R2(T2_SLKM + p), rdv = R2(T2_SLRD + p);
@@ -412,7 +478,7 @@ struct EnvT {
     while (avail != 0u) {
       // --- next job in (key, id) order: the first of the unpicked running jobs, or the heap's minimum
       uint2 bkm = make_uint2(0x7FFFFFFFu, 0xFFFFFFFFu); int bp = -1;
-      if (algo < MIG_ALGO_LLF) {                    // EDF keys are static: the running jobs are still in last time's order
+      if (!is_lax()) {                    // EDF keys are static: the running jobs are still in last time's order
         while ((ro & 15u) != 15u && !((rmask >> (ro & 15u)) & 1u)) ro >>= 4;
         if ((ro & 15u) != 15u) { bp = (int)(ro & 15u); bkm = R2(T2_SLKM + bp); }
       } else {
@@ -600,7 +666,7 @@ struct EnvT {
     e_ep += a.repart_energy; repartitioned = 1;
     count(C_REPART, 1u);
     emit(MIG_EV_REPART, 0xFF, ((uint32_t)old << 8) | action, MIG_NOJOB, 0);
-    if (algo >= MIG_ALGO_LLF && n_wait) {                     // laxity keys are measured against the configuration: re-key, re-sort
+    if (is_lax() && n_wait) {                     // laxity keys are measured against the configuration: re-key, re-sort
       for (uint32_t i = 0; i < n_wait; ++i) {
         const uint2 km = ld_km(i), rdv = ld_rd(i);
         st_km(i, make_uint2((uint32_t)skey_of((int)rdv.y, (int)rdv.x, m_cls(km.y)), km.y));
@@ -693,7 +759,7 @@ struct EnvT {
 
   // ------------------------------------------------------------------ init / load / save
   __device__ __forceinline__ void init(uint32_t env_local) {
-    algo = a.algo[env_local] & 3; t = 0; epoch = 0; status = 0; n_sys = 0; n_wait = 0; q_head = 0; q_ns = 0; g_head = 0; q_ng = 0;
+    algo = a.algo[env_local]; if (algo > MIG_ALGO_EDF_SS_R) algo &= 3; t = 0; epoch = 0; status = 0; n_sys = 0; n_wait = 0; q_head = 0; q_ns = 0; g_head = 0; q_ng = 0;
     h_lo = 0x84222325u; h_hi = 0xcbf29ce4u;                   // FNV-1a-64 offset basis
     uint32_t c0 = a.cfg0[env_local];
     if (c0 >= a.n_configs) { c0 = 0; status |= MIG_ST_BAD_ACTION; }

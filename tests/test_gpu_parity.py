@@ -157,6 +157,8 @@ def gpu_script(sp, rows, algo, cfg, n_envs=1, actions=None, cap_events=4096):
     ("E", [0, 1, 2, 3], (LINEAR,), dict(crit_laxity_s=5, crit_max=3)),
     ("F", [0, 2, 3], (LINEAR, SUB05), dict(crit_laxity_s=1)),
     ("G", [0, 1, 2, 3], (CAP3,), {}),
+    ("H", [4, 1], (LINEAR,), {}),
+    ("I", [4, 1], (LINEAR,), {}),
 ])
 def test_handworked_schedules_trace_equal(case, algos, speeds, kw):
     g = G[case]
@@ -287,7 +289,7 @@ def test_hourly_random_repartitions_all_algorithms(downtime, theta):
     sp = dataclasses.replace(base.params, repart_downtime_s=downtime, crit_laxity_s=theta)
     rng = np.random.default_rng(downtime + theta)
     table = rng.integers(0, 12, size=(n, 24, 4)).astype(np.uint8)
-    algo = (np.arange(n) % 4).astype(np.uint8)
+    algo = (np.arange(n) % 5).astype(np.uint8)               # EDF-FS, EDF-SS, LLF, LALF, EDF-SS with restricted preemption
     cfg0 = rng.integers(0, 12, size=n).astype(np.uint8)
     sim = B.MigSim(sp, n, 77)
     recs, tot = sim.alloc_recs(), sim.alloc_totals()
@@ -300,7 +302,7 @@ def test_hourly_random_repartitions_all_algorithms(downtime, theta):
     g_recs, g_tot = B.recs_to_numpy(recs), B.totals_to_numpy(tot)
     with cf.ProcessPoolExecutor(min(n, os.cpu_count() or 1)) as ex:
         res = list(ex.map(_oracle_custom, [(sp, 77, e, int(algo[e]), int(cfg0[e]), table[e]) for e in range(n)]))
-    assert g_tot["n_repart"].min() > 10 and (theta > 60 or g_tot["n_crit"][2::4].sum() > 0)
+    assert g_tot["n_repart"].min() > 10 and (theta > 60 or g_tot["n_crit"][2::5].sum() > 0)
     for e, o_recs, o_tot, o_trace, o_states in res:
         assert_same_records(g_recs[:, e], g_tot[e], o_recs, o_tot, "env %d algo %d" % (e, algo[e]))
     for e, o_recs, o_tot, o_trace, o_states in res[:16]:
@@ -314,6 +316,35 @@ def test_hourly_random_repartitions_all_algorithms(downtime, theta):
         s_k = state.cpu().numpy()
         for e, o_recs, o_tot, o_trace, o_states in res:
             assert np.array_equal(s_k[e], o_states[k + 1]), (e, k)
+    sim.close()
+
+
+def _oracle_static(args):
+    sp, seed, e, algo, cfg0, want_trace = args
+    r = O.rollout(sp, seed, e, algo=algo, cfg0=cfg0, trace_cap=400000 if want_trace else 0)
+    return e, r.recs, r.totals, r.trace if want_trace else None
+
+
+@pytest.mark.parametrize("name,seed", [("C2", 21), ("C5", 22)])
+def test_restricted_preemption_static_configs(name, seed):
+    # EDF-SS with restricted preemption on every configuration of Fig. 1, light and heavy load
+    n = 96
+    sp = W.CONFIGS[name](n).params
+    algo = np.full(n, 4, np.uint8)
+    cfg0 = (np.arange(n) % 12).astype(np.uint8)
+    sim = B.MigSim(sp, n, seed)
+    recs, tot = sim.alloc_recs(), sim.alloc_totals()
+    sim.reset(0, dev(algo), dev(cfg0))
+    sim.rollout(W.POLICY_STATIC, recs_out=recs, totals_out=tot)
+    torch.cuda.synchronize()
+    g_recs, g_tot = B.recs_to_numpy(recs), B.totals_to_numpy(tot)
+    with cf.ProcessPoolExecutor(min(n, os.cpu_count() or 1)) as ex:
+        res = list(ex.map(_oracle_static, [(sp, seed, e, 4, int(cfg0[e]), e < 12) for e in range(n)]))
+    for e, o_recs, o_tot, o_trace in res:
+        assert_same_records(g_recs[:, e], g_tot[e], o_recs, o_tot, "%s env %d cfg %d" % (name, e, cfg0[e]))
+        if o_trace is not None:
+            ev, t1 = sim.debug_trace(e, cap_events=400000)
+            assert len(ev) == len(o_trace) and ev.tobytes() == o_trace.tobytes(), "env %d" % e
     sim.close()
 
 
