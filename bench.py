@@ -82,11 +82,16 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ oracle arm
+_ALGO_OVERRIDE = -1
+
+
 def _oracle_chunk(args):
     name, n_envs, lo, hi = args
     from oracle import oracle as O
     from paper_2606_25082_b200 import workloads as W
     wl = W.CONFIGS[name](n_envs)
+    if _ALGO_OVERRIDE >= 0:
+        wl.algo[:] = _ALGO_OVERRIDE
     ph = O.ParamsHolder(wl.params)
     qh = O.QNetHolder(wl.qnet) if wl.qnet is not None else None
     ev = 0
@@ -160,6 +165,8 @@ def run_ours(args):
     peaks, peak_src = _peaks()
     n_envs = args.envs                                   # per GPU (weak scaling: every rank simulates a full batch)
     wl = W.CONFIGS[args.workload](n_envs)
+    if args.algo >= 0:
+        wl.algo[:] = args.algo
     sp = dataclasses.replace(wl.params, env_offset=rank * n_envs)      # Philox keyed by global env id
     sim = B.MigSim(sp, n_envs, wl.seed, tile=args.tile)
     qnet = B.QNet(wl.qnet) if wl.qnet is not None else None
@@ -269,7 +276,7 @@ def run_ours(args):
         line = {
             "metric": "job_events_per_s", "value": ev_total / t_s, "unit": "job-events/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
-            "config": {"workload": args.workload, "n_envs_per_gpu": n_envs, "n_envs_total": n_envs * world, "policy": ["static", "table", "dqn"][wl.policy], "lanes_per_env": sim.get_tile(),
+            "config": {"workload": args.workload, "n_envs_per_gpu": n_envs, "n_envs_total": n_envs * world, "policy": ["static", "table", "dqn"][wl.policy], "algo": W.ALGO_NAMES[int(wl.algo[0])] if len(set(wl.algo.tolist())) == 1 else "mixed", "lanes_per_env": sim.get_tile(),
                        "job_events_per_step": ev_total / args.steps, "l2": "flushed between iterations (256 MiB write)", "parallelism": "env-range sharding, no data-path collective"},
             "day_episodes_per_s": n_envs * world * args.steps / t_s,
             "e2e": {"value": float(e2e_ev.item()) / float(e2e_t.item()), "unit": "job-events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
@@ -291,12 +298,15 @@ def main():
     ap.add_argument("--envs", type=int, default=0, help="environments per GPU (default: the workload's BASELINE size)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--algo", type=int, default=-1, choices=[-1, 0, 1, 2, 3, 4], help="override the workload's scheduling algorithm for every env (4 = EDF-SS with restricted preemption); -1 = the workload's own")
     ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 8, 16, 32], help="lanes per environment (0 = library default: 1 = thread per environment for >= 12288 envs, else 8)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     if not args.envs:
         args.envs = {"C1": 1, "C2": 1024, "C3": 4096, "C4": 8192, "C5": 65536}[args.workload]
+    global _ALGO_OVERRIDE
+    _ALGO_OVERRIDE = args.algo                            # (worker processes are forked after this)
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 

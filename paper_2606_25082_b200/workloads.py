@@ -32,8 +32,8 @@ V7 = 840                           # work units per second on a 7g slice (divisi
 STATE_DIM = 64
 N_THR_BINS = 1440                  # one acceptance threshold per minute of the day
 
-ALGO_EDF_FS, ALGO_EDF_SS, ALGO_LLF, ALGO_LALF = 0, 1, 2, 3
-ALGO_NAMES = ("EDF-FS", "EDF-SS", "LLF", "LALF")
+ALGO_EDF_FS, ALGO_EDF_SS, ALGO_LLF, ALGO_LALF, ALGO_EDF_SS_R = 0, 1, 2, 3, 4
+ALGO_NAMES = ("EDF-FS", "EDF-SS", "LLF", "LALF", "EDF-SS-R")     # EDF-SS-R: restricted preemption
 POLICY_STATIC, POLICY_TABLE, POLICY_DQN = 0, 1, 2
 
 # PAPER.md:L75-88 (Fig. 1): (size, start slot) per slice; config ids here are 0-based (paper id - 1).
