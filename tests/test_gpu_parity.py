@@ -436,7 +436,21 @@ def test_queue_cap_overflows_shared_table_and_drops():
     assert ev.tobytes() == r.trace.tobytes() and tot.tobytes() == r.totals.tobytes()
 
 
-@pytest.mark.parametrize("algo", [0, 1, 2, 3])
+@pytest.mark.parametrize("cap", [1, 3, 13])
+def test_tiny_queue_caps(cap):
+    # caps below the shared-memory ring / table sizes: admission, drops and every algorithm still agree with the oracle
+    sp = tiny_params(speeds=(LINEAR, SUB05), cap=cap, crit_laxity_s=3)
+    rng = np.random.default_rng(cap)
+    rows = sorted((int(rng.integers(0, 400)), int(rng.integers(0, 2)), int(rng.integers(1, 30)), 0) for _ in range(120))
+    rows = [(a, c, d, a + int(rng.integers(1, 200))) for (a, c, d, _) in rows]
+    for algo in range(5):
+        ev, tot = gpu_script(sp, rows, algo, 6, cap_events=4096)
+        r = O.rollout(sp, 0, 0, algo=algo, cfg0=6, jobs=O.make_jobs(rows), trace_cap=4096)
+        assert int(tot["n_dropped"]) > 0 and int(tot["n_sys_max"]) == cap
+        assert ev.tobytes() == r.trace.tobytes() and tot.tobytes() == r.totals.tobytes(), (cap, algo)
+
+
+@pytest.mark.parametrize("algo", [0, 1, 2, 3, 4])
 def test_long_queue_all_algorithms(algo):
     # ~500 jobs in system (beyond the entries kept in shared memory), all 4 algorithms, mixed classes; the LLF / LALF
     # runs also raise several hundred critical-laxity events
