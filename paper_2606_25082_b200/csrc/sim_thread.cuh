@@ -48,6 +48,14 @@ struct HotTablesT {              // per CTA, shared memory
   uint32_t class_cum[MIG_MAX_CLASSES];    // padded with 0xFFFFFFFF beyond n_classes
 };
 
+// The generator's larger tables, copied over the (not yet used) per-thread rows while a launch pre-generates its arrivals:
+// the thinning / duration lookups sit on the dependent chain of every candidate and would otherwise be L2 round trips.
+struct GenTables {
+  uint32_t thr[MIG_THR_BINS];
+  int32_t dur7_q[MIG_MAX_CLASSES * 65];
+  uint32_t slack_lo[MIG_MAX_CLASSES], slack_span[MIG_MAX_CLASSES];
+};
+
 __host__ __device__ constexpr size_t thread_smem_bytes(uint32_t smem_entries, int nt) {
   return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * ((T2_HEAP + 2 * (size_t)smem_entries) * 8 + T1_WORDS * 4);
 }
@@ -76,6 +84,7 @@ struct EnvT {
   uint4 *arr;              // this env's arrival list (NULL: generate inline)
   uint32_t a_head, a_count, a_id0, a_more; int a_horizon;
   uint4 a_nxt;             // arr[a_head], prefetched
+  const GenTables *gt;     // the generator's tables in shared memory (valid during pre-generation only)
 
   __device__ __forceinline__ EnvT(const SimArgs &a_, const HotTablesT &h_, uint2 *r2_, uint32_t *r1_)
       : a(a_), hot(h_), r2(r2_), r1(r1_), S(a_.smem_entries) {}
@@ -291,16 +300,16 @@ struct EnvT {
   }
 
   // class, work and due date of the accepted candidate k (R5): {tick, class, work, due}
+  template <bool TS>
   __device__ __forceinline__ uint4 job_attributes(uint32_t k, uint4 w, uint32_t tick) const {
-    const DevTables *tb_ = a.tab;
     uint32_t c = 0;
 #pragma unroll
     for (int i = 0; i < MIG_MAX_CLASSES - 1; ++i) c += (w.z > hot.class_cum[i]) ? 1u : 0u;    // first c with w.z <= cum[c]
     const uint4 wd = philox4x32_10(k, 1u, env_g, a.episode, a.k0, a.k1);     // stream 1: duration
     const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
-    const int q0 = __ldg(&tb_->dur7_q[c * 65 + qi]), q1 = __ldg(&tb_->dur7_q[c * 65 + qi + 1]);
+    const int q0 = TS ? gt->dur7_q[c * 65 + qi] : __ldg(&a.tab->dur7_q[c * 65 + qi]), q1 = TS ? gt->dur7_q[c * 65 + qi + 1] : __ldg(&a.tab->dur7_q[c * 65 + qi + 1]);
     const int dur7 = q0 + (int)(((long long)(q1 - q0) * (long long)f) >> 10);
-    const uint32_t slack = __ldg(&tb_->slack_lo[c]) + __umulhi(w.w, __ldg(&tb_->slack_span[c]));
+    const uint32_t slack = (TS ? gt->slack_lo[c] : __ldg(&a.tab->slack_lo[c])) + __umulhi(w.w, TS ? gt->slack_span[c] : __ldg(&a.tab->slack_span[c]));
     unsigned long long rel = ((unsigned long long)(uint32_t)dur7 * slack) >> 10;
     if (rel < 1) rel = 1;
     return make_uint4(tick, c, (uint32_t)dur7 * hot.h.speed[c * 5 + 4].x, (uint32_t)((long long)tick + (long long)rel));
@@ -312,6 +321,7 @@ struct EnvT {
   // the inline generator below runs a lane-dependent number of trips per arrival) -- and appends the accepted ones to
   // its arrival list in global memory, from which the event loop then reads its look-ahead.  A candidate beyond the
   // horizon or the list's capacity is NOT committed (g_k, g_T stay before it), so generation resumes exactly there.
+  template <bool TS>
   __device__ __forceinline__ void fill_arrivals() {
     a_head = 0; a_count = 0; a_more = 0;
     a_id0 = n_accepted;
@@ -320,7 +330,6 @@ struct EnvT {
       a_id0 = look_id; a_count = 1; look_valid = 0;
     }
     const uint32_t limit = job_limit();
-    const DevTables *tb_ = a.tab;
     while (!g_done && n_accepted < limit) {
       const uint32_t k = g_k;
       const uint4 w = philox4x32_10(k, 0u, env_g, a.episode, a.k0, a.k1);    // stream 0: gap, accept, class, slack
@@ -330,8 +339,8 @@ struct EnvT {
       if (tick > (unsigned long long)a_horizon) break;
       if (a_count == a.arr_cap) { a_more = 1; break; }
       g_k = k + 1; g_T = T;
-      if (w.y <= __ldg(&tb_->thr[(uint32_t)tick / 60u])) {                    // Lewis-Shedler thinning
-        __stcg(&arr[a_count++], job_attributes(k, w, (uint32_t)tick));       // streamed: keep L1 for the tables
+      if (w.y <= (TS ? gt->thr[(uint32_t)tick / 60u] : __ldg(&a.tab->thr[(uint32_t)tick / 60u]))) {     // Lewis-Shedler thinning
+        __stcg(&arr[a_count++], job_attributes<TS>(k, w, (uint32_t)tick));       // streamed: keep L1 for the tables
         n_accepted++;
       }
     }
@@ -352,7 +361,7 @@ struct EnvT {
     if (arr) {                                                                // pre-generated list (kernel-uniform branch)
       if (a_head == a_count) {
         if (!a_more) return;
-        fill_arrivals();                                                      // the list was full: next stretch (rare)
+        fill_arrivals<false>();                                               // the list was full: next stretch (rare; tables in global memory)
         if (a_count == 0) return;
         a_nxt = __ldcg(&arr[0]);
       }
@@ -378,7 +387,7 @@ struct EnvT {
       if (tick >= (unsigned long long)a.day_s) { g_done = 1; return; }        // arrivals stop at the end of the day
       if (w.y <= __ldg(&tb_->thr[(uint32_t)tick / 60u])) break;               // Lewis-Shedler thinning
     }
-    const uint4 e = job_attributes(k, w, (uint32_t)tick);
+    const uint4 e = job_attributes<false>(k, w, (uint32_t)tick);
     look_tick = (int)e.x; look_cls = e.y; look_work = (int)e.z; look_due = (int)e.w;
     look_id = n_accepted++;
     look_valid = 1;
@@ -758,7 +767,9 @@ struct EnvT {
   }
 
   // ------------------------------------------------------------------ init / load / save
-  __device__ __forceinline__ void init(uint32_t env_local) {
+  // init / load come in two parts: registers first (no per-thread shared-memory row is touched: the rows' space still
+  // holds the generator's tables during pre-generation), then the rows
+  __device__ __forceinline__ void init_regs(uint32_t env_local) {
     algo = a.algo[env_local]; if (algo > MIG_ALGO_EDF_SS_R) algo &= 3; t = 0; epoch = 0; status = 0; n_sys = 0; n_wait = 0; q_head = 0; q_ns = 0; g_head = 0; q_ng = 0;
     h_lo = 0x84222325u; h_hi = 0xcbf29ce4u;                   // FNV-1a-64 offset basis
     uint32_t c0 = a.cfg0[env_local];
@@ -769,6 +780,8 @@ struct EnvT {
     look_valid = 0; look_tick = 0; look_work = 0; look_due = 0; look_cls = 0; look_id = 0;
     n_trace = 0; i_script = 0;
     for (int w = H1_DROPS; w < kHeaderWords; ++w) hdr[w] = 0u;      // running totals, drops
+  }
+  __device__ __forceinline__ void init_rows() {
     begin_span();
     update_power();
   }
@@ -787,7 +800,7 @@ struct EnvT {
     for (uint32_t p = 0; p < S; ++p) { const uint2 km = SK(p), rdv = SR(p); gtab[a.ring_cap + p] = make_uint4(km.x, km.y, rdv.x, rdv.y); }
   }
 
-  __device__ __forceinline__ void load() {
+  __device__ __forceinline__ void load_regs() {
     t = (int)hdr[H1_T];
     const uint32_t pk = hdr[H1_PK];
     epoch = pk & 0xFF; algo = (pk >> 16) & 0xFF; status = pk >> 24;
@@ -799,6 +812,8 @@ struct EnvT {
     busy_mask = hdr[H1_MASKS] & 0x7Fu; down_mask = (hdr[H1_MASKS] >> 8) & 0x7Fu; run_order = hdr[H1_ORDER];
     look_valid = (int)hdr[H1_LOOKV]; look_tick = (int)hdr[H1_LOOKTICK]; look_cls = hdr[H1_LOOKCLS];
     look_work = (int)hdr[H1_LOOKWORK]; look_due = (int)hdr[H1_LOOKDUE]; look_id = hdr[H1_LOOKID];
+  }
+  __device__ __forceinline__ void load_rows() {
     for (uint32_t p = 0; p < S; ++p) { const uint4 e = gtab[a.ring_cap + p]; SK(p) = make_uint2(e.x, e.y); SR(p) = make_uint2(e.z, e.w); }
     int nd = MIG_INF, nu = MIG_INF;
 #pragma unroll
@@ -881,24 +896,40 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
     for (int i = threadIdx.x; i < 257; i += NT) hot.logT[i] = tb->logT[i];
     if (threadIdx.x < MIG_MAX_CLASSES) hot.class_cum[threadIdx.x] = threadIdx.x < a.n_classes ? tb->class_cum[threadIdx.x] : 0xFFFFFFFFu;
   }
+  unsigned char *base = smem_raw + ((sizeof(HotTablesT) + 127) & ~(size_t)127);
+  const bool pregen = a.arr && !a.script && a.n_steps > 0;      // kernel-uniform
+  if (pregen) {
+    GenTables *g = reinterpret_cast<GenTables *>(base);
+    const DevTables *tb = a.tab;
+    for (int i = threadIdx.x; i < MIG_THR_BINS; i += NT) g->thr[i] = tb->thr[i];
+    for (int i = threadIdx.x; i < MIG_MAX_CLASSES * 65; i += NT) g->dur7_q[i] = tb->dur7_q[i];
+    if (threadIdx.x < MIG_MAX_CLASSES) { g->slack_lo[threadIdx.x] = tb->slack_lo[threadIdx.x]; g->slack_span[threadIdx.x] = tb->slack_span[threadIdx.x]; }
+  }
   __syncthreads();
   const uint32_t li = blockIdx.x * NT + threadIdx.x;            // index inside this launch's env range
-  if (li >= a.n_envs) return;
-  unsigned char *base = smem_raw + ((sizeof(HotTablesT) + 127) & ~(size_t)127);
+  const bool alive = li < a.n_envs;
   uint2 *r2 = reinterpret_cast<uint2 *>(base) + threadIdx.x;
   uint32_t *r1 = reinterpret_cast<uint32_t *>(base + (size_t)NT * (T2_HEAP + 2 * (size_t)a.smem_entries) * 8) + threadIdx.x;
   EnvT<NT, TRACE> e(a, hot, r2, r1);
-  const uint32_t env = a.env_first + li;
+  const uint32_t env = a.env_first + (alive ? li : 0u);
+  e.gt = reinterpret_cast<const GenTables *>(base);
   e.env_g = a.env_base + env;
   e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * (a.ring_cap + kThreadTabExtra);
   e.hdr = a.hdr_override ? a.hdr_override : a.hdr + (size_t)env * kHeaderWords;
   e.arr = (a.arr && !a.script) ? a.arr + (size_t)env * a.arr_cap : nullptr;
   e.a_head = 0; e.a_count = 0; e.a_id0 = 0; e.a_more = 0;
-  if (a.from_init) e.init(env); else e.load();
-  if (a.n_steps > 0 && e.epoch < a.n_epochs) {
-    if (e.arr) {                                                // arrivals up to the end of the last epoch of this launch
+  if (alive) {
+    if (a.from_init) e.init_regs(env); else e.load_regs();
+    if (pregen && e.epoch < a.n_epochs) {                       // arrivals up to the end of the last epoch of this launch
       e.a_horizon = min(e.epoch + a.n_steps, a.n_epochs) * a.epoch_s;
-      e.fill_arrivals();
+      e.template fill_arrivals<true>();
+    }
+  }
+  __syncthreads();                                              // the tables make room for the per-thread rows
+  if (!alive) return;
+  if (a.from_init) e.init_rows(); else e.load_rows();
+  if (a.n_steps > 0 && e.epoch < a.n_epochs) {
+    if (e.arr) {
       if (e.a_count) e.a_nxt = __ldcg(&e.arr[0]);
       e.gen_next();
     } else if (!e.look_valid) e.gen_next();                     // prime the inline generator's look-ahead
