@@ -172,9 +172,9 @@ static int configure_tile(mig_sim *s, int tile) {
   const uint32_t cap4 = (s->p.cap + 3u) & ~3u, cap8 = (s->p.cap + 7u) & ~7u;
   uint32_t entries; size_t bytes; int threads;
   if (tile == 1) {
-    // 12 heap entries in shared memory per environment: 456 B per thread, 7 CTAs of 64 threads per SM = 448 resident
+    // 11 ring slots of the waiting queue in shared memory per environment: 456 B per thread, 7 CTAs of 64 threads per SM = 448 resident
     // environments per SM (66 304 per B200: BASELINE C5's 65 536 run as ONE resident wave)
-    entries = cap4 < 12u ? cap4 : 12u; threads = kThreadCta;
+    entries = cap4 < 11u ? cap4 : 11u; threads = kThreadCta;
     bytes = thread_smem_bytes(entries, kThreadCta);
   } else {
     entries = cap8 < 64u ? cap8 : 64u; threads = kWarpsPerCta * 32;

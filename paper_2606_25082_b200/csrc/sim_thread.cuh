@@ -57,7 +57,7 @@ struct GenTables {
 };
 
 __host__ __device__ constexpr size_t thread_smem_bytes(uint32_t smem_entries, int nt) {
-  return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * ((T2_HEAP + 2 * (size_t)smem_entries) * 8 + T1_WORDS * 4);
+  return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * ((T2_HEAP + 2 * (size_t)smem_entries) * 8 + T1_WORDS * 4 + 16);   // + one 16-byte landing slot
 }
 
 template <int NT, bool TRACE>
@@ -83,7 +83,7 @@ struct EnvT {
   uint32_t n_trace, i_script, n_events;
   uint4 *arr;              // this env's arrival list (NULL: generate inline)
   uint32_t a_head, a_count, a_id0, a_more; int a_horizon;
-  uint4 a_nxt;             // arr[a_head], prefetched
+  uint4 *a_slot;           // shared-memory landing slot of the asynchronous copy of arr[a_head] (cp.async)
   const GenTables *gt;     // the generator's tables in shared memory (valid during pre-generation only)
 
   __device__ __forceinline__ EnvT(const SimArgs &a_, const HotTablesT &h_, uint2 *r2_, uint32_t *r1_)
@@ -346,6 +346,13 @@ struct EnvT {
     }
   }
 
+  // start the asynchronous copy of arr[a_head] into this thread's landing slot (LDGSTS: no register waits for it)
+  __device__ __forceinline__ void fetch_arrival() {
+    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(a_slot);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n\tcp.async.commit_group;" ::"r"(dst), "l"(arr + a_head) : "memory");
+    if ((a_head & 7u) == 0u && a_head + 8u < a_count) asm volatile("prefetch.global.L2 [%0];" ::"l"(arr + a_head + 8));   // next 128-byte line
+  }
+
   // advance the look-ahead to the next accepted arrival (or none)
   __device__ __forceinline__ void gen_next() {
     look_valid = 0;
@@ -363,16 +370,14 @@ struct EnvT {
         if (!a_more) return;
         fill_arrivals<false>();                                               // the list was full: next stretch (rare; tables in global memory)
         if (a_count == 0) return;
-        a_nxt = __ldcg(&arr[0]);
+        fetch_arrival();
       }
-      const uint4 e = a_nxt;                                                  // loaded one arrival ago: its latency is hidden
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      const uint4 e = *a_slot;                                                // copied one arrival ago: its latency is hidden
       look_tick = (int)e.x; look_cls = e.y; look_work = (int)e.z; look_due = (int)e.w;
       look_id = a_id0 + a_head++;
       look_valid = 1;
-      if (a_head < a_count) {
-        a_nxt = __ldcg(&arr[a_head]);
-        if ((a_head & 7u) == 0u && a_head + 8u < a_count) asm volatile("prefetch.global.L2 [%0];" ::"l"(arr + a_head + 8));   // next 128-byte line
-      }
+      if (a_head < a_count) fetch_arrival();
       return;
     }
     if (n_accepted >= job_limit()) return;
@@ -911,6 +916,7 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   uint2 *r2 = reinterpret_cast<uint2 *>(base) + threadIdx.x;
   uint32_t *r1 = reinterpret_cast<uint32_t *>(base + (size_t)NT * (T2_HEAP + 2 * (size_t)a.smem_entries) * 8) + threadIdx.x;
   EnvT<NT, TRACE> e(a, hot, r2, r1);
+  e.a_slot = reinterpret_cast<uint4 *>(base + (size_t)NT * ((T2_HEAP + 2 * (size_t)a.smem_entries) * 8 + T1_WORDS * 4)) + threadIdx.x;
   const uint32_t env = a.env_first + (alive ? li : 0u);
   e.gt = reinterpret_cast<const GenTables *>(base);
   e.env_g = a.env_base + env;
@@ -930,7 +936,7 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   if (a.from_init) e.init_rows(); else e.load_rows();
   if (a.n_steps > 0 && e.epoch < a.n_epochs) {
     if (e.arr) {
-      if (e.a_count) e.a_nxt = __ldcg(&e.arr[0]);
+      if (e.a_count) e.fetch_arrival();
       e.gen_next();
     } else if (!e.look_valid) e.gen_next();                     // prime the inline generator's look-ahead
   }
