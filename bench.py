@@ -32,7 +32,7 @@ if ROOT not in sys.path:
 ALG_THREAD_INSTR_PER_JOB_EVENT = 316.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE rollout launch from the ncu --set full capture in profiles/
 # (per launch like `achieved`); None where no capture of that launch configuration exists.
-NCU_DRAM_BYTES_PER_LAUNCH = {("C5", 65536, 1): 10.19e9 + 9.62e9}
+NCU_DRAM_BYTES_PER_LAUNCH = {("C5", 65536, 1): 9.90e9 + 9.61e9}
 CPU_SAMPLE_ENVS = 2048
 
 
