@@ -381,6 +381,26 @@ def test_thread_kernel_arrival_lists_of_any_capacity_give_the_same_day(entries):
         sim.close()
 
 
+@pytest.mark.parametrize("algo", [None, 4])
+def test_c5_full_size_every_env_agrees_between_kernel_families(algo):
+    # the two kernel families are independent implementations (warp tiles with an unordered table and argmin passes;
+    # one thread per env with a sorted queue and pre-generated arrivals): every record and every trace hash of all
+    # 65 536 env-days of BASELINE C5 must agree (the oracle checks a sample of the same days in test_c5_full_size_sampled)
+    if B.DEFAULT_TILE != 1:
+        pytest.skip("runs once")
+    wl = W.CONFIGS["C5"](65536)
+    if algo is not None:
+        wl.algo[:] = algo                                     # EDF-SS with restricted preemption
+    out = []
+    for tile in (1, 8):
+        sim, recs, tot, _ = gpu_rollout(wl, sim=B.MigSim(wl.params, 65536, wl.seed, tile=tile))
+        out.append((recs, tot))
+        sim.close()
+    assert out[0][1].tobytes() == out[1][1].tobytes()
+    assert out[0][0].tobytes() == out[1][0].tobytes()
+    assert len(np.unique(out[0][1]["trace_hash"])) == 65536
+
+
 def test_set_tile_between_kernel_families_needs_a_reset():
     wl = W.config_c3(32)
     sim = B.MigSim(wl.params, 32, wl.seed, tile=8)
