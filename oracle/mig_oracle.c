@@ -114,6 +114,8 @@ struct orc_env {
   uint32_t last_epoch_drops;
   /* trace */
   orc_event_t *trace; uint32_t trace_cap, n_trace;
+  /* event-driven decisions (reading #27): this env's table [n_epochs][4], or NULL */
+  const uint8_t *ev_table;
 };
 
 static void *dup_mem(const void *src, size_t n) { void *d = malloc(n ? n : 1); if (n) memcpy(d, src, n); return d; }
@@ -419,6 +421,8 @@ static void remove_job(orc_env_t *e, uint32_t idx)
 }
 
 /* ---------------------------------------------------------------------------------------------- event loop */
+static void repartition(orc_env_t *e, uint8_t action);
+
 static void run_until(orc_env_t *e, int32_t t_end, int drain)
 {
   for (;;) {
@@ -444,7 +448,7 @@ static void run_until(orc_env_t *e, int32_t t_end, int drain)
     }
     e->t = (int32_t)tn;
     /* 3. same-tick order (reading #10): completions, slice-ups, arrivals, critical laxity, then ONE reschedule */
-    int happened = 0;
+    int happened = 0, job_event = 0;
     for (int p = 0; p < ORC_SLOTS; ++p) {                                   /* (i) completions, ascending slot */
       slice_t *s = &e->sl[p];
       if (!s->size || s->job == NONE_JOB) continue;
@@ -456,7 +460,7 @@ static void run_until(orc_env_t *e, int32_t t_end, int drain)
       if (tard > 0) { e->ep.n_tardy++; e->tot.n_tardy++; }
       s->job = NONE_JOB;
       remove_job(e, (uint32_t)(j - e->jobs));
-      happened = 1;
+      happened = 1; job_event = 1;
     }
     for (int p = 0; p < ORC_SLOTS; ++p) {                                   /* (ii) slices coming up */
       slice_t *s = &e->sl[p];
@@ -475,7 +479,7 @@ static void run_until(orc_env_t *e, int32_t t_end, int drain)
         if (e->n_sys > e->ep.n_sys_max) e->ep.n_sys_max = e->n_sys;
         if (e->n_sys > e->tot.n_sys_max) e->tot.n_sys_max = e->n_sys;
       }
-      happened = 1;
+      happened = 1; job_event = 1;
       gen_next(e);
     }
     for (uint32_t i = 0; i < e->n_sys; ++i) {                              /* (iv) critical laxity, ascending id */
@@ -486,6 +490,15 @@ static void run_until(orc_env_t *e, int32_t t_end, int drain)
         e->ep.n_crit++; e->tot.n_crit++;
         happened = 1;
       }
+    }
+    /* Event-driven decision ("re-partitioning can happen when a job arrives or is completed"; reading
+     * #27): after a tick of the day in which a job arrived or completed, the tabulated policy is looked up again with
+     * the load bucket of that moment; a different configuration is a repartition at this very tick (it reschedules). */
+    if (job_event && e->ev_table && !drain) {
+      uint32_t n = e->n_sys; int b = n == 0 ? 0 : (n < 8 ? 1 : (n < 64 ? 2 : 3));
+      uint8_t action = e->ev_table[e->epoch * 4 + b];
+      if (action >= e->p.n_configs) e->status |= ORC_ST_BAD_ACTION;
+      else if ((int)action != e->cfg) { repartition(e, action); happened = 0; }
     }
     if (happened) reschedule(e);                                           /* (v) */
     if (e->t == t_end) break;
@@ -498,6 +511,12 @@ static void prologue(orc_env_t *e, uint8_t action)
   e->ep.repartitioned = 0;
   if (action >= e->p.n_configs) { e->status |= ORC_ST_BAD_ACTION; return; }
   if ((int)action == e->cfg) return;                      /* "remain on the current configuration": no cost, no event */
+  repartition(e, action);
+}
+
+/* action is a valid configuration other than the current one */
+static void repartition(orc_env_t *e, uint8_t action)
+{
   const uint8_t *row = &e->size_at_slot[(uint32_t)action * 7];
   for (int p = 0; p < ORC_SLOTS; ++p) {                   /* destroyed slices, ascending slot: running job goes back to waiting */
     slice_t *s = &e->sl[p];
@@ -667,6 +686,7 @@ int orc_rollout(const orc_params_t *p, uint64_t seed, uint32_t env_id, uint32_t 
   if (jobs) orc_env_set_jobs(e, jobs, n_jobs);
   if (trace_buf) orc_env_set_trace(e, trace_buf, trace_cap);
   orc_env_reset(e, episode, algo, cfg0);
+  e->ev_table = (policy == ORC_POLICY_TABLE && p->decide_on_events) ? table : NULL;
   float x[ORC_STATE_DIM];
   orc_env_observe(e, x);
   double et = (double)epsilon * 4294967296.0;

@@ -56,6 +56,7 @@ typedef struct {
   int32_t crit_laxity_s;
   uint32_t crit_max;
   float w_energy, w_tardy;
+  uint32_t decide_on_events;    /* TABLE policy: also decide after every tick with an arrival or a completion */
 } orc_params_t;
 
 typedef struct { int32_t arr; uint32_t cls; int32_t dur7; int32_t due; } orc_job_in_t;

@@ -44,6 +44,7 @@ class _Params(C.Structure):
         ("repart_downtime_s", C.c_int32), ("repart_energy_mj", C.c_int64),
         ("crit_laxity_s", C.c_int32), ("crit_max", C.c_uint32),
         ("w_energy", C.c_float), ("w_tardy", C.c_float),
+        ("decide_on_events", C.c_uint32),
     ]
 
 
@@ -113,6 +114,7 @@ class ParamsHolder:
         s.repart_downtime_s, s.repart_energy_mj = sp.repart_downtime_s, sp.repart_energy_mj
         s.crit_laxity_s, s.crit_max = sp.crit_laxity_s, sp.crit_max
         s.w_energy, s.w_tardy = sp.w_energy, sp.w_tardy
+        s.decide_on_events = int(getattr(sp, "decide_on_events", 0))
         self.c = s
 
     @property

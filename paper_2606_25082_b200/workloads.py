@@ -164,6 +164,7 @@ class SimParams:
     w_energy: float = 0.5
     w_tardy: float = 0.5
     env_offset: int = 0
+    decide_on_events: int = 0    # TABLE policy: also decide after every tick with an arrival or a completion
 
     @property
     def n_classes(self) -> int:

@@ -183,6 +183,30 @@ def test_I_restricted_preemption_fallback_wait_and_no_eviction_of_earlier_deadli
     assert int(r.totals["n_preempt"]) == g["n_preempt"] and int(r.totals["tardiness_s"]) == g["tardiness_s"]
 
 
+def _table_J(g):
+    t = np.zeros((24, 4), np.uint8)
+    t[:, 0] = g["table"]["bucket0"]; t[:, 1:] = g["table"]["bucket1_3"]
+    return t
+
+
+def test_J_event_driven_decisions_repartition_at_arrival_and_completion():
+    import dataclasses
+    from util import EV_NAMES
+    g = G["J"]
+    sp = dataclasses.replace(tiny_params(repart_downtime_s=g["downtime_s"], repart_energy_mj=g["repart_energy_mj"]), decide_on_events=1)
+    jobs = O.make_jobs(g["jobs"])
+    r = O.rollout(sp, 0, 0, algo=g["algo"], cfg0=g["cfg0"], policy=W.POLICY_TABLE, table=_table_J(g), jobs=jobs, trace_cap=64)
+    trace_check.check_against_records(sp, g["cfg0"], r.trace, r.recs, r.totals, jobs_in=jobs)
+    assert [[int(e["t"]), EV_NAMES[int(e["type"])], int(e["job"]), int(e["slot"])] for e in r.trace] == g["events"]
+    assert [int(e["aux"]) for e in r.trace if e["type"] == 8] == g["repart_aux"]
+    assert int(r.recs[0]["energy_mj"]) == g["epoch0_energy_mj"]
+    assert int(r.totals["n_repart"]) == g["n_repart"] and int(r.recs[0]["repartitioned"]) == 1 and int(r.recs[0]["cfg"]) == g["cfg0"]
+    # without the flag the table is consulted at epoch starts only: the system is empty then, nothing ever changes
+    sp0 = dataclasses.replace(sp, decide_on_events=0)
+    r0 = O.rollout(sp0, 0, 0, algo=g["algo"], cfg0=g["cfg0"], policy=W.POLICY_TABLE, table=_table_J(g), jobs=jobs, trace_cap=64)
+    assert int(r0.totals["n_repart"]) == 0
+
+
 def test_speed_tables_match_survey_values():
     assert LINEAR == [120, 240, 360, 480, 840]
     assert SUB05 == [317, 449, 550, 635, 840]

@@ -121,6 +121,32 @@ def test_restricted_preemption_with_repartitions_keeps_the_invariants():
     assert int(r.totals["n_repart"]) > 10 and int(r.totals["n_jobs"]) == int(r.totals["n_completed"]) + int(r.totals["n_dropped"])
 
 
+def test_event_driven_decisions_with_a_load_blind_table_equal_hourly_decisions():
+    # reading #27: a table whose four load buckets agree gives the same action at every event of an epoch as at its
+    # start, so the event-driven run must be the hourly run, event for event
+    import dataclasses
+    wl = W.config_c3(4)
+    for e in range(3):
+        a = O.rollout(wl.params, 3, e, algo=1, cfg0=int(wl.cfg0[e]), policy=W.POLICY_TABLE, table=wl.table[e], trace_cap=100000)
+        b = O.rollout(dataclasses.replace(wl.params, decide_on_events=1), 3, e, algo=1, cfg0=int(wl.cfg0[e]), policy=W.POLICY_TABLE,
+                      table=wl.table[e], trace_cap=100000)
+        assert int(a.totals["n_repart"]) == 2 and a.trace.tobytes() == b.trace.tobytes() and a.recs.tobytes() == b.recs.tobytes()
+
+
+@pytest.mark.parametrize("algo", [1, 2, 4])
+def test_event_driven_decisions_keep_the_invariants(algo):
+    import dataclasses
+    wl = W.config_c3(4)
+    sp = dataclasses.replace(wl.params, decide_on_events=1, repart_downtime_s=4, repart_energy_mj=1000)
+    table = np.random.default_rng(algo).integers(0, 12, size=(24, 4)).astype(np.uint8)
+    r = O.rollout(sp, 9, 1, algo=algo, cfg0=3, policy=W.POLICY_TABLE, table=table, trace_cap=400000)
+    assert int(r.totals["status"]) == 0 and int(r.totals["n_repart"]) > 100       # the load crosses bucket borders all day
+    trace_check.check_against_records(sp, 3, r.trace, r.recs, r.totals)
+    rep = [int(ev["t"]) for ev in r.trace if ev["type"] == 8 and ev["t"] % 3600 != 0]
+    job_ticks = {int(ev["t"]) for ev in r.trace if ev["type"] in (1, 2, 5)}
+    assert rep and all(t in job_ticks for t in rep)                                # only where a job arrived or completed
+
+
 @pytest.mark.parametrize("cfg", [0, 4])
 def test_uniform_slice_configs_make_variants_coincide(cfg):
     # "configurations 1 and 5 ... the EDF variants produce the same value, as do the LLF variants"
