@@ -92,6 +92,11 @@ typedef struct {
   uint32_t crit_max;            /* max critical-laxity preemptions per job (paper: 3), <= 15 */
   float w_energy, w_tardy;      /* reward weights: r = -(w_energy * dE + w_tardy * dT) */
   uint32_t env_base;            /* global id of local env 0 (multi-GPU sharding: Philox is keyed by global env id) */
+  uint32_t decide_on_events;    /* 0: the policy decides at epoch starts only.  1: with the TABLE policy of mig_sim_rollout /
+                                 * mig_sim_debug_trace the table is looked up again (row of the current epoch, load bucket of that
+                                 * moment) after every tick of the day in which a job arrived or completed; a different
+                                 * configuration is a repartition at that tick ("re-partitioning can happen when a
+                                 * job arrives or is completed"; reading #27).  Ignored by mig_sim_step. */
 } mig_params_t;
 
 /* One record per env per epoch (index n_epochs = the drain).  64 bytes. */

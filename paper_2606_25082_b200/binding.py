@@ -54,7 +54,7 @@ class _Params(C.Structure):
         ("cap", C.c_uint32), ("job_limit", C.c_uint32),
         ("repart_downtime_s", C.c_int32), ("repart_energy_mj", C.c_int64),
         ("crit_laxity_s", C.c_int32), ("crit_max", C.c_uint32),
-        ("w_energy", C.c_float), ("w_tardy", C.c_float), ("env_base", C.c_uint32),
+        ("w_energy", C.c_float), ("w_tardy", C.c_float), ("env_base", C.c_uint32), ("decide_on_events", C.c_uint32),
     ]
 
 
@@ -143,6 +143,7 @@ def _fill_params(sp: SimParams) -> tuple[_Params, tuple]:
     s.repart_downtime_s, s.repart_energy_mj = sp.repart_downtime_s, sp.repart_energy_mj
     s.crit_laxity_s, s.crit_max = sp.crit_laxity_s, sp.crit_max
     s.w_energy, s.w_tardy, s.env_base = sp.w_energy, sp.w_tardy, sp.env_offset
+    s.decide_on_events = int(sp.decide_on_events)
     return s, keep
 
 

@@ -157,9 +157,9 @@ constexpr uint32_t kThreadKernelMinEnvs = 12288;
 static int default_tile(uint32_t n_envs) { return n_envs >= kThreadKernelMinEnvs ? 1 : 8; }
 
 template <bool TRACE>
-static const void *kernel_ptr(int tile) {
+static const void *kernel_ptr(int tile, bool evd = false) {
   switch (tile) {
-    case 1: return (const void *)sim_thread_kernel<kThreadCta, TRACE>;
+    case 1: return evd ? (const void *)sim_thread_kernel<kThreadCta, TRACE, true> : (const void *)sim_thread_kernel<kThreadCta, TRACE, false>;
     case 8: return (const void *)sim_kernel<8, TRACE>;
     case 16: return (const void *)sim_kernel<16, TRACE>;
     default: return (const void *)sim_kernel<32, TRACE>;
@@ -181,15 +181,16 @@ static int configure_tile(mig_sim *s, int tile) {
     bytes = ((sizeof(HotTables) + 127) & ~(size_t)127) + (size_t)kWarpsPerCta * (32 / tile) * tile_smem_bytes(entries);
   }
   int occ = 0;
-  for (int trace = 0; trace < 2; ++trace) {
-    const void *k = trace ? kernel_ptr<true>(tile) : kernel_ptr<false>(tile);
+  for (int v = 0; v < (tile == 1 ? 4 : 2); ++v) {          // every instantiation that a launch may pick
+    const int trace = v & 1;
+    const void *k = trace ? kernel_ptr<true>(tile, v >= 2) : kernel_ptr<false>(tile, v >= 2);
     if (bytes > 48 * 1024 && cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess)
       return fail(MIG_ECUDA, "set_tile: %zu bytes of shared memory per CTA refused (%s)", bytes, cudaGetErrorString(cudaGetLastError()));
     if (tile == 1) cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     int o = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k, threads, bytes) != cudaSuccess || o < 1)
       return fail(MIG_ECUDA, "set_tile: the rollout kernel does not fit this device (%s)", cudaGetErrorString(cudaGetLastError()));
-    if (!trace) occ = o;
+    if (v == 0) occ = o;
   }
   if ((tile == 1) != (s->tile == 1)) s->epoch = -1;      // the saved per-env state has another layout: reset first
   s->tile = tile; s->smem_entries = entries; s->smem_bytes = bytes; s->grid_max = occ * s->n_sm;
@@ -308,7 +309,8 @@ static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
     SimArgs b = a;
     b.arr = s->arr_want ? s->d_arr : nullptr; b.arr_cap = s->arr_cap;
     const dim3 grid((b.n_envs + kThreadCta - 1) / kThreadCta), block(kThreadCta);
-    sim_thread_kernel<kThreadCta, TRACE><<<grid, block, s->smem_bytes, st>>>(b);
+    if (b.ev_decide) sim_thread_kernel<kThreadCta, TRACE, true><<<grid, block, s->smem_bytes, st>>>(b);
+    else sim_thread_kernel<kThreadCta, TRACE, false><<<grid, block, s->smem_bytes, st>>>(b);
     CU(cudaGetLastError());
     s->launches++;
     return MIG_OK;
@@ -384,6 +386,7 @@ extern "C" int mig_sim_rollout(mig_sim_t *s, int policy, const uint8_t *table, c
   if (policy != MIG_POLICY_DQN) {
     SimArgs a; base_args(s, a);
     a.save = 1; a.n_steps = ne - s->epoch; a.policy = policy; a.table = table;
+    a.ev_decide = policy == MIG_POLICY_TABLE && s->p.decide_on_events;
     a.recs = recs_out; a.rec_k0 = 0; a.drain_rec = recs_out ? recs_out + (size_t)ne * s->n_envs : nullptr;
     a.totals = totals_out;
     int rc = launch_sim<false>(s, a, st);
@@ -510,7 +513,7 @@ extern "C" int mig_sim_debug_trace(mig_sim_t *s, uint32_t env, int policy, const
   a.n_envs = 1; a.env_first = env; a.tab_override = s->d_dbgtab; a.hdr_override = s->d_dbghdr;
   a.from_init = 1; a.save = 0; a.n_steps = s->p.n_epochs;
   if (actions) { a.policy = 3; a.actions = actions; a.act_stride_env = 0; a.act_stride_k = 1; }
-  else { a.policy = policy; a.table = table; }
+  else { a.policy = policy; a.table = table; a.ev_decide = policy == MIG_POLICY_TABLE && s->p.decide_on_events; }
   a.trace = buf; a.trace_cap = buf ? cap_events : 0; a.trace_n = n_out; a.totals = totals_out;
   return launch_sim<true>(s, a, (cudaStream_t)stream);
 }

@@ -54,6 +54,7 @@ struct SimArgs {
   int policy;           // 0 static, 1 table, 3 explicit actions
   const uint8_t *algo, *cfg0;                        // from_init
   const uint8_t *table;                              // [n_envs][n_epochs][4]
+  int ev_decide;                                     // TABLE policy: look the table up again after every tick with an arrival or a completion
   const uint8_t *actions; uint32_t act_stride_env, act_stride_k;   // action = actions[env * se + (k - k_first) * sk]
   const mig_job_t *script; uint32_t n_script;
   uint4 *arr; uint32_t arr_cap;                      // thread-per-env kernel: pre-generated arrival lists [n_envs][arr_cap] {tick, class, work, due}, or NULL

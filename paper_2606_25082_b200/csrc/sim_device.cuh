@@ -131,6 +131,7 @@ struct Env {
   uint4 *gtab;             // overflow part (and save area) in global memory, indexed by the same entry index
   const int lane, gl, gshift;   // warp lane, tile lane, first warp lane of the tile
   bool alive;              // the tile holds an environment
+  uint32_t env_l;          // its index in the handle's arrays
   uint32_t env_g;          // global env id (Philox counter word)
   // tile-uniform
   int t, epoch, cfg, algo; uint32_t status, n_sys, cfg_sizes;
@@ -546,6 +547,7 @@ struct Env {
       // 3. same-tick order (reading #10): completions, slice-ups, arrivals, critical laxity, then ONE reschedule
       bool happened = false;
       uint32_t cm = T::tballot(running && sl_pos >= 0 && rj_rem <= 0, gshift);
+      bool job_event = cm != 0u;                                  // a job completed or arrived at this tick
       while (MIG_ANY(cm != 0u)) {                                   // (i) completions, ascending slot
         const bool has = cm != 0u;
         int p = __ffs((int)cm) - 1;
@@ -584,7 +586,7 @@ struct Env {
         }
         emit(arr, drop ? MIG_EV_DROP : MIG_EV_ARRIVE, 0xFF, look_cls, look_id, look_due);
         count_max<C_SYSMAX>(ins ? n_sys : 0u);
-        happened |= arr;
+        happened |= arr; job_event |= arr;
         gen_next(arr);
       }
       __syncwarp();
@@ -617,6 +619,18 @@ struct Env {
           happened |= scan;
         }
       }
+      if (a.ev_decide && !drain) {                            // event-driven decision (reading #27)
+        const bool dec = running && job_event;
+        uint32_t action = (uint32_t)cfg;
+        if (dec) {
+          const uint32_t b = n_sys == 0 ? 0u : (n_sys < 8 ? 1u : (n_sys < 64 ? 2u : 3u));
+          action = a.table[((size_t)env_l * a.n_epochs + epoch) * 4 + b];
+        }
+        const bool bad = dec && action >= a.n_configs;
+        if (bad) status |= MIG_ST_BAD_ACTION;
+        const bool rp = dec && !bad && (int)action != cfg;
+        if (MIG_ANY(rp)) { repartition(rp, action); happened = happened && !rp; }   // (it reschedules those tiles)
+      }
       if (MIG_ANY(happened)) reschedule(happened);            // (v)
       running = running && t != t_end && !(drain && n_sys == 0);
     }
@@ -629,6 +643,10 @@ struct Env {
     if (bad) status |= MIG_ST_BAD_ACTION;
     const bool rp = alive && !bad && (int)action != cfg;      // "remain on the current configuration": no cost, no event
     if (!MIG_ANY(rp)) return;
+    repartition(rp, action);
+  }
+  // tiles with rp change to the valid configuration `action` (tile-uniform, != cfg); ends with ONE reschedule of those tiles
+  __device__ __forceinline__ void repartition(const bool rp, uint32_t action) {
     const uint32_t newsizes = hot.cfg_pack[action & (MIG_MAX_CONFIGS - 1)];
     const int mynew = gl < kSlots ? (int)((newsizes >> (4 * gl)) & 15u) : 0;
     const bool destroyed = rp && sl_size && sl_size != mynew;
@@ -956,7 +974,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) sim_kernel(const SimArgs
     const uint32_t li = idx * NG + (uint32_t)(lane / G);      // index inside this launch's env range
     e.alive = li < a.n_envs;
     const uint32_t env = a.env_first + (e.alive ? li : 0u);   // idle tiles shadow a valid env and never write
-    e.env_g = a.env_base + env;
+    e.env_g = a.env_base + env; e.env_l = env;
     e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * a.cap;
     if (a.from_init) e.init(env); else e.load(env);
     for (int s = 0; s < a.n_steps && e.epoch < a.n_epochs; ++s) {

@@ -60,7 +60,7 @@ __host__ __device__ constexpr size_t thread_smem_bytes(uint32_t smem_entries, in
   return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * ((T2_HEAP + 2 * (size_t)smem_entries) * 8 + T1_WORDS * 4 + 16);   // + one 16-byte landing slot
 }
 
-template <int NT, bool TRACE>
+template <int NT, bool TRACE, bool EVD>     // EVD: event-driven decisions of the tabulated policy compiled in (reading #27)
 struct EnvT {
   // ------------------------------------------------------------------ environment state
   const SimArgs &a;
@@ -81,6 +81,7 @@ struct EnvT {
   uint32_t g_k, g_done, n_accepted; unsigned long long g_T;
   int look_valid, look_tick, look_work, look_due; uint32_t look_cls, look_id;
   uint32_t n_trace, i_script, n_events;
+  uint32_t env_l; bool in_drain;   // env index in the handle's arrays; the drain after the last epoch is running
   uint4 *arr;              // this env's arrival list (NULL: generate inline)
   uint32_t a_head, a_count, a_id0, a_more; int a_horizon;
   uint4 *a_slot;           // shared-memory landing slot of the asynchronous copy of arr[a_head] (cp.async)
@@ -584,7 +585,7 @@ struct EnvT {
         R2(T2_SLRD + p).x = (uint32_t)rem;
         if (rem <= 0) done |= 1u << p;
       }
-    bool happened = false;
+    bool happened = false, job_event = done != 0u;
     for (; done; done &= done - 1) {                                  // (i) completions, ascending slot
       const int p = __ffs((int)done) - 1;
       const int tard = max(t - (int)R2(T2_SLRD + p).y, 0);            // l_j = max(c_j - d_j, 0)
@@ -618,7 +619,7 @@ struct EnvT {
         if (n_sys > R1(T1_CNT + C_SYSMAX)) R1(T1_CNT + C_SYSMAX) = n_sys;
       }
       emit(drop ? MIG_EV_DROP : MIG_EV_ARRIVE, 0xFF, look_cls, look_id, look_due);
-      happened = true;
+      happened = true; job_event = true;
       gen_next();
     }
     if (next_crit == t) {                                             // (iv) critical laxity, ascending id
@@ -640,6 +641,14 @@ struct EnvT {
         happened = true;
       }
     }
+    // event-driven decision (reading #27): after a tick of the day with an arrival or a
+    // completion the tabulated policy is looked up with the load bucket of this moment
+    if (EVD && a.ev_decide && job_event && !in_drain) {
+      const uint32_t b = n_sys == 0 ? 0u : (n_sys < 8 ? 1u : (n_sys < 64 ? 2u : 3u));
+      const uint32_t action = a.table[((size_t)env_l * a.n_epochs + epoch) * 4 + b];
+      if (action >= a.n_configs) status |= MIG_ST_BAD_ACTION;
+      else if ((int)action != cfg) { repartition(action); return; }   // (it reschedules)
+    }
     if (happened) reschedule();                                       // (v)
   }
 
@@ -648,6 +657,10 @@ struct EnvT {
     repartitioned = 0;
     if (action >= a.n_configs) { status |= MIG_ST_BAD_ACTION; return; }
     if ((int)action == cfg) return;                           // "remain on the current configuration": no cost, no event
+    repartition(action);
+  }
+  // action is a valid configuration other than the current one; ends with ONE reschedule
+  __device__ __forceinline__ void repartition(uint32_t action) {
     const uint32_t newsizes = hot.h.cfg_pack[action];
     uint32_t changed = 0;                                     // slots whose (start, size) differs between the two rows
 #pragma unroll
@@ -846,10 +859,11 @@ struct EnvT {
     if (steps_left <= 0 || epoch >= a.n_epochs) return;
     const uint32_t out_i = TRACE ? 0u : env;
     bool drain = false, fresh = true;
+    in_drain = false;
     long long dE = 0, dT = 0;
     for (int s = 0;;) {
       if (fresh) {                                            // ---- the next decision epoch begins
-        fresh = false; drain = false; dE = 0; dT = 0;
+        fresh = false; drain = false; in_drain = false; dE = 0; dT = 0;
         uint32_t action = (uint32_t)cfg;                                            // STATIC: stay
         if (a.policy == MIG_POLICY_TABLE) {                                         // load bucket
           const uint32_t b = n_sys == 0 ? 0u : (n_sys < 8 ? 1u : (n_sys < 64 ? 2u : 3u));
@@ -868,7 +882,7 @@ struct EnvT {
         hdr[H1_DROPS] = R1(T1_CNT + C_DROPPED);
         close_record(a.recs ? a.recs + (size_t)(epoch - a.rec_k0) * a.rec_stride + out_i : nullptr);
         if (epoch == a.n_epochs - 1) {                        // 4. drain (reading #11): energy stops at the last completion
-          drain = true; begin_span(); t_end = a.t_limit_s;
+          drain = true; in_drain = true; begin_span(); t_end = a.t_limit_s;
           continue;
         }
       } else {
@@ -887,7 +901,7 @@ struct EnvT {
   }
 };
 
-template <int NT, bool TRACE>
+template <int NT, bool TRACE, bool EVD>
 __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   HotTablesT &hot = *reinterpret_cast<HotTablesT *>(smem_raw);
@@ -915,11 +929,11 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   const bool alive = li < a.n_envs;
   uint2 *r2 = reinterpret_cast<uint2 *>(base) + threadIdx.x;
   uint32_t *r1 = reinterpret_cast<uint32_t *>(base + (size_t)NT * (T2_HEAP + 2 * (size_t)a.smem_entries) * 8) + threadIdx.x;
-  EnvT<NT, TRACE> e(a, hot, r2, r1);
+  EnvT<NT, TRACE, EVD> e(a, hot, r2, r1);
   e.a_slot = reinterpret_cast<uint4 *>(base + (size_t)NT * ((T2_HEAP + 2 * (size_t)a.smem_entries) * 8 + T1_WORDS * 4)) + threadIdx.x;
   const uint32_t env = a.env_first + (alive ? li : 0u);
   e.gt = reinterpret_cast<const GenTables *>(base);
-  e.env_g = a.env_base + env;
+  e.env_g = a.env_base + env; e.env_l = env; e.in_drain = false;
   e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * (a.ring_cap + kThreadTabExtra);
   e.hdr = a.hdr_override ? a.hdr_override : a.hdr + (size_t)env * kHeaderWords;
   e.arr = (a.arr && !a.script) ? a.arr + (size_t)env * a.arr_cap : nullptr;

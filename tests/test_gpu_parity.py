@@ -319,6 +319,54 @@ def test_hourly_random_repartitions_all_algorithms(downtime, theta):
     sim.close()
 
 
+@pytest.mark.parametrize("downtime", [4, 60])
+def test_event_driven_table_decisions(downtime):
+    # PAPER.md:L212 / reading #27: the tabulated policy is looked up again after every tick with an arrival or a
+    # completion; random bucket-dependent tables make the configuration follow the load all day, all five algorithms
+    import dataclasses
+    n = 60
+    base = W.config_c3(n)
+    sp = dataclasses.replace(base.params, repart_downtime_s=downtime, repart_energy_mj=1000, decide_on_events=1)
+    rng = np.random.default_rng(downtime)
+    table = rng.integers(0, 12, size=(n, 24, 4)).astype(np.uint8)
+    table[::7] = table[::7, :, :1]                                   # some load-blind tables: decisions stay hourly
+    algo = (np.arange(n) % 5).astype(np.uint8)
+    cfg0 = rng.integers(0, 12, size=n).astype(np.uint8)
+    sim = B.MigSim(sp, n, 55)
+    recs, tot = sim.alloc_recs(), sim.alloc_totals()
+    d_table = dev(table)
+    sim.reset(0, dev(algo), dev(cfg0))
+    sim.rollout(W.POLICY_TABLE, table=d_table, recs_out=recs, totals_out=tot)
+    torch.cuda.synchronize()
+    g_recs, g_tot = B.recs_to_numpy(recs), B.totals_to_numpy(tot)
+    with cf.ProcessPoolExecutor(min(n, os.cpu_count() or 1)) as ex:
+        res = list(ex.map(_oracle_custom, [(sp, 55, e, int(algo[e]), int(cfg0[e]), table[e]) for e in range(n)]))
+    assert np.median(g_tot["n_repart"]) > 100 and g_tot["n_repart"][::7].max() <= 24
+    for e, o_recs, o_tot, o_trace, o_states in res:
+        assert_same_records(g_recs[:, e], g_tot[e], o_recs, o_tot, "env %d algo %d" % (e, algo[e]))
+    for e, o_recs, o_tot, o_trace, o_states in res[:10]:
+        ev, t1 = sim.debug_trace(e, policy=W.POLICY_TABLE, table=d_table, cap_events=400000)
+        assert len(ev) == len(o_trace) and ev.tobytes() == o_trace.tobytes(), "env %d" % e
+    sim.close()
+
+
+def test_event_driven_handworked_J():
+    import dataclasses
+    g = G["J"]
+    sp = dataclasses.replace(tiny_params(repart_downtime_s=g["downtime_s"], repart_energy_mj=g["repart_energy_mj"]), decide_on_events=1)
+    table = np.zeros((1, 24, 4), np.uint8)
+    table[:, :, 0] = g["table"]["bucket0"]; table[:, :, 1:] = g["table"]["bucket1_3"]
+    sim = B.MigSim(sp, 1, 0)
+    sim.debug_set_jobs(O.make_jobs(g["jobs"]).astype(B.JOB_DTYPE))
+    sim.reset(0, dev(np.array([g["algo"]], np.uint8)), dev(np.array([g["cfg0"]], np.uint8)))
+    ev, tot = sim.debug_trace(0, policy=W.POLICY_TABLE, table=dev(table), cap_events=64)
+    assert [[int(e["t"]), int(e["type"]), int(e["slot"])] for e in ev] == [[t, {"ARRIVE": 1, "START": 3, "PREEMPT": 4, "COMPLETE": 5, "SLICE_UP": 7, "REPART": 8}[nm], sl] for t, nm, jb, sl in g["events"]]
+    assert int(tot["n_repart"]) == g["n_repart"]
+    r = O.rollout(sp, 0, 0, algo=g["algo"], cfg0=g["cfg0"], policy=W.POLICY_TABLE, table=table[0], jobs=O.make_jobs(g["jobs"]), trace_cap=64)
+    assert ev.tobytes() == r.trace.tobytes() and tot.tobytes() == r.totals.tobytes()
+    sim.close()
+
+
 def _oracle_static(args):
     sp, seed, e, algo, cfg0, want_trace = args
     r = O.rollout(sp, seed, e, algo=algo, cfg0=cfg0, trace_cap=400000 if want_trace else 0)
