@@ -299,7 +299,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--algo", type=int, default=-1, choices=[-1, 0, 1, 2, 3, 4], help="override the workload's scheduling algorithm for every env (4 = EDF-SS with restricted preemption); -1 = the workload's own")
-    ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 8, 16, 32], help="lanes per environment (0 = library default: 1 = thread per environment for >= 12288 envs, else 8)")
+    ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 8, 16, 32], help="lanes per environment (0 = library default = 1: one thread per environment; 8, 16, 32: warp tiles)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -195,12 +195,17 @@ int mig_sim_debug_set_jobs(mig_sim_t *s, const mig_job_t *jobs, uint32_t n);
  * (umulhi(x, m) >> sh) for every 0 <= x < 2^31. */
 int mig_debug_div_magic(uint32_t v, uint32_t *m, uint32_t *sh);
 /* Lanes per environment of the rollout kernel.  1 = one THREAD per environment (running jobs in the slice table, waiting
- * jobs in a sorted two-level queue, no cross-lane traffic; needs >= ~12 000 environments to fill a B200 and is then 3-5x
- * faster); 8 = four environments per warp in lockstep, 16, 32 = one warp per environment (north_star's layout).
- * 0 = default: 1 if n_envs >= 12288, else 8.  Results are identical for every value (tested); only the launch geometry
+ * jobs in a sorted two-level queue, arrivals drawn before the event loop, no cross-lane traffic; 5x faster than the
+ * tiles on batches that fill a B200, on a par with them below); 8 = four environments per warp in lockstep, 16, 32 = one warp per environment (north_star's layout).
+ * 0 = default: 1.  Results are identical for every value (tested); only the launch geometry
  * and the memory footprint change.  Switching between 1 and {8, 16, 32} changes the layout of the saved per-env state:
  * allowed at any time, but the next call must then be mig_sim_reset (MIG_ESTATE otherwise).  Other values: MIG_EINVAL. */
 int mig_sim_set_tile(mig_sim_t *s, int lanes_per_env);
+/* Thread-per-environment kernel only: environments per warp (lanes 0 .. n-1 of every warp hold one each): 1, 2, 4, 8, 16
+ * or 32; 0 = default: the smallest power of two that keeps a launch one resident wave, so that a small batch is spread
+ * over many warps (little divergence, latency hidden) and a full batch uses every lane.  Launch geometry only: results
+ * are identical for every value (tested).  Allowed between any two calls. */
+int mig_sim_set_envs_per_warp(mig_sim_t *s, uint32_t envs_per_warp);
 /* Thread-per-environment kernel only: capacity (records of 16 bytes per environment) of the arrival lists that a launch
  * fills, in one loop that all lanes of a warp run in step, before it simulates (the arrival process does
  * not depend on the schedule).  Default: the expected number of accepted arrivals per day + 8 sigma, computed from

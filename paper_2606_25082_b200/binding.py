@@ -34,7 +34,7 @@ EXPORTS = (
     "mig_last_error", "mig_version", "mig_sim_create", "mig_sim_destroy", "mig_sim_reset", "mig_sim_step",
     "mig_sim_rollout", "mig_sim_totals", "mig_sim_rollout_host", "mig_qnet_create", "mig_qnet_destroy", "mig_q_eval",
     "mig_sim_debug_trace", "mig_sim_debug_set_jobs", "mig_debug_div_magic", "mig_sim_launch_count", "mig_sim_set_tile",
-    "mig_sim_get_tile", "mig_sim_set_arrival_buffer")
+    "mig_sim_get_tile", "mig_sim_set_arrival_buffer", "mig_sim_set_envs_per_warp")
 
 
 class MigError(RuntimeError):
@@ -88,6 +88,7 @@ def lib():
         L.mig_sim_set_tile.argtypes = [vp, i32]
         L.mig_sim_get_tile.argtypes = [vp]
         L.mig_sim_set_arrival_buffer.argtypes = [vp, C.c_uint32]
+        L.mig_sim_set_envs_per_warp.argtypes = [vp, C.c_uint32]
         _lib = L
     return _lib
 
@@ -195,6 +196,9 @@ class MigSim:
 
     def get_tile(self) -> int:
         return int(lib().mig_sim_get_tile(self.h))
+
+    def set_envs_per_warp(self, envs_per_warp: int):
+        _check(lib().mig_sim_set_envs_per_warp(self.h, int(envs_per_warp)))
 
     def set_arrival_buffer(self, entries_per_env: int):
         _check(lib().mig_sim_set_arrival_buffer(self.h, int(entries_per_env)))

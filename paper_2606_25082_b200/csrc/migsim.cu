@@ -44,6 +44,7 @@ struct mig_sim {
   uint32_t ring_cap = 1;     // power of two >= cap
   uint4 *d_arr = nullptr; uint32_t arr_cap = 0;      // thread-per-env kernel: pre-generated arrival lists (allocated on first use)
   uint32_t arr_want = 0;     // entries per env wanted (0 = generate inline)
+  uint32_t envs_per_warp = 0;   // thread-per-env kernel: 0 = chosen per launch so that the batch is one resident wave
   DevTables *d_tab = nullptr;
   uint32_t *d_hdr = nullptr; uint4 *d_jobtab = nullptr; uint4 *d_dbgtab = nullptr; uint32_t *d_dbghdr = nullptr;
   unsigned int *d_counter = nullptr;
@@ -149,12 +150,11 @@ static int build_tables(const mig_params_t *p, DevTables *t) {
 }
 
 // ------------------------------------------------------------------------------------------------ tile width
-// Default lanes per environment: the thread-per-environment kernel takes a whole simulated day of latency whatever the
-// batch (about 80-100 ms for the C5 shape) and wins as soon as the batch fills the machine with warps; measured
-// crossover against the 8-lane tiles on B200 (C5 shape): 8192 envs 78 vs 90 ms, 16384 envs 82 vs 152 ms; C3 (4096 envs)
-// and C4 (8192 envs, one launch per epoch) are faster on the tiles.
-constexpr uint32_t kThreadKernelMinEnvs = 12288;
-static int default_tile(uint32_t n_envs) { return n_envs >= kThreadKernelMinEnvs ? 1 : 8; }
+// Default lanes per environment: 1 = the thread-per-environment kernel, for every batch size.  Small batches put few
+// environments in each warp (auto_envs_per_warp below), which makes it as fast as the 8-lane tiles where the batch cannot
+// fill the machine (B200, ms per day-batch, thread kernel vs tiles: C2 1024 envs 20.6 vs 23.1, C3 4096 envs 20.9 vs 20.8,
+// C4 8192 envs 31.3 vs 32.1) and 5x faster where it can (C5 65536 envs 93 vs 499).
+static int default_tile(uint32_t) { return 1; }
 
 template <bool TRACE>
 static const void *kernel_ptr(int tile, bool evd = false) {
@@ -203,6 +203,13 @@ extern "C" int mig_sim_set_tile(mig_sim_t *s, int lanes_per_env) {
 }
 
 extern "C" int mig_sim_get_tile(const mig_sim_t *s) { return s ? s->tile : 0; }
+
+extern "C" int mig_sim_set_envs_per_warp(mig_sim_t *s, uint32_t envs_per_warp) {
+  if (!s) return fail(MIG_EINVAL, "set_envs_per_warp: NULL handle");
+  if (envs_per_warp > 32 || (envs_per_warp & (envs_per_warp - 1))) return fail(MIG_EINVAL, "set_envs_per_warp: %u is not 0 or a power of two <= 32", envs_per_warp);
+  s->envs_per_warp = envs_per_warp;
+  return MIG_OK;
+}
 
 extern "C" int mig_sim_set_arrival_buffer(mig_sim_t *s, uint32_t entries_per_env) {
   if (!s) return fail(MIG_EINVAL, "set_arrival_buffer: NULL handle");
@@ -294,6 +301,16 @@ static void base_args(const mig_sim *s, SimArgs &a) {
   a.rec_stride = s->n_envs;
 }
 
+// Environments per warp of the thread-per-env kernel: the smallest power of two that keeps the launch one resident wave
+// (grid_max CTAs of kThreadCta / 32 warps): a small batch gets few environments per warp -- less serialisation of
+// divergent lanes, more warps to hide latency -- and a full batch all 32 lanes.
+static uint32_t auto_envs_per_warp(const mig_sim *s, uint32_t n_envs) {
+  const uint64_t warps = (uint64_t)(s->grid_max > 0 ? s->grid_max : 1) * (kThreadCta / 32);
+  uint32_t l = 1;
+  while (l < 32 && (uint64_t)l * warps < n_envs) l <<= 1;
+  return l;
+}
+
 template <bool TRACE>
 static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
   if (s->tile == 1) {                                     // one thread per environment, one CTA per 64 environments
@@ -308,7 +325,9 @@ static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
     }
     SimArgs b = a;
     b.arr = s->arr_want ? s->d_arr : nullptr; b.arr_cap = s->arr_cap;
-    const dim3 grid((b.n_envs + kThreadCta - 1) / kThreadCta), block(kThreadCta);
+    b.envs_per_warp = s->envs_per_warp ? s->envs_per_warp : auto_envs_per_warp(s, b.n_envs);
+    const uint32_t per_cta = b.envs_per_warp * (kThreadCta / 32);
+    const dim3 grid((b.n_envs + per_cta - 1) / per_cta), block(kThreadCta);
     if (b.ev_decide) sim_thread_kernel<kThreadCta, TRACE, true><<<grid, block, s->smem_bytes, st>>>(b);
     else sim_thread_kernel<kThreadCta, TRACE, false><<<grid, block, s->smem_bytes, st>>>(b);
     CU(cudaGetLastError());

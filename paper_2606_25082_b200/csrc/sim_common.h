@@ -43,6 +43,7 @@ struct SimArgs {
   uint64_t gap_scale;
   int32_t day_s, epoch_s, n_epochs, t_limit_s;
   uint32_t cap, job_limit, smem_entries;
+  uint32_t envs_per_warp;  // thread-per-env kernel: active lanes per warp (1, 2, 4, ... 32): fewer = less divergence, more warps
   uint32_t ring_cap;    // thread-per-env kernel: capacity of the global part of the waiting queue (power of two >= cap)
   int32_t downtime_s; int64_t repart_energy;
   int32_t theta; uint32_t crit_max;

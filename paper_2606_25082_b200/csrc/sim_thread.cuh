@@ -925,8 +925,11 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
     if (threadIdx.x < MIG_MAX_CLASSES) { g->slack_lo[threadIdx.x] = tb->slack_lo[threadIdx.x]; g->slack_span[threadIdx.x] = tb->slack_span[threadIdx.x]; }
   }
   __syncthreads();
-  const uint32_t li = blockIdx.x * NT + threadIdx.x;            // index inside this launch's env range
-  const bool alive = li < a.n_envs;
+  // lanes 0 .. envs_per_warp-1 of every warp hold an environment: small batches are spread over more warps (less
+  // divergence per warp, more warps to hide latency); a full batch uses all 32 lanes
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t li = (blockIdx.x * (NT / 32) + (threadIdx.x >> 5)) * a.envs_per_warp + lane;   // index inside this launch's env range
+  const bool alive = lane < a.envs_per_warp && li < a.n_envs;
   uint2 *r2 = reinterpret_cast<uint2 *>(base) + threadIdx.x;
   uint32_t *r1 = reinterpret_cast<uint32_t *>(base + (size_t)NT * (T2_HEAP + 2 * (size_t)a.smem_entries) * 8) + threadIdx.x;
   EnvT<NT, TRACE, EVD> e(a, hot, r2, r1);

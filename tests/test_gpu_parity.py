@@ -449,6 +449,21 @@ def test_c5_full_size_every_env_agrees_between_kernel_families(algo):
     assert len(np.unique(out[0][1]["trace_hash"])) == 65536
 
 
+@pytest.mark.parametrize("epw", [1, 4, 32])
+def test_thread_kernel_envs_per_warp_gives_the_same_day(epw):
+    for name, n in (("C3", 200), ("C4", 70)):
+        wl = W.CONFIGS[name](n)
+        _, recs_ref, tot_ref, _ = gpu_rollout(wl, sim=B.MigSim(wl.params, n, wl.seed, tile=8))
+        sim = B.MigSim(wl.params, n, wl.seed, tile=1)
+        sim.set_envs_per_warp(epw)
+        _, recs, tot, _ = gpu_rollout(wl, sim=sim)
+        assert tot.tobytes() == tot_ref.tobytes() and recs.tobytes() == recs_ref.tobytes()
+        sim.close()
+    with pytest.raises(B.MigError):
+        sim = B.MigSim(wl.params, n, wl.seed, tile=1)
+        sim.set_envs_per_warp(3)
+
+
 def test_set_tile_between_kernel_families_needs_a_reset():
     wl = W.config_c3(32)
     sim = B.MigSim(wl.params, 32, wl.seed, tile=8)
