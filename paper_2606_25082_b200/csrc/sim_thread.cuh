@@ -1,12 +1,12 @@
-// sim_thread.cuh -- the rollout kernel with ONE THREAD PER ENVIRONMENT (mig_sim_set_tile(s, 1)).
+// sim_thread.cuh -- the rollout kernel with ONE THREAD PER ENVIRONMENT (the library default; mig_sim_set_tile(s, 1)).
 //
 // Why: the warp-tile kernel of sim_device.cuh spends most of its issue slots on cross-lane plumbing (butterfly
 // reductions, ballots, broadcasts) for queues that hold about a dozen jobs and a GPU that has 7 slots.  With one
 // environment per lane there is NO cross-lane traffic at all: every lane runs the serial event loop of DESIGN.md 3.3 on
-// its own environment and a warp instruction advances 32 environments at once; the price is branch divergence between
-// lanes, which the hardware reconverges (profiles/ has the measured threads-per-instruction).  It needs enough
-// environments to fill the machine (one resident wave = 148 SMs x 448 threads = 66 304 environments), which is what
-// the heavy batches (BASELINE C5: 65 536) have; small batches stay on the 8-lane tiles.
+// its own environment and a warp instruction advances up to 32 environments at once; the price is branch divergence
+// between lanes, which the hardware reconverges (profiles/ has the measured threads-per-instruction).  One resident
+// wave is 148 SMs x 448 threads = 66 304 environments (BASELINE C5: 65 536); smaller batches put fewer environments in
+// each warp (SimArgs::envs_per_warp) so that they still spread over the whole machine.
 //
 // Data structures are chosen so that no step scans the queue (a lane with a 300-job queue would otherwise hold its 31
 // neighbours for the length of its scan) and that lanes doing the same thing run the same instructions:
