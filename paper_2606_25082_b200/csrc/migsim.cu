@@ -388,7 +388,7 @@ static int launch_qnet(const mig_qnet *q, QArgs &qa, cudaStream_t st) {
     attr_set = smem;
   }
   uint32_t blocks = (qa.B + kQRows - 1) / kQRows;
-  qnet_kernel<<<blocks, q->H, smem, st>>>(qa);
+  qnet_kernel<<<blocks, q->H / kQCols * (kQRows / kQRpt), smem, st>>>(qa);
   CU(cudaGetLastError());
   return MIG_OK;
 }
