@@ -381,7 +381,7 @@ extern "C" int mig_sim_step(mig_sim_t *s, const uint8_t *action, float *state_ou
 
 static int launch_qnet(const mig_qnet *q, QArgs &qa, cudaStream_t st) {
   qa.W1 = q->W1; qa.b1 = q->b1; qa.W2 = q->W2; qa.b2 = q->b2; qa.W3 = q->W3; qa.b3 = q->b3; qa.H = q->H; qa.A = q->A;
-  size_t smem = (size_t)(MIG_STATE_DIM + 2 * q->H + q->A) * kQRows * sizeof(float);
+  size_t smem = (size_t)(MIG_STATE_DIM + 2 * q->H + q->A) * kQRows * sizeof(float) + (size_t)kQStages * kQChunk * q->H * sizeof(float);
   static thread_local size_t attr_set = 0;
   if (smem > 48 * 1024 && attr_set < smem) {
     CU(cudaFuncSetAttribute(qnet_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -4,7 +4,7 @@
 // term, fixed order, so the result is bit-identical to a sequential CPU fmaf loop.  That is why this is a CUDA-core
 // register-tiled kernel and not a tensor-core GEMM (split accumulation would change the argmax on near-ties and
 // fork the DQN-driven event trace).  One CTA = 32 batch rows, H threads; activations live in shared memory
-// k-major ([k][row]); weights stream from L2 (334 KB, resident), coalesced 16 bytes per thread.
+// k-major ([k][row]); weights stream from L2 (334 KB, resident) through a cp.async double buffer.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -40,39 +40,64 @@ __device__ __forceinline__ uint4 philox_q(uint32_t c0, uint32_t c1, uint32_t c2,
 }
 
 // one dense layer for the CTA's 32 rows.  A thread computes a register tile of kQCols adjacent columns x kQRpt rows
-// (32 accumulators): per k one LDG.128 of weights and kQRpt / 4 broadcast LDS.128 of activations feed 32 FFMAs, eight
-// k steps in flight (the weights come from L2: one column x 32 rows per thread with four steps in flight, the first
-// version, reached 24.6 TFLOP/s; this one 35.5 = 48 % of the FP32 peak, ncu: FMA pipe 52 % busy, the rest is waiting
-// for weights -- each row of W is still fetched by the CTA's four row groups).  Each output is still ONE chain
+// (32 accumulators); W is streamed through shared memory in chunks of kQChunk rows with cp.async (one copy per CTA, no
+// register waits for a weight), activations are read as broadcast LDS.128: per k three LDS.128 feed 32 FFMAs.
+// Measured on B200: 34.2 TFLOP/s at B = 262 144 (46 % of the FP32 peak), 25.7 at C4's B = 8192; the first version (one
+// column x 32 rows per thread, weights by LDG from L2) reached 24.6 / 18.5.  Each output is still ONE chain
 // acc = fmaf(in[k], W[k][n], acc) in ascending k: the tiling changes which thread owns an output, not its arithmetic.
 // in: [K][32] k-major, out: [H][32].
 constexpr int kQCols = 4, kQRpt = 8;
 
+constexpr int kQChunk = 16, kQStages = 2;    // rows of W per cp.async stage; stages in flight
+
+// W is streamed through shared memory in chunks of kQChunk rows (cp.async, kQStages deep): one copy per CTA instead of
+// one L2 fetch per row group, and no register waits for a weight.
 template <bool RELU>
 __device__ __forceinline__ void q_layer(const float *__restrict__ W, const float *__restrict__ b, int K, int H,
-                                        const float *in, float *out, int tid) {
+                                        const float *in, float *out, float4 *stage, int tid) {
   const int n0 = (tid / (kQRows / kQRpt)) * kQCols, r0 = (tid % (kQRows / kQRpt)) * kQRpt;
   float acc[kQCols][kQRpt];
   const float4 bias = *reinterpret_cast<const float4 *>(b + n0);
 #pragma unroll
   for (int r = 0; r < kQRpt; ++r) { acc[0][r] = bias.x; acc[1][r] = bias.y; acc[2][r] = bias.z; acc[3][r] = bias.w; }
-#pragma unroll 8
-  for (int k = 0; k < K; ++k) {
-    const float4 w = __ldg(reinterpret_cast<const float4 *>(W + (size_t)k * H + n0));
-    const float4 *row = reinterpret_cast<const float4 *>(in + k * kQRows + r0);
+  const int nch = K / kQChunk, per = kQChunk * H / 4;          // float4 per chunk = 2 per thread (blockDim.x == H)
+  auto issue = [&](int c) {
+    if (c < nch) {
+      const float4 *src = reinterpret_cast<const float4 *>(W + (size_t)c * kQChunk * H);
+      float4 *dst = stage + (c % kQStages) * per;
+      for (int e = tid; e < per; e += H) {
+        const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst + e);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src + e) : "memory");
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");        // (an empty group keeps the count uniform)
+  };
+  for (int c = 0; c < kQStages - 1; ++c) issue(c);
+  for (int c = 0; c < nch; ++c) {
+    asm volatile("cp.async.wait_group %0;" ::"n"(kQStages - 2) : "memory");   // chunk c has landed
+    __syncthreads();                                            // ... for every thread; and chunk c - 1 is consumed
+    issue(c + kQStages - 1);
+    const float *ws = reinterpret_cast<const float *>(stage + (c % kQStages) * per) + n0;
+    const float *xs = in + c * kQChunk * kQRows + r0;
 #pragma unroll
-    for (int r4 = 0; r4 < kQRpt / 4; ++r4) {
-      const float4 x = row[r4];
-      const float xv[4] = {x.x, x.y, x.z, x.w};
+    for (int kk = 0; kk < kQChunk; ++kk) {
+      const float4 w = *reinterpret_cast<const float4 *>(ws + kk * H);
+      const float4 *row = reinterpret_cast<const float4 *>(xs + kk * kQRows);
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        acc[0][4 * r4 + j] = __fmaf_rn(xv[j], w.x, acc[0][4 * r4 + j]);
-        acc[1][4 * r4 + j] = __fmaf_rn(xv[j], w.y, acc[1][4 * r4 + j]);
-        acc[2][4 * r4 + j] = __fmaf_rn(xv[j], w.z, acc[2][4 * r4 + j]);
-        acc[3][4 * r4 + j] = __fmaf_rn(xv[j], w.w, acc[3][4 * r4 + j]);
+      for (int r4 = 0; r4 < kQRpt / 4; ++r4) {
+        const float4 x = row[r4];
+        const float xv[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          acc[0][4 * r4 + j] = __fmaf_rn(xv[j], w.x, acc[0][4 * r4 + j]);
+          acc[1][4 * r4 + j] = __fmaf_rn(xv[j], w.y, acc[1][4 * r4 + j]);
+          acc[2][4 * r4 + j] = __fmaf_rn(xv[j], w.z, acc[2][4 * r4 + j]);
+          acc[3][4 * r4 + j] = __fmaf_rn(xv[j], w.w, acc[3][4 * r4 + j]);
+        }
       }
     }
   }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
 #pragma unroll
   for (int c = 0; c < kQCols; ++c)
 #pragma unroll
@@ -90,6 +115,7 @@ __global__ void __launch_bounds__(256) qnet_kernel(const QArgs a) {      // H / 
   float *h1 = x + MIG_STATE_DIM * kQRows;       // [H][32]
   float *h2 = h1 + H * kQRows;                  // [H][32]
   float *qo = h2 + H * kQRows;                  // [A][32]
+  float4 *stage = reinterpret_cast<float4 *>(qo + ((A * kQRows + 3) & ~3));   // [kQStages][kQChunk * H / 4]
   const int tid = threadIdx.x;
   const uint32_t row0 = blockIdx.x * kQRows;
   for (int i = tid; i < MIG_STATE_DIM * kQRows; i += blockDim.x) {   // coalesced read of [row][k], transposed store
@@ -98,9 +124,9 @@ __global__ void __launch_bounds__(256) qnet_kernel(const QArgs a) {      // H / 
     x[k * kQRows + r] = row < a.B ? a.state[(size_t)row * MIG_STATE_DIM + k] : 0.0f;
   }
   __syncthreads();
-  q_layer<true>(a.W1, a.b1, MIG_STATE_DIM, H, x, h1, tid);
+  q_layer<true>(a.W1, a.b1, MIG_STATE_DIM, H, x, h1, stage, tid);
   __syncthreads();
-  q_layer<true>(a.W2, a.b2, H, H, h1, h2, tid);
+  q_layer<true>(a.W2, a.b2, H, H, h1, h2, stage, tid);
   __syncthreads();
   for (int o = tid; o < A * kQRows; o += blockDim.x) {                // output layer: (n, row) pairs
     int n = o / kQRows, r = o % kQRows;
