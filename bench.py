@@ -214,13 +214,7 @@ def run_ours(args):
     barrier()
     launches = sim.launch_count() - launches0
     clocks = sampler.stop() if sampler else None
-    t_ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-    ev_all = job_events.clone()
-    if world > 1:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-        dist.all_reduce(ev_all, op=dist.ReduceOp.SUM)
-    t_s = float(t_ms.item()) / 1e3
-    ev_total = int(ev_all.item())
+    t_s, ev_total = W.reduce_over_ranks(e0.elapsed_time(e1) / 1e3, int(job_events.item()), device="cuda")   # max time, summed events
     kern_ms = statistics.mean(a.elapsed_time(b) for a, b in pairs)
     ev_per_launch = int(job_events.item()) / args.steps
     # ---- end to end: HOST buffers through the C ABI, copies inside the timed region ---------------------------------
@@ -239,11 +233,7 @@ def run_ours(args):
         sim.rollout_host(100 + k, wl.algo, wl.cfg0, wl.policy, wl.table, qnet, wl.epsilon, h_recs, h_tot)
         ev_e2e += int(h_tot["n_jobs"].sum() + h_tot["n_completed"].sum() + h_tot["n_dropped"].sum())
     torch.cuda.synchronize()
-    e2e_t = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-    e2e_ev = torch.tensor([ev_e2e], dtype=torch.int64, device="cuda")
-    if world > 1:
-        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(e2e_ev, op=dist.ReduceOp.SUM)
+    e2e_t, e2e_ev = W.reduce_over_ranks(time.perf_counter() - t0, ev_e2e, device="cuda")
     h2d = wl.algo.nbytes + wl.cfg0.nbytes + (wl.table.nbytes if wl.table is not None else 0)
     d2h = h_tot.nbytes + h_recs.nbytes
     # ---- roofline of the dominant kernel (sim_kernel): plain ALU / issue slots --------------------------------------
@@ -279,7 +269,7 @@ def run_ours(args):
             "config": {"workload": args.workload, "n_envs_per_gpu": n_envs, "n_envs_total": n_envs * world, "policy": ["static", "table", "dqn"][wl.policy], "algo": W.ALGO_NAMES[int(wl.algo[0])] if len(set(wl.algo.tolist())) == 1 else "mixed", "lanes_per_env": sim.get_tile(),
                        "job_events_per_step": ev_total / args.steps, "l2": "flushed between iterations (256 MiB write)", "parallelism": "env-range sharding, no data-path collective"},
             "day_episodes_per_s": n_envs * world * args.steps / t_s,
-            "e2e": {"value": float(e2e_ev.item()) / float(e2e_t.item()), "unit": "job-events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
+            "e2e": {"value": e2e_ev / e2e_t, "unit": "job-events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
             "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
         }
         print(json.dumps(line))

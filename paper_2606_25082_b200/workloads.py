@@ -363,3 +363,17 @@ def shard_range(n_total: int, rank: int, world: int) -> tuple[int, int]:
     lo = (n_total * rank) // world
     hi = (n_total * (rank + 1)) // world
     return lo, hi
+
+
+def reduce_over_ranks(seconds: float, units: int, device="cpu") -> tuple[float, int]:
+    """Whole-job timing of a data-parallel run: the slowest rank's time and the units of all ranks.  Works
+    on any initialised torch.distributed backend (NCCL with a CUDA device, gloo on CPU); a no-op without one."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(seconds), int(units)
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    n = torch.tensor([units], dtype=torch.int64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(n.item())
