@@ -31,7 +31,7 @@ constexpr int kThreadTabExtra = 32;   // job-table entries per env beyond the gl
 
 // per-thread rows of 8 bytes (uint2): slice records, pick staging, then the queue's shared ring; rows of 4 bytes follow
 enum { T2_SLKM = 0 /* 7: {skey, meta} of the job running on slot p */, T2_SLRD = 7 /* 7: {rem, due}; a DOWN slice keeps up_at in .x */,
-       T2_STG = 14 /* 7: {meta | slot | moved << 3, rem} of pick k */, T2_HEAP = 21 };
+       T2_STG = 14 /* 7: {meta | slot | moved << 3, rem} of pick k */, T2_RING = 21 };
 enum { T1_V = 0 /* 7: speed of the running job */, T1_STGDUE = 7 /* 7 */, T1_CNT = 14 /* C_COUNT = 10 */, T1_WORDS = 24 };
 
 // saved per-env header of this kernel (kHeaderWords words); the running totals H1_TOT / H1_CNT live here all the time
@@ -57,7 +57,7 @@ struct GenTables {
 };
 
 __host__ __device__ constexpr size_t thread_smem_bytes(uint32_t smem_entries, int nt) {
-  return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * ((T2_HEAP + 2 * (size_t)smem_entries) * 8 + T1_WORDS * 4 + 16);   // + one 16-byte landing slot
+  return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * ((T2_RING + 2 * (size_t)smem_entries) * 8 + T1_WORDS * 4 + 16);   // + one 16-byte landing slot
 }
 
 template <int NT, bool TRACE, bool EVD>     // EVD: event-driven decisions of the tabulated policy compiled in (reading #27)
@@ -104,8 +104,8 @@ struct EnvT {
   // sifts of queue-dependent depth serialised the lanes of a warp (profiles/r1_thread.md).
   __device__ __forceinline__ uint32_t s_phys(uint32_t i) const { const uint32_t p = q_head + i; return p >= S ? p - S : p; }
   __device__ __forceinline__ uint32_t g_phys(uint32_t i) const { return (g_head + i) & (a.ring_cap - 1u); }
-  __device__ __forceinline__ uint2 &SK(uint32_t phys) { return r2[(T2_HEAP + 2 * phys) * NT]; }
-  __device__ __forceinline__ uint2 &SR(uint32_t phys) { return r2[(T2_HEAP + 2 * phys + 1) * NT]; }
+  __device__ __forceinline__ uint2 &SK(uint32_t phys) { return r2[(T2_RING + 2 * phys) * NT]; }
+  __device__ __forceinline__ uint2 &SR(uint32_t phys) { return r2[(T2_RING + 2 * phys + 1) * NT]; }
   // rare paths (critical-laxity scans, state vector, save): record at LOGICAL index i in (key, id) order
   __device__ __forceinline__ uint2 ld_km(uint32_t i) {
     if (i < q_ns) return SK(s_phys(i));
@@ -477,7 +477,7 @@ struct EnvT {
   }
 
   // Every job in the system is re-evaluated: in (key, id) order, while an up slice is left, each job picks a slice by its
-  // rule.  The order is produced by merging the running jobs (slice table) with successive minima of the waiting heap.
+  // rule.  The order is produced by merging the running jobs (slice table) with the front of the waiting queue.
   __device__ __forceinline__ void reschedule() {
     if (algo == MIG_ALGO_EDF_SS_R) { reschedule_restricted(); return; }
     if (is_lax())                       // the keys of running jobs move with their remaining work
@@ -491,7 +491,7 @@ struct EnvT {
     uint32_t keep = 0, nb = 0; int K = 0, nd = MIG_INF, u = 0, pd = 0;
     uint32_t ro = run_order | 0xF0000000u, new_order = 0xFFFFFFFFu;
     while (avail != 0u) {
-      // --- next job in (key, id) order: the first of the unpicked running jobs, or the heap's minimum
+      // --- next job in (key, id) order: the first of the unpicked running jobs, or the front of the queue
       uint2 bkm = make_uint2(0x7FFFFFFFu, 0xFFFFFFFFu); int bp = -1;
       if (!is_lax()) {                    // EDF keys are static: the running jobs are still in last time's order
         while ((ro & 15u) != 15u && !((rmask >> (ro & 15u)) & 1u)) ro >>= 4;
@@ -743,7 +743,7 @@ struct EnvT {
   }
 
   // ------------------------------------------------------------------ state vector
-  // job j of the system, running ones first: j < 7 = slot j (valid if busy), j >= 7 = heap entry j - 7
+  // job j of the system, running ones first: j < 7 = slot j (valid if busy), j >= 7 = queue record j - 7
   __device__ __forceinline__ bool job_at(uint32_t j, uint2 &km, uint2 &rd) {
     if (j < 7u) { if (!((busy_mask >> j) & 1u)) return false; km = R2(T2_SLKM + (int)j); rd = R2(T2_SLRD + (int)j); return true; }
     km = ld_km(j - 7u); rd = ld_rd(j - 7u); return true;
@@ -931,9 +931,9 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   const uint32_t li = (blockIdx.x * (NT / 32) + (threadIdx.x >> 5)) * a.envs_per_warp + lane;   // index inside this launch's env range
   const bool alive = lane < a.envs_per_warp && li < a.n_envs;
   uint2 *r2 = reinterpret_cast<uint2 *>(base) + threadIdx.x;
-  uint32_t *r1 = reinterpret_cast<uint32_t *>(base + (size_t)NT * (T2_HEAP + 2 * (size_t)a.smem_entries) * 8) + threadIdx.x;
+  uint32_t *r1 = reinterpret_cast<uint32_t *>(base + (size_t)NT * (T2_RING + 2 * (size_t)a.smem_entries) * 8) + threadIdx.x;
   EnvT<NT, TRACE, EVD> e(a, hot, r2, r1);
-  e.a_slot = reinterpret_cast<uint4 *>(base + (size_t)NT * ((T2_HEAP + 2 * (size_t)a.smem_entries) * 8 + T1_WORDS * 4)) + threadIdx.x;
+  e.a_slot = reinterpret_cast<uint4 *>(base + (size_t)NT * ((T2_RING + 2 * (size_t)a.smem_entries) * 8 + T1_WORDS * 4)) + threadIdx.x;
   const uint32_t env = a.env_first + (alive ? li : 0u);
   e.gt = reinterpret_cast<const GenTables *>(base);
   e.env_g = a.env_base + env; e.env_l = env; e.in_drain = false;
