@@ -247,7 +247,7 @@ def run_ours(args):
         alg_bytes += int(2 * 16 * ev_per_launch / 2)                              # arrival lists: 16 B per job written once, read once
     roofline = {"bound": "alu", "achieved": achieved_gips, "peak": peak_gips, "unit": "Glane-instr/s", "frac": achieved_gips / peak_gips,
                 "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.workload, n_envs, tile)),
-                "kernel": "sim_thread_kernel<64,false>" if tile == 1 else "sim_kernel<%d,false>" % tile, "kernel_ms": kern_ms,
+                "kernel": "sim_thread_kernel<64,false,false>" if tile == 1 else "sim_kernel<%d,false>" % tile, "kernel_ms": kern_ms,
                 "alg_thread_instr_per_job_event": ALG_THREAD_INSTR_PER_JOB_EVENT, "peak_source": "%d SMs x 128 lanes x %s sm_max_mhz %.0f" % (props.multi_processor_count, peak_src, sm_mhz),
                 "hbm_algorithmic_bytes_per_launch": alg_bytes, "hbm_gbs_at_that": alg_bytes / (kern_ms / 1e3) / 1e9,
                 "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_frac": alg_bytes / (kern_ms / 1e3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0))}
