@@ -164,9 +164,9 @@ class QNet:
                                 _dp(argmax_out, torch.uint8, B), _stream(stream)))
 
     def close(self):
-        if getattr(self, "h", None):
-            lib().mig_qnet_destroy(self.h)
-            self.h = None
+        if getattr(self, "h", None) and _lib is not None:      # (at interpreter shutdown the module may be gone already)
+            _lib.mig_qnet_destroy(self.h)
+        self.h = None
 
     __del__ = close
 
@@ -204,9 +204,9 @@ class MigSim:
         _check(lib().mig_sim_set_arrival_buffer(self.h, int(entries_per_env)))
 
     def close(self):
-        if getattr(self, "h", None):
-            lib().mig_sim_destroy(self.h)
-            self.h = None
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.mig_sim_destroy(self.h)
+        self.h = None
 
     __del__ = close
 

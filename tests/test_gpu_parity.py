@@ -5,6 +5,7 @@ construction (small integers times powers of two); Q-values and rewards are comp
 fmaf / two products and an add), which is stricter than the 1e-4 relative tolerance north_star allows.
 """
 import concurrent.futures as cf
+import dataclasses
 import os
 
 import numpy as np
@@ -462,6 +463,62 @@ def test_thread_kernel_envs_per_warp_gives_the_same_day(epw):
     with pytest.raises(B.MigError):
         sim = B.MigSim(wl.params, n, wl.seed, tile=1)
         sim.set_envs_per_warp(3)
+
+
+def _random_setup(seed, n):
+    """A random but valid parameter set: classes, speeds (not even monotone in the slice size), duration tables, slack
+    ranges, a random subset of Fig. 1 plus a made-up partition, power tables, cap, rates, repartition costs, thresholds,
+    a random bucket-dependent table, mixed algorithms."""
+    rng = np.random.default_rng(1000 + seed)
+    nc = int(rng.integers(1, 17))
+    speeds = [[int(x) for x in rng.integers(1, 2000, size=5)] for _ in range(nc)]
+    durs = []
+    for _ in range(nc):
+        q = np.sort(rng.integers(1, int(rng.choice([20, 200, 3000])), size=65))
+        durs.append([int(x) for x in q])
+    weights = [float(x) for x in rng.uniform(0.1, 1.0, size=nc)]
+    cfgs = [W.FIG1_CONFIGS[i] for i in rng.choice(12, size=int(rng.integers(1, 12)), replace=False)]
+    cfgs.append(((3, 0), (2, 3), (1, 5)))                               # not in Fig. 1: slot 6 unused
+    sp = W.make_params(speeds, durs, weights, jobs_per_day=float(rng.choice([300, 2000, 9000])), amplitude=float(rng.uniform(0, 0.9)),
+                       slack=(int(rng.integers(1024, 2000)), int(rng.integers(2000, 5000))), configs=tuple(cfgs),
+                       cap=int(rng.choice([1, 5, 11, 12, 40, 256, 1024])), repart_downtime_s=int(rng.choice([0, 1, 4, 60, 900])),
+                       repart_energy_mj=int(rng.choice([0, 1000, 6_000_000])), crit_laxity_s=int(rng.choice([0, 1, 60, 600])),
+                       crit_max=int(rng.integers(0, 6)), job_limit=int(rng.choice([0, 0, 50])), decide_on_events=int(rng.integers(0, 2)))
+    sp = dataclasses.replace(sp, curve_mw=rng.integers(0, 50000, size=8).astype(np.int32), p_idle_mw=rng.integers(0, 60000, size=5).astype(np.int32),
+                             p_busy_mw=rng.integers(60000, 250000, size=5).astype(np.int32)).normalised()
+    ncfg = len(cfgs)
+    table = rng.integers(0, ncfg, size=(n, 24, 4)).astype(np.uint8)
+    table[::5, :, :] = rng.integers(0, ncfg + 2, size=(len(table[::5]), 24, 4))    # some actions are invalid: stay + flag
+    algo = rng.integers(0, 5, size=n).astype(np.uint8)
+    cfg0 = rng.integers(0, ncfg, size=n).astype(np.uint8)
+    return sp, table, algo, cfg0
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_random_parameter_sets(seed):
+    # differential test over parameter space: both kernel families on every env, the oracle on a sample with full traces
+    if B.DEFAULT_TILE != 1:
+        pytest.skip("runs once")
+    n = 48
+    sp, table, algo, cfg0 = _random_setup(seed, n)
+    out = []
+    for tile in (1, 8):
+        sim = B.MigSim(sp, n, 4242 + seed, tile=tile)
+        recs, tot = sim.alloc_recs(), sim.alloc_totals()
+        d_table = dev(table)
+        sim.reset(seed, dev(algo), dev(cfg0))
+        sim.rollout(W.POLICY_TABLE, table=d_table, recs_out=recs, totals_out=tot)
+        torch.cuda.synchronize()
+        out.append((B.recs_to_numpy(recs), B.totals_to_numpy(tot)))
+        if tile == 1:
+            traces = [sim.debug_trace(e, policy=W.POLICY_TABLE, table=d_table, cap_events=600000) for e in range(4)]
+        sim.close()
+    assert out[0][1].tobytes() == out[1][1].tobytes() and out[0][0].tobytes() == out[1][0].tobytes()
+    for e in range(4):
+        r = O.rollout(sp, 4242 + seed, e, episode=seed, algo=int(algo[e]), cfg0=int(cfg0[e]), policy=W.POLICY_TABLE, table=table[e], trace_cap=600000)
+        assert_same_records(out[0][0][:, e], out[0][1][e], r.recs, r.totals, "seed %d env %d" % (seed, e))
+        ev, t1 = traces[e]
+        assert len(ev) == len(r.trace) and ev.tobytes() == r.trace.tobytes(), (seed, e)
 
 
 def test_set_tile_between_kernel_families_needs_a_reset():
