@@ -236,6 +236,26 @@ def run_ours(args):
     e2e_t, e2e_ev = W.reduce_over_ranks(time.perf_counter() - t0, ev_e2e, device="cuda")
     h2d = wl.algo.nbytes + wl.cfg0.nbytes + (wl.table.nbytes if wl.table is not None else 0)
     d2h = h_tot.nbytes + h_recs.nbytes
+    # ---- secondary number: the same day through mig_sim_step, one launch per decision epoch with the
+    # actions given by the caller (here: the configurations the timed rollout chose), state, reward and record outputs on
+    step_api = None
+    if rank == 0 and not args.no_step_api:
+        acts = [recs[k, :, 52].contiguous() for k in range(sp.n_epochs)]             # byte 52 of a record = cfg
+        totals_roll = totals.clone()                                                  # of the last timed rollout
+        state, reward = sim.alloc_state(), torch.zeros(n_envs, dtype=torch.float32, device="cuda")
+        rec1, drain1 = torch.zeros((n_envs, 64), dtype=torch.uint8, device="cuda"), torch.zeros((n_envs, 64), dtype=torch.uint8, device="cuda")
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for it in range(2):                                                           # first day: warm-up
+            sim.reset(args.warmup + args.steps - 1, d_algo, d_cfg0, state_out=state)
+            s0.record(stream)
+            for k in range(sp.n_epochs):
+                sim.step(acts[k], state_out=state, reward_out=reward, rec_out=rec1, drain_rec_out=drain1)
+            sim.totals(totals)
+            s1.record(stream)
+            torch.cuda.synchronize()
+        ev_step = int(count_events().item())
+        step_api = {"value": ev_step / (s0.elapsed_time(s1) / 1e3), "unit": "job-events/s", "ms_per_day": s0.elapsed_time(s1),
+                    "launches_per_day": sp.n_epochs + 1, "identical_to_rollout": bool(torch.equal(totals, totals_roll))}
     # ---- roofline of the dominant kernel (sim_kernel): plain ALU / issue slots --------------------------------------
     props = torch.cuda.get_device_properties(local)
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
@@ -270,7 +290,7 @@ def run_ours(args):
                        "job_events_per_step": ev_total / args.steps, "l2": "flushed between iterations (256 MiB write)", "parallelism": "env-range sharding, no data-path collective"},
             "day_episodes_per_s": n_envs * world * args.steps / t_s,
             "e2e": {"value": e2e_ev / e2e_t, "unit": "job-events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
-            "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+            "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "step_api": step_api,
         }
         print(json.dumps(line))
     sim.close()
@@ -288,6 +308,7 @@ def main():
     ap.add_argument("--envs", type=int, default=0, help="environments per GPU (default: the workload's BASELINE size)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-step-api", action="store_true", help="skip the secondary mig_sim_step measurement")
     ap.add_argument("--algo", type=int, default=-1, choices=[-1, 0, 1, 2, 3, 4], help="override the workload's scheduling algorithm for every env (4 = EDF-SS with restricted preemption); -1 = the workload's own")
     ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 8, 16, 32], help="lanes per environment (0 = library default = 1: one thread per environment; 8, 16, 32: warp tiles)")
     args = ap.parse_args()
