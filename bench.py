@@ -281,7 +281,10 @@ def run_ours(args):
             with cf.ProcessPoolExecutor(cores) as pool:
                 time_oracle(args.workload, n_envs, min(n_sample, cores * 2), pool, cores)
                 ev, dt = time_oracle(args.workload, n_envs, n_sample, pool, cores)
-            cpu = {"value": ev / dt, "unit": "job-events/s", "cores": cores, "kind": "oracle",
+            n1 = min(n_envs, 128)                                                        # (i) of SURVEY 8(d): one core
+            t1 = time.perf_counter(); ev1 = _oracle_chunk((args.workload, n_envs, 0, n1)); dt1 = time.perf_counter() - t1
+            cpu = {"value": ev / dt, "unit": "job-events/s", "cores": cores, "kind": "oracle", "one_core_value": ev1 / dt1,
+                   "one_core_sample": "first %d envs, one process (%.1f s)" % (n1, dt1),
                    "sample": "first %d of %d envs of %s, one simulated day each, split statically over %d processes (%.1f s wall)" % (n_sample, n_envs, args.workload, cores, dt)}
         line = {
             "metric": "job_events_per_s", "value": ev_total / t_s, "unit": "job-events/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
