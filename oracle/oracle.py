@@ -7,6 +7,7 @@ from ``paper_2606_25082_b200.workloads`` (input recipes only).
 from __future__ import annotations
 
 import ctypes as C
+import os
 
 import numpy as np
 
@@ -60,7 +61,8 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(_build.build())
+        # MIG_ORACLE_LIB: an alternative build of the same source (tests/test_oracle_sanitizers.py: ASan + UBSan)
+        _lib = C.CDLL(os.environ.get("MIG_ORACLE_LIB") or _build.build())
         _lib.orc_neglog2_q24.restype = C.c_uint32
         _lib.orc_neglog2_q24.argtypes = [C.c_uint32]
         _lib.orc_fnv1a_words.restype = C.c_uint64

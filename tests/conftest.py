@@ -10,6 +10,7 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu on the GPU box")
+    config.addinivalue_line("markers", "sanitize: opt-in (MIG_SANITIZE=1): the oracle's tests under ASan + UBSan")
 
 
 @pytest.fixture(scope="session")
