@@ -25,14 +25,15 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# Algorithmic LANE-instructions per job-event (DESIGN.md section 6 derives it by hand from what the serial method must
-# execute per ARRIVE/COMPLETE: generator 136, event advance 22, arrival/completion accounting + trace hash 30,
-# reschedule 128); the roofline numerator uses THIS, not the executed count, so that neither instruction bloat nor
-# idle lanes can inflate the fraction.  Peak = SMs x 128 FP32/INT32 lanes x f_max lane-instructions per second.
-ALG_THREAD_INSTR_PER_JOB_EVENT = 316.0
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE rollout launch from the ncu --set full capture in profiles/
-# (per launch like `achieved`); None where no capture of that launch configuration exists.
-NCU_DRAM_BYTES_PER_LAUNCH = {("C5", 65536, 1): 9.90e9 + 9.61e9}
+# Algorithmic LANE-instructions per job-event (DESIGN.md section 6 derives them by hand from what the serial method must
+# execute per ARRIVE/COMPLETE): arrival generator 136 (gen_arrivals_kernel); event loop 185 = event advance 22 +
+# arrival/completion accounting and trace hash 30 + reschedule 128 + taking one list record 5 (the rollout kernel).  The
+# roofline numerator uses THESE, not the executed counts, so that neither instruction bloat nor idle lanes can inflate the
+# fraction.  Peak = SMs x 128 FP32/INT32 lanes x f_max lane-instructions per second.
+ALG_LANE_INSTR = {"gen": 136.0, "sim": 185.0}
+# profiles/ncu_summary.json: per-kernel numbers of the committed `ncu --set full` captures (written by
+# `python -m paper_2606_25082_b200.ncu_summary`), keyed "kernel|workload|n_envs" and stamped with the hash of csrc/.
+NCU_SUMMARY = os.path.join(ROOT, "profiles", "ncu_summary.json")
 CPU_SAMPLE_ENVS = 2048
 
 
@@ -98,7 +99,7 @@ def _oracle_chunk(args):
     for e in range(lo, hi):
         r = O.rollout(ph, wl.seed, e, algo=int(wl.algo[e]), cfg0=int(wl.cfg0[e]), policy=wl.policy,
                       table=None if wl.table is None else wl.table[e], qnet=qh, epsilon=wl.epsilon)
-        ev += int(r.totals["n_jobs"]) + int(r.totals["n_completed"]) + int(r.totals["n_dropped"])
+        ev += int(r.totals["n_jobs"]) + int(r.totals["n_completed"])
     return ev
 
 
@@ -189,9 +190,9 @@ def run_ours(args):
         if ev_pair:
             ev_pair[1].record(stream)
 
-    def count_events():                                                                      # n_jobs + n_completed + n_dropped
+    def count_events():                                                                      # one ARRIVE-or-DROP per generated job (n_jobs) + one COMPLETE (n_completed)
         t = totals.view(torch.int32).view(n_envs, 20)
-        return (t[:, 8].long() + t[:, 9].long() + t[:, 10].long()).sum()
+        return (t[:, 8].long() + t[:, 9].long() ).sum()
 
     job_events = torch.zeros(1, dtype=torch.int64, device="cuda")
     for w in range(args.warmup):                                                             # the same work as a timed step
@@ -215,8 +216,26 @@ def run_ours(args):
     launches = sim.launch_count() - launches0
     clocks = sampler.stop() if sampler else None
     t_s, ev_total = W.reduce_over_ranks(e0.elapsed_time(e1) / 1e3, int(job_events.item()), device="cuda")   # max time, summed events
-    kern_ms = statistics.mean(a.elapsed_time(b) for a, b in pairs)
+    kern_ms = statistics.mean(a.elapsed_time(b) for a, b in pairs)                  # the whole mig_sim_rollout call: generator + event loop
     ev_per_launch = int(job_events.item()) / args.steps
+    sim.kernel_times()                                                             # forget the timed region's spans (profiling was off)
+    # ---- per-kernel durations: a second, short region with the library's own event pairs around every launch -------
+    sim.set_profiling(True)
+    n_prof = max(1, min(args.steps, 3))
+    for k in range(n_prof):
+        sim.reset(args.warmup + args.steps + k, d_algo, d_cfg0)
+        sim.kernel_times()                                                         # (drops the reset launch)
+        sim.rollout(wl.policy, table=d_table, qnet=qnet, epsilon=wl.epsilon, recs_out=recs, totals_out=totals)
+        ms_k, n_k = sim.kernel_times()
+        if k == 0:
+            ms_sum, n_sum = dict(ms_k), dict(n_k)
+        else:
+            for key in ms_sum:
+                ms_sum[key] += ms_k[key]; n_sum[key] += n_k[key]
+        flush.fill_(k & 0xFF)
+    sim.set_profiling(False)
+    torch.cuda.synchronize()
+    per_day_ms = {key: ms_sum[key] / n_prof for key in ms_sum}                      # per day-batch, all launches of that family
     # ---- end to end: HOST buffers through the C ABI, copies inside the timed region ---------------------------------
     h_tot = np.zeros(n_envs, dtype=B.TOTALS_DTYPE)
     h_recs = np.zeros((sp.n_epochs + 1, n_envs), dtype=B.REC_DTYPE)
@@ -231,7 +250,7 @@ def run_ours(args):
     n_e2e = max(1, min(args.steps, 3))
     for k in range(n_e2e):
         sim.rollout_host(100 + k, wl.algo, wl.cfg0, wl.policy, wl.table, qnet, wl.epsilon, h_recs, h_tot)
-        ev_e2e += int(h_tot["n_jobs"].sum() + h_tot["n_completed"].sum() + h_tot["n_dropped"].sum())
+        ev_e2e += int(h_tot["n_jobs"].sum() + h_tot["n_completed"].sum())
     torch.cuda.synchronize()
     e2e_t, e2e_ev = W.reduce_over_ranks(time.perf_counter() - t0, ev_e2e, device="cuda")
     h2d = wl.algo.nbytes + wl.cfg0.nbytes + (wl.table.nbytes if wl.table is not None else 0)
@@ -256,21 +275,41 @@ def run_ours(args):
         ev_step = int(count_events().item())
         step_api = {"value": ev_step / (s0.elapsed_time(s1) / 1e3), "unit": "job-events/s", "ms_per_day": s0.elapsed_time(s1),
                     "launches_per_day": sp.n_epochs + 1, "identical_to_rollout": bool(torch.equal(totals, totals_roll))}
-    # ---- roofline of the dominant kernel (sim_kernel): plain ALU / issue slots --------------------------------------
+    # ---- roofline of the dominant kernel: plain ALU / issue slots ------------------------------------------------------
     props = torch.cuda.get_device_properties(local)
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     tile = sim.get_tile()
+    kname = sim.kernel_name()
     peak_gips = props.multi_processor_count * 128 * sm_mhz * 1e6 / 1e9           # G lane-instr/s: SMs x 128 lanes x f_max
-    achieved_gips = ALG_THREAD_INSTR_PER_JOB_EVENT * ev_per_launch / (kern_ms / 1e3) / 1e9
-    alg_bytes = n_envs * ((sp.n_epochs + 1) * 64 + 80 + 2 * 256)                  # records + totals + state header in/out
-    if tile == 1:
-        alg_bytes += int(2 * 16 * ev_per_launch / 2)                              # arrival lists: 16 B per job written once, read once
+    sim_ms = per_day_ms["sim"] if per_day_ms["sim"] > 0 else kern_ms
+    alg_sim = ALG_LANE_INSTR["sim"] + (0.0 if per_day_ms["gen"] > 0 else ALG_LANE_INSTR["gen"])   # tiles draw arrivals inside the rollout kernel
+    achieved_gips = alg_sim * ev_per_launch / (sim_ms / 1e3) / 1e9
+    path_gips = (ALG_LANE_INSTR["sim"] + ALG_LANE_INSTR["gen"]) * ev_per_launch / (kern_ms / 1e3) / 1e9
+    # algorithmic HBM bytes per launch: the outputs the caller asked for + the per-env inputs, nothing else
+    alg_bytes = n_envs * ((sp.n_epochs + 1) * 64 + 80) + d_algo.numel() + d_cfg0.numel() + (d_table.numel() if d_table is not None else 0)
+    cap = None
+    try:
+        with open(NCU_SUMMARY) as f:
+            cap = json.load(f).get("%s|%s|%d" % (kname, args.workload, n_envs))
+    except Exception:
+        cap = None
+    from paper_2606_25082_b200 import ncu_summary
+    fresh = bool(cap) and cap.get("csrc_sha16") == ncu_summary.csrc_sha16()
+    traffic = cap.get("dram_bytes") if fresh else None
     roofline = {"bound": "alu", "achieved": achieved_gips, "peak": peak_gips, "unit": "Glane-instr/s", "frac": achieved_gips / peak_gips,
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.workload, n_envs, tile)),
-                "kernel": "sim_thread_kernel<64,false,false>" if tile == 1 else "sim_kernel<%d,false>" % tile, "kernel_ms": kern_ms,
-                "alg_thread_instr_per_job_event": ALG_THREAD_INSTR_PER_JOB_EVENT, "peak_source": "%d SMs x 128 lanes x %s sm_max_mhz %.0f" % (props.multi_processor_count, peak_src, sm_mhz),
-                "hbm_algorithmic_bytes_per_launch": alg_bytes, "hbm_gbs_at_that": alg_bytes / (kern_ms / 1e3) / 1e9,
-                "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_frac": alg_bytes / (kern_ms / 1e3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0))}
+                "traffic": traffic, "kernel": kname, "kernel_ms": sim_ms, "alg_lane_instr_per_job_event": alg_sim,
+                "peak_source": "%d SMs x 128 lanes x %s sm_max_mhz %.0f" % (props.multi_processor_count, peak_src, sm_mhz),
+                "hot_path": {"frac": path_gips / peak_gips, "achieved": path_gips, "ms": kern_ms, "alg_lane_instr_per_job_event": ALG_LANE_INSTR["sim"] + ALG_LANE_INSTR["gen"],
+                             "what": "generator + event loop: the whole mig_sim_rollout call (round 1's definition of frac)"},
+                "kernels_ms_per_day": per_day_ms, "launches_per_day": {key: n_sum[key] / n_prof for key in n_sum},
+                "hbm_algorithmic_bytes_per_launch": alg_bytes, "traffic_over_algorithmic": (traffic / alg_bytes) if traffic else None,
+                "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_frac": alg_bytes / (sim_ms / 1e3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0)),
+                "arrival_list_records_per_env": sim.get_arrival_buffer() if tile == 1 else 0,
+                "ncu_capture": None if not cap else {"fresh": fresh, "csrc_sha16": cap.get("csrc_sha16"), "duration_ms": cap.get("duration_ms"),
+                                                     "active_threads_per_inst": cap.get("active_threads_per_inst"),
+                                                     "issue_frac_executed": (cap.get("issue_pct_of_peak_elapsed") or 0.0) / 100.0 or None,
+                                                     "executed_lane_instr_per_job_event": (cap.get("thread_inst_executed_true") / ev_per_launch) if cap.get("thread_inst_executed_true") else None,
+                                                     "global_ld_bytes_per_sector": cap.get("global_ld_bytes_per_sector")}}
     line = None
     if rank == 0:
         import concurrent.futures as cf

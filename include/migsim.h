@@ -62,6 +62,7 @@ enum { MIG_POLICY_STATIC = 0, MIG_POLICY_TABLE = 1, MIG_POLICY_DQN = 2 };
 /* per-environment status bits */
 #define MIG_ST_TRUNCATED 1u  /* t_limit_s reached with jobs still in the system */
 #define MIG_ST_BAD_ACTION 2u /* an action >= n_configs was treated as "stay" */
+#define MIG_ST_BAD_ALGO 4u   /* an algorithm id > MIG_ALGO_EDF_SS_R was given at reset: the env runs EDF-FS (reading #28) */
 /* event types of the trace */
 enum { MIG_EV_ARRIVE = 1, MIG_EV_DROP = 2, MIG_EV_START = 3, MIG_EV_PREEMPT = 4, MIG_EV_COMPLETE = 5, MIG_EV_CRIT = 6,
        MIG_EV_SLICE_UP = 7, MIG_EV_REPART = 8 };
@@ -176,7 +177,8 @@ int mig_sim_rollout_host(mig_sim_t *s, uint32_t episode, const uint8_t *algo, co
                          mig_totals_t *totals_out);
 
 /* Q-network MLP 64 -> H -> H -> n_actions, ReLU, fp32.  Host arrays, copied; W row-major [in][out].
- * Every output is accumulated in ascending k with one fused multiply-add per term (bit-reproducible). H in {64,128,256}. */
+ * Every output is accumulated in ascending k with one fused multiply-add per term (bit-reproducible).  hidden: any
+ * multiple of 32 in 32..256 (MIG_EINVAL otherwise). */
 int mig_qnet_create(mig_qnet_t **out, const float *W1, const float *b1, const float *W2, const float *b2,
                     const float *W3, const float *b3, uint32_t hidden, uint32_t n_actions);
 int mig_qnet_destroy(mig_qnet_t *q);
@@ -206,16 +208,30 @@ int mig_sim_set_tile(mig_sim_t *s, int lanes_per_env);
  * over many warps (little divergence, latency hidden) and a full batch uses every lane.  Launch geometry only: results
  * are identical for every value (tested).  Allowed between any two calls. */
 int mig_sim_set_envs_per_warp(mig_sim_t *s, uint32_t envs_per_warp);
-/* Thread-per-environment kernel only: capacity (records of 16 bytes per environment) of the arrival lists that a launch
- * fills, in one loop that all lanes of a warp run in step, before it simulates (the arrival process does
- * not depend on the schedule).  Default: the expected number of accepted arrivals per day + 8 sigma, computed from
- * accept_thr and gap_scale_q16 (C5: 8 784 records = 140 KB per environment).  0 = draw arrivals inside the event loop
- * (no global buffer).  A list that fills up is refilled when it runs empty, so ANY capacity >= 1 gives the same results
- * (tested); memory is allocated at the next launch (inline generation if it does not fit).  Allowed between any two calls. */
+/* Thread-per-environment kernel only: capacity (records of 8 bytes per environment, rounded up to a multiple of 4) of the
+ * arrival lists.  Before every launch that simulates, a generator kernel (one warp per environment, 32 thinning candidates
+ * per pass) draws the arrivals of that launch's horizon into them (the arrival process does not depend
+ * on the schedule).  Default, allocated by mig_sim_create: the expected number of accepted arrivals per day + 8 sigma,
+ * computed from accept_thr and gap_scale_q16 (C5: 8 784 records = 70 KB per environment); if that allocation fails,
+ * create fails with MIG_ENOMEM.  0 = no lists: arrivals are drawn inside the event loop, one at a time (slower).  A list
+ * that is too small for a launch is simply continued that way, so ANY capacity gives the same results (tested).
+ * 0xFFFFFFFF = back to the default.  Synchronises the device and reallocates; on MIG_ENOMEM the handle is left WITHOUT
+ * lists (still correct, slower) and mig_last_error() says so.  Allowed between any two calls. */
 int mig_sim_set_arrival_buffer(mig_sim_t *s, uint32_t entries_per_env);
+/* Capacity of the arrival lists in use (records per environment); 0 = arrivals are drawn inside the event loop. */
+uint32_t mig_sim_get_arrival_buffer(const mig_sim_t *s);
 int mig_sim_get_tile(const mig_sim_t *s);
 /* Number of kernel launches issued through this handle so far (bench.py's gpu_launches). */
 uint64_t mig_sim_launch_count(const mig_sim_t *s);
+/* Name of the rollout kernel that mig_sim_rollout launches with the handle's current settings, as ncu prints it
+ * (bench.py's roofline.kernel; the ncu summaries under profiles/ are keyed by it).  Static string. */
+const char *mig_sim_kernel_name(const mig_sim_t *s);
+/* Measurement aid: with on != 0 every kernel launch of this handle is bracketed by two CUDA events on the launching
+ * stream.  mig_sim_kernel_times synchronises on them, adds up the elapsed milliseconds per kernel family since its last
+ * call -- ms_out[0] arrival generator, [1] rollout kernel, [2] Q-network -- with the launch counts (host arrays of 3,
+ * launches_out may be NULL), and forgets them.  Results are unaffected. */
+int mig_sim_set_profiling(mig_sim_t *s, int on);
+int mig_sim_kernel_times(mig_sim_t *s, float ms_out[3], uint32_t launches_out[3]);
 
 #ifdef __cplusplus
 }

@@ -547,6 +547,7 @@ void orc_env_reset(orc_env_t *e, uint32_t episode, uint8_t algo, uint8_t cfg0)
 {
   e->episode = episode; e->algo = algo; e->cfg = cfg0;
   e->t = 0; e->epoch = 0; e->status = 0; e->n_sys = 0;
+  if (algo > ORC_ALGO_EDF_SS_R) { e->algo = ORC_ALGO_EDF_FS; e->status |= ORC_ST_BAD_ALGO; }   /* reading #28 */
   e->hash = 0xcbf29ce484222325ull;
   memset(&e->ep, 0, sizeof(e->ep)); memset(&e->tot, 0, sizeof(e->tot));
   e->last_epoch_drops = 0; e->n_trace = 0;

@@ -28,6 +28,7 @@ extern "C" {
 /* status flags */
 #define ORC_ST_TRUNCATED 1u  /* t_limit_s reached with jobs still in system */
 #define ORC_ST_BAD_ACTION 2u /* an action >= n_configs was treated as "stay" */
+#define ORC_ST_BAD_ALGO 4u   /* an algorithm id > 4 was given at reset: the env runs EDF-FS (reading #28) */
 
 /* event types */
 enum { ORC_EV_ARRIVE = 1, ORC_EV_DROP = 2, ORC_EV_START = 3, ORC_EV_PREEMPT = 4, ORC_EV_COMPLETE = 5,

@@ -30,7 +30,7 @@ JOB_IN_DTYPE = np.dtype([("arr", "<i4"), ("cls", "<u4"), ("dur7", "<i4"), ("due"
 assert EVENT_DTYPE.itemsize == 16 and REC_DTYPE.itemsize == 64 and TOTALS_DTYPE.itemsize == 80
 
 EV_ARRIVE, EV_DROP, EV_START, EV_PREEMPT, EV_COMPLETE, EV_CRIT, EV_SLICE_UP, EV_REPART = range(1, 9)
-ST_TRUNCATED, ST_BAD_ACTION = 1, 2
+ST_TRUNCATED, ST_BAD_ACTION, ST_BAD_ALGO = 1, 2, 4
 
 
 class _Params(C.Structure):

@@ -1,6 +1,7 @@
 """Builds libmigsim.so (hand-written CUDA for sm_100a + the C ABI of include/migsim.h) in-tree with nvcc."""
 from __future__ import annotations
 
+import glob
 import os
 import subprocess
 
@@ -8,7 +9,17 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmigsim.so")
 SOURCES = ["migsim.cu"]
-DEPS = ["migsim.cu", "sim_device.cuh", "qnet_device.cuh", "sim_common.h", os.path.join("..", "..", "include", "migsim.h")]
+
+
+def _deps() -> list[str]:
+    """Every source the library is compiled from: csrc/*.cu, *.cuh, *.h and the public header (a stale .so must never
+    pass a parity test: binding.lib() rebuilds when any of these is newer than libmigsim.so)."""
+    out = []
+    for pat in ("*.cu", "*.cuh", "*.h"):
+        out += glob.glob(os.path.join(CSRC, pat))
+    out += glob.glob(os.path.join(HERE, "..", "include", "*.h"))
+    return sorted(out)
+
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-shared",
               "-Xcompiler", "-fPIC", "-cudart", "shared"]
 
@@ -24,7 +35,7 @@ def stale() -> bool:
     if not os.path.exists(LIB):
         return True
     mt = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, d)) > mt for d in DEPS)
+    return any(os.path.getmtime(d) > mt for d in _deps())
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -34,7 +34,8 @@ EXPORTS = (
     "mig_last_error", "mig_version", "mig_sim_create", "mig_sim_destroy", "mig_sim_reset", "mig_sim_step",
     "mig_sim_rollout", "mig_sim_totals", "mig_sim_rollout_host", "mig_qnet_create", "mig_qnet_destroy", "mig_q_eval",
     "mig_sim_debug_trace", "mig_sim_debug_set_jobs", "mig_debug_div_magic", "mig_sim_launch_count", "mig_sim_set_tile",
-    "mig_sim_get_tile", "mig_sim_set_arrival_buffer", "mig_sim_set_envs_per_warp")
+    "mig_sim_get_tile", "mig_sim_set_arrival_buffer", "mig_sim_get_arrival_buffer", "mig_sim_set_envs_per_warp",
+    "mig_sim_kernel_name", "mig_sim_set_profiling", "mig_sim_kernel_times")
 
 
 class MigError(RuntimeError):
@@ -89,6 +90,12 @@ def lib():
         L.mig_sim_get_tile.argtypes = [vp]
         L.mig_sim_set_arrival_buffer.argtypes = [vp, C.c_uint32]
         L.mig_sim_set_envs_per_warp.argtypes = [vp, C.c_uint32]
+        L.mig_sim_kernel_name.argtypes = [vp]
+        L.mig_sim_kernel_name.restype = C.c_char_p
+        L.mig_sim_set_profiling.argtypes = [vp, i32]
+        L.mig_sim_kernel_times.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_uint32)]
+        L.mig_sim_get_arrival_buffer.argtypes = [vp]
+        L.mig_sim_get_arrival_buffer.restype = C.c_uint32
         _lib = L
     return _lib
 
@@ -203,6 +210,9 @@ class MigSim:
     def set_arrival_buffer(self, entries_per_env: int):
         _check(lib().mig_sim_set_arrival_buffer(self.h, int(entries_per_env)))
 
+    def get_arrival_buffer(self) -> int:
+        return int(lib().mig_sim_get_arrival_buffer(self.h))
+
     def close(self):
         if getattr(self, "h", None) and _lib is not None:
             _lib.mig_sim_destroy(self.h)
@@ -281,6 +291,19 @@ class MigSim:
 
     def launch_count(self) -> int:
         return int(lib().mig_sim_launch_count(self.h))
+
+    def kernel_name(self) -> str:
+        return lib().mig_sim_kernel_name(self.h).decode()
+
+    def set_profiling(self, on: bool):
+        _check(lib().mig_sim_set_profiling(self.h, int(bool(on))))
+
+    def kernel_times(self):
+        """({"gen": ms, "sim": ms, "qnet": ms}, {... launches}) since the last call (needs set_profiling(True))."""
+        ms, n = (C.c_float * 3)(), (C.c_uint32 * 3)()
+        _check(lib().mig_sim_kernel_times(self.h, ms, n))
+        names = ("gen", "sim", "qnet")
+        return {k: float(ms[i]) for i, k in enumerate(names)}, {k: int(n[i]) for i, k in enumerate(names)}
 
 
 def recs_to_numpy(t: torch.Tensor) -> np.ndarray:

@@ -1,0 +1,152 @@
+// gen_kernel.cuh -- the arrival generator of the thread-per-environment path as its OWN kernel (
+// DESIGN.md R1-R5), launched on the same stream right before sim_thread_kernel.
+//
+// The arrival process does not depend on the schedule, so a launch's arrivals can all be drawn before
+// it simulates -- and drawing them is embarrassingly parallel over thinning CANDIDATES, where the event loop is serial:
+//   * ONE WARP PER ENVIRONMENT, 32 candidates per pass: lane l draws candidate k + l (Philox stream 0: gap, accept,
+//     class, slack), the integer -log2 turns w_gap into a Q16 gap, a 64-bit inclusive warp scan (SHFL.UP) plus the
+//     running sum gives every candidate its arrival tick -- integer addition is associative, so this IS the oracle's
+//     sequential accumulation;
+//   * Lewis-Shedler thinning against the per-minute threshold table; ballot + popc compact the accepted candidates;
+//   * only accepted candidates draw Philox stream 1 (duration) and look their class / duration / slack up;
+//   * each accepted job becomes ONE 8-BYTE record {dur7 | class | slack, tick} appended to the environment's list; the
+//     32 lanes of a pass write neighbouring records (coalesced).  The event loop recomputes work = dur7 * v7[class] and
+//     due = tick + max(1, dur7 * slack >> 10) when it takes the record (two multiplies) -- half the bytes of a
+//     {tick, class, work, due} record through HBM.
+// A candidate is COMMITTED (the saved generator state moves past it) only if it lies inside the day and the launch's
+// horizon and the list still has room; generation resumes exactly at the first uncommitted candidate, in the next
+// launch's generator or -- when a list is too small for its launch -- in the event loop's own one-at-a-time generator
+// (EnvT::gen_next_inline).  Any list capacity therefore gives the same day (tested).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "philox.cuh"
+#include "sim_common.h"
+
+namespace migsim {
+
+constexpr int kGenWarps = 8;     // environments (= warps) per CTA of the generator
+
+// generator state of the thread-per-environment path inside the saved per-env header (word indices; sim_thread.cuh
+// owns the rest of the layout)
+enum { HG_PK = 1 /* epoch in the low byte */, HG_GK = 6, HG_GT_LO, HG_GT_HI, HG_GDONE, HG_NACC,
+       HG_ACOUNT = 32 /* records in this launch's list */, HG_AMORE /* the list filled up before the horizon */, HG_AID0 /* job id of record 0 */ };
+
+struct GenArgs {
+  const DevTables *tab;
+  uint32_t *hdr;                       // [n_envs][kHeaderWords]
+  uint2 *arr; uint32_t arr_cap;        // [n_envs][arr_cap] records
+  uint32_t n_envs, env_first;
+  uint32_t k0, k1, episode, env_base;  // Philox key, counter words
+  uint64_t gap_scale;
+  int32_t day_s, epoch_s, n_epochs, n_steps;
+  uint32_t job_limit;
+};
+
+struct GenSmem {
+  uint32_t thr[MIG_THR_BINS];
+  int32_t dur7_q[MIG_MAX_CLASSES * 65];
+  uint32_t class_cum[MIG_MAX_CLASSES];      // padded with 0xFFFFFFFF beyond n_classes
+  uint32_t slack_lo[MIG_MAX_CLASSES], slack_span[MIG_MAX_CLASSES];
+  uint32_t logT[257];
+};
+
+// arrival record: x = dur7[0:25) | class[25:29) | slack_q10 bits 13..15 [29:32);  y = tick[0:17) | slack_q10 bits 0..12 [17:30)
+__device__ __forceinline__ uint2 pack_arrival(uint32_t tick, uint32_t cls, uint32_t dur7, uint32_t slack) {
+  return make_uint2(dur7 | (cls << 25) | ((slack >> 13) << 29), tick | ((slack & 0x1FFFu) << 17));
+}
+
+// E24 = -log2((w|1) / 2^32) * 2^24 by table + linear interpolation, all integer (R3)
+__device__ __forceinline__ uint32_t neglog2_q24_tab(uint32_t w, const uint32_t *logT) {
+  const uint32_t m = w | 1u;
+  const int lz = __clz((int)m);
+  const uint32_t y = m << lz;
+  const uint32_t i = (y >> 23) & 0xFFu, f = (y >> 7) & 0xFFFFu;
+  const uint32_t T0 = logT[i], T1 = logT[i + 1];
+  const uint32_t L = T0 + (uint32_t)(((unsigned long long)(T1 - T0) * f) >> 16);
+  return ((uint32_t)(1 + lz) << 24) - L;
+}
+
+// first c with w <= cum[c] over 16 non-decreasing thresholds whose last is 0xFFFFFFFF: four dependent compares
+__device__ __forceinline__ uint32_t class_of(uint32_t w, const uint32_t *cum) {
+  uint32_t c = (w > cum[7]) ? 8u : 0u;
+  c += (w > cum[c + 3]) ? 4u : 0u;
+  c += (w > cum[c + 1]) ? 2u : 0u;
+  c += (w > cum[c]) ? 1u : 0u;
+  return c;
+}
+
+__global__ void __launch_bounds__(kGenWarps * 32) gen_arrivals_kernel(const GenArgs a) {
+  __shared__ GenSmem sm;
+  {
+    const DevTables *tb = a.tab;
+    for (int i = threadIdx.x; i < MIG_THR_BINS; i += kGenWarps * 32) sm.thr[i] = tb->thr[i];
+    for (int i = threadIdx.x; i < MIG_MAX_CLASSES * 65; i += kGenWarps * 32) sm.dur7_q[i] = tb->dur7_q[i];
+    for (int i = threadIdx.x; i < 257; i += kGenWarps * 32) sm.logT[i] = tb->logT[i];
+    if (threadIdx.x < MIG_MAX_CLASSES) {
+      sm.class_cum[threadIdx.x] = tb->class_cum[threadIdx.x];
+      sm.slack_lo[threadIdx.x] = tb->slack_lo[threadIdx.x]; sm.slack_span[threadIdx.x] = tb->slack_span[threadIdx.x];
+    }
+  }
+  __syncthreads();
+  const uint32_t lane = threadIdx.x & 31u, li = blockIdx.x * kGenWarps + (threadIdx.x >> 5);
+  if (li >= a.n_envs) return;
+  const uint32_t env = a.env_first + li, env_g = a.env_base + env;
+  uint32_t *hdr = a.hdr + (size_t)env * kHeaderWords;
+  uint2 *out = a.arr + (size_t)env * a.arr_cap;
+  const int epoch = (int)(hdr[HG_PK] & 0xFFu);
+  uint32_t k = hdr[HG_GK], done = hdr[HG_GDONE], nacc = hdr[HG_NACC];
+  unsigned long long T = (unsigned long long)hdr[HG_GT_LO] | ((unsigned long long)hdr[HG_GT_HI] << 32);
+  const uint32_t id0 = nacc, limit = a.job_limit ? min(a.job_limit, MIG_MAX_JOBS) : MIG_MAX_JOBS;
+  uint32_t count = 0, more = 0;
+  if (epoch < a.n_epochs && !done) {
+    const unsigned long long horizon = (unsigned long long)(min(epoch + a.n_steps, a.n_epochs) * a.epoch_s);
+    const uint32_t lt = (1u << lane) - 1u;
+    for (;;) {                                                    // every condition below is warp-uniform
+      if (nacc >= limit) break;
+      if (count >= a.arr_cap) { more = 1; break; }
+      const uint32_t kl = k + lane;
+      const uint4 w = philox4x32_10(kl, 0u, env_g, a.episode, a.k0, a.k1);       // stream 0: gap, accept, class, slack
+      unsigned long long gap = ((unsigned long long)neglog2_q24_tab(w.x, sm.logT) * a.gap_scale) >> 24;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {                          // inclusive prefix sum of the gaps, 64-bit integer
+        const unsigned long long o = __shfl_up_sync(0xffffffffu, gap, d);
+        if (lane >= (uint32_t)d) gap += o;
+      }
+      const unsigned long long Tl = T + gap, tick = Tl >> 16;
+      const bool in_day = tick < (unsigned long long)a.day_s;     // arrivals stop at the end of the day
+      const bool ok = in_day && tick <= horizon;
+      const bool acc0 = ok && w.y <= sm.thr[(uint32_t)tick / 60u];               // Lewis-Shedler thinning
+      const uint32_t accm = __ballot_sync(0xffffffffu, acc0);
+      const uint32_t before = __popc(accm & lt);                  // accepted among the earlier candidates of this pass
+      const uint32_t room = min(a.arr_cap - count, limit - nacc);
+      const bool commit = ok && before < room;                    // a prefix of the pass: ticks and `before` are monotone
+      const uint32_t cm = __ballot_sync(0xffffffffu, commit);
+      const int nc = __popc(cm);
+      if (acc0 && commit) {                                       // job attributes (R5)
+        const uint32_t c = class_of(w.z, sm.class_cum);
+        const uint4 wd = philox4x32_10(kl, 1u, env_g, a.episode, a.k0, a.k1);    // stream 1: duration
+        const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
+        const int q0 = sm.dur7_q[c * 65 + qi], q1 = sm.dur7_q[c * 65 + qi + 1];
+        const int dur7 = q0 + (int)(((long long)(q1 - q0) * (long long)f) >> 10);
+        const uint32_t slack = sm.slack_lo[c] + __umulhi(w.w, sm.slack_span[c]);
+        __stcg(&out[count + before], pack_arrival((uint32_t)tick, c, (uint32_t)dur7, slack));   // streamed past L1
+      }
+      const uint32_t na = __popc(accm & cm);
+      count += na; nacc += na;
+      if (nc) { T = __shfl_sync(0xffffffffu, Tl, nc - 1); k += (uint32_t)nc; }
+      if (nc < 32) {                                              // the first uncommitted candidate says why we stop
+        const bool s_in_day = __shfl_sync(0xffffffffu, (int)in_day, nc) != 0, s_ok = __shfl_sync(0xffffffffu, (int)ok, nc) != 0;
+        if (!s_in_day) done = 1;                                  // end of the day
+        else if (s_ok && nacc < limit) more = 1;                  // inside the horizon: the list is full
+        break;
+      }
+    }
+  }
+  if (lane == 0) {
+    hdr[HG_GK] = k; hdr[HG_GT_LO] = (uint32_t)T; hdr[HG_GT_HI] = (uint32_t)(T >> 32); hdr[HG_GDONE] = done; hdr[HG_NACC] = nacc;
+    hdr[HG_ACOUNT] = count; hdr[HG_AMORE] = more; hdr[HG_AID0] = id0;
+  }
+}
+
+}  // namespace migsim

@@ -42,8 +42,8 @@ struct mig_sim {
   int tile = 8;              // lanes per environment (8, 16 or 32): 32 / tile environments per warp
   uint32_t smem_entries = 0; size_t smem_bytes = 0; int grid_max = 0;
   uint32_t ring_cap = 1;     // power of two >= cap
-  uint4 *d_arr = nullptr; uint32_t arr_cap = 0;      // thread-per-env kernel: pre-generated arrival lists (allocated on first use)
-  uint32_t arr_want = 0;     // entries per env wanted (0 = generate inline)
+  uint2 *d_arr = nullptr; uint32_t arr_cap = 0;      // thread-per-env kernel: arrival lists [n_envs][arr_cap] of 8-byte records (0 = none: arrivals are drawn inside the event loop)
+  uint32_t arr_default = 0;  // capacity chosen at create: expected accepted arrivals per day + 8 sigma
   uint32_t envs_per_warp = 0;   // thread-per-env kernel: 0 = chosen per launch so that the batch is one resident wave
   DevTables *d_tab = nullptr;
   uint32_t *d_hdr = nullptr; uint4 *d_jobtab = nullptr; uint4 *d_dbgtab = nullptr; uint32_t *d_dbghdr = nullptr;
@@ -55,6 +55,23 @@ struct mig_sim {
   mig_job_t *d_script = nullptr; uint32_t n_script = 0;
   int epoch = -1;            // -1: never reset
   uint64_t launches = 0;
+  // optional per-kernel timing (mig_sim_set_profiling): CUDA events around every launch, on the launching stream
+  bool prof = false;
+  struct Span { int cat; cudaEvent_t a, b; };
+  std::vector<Span> spans; std::vector<cudaEvent_t> ev_pool;
+};
+
+enum { CAT_GEN = 0, CAT_SIM = 1, CAT_QNET = 2, CAT_COUNT = 3 };
+
+// brackets one kernel launch with two events when profiling is on (otherwise free)
+struct ProfSpan {
+  mig_sim *s; cudaStream_t st; int cat; cudaEvent_t a = nullptr;
+  static cudaEvent_t get(mig_sim *s) {
+    if (!s->ev_pool.empty()) { cudaEvent_t e = s->ev_pool.back(); s->ev_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr; cudaEventCreate(&e); return e;
+  }
+  ProfSpan(mig_sim *s_, cudaStream_t st_, int cat_) : s(s_), st(st_), cat(cat_) { if (s->prof) { a = get(s); cudaEventRecord(a, st); } }
+  ~ProfSpan() { if (a) { cudaEvent_t b = get(s); cudaEventRecord(b, st); s->spans.push_back({cat, a, b}); } }
 };
 
 // ------------------------------------------------------------------------------------------------ exact division constants
@@ -144,6 +161,7 @@ static int build_tables(const mig_params_t *p, DevTables *t) {
     t->slack_lo[c] = lo; t->slack_span[c] = hi - lo + 1;
   }
   if (p->class_cum[p->n_classes - 1] != 0xFFFFFFFFu) return fail(MIG_EINVAL, "create: class_cum[last] must be 0xFFFFFFFF");
+  for (uint32_t c = p->n_classes; c < MIG_MAX_CLASSES; ++c) t->class_cum[c] = 0xFFFFFFFFu;      // padded: the class search needs no bound
   for (int i = 0; i < MIG_THR_BINS; ++i) t->thr[i] = p->accept_thr[i];
   for (int i = 0; i <= 256; ++i) t->logT[i] = (uint32_t)llround(16777216.0 * log2(1.0 + (double)i / 256.0));
   return MIG_OK;
@@ -211,12 +229,30 @@ extern "C" int mig_sim_set_envs_per_warp(mig_sim_t *s, uint32_t envs_per_warp) {
   return MIG_OK;
 }
 
+// (Re)allocates the arrival lists: n_envs x entries x 8 bytes, entries rounded up to a multiple of 4 (one 32-byte sector).
+static int alloc_arrival_lists(mig_sim *s, uint32_t entries) {
+  if (cudaDeviceSynchronize() != cudaSuccess) return fail(MIG_ECUDA, "set_arrival_buffer: %s", cudaGetErrorString(cudaGetLastError()));
+  cudaFree(s->d_arr); s->d_arr = nullptr; s->arr_cap = 0;
+  if (entries == 0) return MIG_OK;
+  entries = (entries + 3u) & ~3u;
+  const size_t need = (size_t)s->n_envs * entries * sizeof(uint2);
+  if (cudaMalloc((void **)&s->d_arr, need) != cudaSuccess) {
+    cudaGetLastError(); s->d_arr = nullptr;
+    return fail(MIG_ENOMEM, "arrival lists: cudaMalloc of %zu bytes (%u envs x %u records x 8 B) failed; the handle now draws arrivals inside the event loop "
+                            "(slower, same results) -- choose a capacity that fits with mig_sim_set_arrival_buffer", need, s->n_envs, entries);
+  }
+  s->arr_cap = entries;
+  return MIG_OK;
+}
+
 extern "C" int mig_sim_set_arrival_buffer(mig_sim_t *s, uint32_t entries_per_env) {
   if (!s) return fail(MIG_EINVAL, "set_arrival_buffer: NULL handle");
   if (entries_per_env > MIG_MAX_JOBS) return fail(MIG_EINVAL, "set_arrival_buffer: more than %u entries per environment", MIG_MAX_JOBS);
-  s->arr_want = entries_per_env;
-  return MIG_OK;
+  if (entries_per_env == 0xFFFFFFFFu) entries_per_env = s->arr_default;
+  return alloc_arrival_lists(s, entries_per_env);
 }
+
+extern "C" uint32_t mig_sim_get_arrival_buffer(const mig_sim_t *s) { return s ? s->arr_cap : 0; }
 
 extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n_envs, uint64_t seed) {
   if (!out || !p) return fail(MIG_EINVAL, "create: NULL argument");
@@ -251,7 +287,7 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
     double want = acc + 8.0 * sqrt(acc + 1.0) + 64.0;
     if (p->job_limit && want > (double)p->job_limit + 1.0) want = (double)p->job_limit + 1.0;
     if (want > (double)MIG_MAX_JOBS) want = (double)MIG_MAX_JOBS;
-    s->arr_want = ((uint32_t)want + 7u) & ~7u;
+    s->arr_default = ((uint32_t)want + 7u) & ~7u;
   }
   ALLOC(s->d_jobtab, n * (s->ring_cap + kThreadTabExtra) * sizeof(uint4));
   ALLOC(s->d_dbgtab, (size_t)(s->ring_cap + kThreadTabExtra) * sizeof(uint4));
@@ -261,6 +297,8 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
   ALLOC(s->d_state, n * MIG_STATE_DIM * sizeof(float));
   ALLOC(s->d_action, n);
 #undef ALLOC
+  rc = alloc_arrival_lists(s, s->arr_default);            // a full day per environment: every launch's horizon fits
+  if (rc) { mig_sim_destroy(s); return rc; }
   if (cudaMemcpy(s->d_tab, host.data(), sizeof(DevTables), cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemset(s->d_hdr, 0, n * kHeaderWords * 4) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) {
     mig_sim_destroy(s); return fail(MIG_ECUDA, "create: table upload failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -275,12 +313,44 @@ extern "C" int mig_sim_destroy(mig_sim_t *s) {
   cudaFree(s->d_tab); cudaFree(s->d_hdr); cudaFree(s->d_jobtab); cudaFree(s->d_dbgtab); cudaFree(s->d_dbghdr); cudaFree(s->d_counter);
   cudaFree(s->d_algo); cudaFree(s->d_cfg0); cudaFree(s->d_state); cudaFree(s->d_action); cudaFree(s->d_table);
   cudaFree(s->d_recs); cudaFree(s->d_totals); cudaFree(s->d_script); cudaFree(s->d_arr);
+  for (auto &sp : s->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+  for (auto e : s->ev_pool) cudaEventDestroy(e);
   cudaGetLastError();
   delete s;
   return MIG_OK;
 }
 
 extern "C" uint64_t mig_sim_launch_count(const mig_sim_t *s) { return s ? s->launches : 0; }
+
+extern "C" const char *mig_sim_kernel_name(const mig_sim_t *s) {
+  if (!s) return "";
+  switch (s->tile) {
+    case 1: return s->p.decide_on_events ? "sim_thread_kernel<64,false,true>" : "sim_thread_kernel<64,false,false>";
+    case 8: return "sim_kernel<8,false>";
+    case 16: return "sim_kernel<16,false>";
+    default: return "sim_kernel<32,false>";
+  }
+}
+
+extern "C" int mig_sim_set_profiling(mig_sim_t *s, int on) {
+  if (!s) return fail(MIG_EINVAL, "set_profiling: NULL handle");
+  s->prof = on != 0;
+  return MIG_OK;
+}
+
+extern "C" int mig_sim_kernel_times(mig_sim_t *s, float ms_out[3], uint32_t launches_out[3]) {
+  if (!s || !ms_out) return fail(MIG_EINVAL, "kernel_times: NULL argument");
+  for (int c = 0; c < CAT_COUNT; ++c) { ms_out[c] = 0.0f; if (launches_out) launches_out[c] = 0; }
+  for (auto &sp : s->spans) {
+    CU(cudaEventSynchronize(sp.b));
+    float ms = 0.0f;
+    CU(cudaEventElapsedTime(&ms, sp.a, sp.b));
+    ms_out[sp.cat] += ms; if (launches_out) launches_out[sp.cat]++;
+    s->ev_pool.push_back(sp.a); s->ev_pool.push_back(sp.b);
+  }
+  s->spans.clear();
+  return MIG_OK;
+}
 
 // ------------------------------------------------------------------------------------------------ launches
 static void base_args(const mig_sim *s, SimArgs &a) {
@@ -314,22 +384,28 @@ static uint32_t auto_envs_per_warp(const mig_sim *s, uint32_t n_envs) {
 template <bool TRACE>
 static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
   if (s->tile == 1) {                                     // one thread per environment, one CTA per 64 environments
-    if (s->arr_want && a.n_steps > 0 && !a.script) {      // arrival lists: allocated on first use; inline generation if they do not fit
-      if (s->d_arr && s->arr_cap != s->arr_want) { CU(cudaStreamSynchronize(st)); cudaFree(s->d_arr); s->d_arr = nullptr; s->arr_cap = 0; }
-      if (!s->d_arr) {
-        size_t free_b = 0, total_b = 0;
-        const size_t need = (size_t)s->n_envs * s->arr_want * sizeof(uint4);
-        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need <= free_b / 2 && cudaMalloc((void **)&s->d_arr, need) == cudaSuccess) s->arr_cap = s->arr_want;
-        else { cudaGetLastError(); s->d_arr = nullptr; s->arr_cap = 0; s->arr_want = 0; }
-      }
-    }
     SimArgs b = a;
-    b.arr = s->arr_want ? s->d_arr : nullptr; b.arr_cap = s->arr_cap;
+    // arrivals of this launch's horizon: drawn by the generator kernel into the per-environment lists, on the same stream,
+    // before the event loop runs (not for scripted arrivals, nor for the one-env debug trace, which draws its own)
+    const bool lists = s->d_arr && a.n_steps > 0 && !a.script && !a.from_init && !a.hdr_override;
+    if (lists) {
+      GenArgs g; memset(&g, 0, sizeof(g));
+      g.tab = a.tab; g.hdr = a.hdr; g.arr = s->d_arr; g.arr_cap = s->arr_cap; g.n_envs = a.n_envs; g.env_first = a.env_first;
+      g.k0 = a.k0; g.k1 = a.k1; g.episode = a.episode; g.env_base = a.env_base; g.gap_scale = a.gap_scale;
+      g.day_s = a.day_s; g.epoch_s = a.epoch_s; g.n_epochs = a.n_epochs; g.n_steps = a.n_steps; g.job_limit = a.job_limit;
+      { ProfSpan ps(s, st, CAT_GEN); gen_arrivals_kernel<<<(a.n_envs + kGenWarps - 1) / kGenWarps, kGenWarps * 32, 0, st>>>(g); }
+      CU(cudaGetLastError());
+      s->launches++;
+    }
+    b.arr = lists ? s->d_arr : nullptr; b.arr_cap = s->arr_cap;
     b.envs_per_warp = s->envs_per_warp ? s->envs_per_warp : auto_envs_per_warp(s, b.n_envs);
     const uint32_t per_cta = b.envs_per_warp * (kThreadCta / 32);
     const dim3 grid((b.n_envs + per_cta - 1) / per_cta), block(kThreadCta);
-    if (b.ev_decide) sim_thread_kernel<kThreadCta, TRACE, true><<<grid, block, s->smem_bytes, st>>>(b);
-    else sim_thread_kernel<kThreadCta, TRACE, false><<<grid, block, s->smem_bytes, st>>>(b);
+    {
+      ProfSpan ps(s, st, CAT_SIM);
+      if (b.ev_decide) sim_thread_kernel<kThreadCta, TRACE, true><<<grid, block, s->smem_bytes, st>>>(b);
+      else sim_thread_kernel<kThreadCta, TRACE, false><<<grid, block, s->smem_bytes, st>>>(b);
+    }
     CU(cudaGetLastError());
     s->launches++;
     return MIG_OK;
@@ -339,10 +415,13 @@ static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
   int ctas = (int)((a.n_envs + envs_per_cta - 1) / envs_per_cta);
   if (ctas > s->grid_max) ctas = s->grid_max;
   const dim3 grid((unsigned)ctas), block(kWarpsPerCta * 32);
-  switch (s->tile) {
-    case 8: sim_kernel<8, TRACE><<<grid, block, s->smem_bytes, st>>>(a); break;
-    case 16: sim_kernel<16, TRACE><<<grid, block, s->smem_bytes, st>>>(a); break;
-    default: sim_kernel<32, TRACE><<<grid, block, s->smem_bytes, st>>>(a); break;
+  {
+    ProfSpan ps(s, st, CAT_SIM);
+    switch (s->tile) {
+      case 8: sim_kernel<8, TRACE><<<grid, block, s->smem_bytes, st>>>(a); break;
+      case 16: sim_kernel<16, TRACE><<<grid, block, s->smem_bytes, st>>>(a); break;
+      default: sim_kernel<32, TRACE><<<grid, block, s->smem_bytes, st>>>(a); break;
+    }
   }
   CU(cudaGetLastError());
   s->launches++;
@@ -428,7 +507,8 @@ extern "C" int mig_sim_rollout(mig_sim_t *s, int policy, const uint8_t *table, c
     QArgs qa; memset(&qa, 0, sizeof(qa));
     qa.state = s->d_state; qa.B = s->n_envs; qa.action_out = s->d_action; qa.eps_thr = eps_thr;
     qa.epoch = (uint32_t)s->epoch; qa.k0 = (uint32_t)s->seed; qa.k1 = (uint32_t)(s->seed >> 32); qa.episode = s->episode; qa.env_base = s->p.env_base;
-    int rc = launch_qnet(q, qa, st);
+    int rc;
+    { ProfSpan ps(s, st, CAT_QNET); rc = launch_qnet(q, qa, st); }
     if (rc) return rc;
     s->launches++;
     SimArgs a; base_args(s, a);

@@ -8,6 +8,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "philox.cuh"
 #include "sim_common.h"
 
 namespace migsim {
@@ -26,18 +27,6 @@ struct QArgs {
   uint32_t eps_thr;     // explore iff w_explore < eps_thr = min(round(eps 2^32), 2^32 - 1)
   uint32_t epoch, k0, k1, episode, env_base;
 };
-
-__device__ __forceinline__ uint4 philox_q(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
-#pragma unroll
-  for (int r = 0; r < 10; ++r) {
-    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-    uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
-    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
-    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
-  }
-  return make_uint4(c0, c1, c2, c3);
-}
 
 // one dense layer for the CTA's 32 rows.  A thread computes a register tile of kQCols adjacent columns x kQRpt rows
 // (32 accumulators); W is streamed through shared memory in chunks of kQChunk rows with cp.async (one copy per CTA, no
@@ -146,7 +135,7 @@ __global__ void __launch_bounds__(256) qnet_kernel(const QArgs a) {      // H / 
     for (int n = 1; n < A; ++n) { float v = qo[n * kQRows + tid]; if (v > bv) { bv = v; best = n; } }   // lowest index on ties
     if (a.argmax_out) a.argmax_out[row] = (uint8_t)best;
     if (a.action_out) {
-      uint4 w = philox_q(a.epoch, 2u, a.env_base + row, a.episode, a.k0, a.k1);
+      uint4 w = philox4x32_10(a.epoch, 2u, a.env_base + row, a.episode, a.k0, a.k1);
       bool explore = w.x < a.eps_thr;
       a.action_out[row] = explore ? (uint8_t)(((unsigned long long)w.y * (unsigned long long)A) >> 32) : (uint8_t)best;
     }

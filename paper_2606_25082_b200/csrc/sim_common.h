@@ -18,7 +18,7 @@ constexpr uint32_t kIdMask = 0xFFFFFu;
 struct DevTables {
   uint4 speed[MIG_MAX_CLASSES * 5];         // {v, magic m, shift (>=32: v == 1), 0}: x / v = umulhi(x, m) >> sh
   int32_t dur7_q[MIG_MAX_CLASSES * 65];
-  uint32_t class_cum[MIG_MAX_CLASSES];
+  uint32_t class_cum[MIG_MAX_CLASSES];       // padded with 0xFFFFFFFF beyond n_classes
   uint32_t slack_lo[MIG_MAX_CLASSES], slack_span[MIG_MAX_CLASSES];  // lo, hi - lo + 1
   uint32_t cfg_pack[MIG_MAX_CONFIGS];       // 7 nibbles: size of the slice starting at slot p
   uint32_t cfg_rank[MIG_MAX_CONFIGS];       // nibble p: rank of that slice among the configuration's in (size, slot) order
@@ -58,7 +58,7 @@ struct SimArgs {
   int ev_decide;                                     // TABLE policy: look the table up again after every tick with an arrival or a completion
   const uint8_t *actions; uint32_t act_stride_env, act_stride_k;   // action = actions[env * se + (k - k_first) * sk]
   const mig_job_t *script; uint32_t n_script;
-  uint4 *arr; uint32_t arr_cap;                      // thread-per-env kernel: pre-generated arrival lists [n_envs][arr_cap] {tick, class, work, due}, or NULL
+  const uint2 *arr; uint32_t arr_cap;                // thread-per-env kernel: arrival lists [n_envs][arr_cap] of 8-byte records (gen_kernel.cuh), or NULL
   // outputs (NULL = skip)
   float *state_out; float *reward_out; int64_t *energy_out; int64_t *tard_out;
   mig_epoch_rec_t *recs; int32_t rec_k0; mig_epoch_rec_t *drain_rec;   // record of epoch k -> recs[(k - rec_k0) * n_envs_total + env]

@@ -19,6 +19,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "philox.cuh"
 #include "sim_common.h"
 
 namespace migsim {
@@ -47,19 +48,6 @@ struct HotTables {               // per CTA, shared memory
 __host__ __device__ constexpr size_t tile_smem_bytes(uint32_t smem_entries) {
   // scratch + two 8-byte arrays; + 64 so that consecutive tiles start 64 B apart modulo 128 (LDS.64 of two tiles = one wavefront)
   return (size_t)WS_WORDS * 4 + (size_t)smem_entries * 16 + 64;
-}
-
-__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
-  // Salmon et al., SC'11: ten rounds of two 32x32->64 multiplies, key bumped by the Weyl constants (R1)
-#pragma unroll
-  for (int r = 0; r < 10; ++r) {
-    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-    uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
-    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
-    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
-  }
-  return make_uint4(c0, c1, c2, c3);
 }
 
 __device__ __forceinline__ int sidx_of(int size) { return size == 7 ? 4 : size - 1; }   // 1,2,3,4,7 -> 0..4
@@ -808,7 +796,8 @@ struct Env {
   }
 
   __device__ __forceinline__ void init(uint32_t env_local) {
-    algo = a.algo[env_local]; if (algo > MIG_ALGO_EDF_SS_R) algo &= 3; t = 0; epoch = 0; status = 0; n_sys = 0;
+    algo = a.algo[env_local]; t = 0; epoch = 0; status = 0; n_sys = 0;
+    if (algo > MIG_ALGO_EDF_SS_R) { algo = MIG_ALGO_EDF_FS; status |= MIG_ST_BAD_ALGO; }   // reading #28
     h_lo = 0x84222325u; h_hi = 0xcbf29ce4u;                   // FNV-1a-64 offset basis
     uint32_t c0 = a.cfg0[env_local];
     if (c0 >= a.n_configs) { c0 = 0; status |= MIG_ST_BAD_ACTION; }

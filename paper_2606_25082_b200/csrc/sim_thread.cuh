@@ -15,13 +15,16 @@
 //     smallest records, a ring in global memory for the rest.  The reschedule's "all jobs in priority order"
 //      is a merge of the <= 7 running jobs with the queue's front; arrivals are inserted from the tail,
 //     re-queued jobs from the front (deadlines grow with arrival time, so both are O(1) in practice);
-//   * ARRIVALS are drawn before the event loop starts, in one loop that all lanes run in step, into a per-environment
-//     list in global memory (the arrival process does not depend on the schedule).
+//   * ARRIVALS are drawn before the event loop starts, by gen_arrivals_kernel (gen_kernel.cuh: one warp per environment,
+//     32 thinning candidates per pass), into a per-environment list of 8-byte records in global memory (the arrival
+//     process does not depend on the schedule); the event loop copies four records at a time into a
+//     shared-memory landing slot with cp.async, one block ahead.
 // Per-thread data is in shared memory, interleaved by thread (row r of thread tid at base[r * NT + tid]: every access
 // of a warp is bank-conflict-free whatever index each lane uses).  Scalars (time, hash, energy, generator, look-ahead
 // arrival) live in registers.  The results are bit-identical to the tile kernels and to the oracle
 // (tests/test_gpu_parity.py); no code is shared with oracle/.
 #pragma once
+#include "gen_kernel.cuh"
 #include "sim_device.cuh"
 
 namespace migsim {
@@ -37,27 +40,48 @@ enum { T1_V = 0 /* 7: speed of the running job */, T1_STGDUE = 7 /* 7 */, T1_CNT
 // saved per-env header of this kernel (kHeaderWords words); the running totals H1_TOT / H1_CNT live here all the time
 enum { H1_T = 0, H1_PK, H1_NSYS, H1_NWAIT, H1_HLO, H1_HHI, H1_GK, H1_GT_LO, H1_GT_HI, H1_GDONE, H1_NACC, H1_ISCRIPT,
        H1_DROPS, H1_MASKS /* busy | down << 8 */, H1_ORDER, H1_QHEAD, H1_QNS, H1_GHEAD, H1_QNG, H1_TOT = 20 /* 6 */, H1_LOOKV = 26, H1_LOOKTICK, H1_LOOKCLS, H1_LOOKWORK,
-       H1_LOOKDUE, H1_LOOKID, H1_CNT = 48 /* 10 */ };
+       H1_LOOKDUE, H1_LOOKID, H1_ACOUNT = 32, H1_AMORE, H1_AID0 /* written by gen_arrivals_kernel */, H1_CNT = 48 /* 10 */ };
+static_assert((int)H1_PK == (int)HG_PK && (int)H1_GK == (int)HG_GK && (int)H1_NACC == (int)HG_NACC && (int)H1_ACOUNT == (int)HG_ACOUNT && (int)H1_AID0 == (int)HG_AID0, "header layout shared with gen_kernel.cuh");
 
 struct HotTablesT {              // per CTA, shared memory
   HotTables h;
   uint32_t cfg_rank[MIG_MAX_CONFIGS];     // nibble p: rank of the slice starting at slot p in (size, slot) order (reading #4)
   uint32_t cfg_slot_of[MIG_MAX_CONFIGS];  // nibble r: start slot of the slice of rank r
   int32_t cfg_pidle[MIG_MAX_CONFIGS];     // sum of p_idle over the slices of the configuration
-  uint32_t logT[257];
-  uint32_t class_cum[MIG_MAX_CLASSES];    // padded with 0xFFFFFFFF beyond n_classes
-};
-
-// The generator's larger tables, copied over the (not yet used) per-thread rows while a launch pre-generates its arrivals:
-// the thinning / duration lookups sit on the dependent chain of every candidate and would otherwise be L2 round trips.
-struct GenTables {
-  uint32_t thr[MIG_THR_BINS];
-  int32_t dur7_q[MIG_MAX_CLASSES * 65];
-  uint32_t slack_lo[MIG_MAX_CLASSES], slack_span[MIG_MAX_CLASSES];
 };
 
 __host__ __device__ constexpr size_t thread_smem_bytes(uint32_t smem_entries, int nt) {
-  return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * ((T2_RING + 2 * (size_t)smem_entries) * 8 + T1_WORDS * 4 + 16);   // + one 16-byte landing slot
+  return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * ((T2_RING + 2 * (size_t)smem_entries) * 8 + T1_WORDS * 4 + 32);   // + a 32-byte landing slot: four arrival records
+}
+
+// The one-at-a-time arrival generator: draws thinning candidates from (g_k, g_T) until one is accepted or the day ends
+// (R2-R5; tables from global memory).  A free function with everything passed and returned BY VALUE and not
+// inlined: it is off the hot path, must not cost the event loop registers, and must not make the environment's state
+// addressable (a non-inlined member function would pin the whole EnvT in local memory).
+struct InlineDraw { uint32_t g_k; unsigned long long g_T; uint32_t done, found, tick, cls, dur7, slack; };
+static __device__ __noinline__ InlineDraw draw_next_arrival(const DevTables *tb, uint32_t env_g, uint32_t episode, uint32_t k0, uint32_t k1,
+                                                            unsigned long long gap_scale, int day_s, uint32_t g_k, unsigned long long g_T) {
+  InlineDraw d; d.done = 0; d.found = 0; d.tick = 0; d.cls = 0; d.dur7 = 0; d.slack = 0;
+  uint4 w; unsigned long long tick; uint32_t k;
+  for (;;) {
+    k = g_k++;
+    w = philox4x32_10(k, 0u, env_g, episode, k0, k1);                          // stream 0: gap, accept, class, slack
+    g_T += ((unsigned long long)neglog2_q24_tab(w.x, tb->logT) * gap_scale) >> 24;
+    tick = g_T >> 16;
+    if (tick >= (unsigned long long)day_s) { d.done = 1; break; }               // arrivals stop at the end of the day
+    if (w.y <= __ldg(&tb->thr[(uint32_t)tick / 60u])) { d.found = 1; break; }   // Lewis-Shedler thinning
+  }
+  d.g_k = g_k; d.g_T = g_T;
+  if (d.found) {
+    const uint32_t c = class_of(w.z, tb->class_cum);                            // (padded with 0xFFFFFFFF beyond n_classes)
+    const uint4 wd = philox4x32_10(k, 1u, env_g, episode, k0, k1);              // stream 1: duration
+    const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
+    const int q0 = __ldg(&tb->dur7_q[c * 65 + qi]), q1 = __ldg(&tb->dur7_q[c * 65 + qi + 1]);
+    d.dur7 = (uint32_t)(q0 + (int)(((long long)(q1 - q0) * (long long)f) >> 10));
+    d.slack = __ldg(&tb->slack_lo[c]) + __umulhi(w.w, __ldg(&tb->slack_span[c]));
+    d.tick = (uint32_t)tick; d.cls = c;
+  }
+  return d;
 }
 
 template <int NT, bool TRACE, bool EVD>     // EVD: event-driven decisions of the tabulated policy compiled in (reading #27)
@@ -82,10 +106,9 @@ struct EnvT {
   int look_valid, look_tick, look_work, look_due; uint32_t look_cls, look_id;
   uint32_t n_trace, i_script, n_events;
   uint32_t env_l; bool in_drain;   // env index in the handle's arrays; the drain after the last epoch is running
-  uint4 *arr;              // this env's arrival list (NULL: generate inline)
-  uint32_t a_head, a_count, a_id0, a_more; int a_horizon;
-  uint4 *a_slot;           // shared-memory landing slot of the asynchronous copy of arr[a_head] (cp.async)
-  const GenTables *gt;     // the generator's tables in shared memory (valid during pre-generation only)
+  const uint2 *arr;        // this env's arrival list, written by gen_arrivals_kernel (NULL: generate inline)
+  uint32_t a_head, a_count, a_id0, a_more;
+  uint4 *land;             // landing slot of the asynchronous copy of four list records: rows land[0], land[NT] (cp.async)
 
   __device__ __forceinline__ EnvT(const SimArgs &a_, const HotTablesT &h_, uint2 *r2_, uint32_t *r1_)
       : a(a_), hot(h_), r2(r2_), r1(r1_), S(a_.smem_entries) {}
@@ -289,69 +312,33 @@ struct EnvT {
     U = u; P = hot.cfg_pidle[cfg] + pd + hot.h.curve[u & 7];
   }
 
-  // ------------------------------------------------------------------ arrival generator (R2-R5)
-  __device__ __forceinline__ uint32_t neglog2_q24(uint32_t w) const {
-    const uint32_t m = w | 1u;
-    const int lz = __clz((int)m);
-    const uint32_t y = m << lz;
-    const uint32_t i = (y >> 23) & 0xFFu, f = (y >> 7) & 0xFFFFu;
-    const uint32_t T0 = hot.logT[i], T1 = hot.logT[i + 1];
-    const uint32_t L = T0 + (uint32_t)(((unsigned long long)(T1 - T0) * f) >> 16);
-    return ((uint32_t)(1 + lz) << 24) - L;
-  }
-
-  // class, work and due date of the accepted candidate k (R5): {tick, class, work, due}
-  template <bool TS>
-  __device__ __forceinline__ uint4 job_attributes(uint32_t k, uint4 w, uint32_t tick) const {
-    uint32_t c = 0;
-#pragma unroll
-    for (int i = 0; i < MIG_MAX_CLASSES - 1; ++i) c += (w.z > hot.class_cum[i]) ? 1u : 0u;    // first c with w.z <= cum[c]
-    const uint4 wd = philox4x32_10(k, 1u, env_g, a.episode, a.k0, a.k1);     // stream 1: duration
-    const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
-    const int q0 = TS ? gt->dur7_q[c * 65 + qi] : __ldg(&a.tab->dur7_q[c * 65 + qi]), q1 = TS ? gt->dur7_q[c * 65 + qi + 1] : __ldg(&a.tab->dur7_q[c * 65 + qi + 1]);
-    const int dur7 = q0 + (int)(((long long)(q1 - q0) * (long long)f) >> 10);
-    const uint32_t slack = (TS ? gt->slack_lo[c] : __ldg(&a.tab->slack_lo[c])) + __umulhi(w.w, TS ? gt->slack_span[c] : __ldg(&a.tab->slack_span[c]));
-    unsigned long long rel = ((unsigned long long)(uint32_t)dur7 * slack) >> 10;
-    if (rel < 1) rel = 1;
-    return make_uint4(tick, c, (uint32_t)dur7 * hot.h.speed[c * 5 + 4].x, (uint32_t)((long long)tick + (long long)rel));
-  }
+  // ------------------------------------------------------------------ arrivals (R2-R5)
   __device__ __forceinline__ uint32_t job_limit() const { return a.job_limit ? min(a.job_limit, MIG_MAX_JOBS) : MIG_MAX_JOBS; }
 
-  // Pre-generation (a.arr != NULL): at the start of a launch every lane draws ALL candidates up to the launch's horizon,
-  // one candidate per trip of ONE loop -- every lane of the warp executes the same instructions (the thinning loop of
-  // the inline generator below runs a lane-dependent number of trips per arrival) -- and appends the accepted ones to
-  // its arrival list in global memory, from which the event loop then reads its look-ahead.  A candidate beyond the
-  // horizon or the list's capacity is NOT committed (g_k, g_T stay before it), so generation resumes exactly there.
-  template <bool TS>
-  __device__ __forceinline__ void fill_arrivals() {
-    a_head = 0; a_count = 0; a_more = 0;
-    a_id0 = n_accepted;
-    if (look_valid) {                               // a look-ahead carried over from a launch of the inline generator
-      arr[0] = make_uint4((uint32_t)look_tick, look_cls, (uint32_t)look_work, (uint32_t)look_due);
-      a_id0 = look_id; a_count = 1; look_valid = 0;
-    }
-    const uint32_t limit = job_limit();
-    while (!g_done && n_accepted < limit) {
-      const uint32_t k = g_k;
-      const uint4 w = philox4x32_10(k, 0u, env_g, a.episode, a.k0, a.k1);    // stream 0: gap, accept, class, slack
-      const unsigned long long T = g_T + (((unsigned long long)neglog2_q24(w.x) * a.gap_scale) >> 24);
-      const unsigned long long tick = T >> 16;
-      if (tick >= (unsigned long long)a.day_s) { g_done = 1; break; }         // arrivals stop at the end of the day
-      if (tick > (unsigned long long)a_horizon) break;
-      if (a_count == a.arr_cap) { a_more = 1; break; }
-      g_k = k + 1; g_T = T;
-      if (w.y <= (TS ? gt->thr[(uint32_t)tick / 60u] : __ldg(&a.tab->thr[(uint32_t)tick / 60u]))) {     // Lewis-Shedler thinning
-        __stcg(&arr[a_count++], job_attributes<TS>(k, w, (uint32_t)tick));       // streamed: keep L1 for the tables
-        n_accepted++;
-      }
-    }
+  // start the asynchronous copy of list records [b, b + 4) (one 32-byte sector) into this thread's landing slot
+  // (LDGSTS: no register waits for it).  b is a multiple of 4; the list's capacity is one too.
+  __device__ __forceinline__ void fetch_block(uint32_t b) {
+    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(land);
+    asm volatile("cp.async.cg.shared.global [%0], [%2], 16;\n\tcp.async.cg.shared.global [%1], [%3], 16;\n\tcp.async.commit_group;"
+                 ::"r"(dst), "r"(dst + (uint32_t)(NT * sizeof(uint4))), "l"(arr + b), "l"(arr + b + 2) : "memory");
   }
 
-  // start the asynchronous copy of arr[a_head] into this thread's landing slot (LDGSTS: no register waits for it)
-  __device__ __forceinline__ void fetch_arrival() {
-    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(a_slot);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n\tcp.async.commit_group;" ::"r"(dst), "l"(arr + a_head) : "memory");
-    if ((a_head & 7u) == 0u && a_head + 8u < a_count) asm volatile("prefetch.global.L2 [%0];" ::"l"(arr + a_head + 8));   // next 128-byte line
+  // The one-at-a-time generator (draw_next_arrival below the struct's forward declaration): used when there is no list
+  // (debug trace, mig_sim_set_arrival_buffer(0)) and for the rest of a launch whose list filled up.
+  __device__ __forceinline__ void gen_next_inline() {
+    if (g_done || n_accepted >= job_limit()) return;
+    const InlineDraw d = draw_next_arrival(a.tab, env_g, a.episode, a.k0, a.k1, a.gap_scale, a.day_s, g_k, g_T);
+    g_k = d.g_k; g_T = d.g_T; g_done = d.done;
+    if (d.found) { set_look(d.tick, d.cls, d.dur7, d.slack); look_id = n_accepted++; }
+  }
+
+  // work and due date from the drawn attributes (R5): work = dur7 * v7, due = tick + max(1, dur7 * slack >> 10)
+  __device__ __forceinline__ void set_look(uint32_t tick, uint32_t cls, uint32_t dur7, uint32_t slack) {
+    unsigned long long rel = ((unsigned long long)dur7 * slack) >> 10;
+    if (rel < 1) rel = 1;
+    look_tick = (int)tick; look_cls = cls; look_work = (int)(dur7 * hot.h.speed[cls * 5 + 4].x);
+    look_due = (int)((long long)tick + (long long)rel);
+    look_valid = 1;
   }
 
   // advance the look-ahead to the next accepted arrival (or none)
@@ -366,37 +353,20 @@ struct EnvT {
       }
       return;
     }
-    if (arr) {                                                                // pre-generated list (kernel-uniform branch)
-      if (a_head == a_count) {
-        if (!a_more) return;
-        fill_arrivals<false>();                                               // the list was full: next stretch (rare; tables in global memory)
-        if (a_count == 0) return;
-        fetch_arrival();
+    if (arr) {                                                                // the launch's pre-generated list
+      if (a_head < a_count) {
+        const uint32_t j = a_head & 3u;
+        if (j == 0u) asm volatile("cp.async.wait_group 0;" ::: "memory");     // requested one block (>= 1 arrival) ago
+        const uint2 e = reinterpret_cast<const uint2 *>(land + (j >> 1) * NT)[j & 1u];
+        set_look(e.y & 0x1FFFFu, (e.x >> 25) & 15u, e.x & 0x1FFFFFFu, ((e.x >> 29) << 13) | (e.y >> 17));
+        look_id = a_id0 + a_head++;
+        if ((a_head & 3u) == 0u && a_head < a_count) fetch_block(a_head);
+        return;
       }
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
-      const uint4 e = *a_slot;                                                // copied one arrival ago: its latency is hidden
-      look_tick = (int)e.x; look_cls = e.y; look_work = (int)e.z; look_due = (int)e.w;
-      look_id = a_id0 + a_head++;
-      look_valid = 1;
-      if (a_head < a_count) fetch_arrival();
-      return;
+      if (!a_more) return;                                                    // nothing more inside this launch's horizon
+      arr = nullptr;                                                          // the list was too small: one at a time from here
     }
-    if (n_accepted >= job_limit()) return;
-    const DevTables *tb_ = a.tab;
-    uint4 w; unsigned long long tick; uint32_t k;
-    for (;;) {                                                                // inline: draw candidates until one is accepted
-      if (g_done) return;
-      k = g_k++;
-      w = philox4x32_10(k, 0u, env_g, a.episode, a.k0, a.k1);                // stream 0: gap, accept, class, slack
-      g_T += ((unsigned long long)neglog2_q24(w.x) * a.gap_scale) >> 24;
-      tick = g_T >> 16;
-      if (tick >= (unsigned long long)a.day_s) { g_done = 1; return; }        // arrivals stop at the end of the day
-      if (w.y <= __ldg(&tb_->thr[(uint32_t)tick / 60u])) break;               // Lewis-Shedler thinning
-    }
-    const uint4 e = job_attributes<false>(k, w, (uint32_t)tick);
-    look_tick = (int)e.x; look_cls = e.y; look_work = (int)e.z; look_due = (int)e.w;
-    look_id = n_accepted++;
-    look_valid = 1;
+    gen_next_inline();
   }
 
   // ------------------------------------------------------------------ reschedule
@@ -785,16 +755,16 @@ struct EnvT {
   }
 
   // ------------------------------------------------------------------ init / load / save
-  // init / load come in two parts: registers first (no per-thread shared-memory row is touched: the rows' space still
-  // holds the generator's tables during pre-generation), then the rows
   __device__ __forceinline__ void init_regs(uint32_t env_local) {
-    algo = a.algo[env_local]; if (algo > MIG_ALGO_EDF_SS_R) algo &= 3; t = 0; epoch = 0; status = 0; n_sys = 0; n_wait = 0; q_head = 0; q_ns = 0; g_head = 0; q_ng = 0;
+    algo = a.algo[env_local]; t = 0; epoch = 0; status = 0; n_sys = 0; n_wait = 0;
+    if (algo > MIG_ALGO_EDF_SS_R) { algo = MIG_ALGO_EDF_FS; status |= MIG_ST_BAD_ALGO; }   // reading #28
+    q_head = 0; q_ns = 0; g_head = 0; q_ng = 0;
     h_lo = 0x84222325u; h_hi = 0xcbf29ce4u;                   // FNV-1a-64 offset basis
     uint32_t c0 = a.cfg0[env_local];
     if (c0 >= a.n_configs) { c0 = 0; status |= MIG_ST_BAD_ACTION; }
     set_cfg_tables((int)c0);
     busy_mask = 0; down_mask = 0; run_order = 0xFFFFFFFFu; next_done = MIG_INF; next_up = MIG_INF; next_crit = MIG_INF;
-    g_k = 0; g_T = 0; g_done = 0; n_accepted = 0;
+    g_k = 0; g_T = 0; g_done = 0; n_accepted = 0; a_count = 0; a_more = 1; a_id0 = 0;
     look_valid = 0; look_tick = 0; look_work = 0; look_due = 0; look_cls = 0; look_id = 0;
     n_trace = 0; i_script = 0;
     for (int w = H1_DROPS; w < kHeaderWords; ++w) hdr[w] = 0u;      // running totals, drops
@@ -830,6 +800,7 @@ struct EnvT {
     busy_mask = hdr[H1_MASKS] & 0x7Fu; down_mask = (hdr[H1_MASKS] >> 8) & 0x7Fu; run_order = hdr[H1_ORDER];
     look_valid = (int)hdr[H1_LOOKV]; look_tick = (int)hdr[H1_LOOKTICK]; look_cls = hdr[H1_LOOKCLS];
     look_work = (int)hdr[H1_LOOKWORK]; look_due = (int)hdr[H1_LOOKDUE]; look_id = hdr[H1_LOOKID];
+    a_count = hdr[H1_ACOUNT]; a_more = hdr[H1_AMORE]; a_id0 = hdr[H1_AID0];      // this launch's list (gen_arrivals_kernel)
   }
   __device__ __forceinline__ void load_rows() {
     for (uint32_t p = 0; p < S; ++p) { const uint4 e = gtab[a.ring_cap + p]; SK(p) = make_uint2(e.x, e.y); SR(p) = make_uint2(e.z, e.w); }
@@ -912,50 +883,29 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
       hot.h.cfg_pack[i] = tb->cfg_pack[i]; hot.cfg_rank[i] = tb->cfg_rank[i]; hot.cfg_slot_of[i] = tb->cfg_slot_of[i]; hot.cfg_pidle[i] = tb->cfg_pidle[i];
     }
     if (threadIdx.x < 8) { hot.h.curve[threadIdx.x] = tb->curve[threadIdx.x]; hot.h.p_idle[threadIdx.x] = tb->p_idle[threadIdx.x]; hot.h.p_busy[threadIdx.x] = tb->p_busy[threadIdx.x]; }
-    for (int i = threadIdx.x; i < 257; i += NT) hot.logT[i] = tb->logT[i];
-    if (threadIdx.x < MIG_MAX_CLASSES) hot.class_cum[threadIdx.x] = threadIdx.x < a.n_classes ? tb->class_cum[threadIdx.x] : 0xFFFFFFFFu;
   }
   unsigned char *base = smem_raw + ((sizeof(HotTablesT) + 127) & ~(size_t)127);
-  const bool pregen = a.arr && !a.script && a.n_steps > 0;      // kernel-uniform
-  if (pregen) {
-    GenTables *g = reinterpret_cast<GenTables *>(base);
-    const DevTables *tb = a.tab;
-    for (int i = threadIdx.x; i < MIG_THR_BINS; i += NT) g->thr[i] = tb->thr[i];
-    for (int i = threadIdx.x; i < MIG_MAX_CLASSES * 65; i += NT) g->dur7_q[i] = tb->dur7_q[i];
-    if (threadIdx.x < MIG_MAX_CLASSES) { g->slack_lo[threadIdx.x] = tb->slack_lo[threadIdx.x]; g->slack_span[threadIdx.x] = tb->slack_span[threadIdx.x]; }
-  }
   __syncthreads();
   // lanes 0 .. envs_per_warp-1 of every warp hold an environment: small batches are spread over more warps (less
   // divergence per warp, more warps to hide latency); a full batch uses all 32 lanes
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t li = (blockIdx.x * (NT / 32) + (threadIdx.x >> 5)) * a.envs_per_warp + lane;   // index inside this launch's env range
   const bool alive = lane < a.envs_per_warp && li < a.n_envs;
+  if (!alive) return;
   uint2 *r2 = reinterpret_cast<uint2 *>(base) + threadIdx.x;
   uint32_t *r1 = reinterpret_cast<uint32_t *>(base + (size_t)NT * (T2_RING + 2 * (size_t)a.smem_entries) * 8) + threadIdx.x;
   EnvT<NT, TRACE, EVD> e(a, hot, r2, r1);
-  e.a_slot = reinterpret_cast<uint4 *>(base + (size_t)NT * ((T2_RING + 2 * (size_t)a.smem_entries) * 8 + T1_WORDS * 4)) + threadIdx.x;
-  const uint32_t env = a.env_first + (alive ? li : 0u);
-  e.gt = reinterpret_cast<const GenTables *>(base);
+  e.land = reinterpret_cast<uint4 *>(base + (size_t)NT * ((T2_RING + 2 * (size_t)a.smem_entries) * 8 + T1_WORDS * 4)) + threadIdx.x;
+  const uint32_t env = a.env_first + li;
   e.env_g = a.env_base + env; e.env_l = env; e.in_drain = false;
   e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * (a.ring_cap + kThreadTabExtra);
   e.hdr = a.hdr_override ? a.hdr_override : a.hdr + (size_t)env * kHeaderWords;
-  e.arr = (a.arr && !a.script) ? a.arr + (size_t)env * a.arr_cap : nullptr;
-  e.a_head = 0; e.a_count = 0; e.a_id0 = 0; e.a_more = 0;
-  if (alive) {
-    if (a.from_init) e.init_regs(env); else e.load_regs();
-    if (pregen && e.epoch < a.n_epochs) {                       // arrivals up to the end of the last epoch of this launch
-      e.a_horizon = min(e.epoch + a.n_steps, a.n_epochs) * a.epoch_s;
-      e.template fill_arrivals<true>();
-    }
-  }
-  __syncthreads();                                              // the tables make room for the per-thread rows
-  if (!alive) return;
-  if (a.from_init) e.init_rows(); else e.load_rows();
+  e.arr = (a.arr && !a.script) ? a.arr + (size_t)env * a.arr_cap : nullptr;   // (the host launches gen_arrivals_kernel first)
+  e.a_head = 0;
+  if (a.from_init) { e.init_regs(env); e.init_rows(); } else { e.load_regs(); e.load_rows(); }
   if (a.n_steps > 0 && e.epoch < a.n_epochs) {
-    if (e.arr) {
-      if (e.a_count) e.fetch_arrival();
-      e.gen_next();
-    } else if (!e.look_valid) e.gen_next();                     // prime the inline generator's look-ahead
+    if (e.arr && e.a_count) e.fetch_block(0);
+    if (!e.look_valid) e.gen_next();                            // prime the look-ahead (one may be carried over from the last launch)
   }
   e.run(li, env);
   if (a.state_out) e.observe(a.state_out + (size_t)(TRACE ? 0u : env) * MIG_STATE_DIM);
