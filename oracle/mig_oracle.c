@@ -21,6 +21,8 @@
 #define NO_SLOT (-1)
 
 static const int SIZE_IDX[8] = { -1, 0, 1, 2, 3, -1, -1, 4 }; /* slice size g -> column of the [..][5] tables */
+/* size code 8 = the whole GPU with MIG disabled (reading #29): own speed and power, 7 compute units */
+static int units_of(int size) { return size == ORC_SIZE_NOMIG ? 7 : size; }
 
 /* ------------------------------------------------------------------------------------------------
  * R1: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11).  counter (c0..c3), key (k0,k1); ten rounds,
@@ -98,6 +100,7 @@ struct orc_env {
   orc_params_t p;
   /* owned copies of the tables */
   uint32_t *speed; int32_t *dur7_q; uint32_t *class_cum; uint16_t *slack_q10; uint8_t *size_at_slot; uint32_t *accept_thr;
+  uint32_t *speed_nomig; int32_t *dbin_edges, *abin_edges;
   uint64_t seed; uint32_t env_id, episode;
   /* scripted arrivals */
   orc_job_in_t *script; uint32_t n_script, i_script; int scripted;
@@ -116,6 +119,8 @@ struct orc_env {
   orc_event_t *trace; uint32_t trace_cap, n_trace;
   /* event-driven decisions (reading #27): this env's table [n_epochs][4], or NULL */
   const uint8_t *ev_table;
+  const uint8_t *bin_table;        /* BINNED policy: the shared table (event-driven look-ups), or NULL */
+  int32_t util_s[8];                /* seconds spent with U busy compute units */
 };
 
 static void *dup_mem(const void *src, size_t n) { void *d = malloc(n ? n : 1); if (n) memcpy(d, src, n); return d; }
@@ -130,6 +135,9 @@ orc_env_t *orc_env_create(const orc_params_t *p, uint64_t seed, uint32_t env_id)
   e->slack_q10 = (uint16_t *)dup_mem(p->slack_q10, sizeof(uint16_t) * 2 * p->n_classes);
   e->size_at_slot = (uint8_t *)dup_mem(p->size_at_slot, 7 * p->n_configs);
   e->accept_thr = (uint32_t *)dup_mem(p->accept_thr, sizeof(uint32_t) * 1440);
+  e->speed_nomig = p->speed_nomig ? (uint32_t *)dup_mem(p->speed_nomig, sizeof(uint32_t) * p->n_classes) : NULL;
+  e->dbin_edges = (p->dbin_edges && p->n_dbins > 1) ? (int32_t *)dup_mem(p->dbin_edges, sizeof(int32_t) * (p->n_dbins - 1)) : NULL;
+  e->abin_edges = (p->abin_edges && p->n_abins > 1) ? (int32_t *)dup_mem(p->abin_edges, sizeof(int32_t) * (p->n_abins - 1)) : NULL;
   e->seed = seed; e->env_id = env_id;
   e->jobs = (job_t *)calloc(p->cap ? p->cap : 1, sizeof(job_t));
   build_log_table();
@@ -140,6 +148,7 @@ void orc_env_destroy(orc_env_t *e)
 {
   if (!e) return;
   free(e->speed); free(e->dur7_q); free(e->class_cum); free(e->slack_q10); free(e->size_at_slot); free(e->accept_thr);
+  free(e->speed_nomig); free(e->dbin_edges); free(e->abin_edges);
   free(e->script); free(e->jobs); free(e);
 }
 
@@ -169,7 +178,11 @@ static void emit(orc_env_t *e, int type, int slot, uint32_t aux, uint32_t job, i
 }
 
 /* ---------------------------------------------------------------------------------------------- generator */
-static uint32_t speed_of(const orc_env_t *e, uint32_t cls, int size) { return e->speed[cls * 5 + SIZE_IDX[size]]; }
+static uint32_t speed_of(const orc_env_t *e, uint32_t cls, int size)
+{
+  if (size == ORC_SIZE_NOMIG) return e->speed_nomig[cls];          /* MIG disabled: its own column */
+  return e->speed[cls * 5 + SIZE_IDX[size]];
+}
 
 /* R2-R5: advance to the next accepted arrival (or mark the generator done) */
 static void gen_next(orc_env_t *e)
@@ -240,6 +253,10 @@ static void power_now(const orc_env_t *e, int64_t *P, int *U)
   for (int p = 0; p < ORC_SLOTS; ++p) {
     const slice_t *sl = &e->sl[p];
     if (!sl->size) continue;
+    if (sl->size == ORC_SIZE_NOMIG) {
+      if (sl->job != NONE_JOB) { u += 7; s += e->p.p_busy_nomig_mw; } else s += e->p.p_idle_nomig_mw;
+      continue;
+    }
     if (sl->job != NONE_JOB) { u += sl->size; s += e->p.p_busy_mw[SIZE_IDX[sl->size]]; }
     else s += e->p.p_idle_mw[SIZE_IDX[sl->size]];
   }
@@ -420,6 +437,44 @@ static void remove_job(orc_env_t *e, uint32_t idx)
   e->n_sys--;
 }
 
+/* ---------------------------------------------------------------------------------------------- binned state */
+/* "2+2m different features: the current MIG configuration, time, and the deadlines and average duration
+ * of the first m jobs ... binned", m = 3.  Reading #31: the first m jobs are the first three in (due, id) order over all
+ * jobs in system; the deadline feature is due - t, the average duration the mean remaining duration over the slices of
+ * the current configuration (as in LALF, L183); a value falls in the first bin i with value < edge[i] (else the last
+ * bin); an absent job has code 0, a present one code 1 + dbin * n_abins + abin; time bin = min(t, day_s - 1) * n_tbins
+ * / day_s.  index = (((cfg * n_tbins + tbin) * B + code_0) * B + code_1) * B + code_2 with B = 1 + n_dbins * n_abins. */
+static uint32_t bin_of(int64_t v, const int32_t *edges, uint32_t n_bins)
+{
+  uint32_t b = 0;
+  while (b + 1 < n_bins && v >= (int64_t)edges[b]) ++b;
+  return b;
+}
+uint32_t orc_env_binned_index(const orc_env_t *e)
+{
+  const orc_params_t *p = &e->p;
+  uint32_t B = 1u + p->n_dbins * p->n_abins;
+  int64_t tc = e->t < p->day_s - 1 ? e->t : p->day_s - 1;
+  uint32_t tbin = (uint32_t)((tc * (int64_t)p->n_tbins) / p->day_s);
+  uint32_t idx = (uint32_t)e->cfg * p->n_tbins + tbin;
+  char *taken = (char *)calloc(e->n_sys ? e->n_sys : 1, 1);
+  for (int m = 0; m < 3; ++m) {
+    int best = -1;                              /* jobs[] is in id order: strict '<' keeps the lowest id on ties */
+    for (uint32_t i = 0; i < e->n_sys; ++i) if (!taken[i] && (best < 0 || e->jobs[i].due < e->jobs[best].due)) best = (int)i;
+    uint32_t code = 0;
+    if (best >= 0) {
+      taken[best] = 1;
+      uint32_t db = bin_of((int64_t)e->jobs[best].due - e->t, e->dbin_edges, p->n_dbins);
+      uint32_t ab = bin_of((int64_t)rd_mean_cfg(e, &e->jobs[best]), e->abin_edges, p->n_abins);
+      code = 1u + db * p->n_abins + ab;
+    }
+    idx = idx * B + code;
+  }
+  free(taken);
+  return idx;
+}
+void orc_env_util_hist(const orc_env_t *e, int32_t out[8]) { memcpy(out, e->util_s, sizeof(e->util_s)); }
+
 /* ---------------------------------------------------------------------------------------------- event loop */
 static void repartition(orc_env_t *e, uint8_t action);
 
@@ -442,6 +497,7 @@ static void run_until(orc_env_t *e, int32_t t_end, int drain)
     /* integrate power and progress over [t, tn) */
     int64_t P; int U; power_now(e, &P, &U);
     e->ep.energy += P * dt; e->ep.busy += (int64_t)U * dt;
+    e->util_s[U] += (int32_t)dt;                                /* time at this utilisation level (Fig. 6) */
     for (int p = 0; p < ORC_SLOTS; ++p) {
       slice_t *s = &e->sl[p];
       if (s->size && s->job != NONE_JOB) { job_t *j = find_job(e, s->job); j->rem -= (int32_t)(dt * (int64_t)speed_of(e, j->cls, s->size)); }
@@ -494,9 +550,9 @@ static void run_until(orc_env_t *e, int32_t t_end, int drain)
     /* Event-driven decision ("re-partitioning can happen when a job arrives or is completed"; reading
      * #27): after a tick of the day in which a job arrived or completed, the tabulated policy is looked up again with
      * the load bucket of that moment; a different configuration is a repartition at this very tick (it reschedules). */
-    if (job_event && e->ev_table && !drain) {
+    if (job_event && (e->ev_table || e->bin_table) && !drain) {
       uint32_t n = e->n_sys; int b = n == 0 ? 0 : (n < 8 ? 1 : (n < 64 ? 2 : 3));
-      uint8_t action = e->ev_table[e->epoch * 4 + b];
+      uint8_t action = e->bin_table ? e->bin_table[orc_env_binned_index(e)] : e->ev_table[e->epoch * 4 + b];
       if (action >= e->p.n_configs) e->status |= ORC_ST_BAD_ACTION;
       else if ((int)action != e->cfg) { repartition(e, action); happened = 0; }
     }
@@ -520,7 +576,7 @@ static void repartition(orc_env_t *e, uint8_t action)
   const uint8_t *row = &e->size_at_slot[(uint32_t)action * 7];
   for (int p = 0; p < ORC_SLOTS; ++p) {                   /* destroyed slices, ascending slot: running job goes back to waiting */
     slice_t *s = &e->sl[p];
-    if (s->size && s->size != row[p]) {
+    if (s->size && (s->size != row[p] || e->p.repart_all_down)) {   /* reading #30: the whole GPU goes down */
       if (s->job != NONE_JOB) {
         job_t *j = find_job(e, s->job);
         emit(e, ORC_EV_PREEMPT, p, (uint32_t)s->size, j->id, j->rem);
@@ -531,7 +587,7 @@ static void repartition(orc_env_t *e, uint8_t action)
   }
   for (int p = 0; p < ORC_SLOTS; ++p) {
     slice_t *s = &e->sl[p];
-    if (s->size == row[p]) continue;                      /* same (start, size) in both rows: keeps job and up_at */
+    if (s->size == row[p] && !e->p.repart_all_down) continue;   /* same (start, size) in both rows: keeps job and up_at */
     s->size = row[p]; s->job = NONE_JOB; s->down = 0; s->up_at = 0;
     if (s->size && e->p.repart_downtime_s > 0) { s->down = 1; s->up_at = e->t + e->p.repart_downtime_s; }
   }
@@ -551,6 +607,7 @@ void orc_env_reset(orc_env_t *e, uint32_t episode, uint8_t algo, uint8_t cfg0)
   e->hash = 0xcbf29ce484222325ull;
   memset(&e->ep, 0, sizeof(e->ep)); memset(&e->tot, 0, sizeof(e->tot));
   e->last_epoch_drops = 0; e->n_trace = 0;
+  memset(e->util_s, 0, sizeof(e->util_s));
   const uint8_t *row = &e->size_at_slot[(uint32_t)cfg0 * 7];
   for (int p = 0; p < ORC_SLOTS; ++p) { e->sl[p].size = row[p]; e->sl[p].down = 0; e->sl[p].up_at = 0; e->sl[p].job = NONE_JOB; }
   e->gen_k = 0; e->gen_Tq16 = 0; e->gen_done = 0; e->n_accepted = 0; e->i_script = 0;
@@ -616,7 +673,7 @@ void orc_env_observe(const orc_env_t *e, float *x)
     const slice_t *s = &e->sl[p];
     if (!s->size) continue;
     float v = s->down ? 0.5f : (s->job != NONE_JOB ? 1.0f : 0.0f);
-    for (int q = p; q < p + s->size && q < ORC_SLOTS; ++q) x[16 + q] = v;
+    for (int q = p; q < p + units_of(s->size) && q < ORC_SLOTS; ++q) x[16 + q] = v;
     x[23 + p] = (float)s->size / 8.0f;
   }
   x[30 + (e->t / 3600) % 24] = 1.0f;
@@ -683,11 +740,25 @@ int orc_rollout(const orc_params_t *p, uint64_t seed, uint32_t env_id, uint32_t 
                 orc_event_t *trace_buf, uint32_t trace_cap, uint32_t *n_trace_out,
                 float *states_out, uint8_t *actions_out, float *rewards_out)
 {
+  return orc_rollout_ex(p, seed, env_id, episode, algo, cfg0, policy, table, q, epsilon, jobs, n_jobs, recs_out, totals_out,
+                        trace_buf, trace_cap, n_trace_out, states_out, actions_out, rewards_out, NULL, NULL);
+}
+
+int orc_rollout_ex(const orc_params_t *p, uint64_t seed, uint32_t env_id, uint32_t episode, uint8_t algo, uint8_t cfg0,
+                   int policy, const uint8_t *table, const orc_qnet_t *q, float epsilon,
+                   const orc_job_in_t *jobs, uint32_t n_jobs,
+                   orc_epoch_rec_t *recs_out, orc_totals_t *totals_out,
+                   orc_event_t *trace_buf, uint32_t trace_cap, uint32_t *n_trace_out,
+                   float *states_out, uint8_t *actions_out, float *rewards_out,
+                   float *return_out, int32_t *util_out)
+{
   orc_env_t *e = orc_env_create(p, seed, env_id);
   if (jobs) orc_env_set_jobs(e, jobs, n_jobs);
   if (trace_buf) orc_env_set_trace(e, trace_buf, trace_cap);
   orc_env_reset(e, episode, algo, cfg0);
   e->ev_table = (policy == ORC_POLICY_TABLE && p->decide_on_events) ? table : NULL;
+  e->bin_table = (policy == ORC_POLICY_BINNED && p->decide_on_events) ? table : NULL;
+  float G = 0.0f, disc = 1.0f;                                               /* discounted return */
   float x[ORC_STATE_DIM];
   orc_env_observe(e, x);
   double et = (double)epsilon * 4294967296.0;
@@ -700,6 +771,8 @@ int orc_rollout(const orc_params_t *p, uint64_t seed, uint32_t env_id, uint32_t 
     if (policy == ORC_POLICY_TABLE) {                                        /* DESIGN.md 3.6 load buckets */
       uint32_t n = e->n_sys; int b = n == 0 ? 0 : (n < 8 ? 1 : (n < 64 ? 2 : 3));
       action = table[k * 4 + b];
+    } else if (policy == ORC_POLICY_BINNED) {                                /* the paper's binned 2+2m state (L210) */
+      action = table[orc_env_binned_index(e)];
     } else if (policy == ORC_POLICY_DQN) {                                   /* eps-greedy */
       uint32_t w[4];
       orc_philox4x32_10((uint32_t)k, 2u, env_id, episode, (uint32_t)seed, (uint32_t)(seed >> 32), w);
@@ -710,11 +783,29 @@ int orc_rollout(const orc_params_t *p, uint64_t seed, uint32_t env_id, uint32_t 
     float r;
     orc_env_step(e, action, x, &r, NULL, NULL, two);
     if (rewards_out) rewards_out[k] = r;
+    G = fmaf(disc, r, G); { volatile float d2 = disc * p->gamma; disc = d2; }
     if (recs_out) { recs_out[k] = two[0]; if (k == p->n_epochs - 1) recs_out[k + 1] = two[1]; }
   }
   if (states_out) memcpy(states_out + (size_t)p->n_epochs * ORC_STATE_DIM, x, sizeof(x));
   if (totals_out) orc_env_totals(e, totals_out);
+  if (return_out) *return_out = G;
+  if (util_out) orc_env_util_hist(e, util_out);
   if (n_trace_out) *n_trace_out = e->n_trace;
   orc_env_destroy(e);
   return 0;
+}
+
+/* ---------------------------------------------------------------------------------------------- ET */
+double orc_et_reduce(const double *x, const double *y, const uint32_t *group, uint32_t n, uint32_t n_groups, double *et_out)
+{
+  double s = 0.0, t = 0.0;                       /* global means of energy and of average tardiness */
+  for (uint32_t i = 0; i < n; ++i) { s += x[i]; t += y[i]; }
+  s /= (double)n; t /= (double)n;
+  double a = t / (2.0 * s);                      /* "we set a to be t / 2s" (L143) */
+  for (uint32_t g = 0; g < n_groups; ++g) {
+    double acc = 0.0; uint32_t cnt = 0;
+    for (uint32_t i = 0; i < n; ++i) if (group[i] == g) { acc += (a * x[i] + y[i]) / (a + 1.0); ++cnt; }
+    et_out[g] = cnt ? acc / (double)cnt : 0.0;
+  }
+  return a;
 }

@@ -36,7 +36,9 @@ enum { ORC_EV_ARRIVE = 1, ORC_EV_DROP = 2, ORC_EV_START = 3, ORC_EV_PREEMPT = 4,
 
 enum { ORC_ALGO_EDF_FS = 0, ORC_ALGO_EDF_SS = 1, ORC_ALGO_LLF = 2, ORC_ALGO_LALF = 3,
        ORC_ALGO_EDF_SS_R = 4 /* EDF-SS with restricted preemption */ };
-enum { ORC_POLICY_STATIC = 0, ORC_POLICY_TABLE = 1, ORC_POLICY_DQN = 2 };
+enum { ORC_POLICY_STATIC = 0, ORC_POLICY_TABLE = 1, ORC_POLICY_DQN = 2,
+       ORC_POLICY_BINNED = 3 /* table over the paper's binned 2+2m state, shared by all envs */ };
+#define ORC_SIZE_NOMIG 8 /* slice size code of the whole GPU with MIG disabled */
 
 typedef struct {
   uint32_t n_classes, n_configs;
@@ -57,7 +59,15 @@ typedef struct {
   int32_t crit_laxity_s;
   uint32_t crit_max;
   float w_energy, w_tardy;
-  uint32_t decide_on_events;    /* TABLE policy: also decide after every tick with an arrival or a completion */
+  uint32_t decide_on_events;    /* TABLE / BINNED policy: also decide after every tick with an arrival or a completion */
+  /* --- round-2 extensions; all 0 / NULL = off (readings #29-#32) ------------------------------------ */
+  const uint32_t *speed_nomig;  /* [n_classes] work units / s on the whole GPU with MIG DISABLED, slice size code 8, or NULL */
+  int32_t p_idle_nomig_mw, p_busy_nomig_mw;
+  uint32_t repart_all_down;     /* 1: a repartition takes the WHOLE GPU down for repart_downtime_s, every running job is requeued */
+  float gamma;                  /* discount of the return sum_k gamma^k r_k ("discounted rewards over time") */
+  uint32_t n_tbins, n_dbins, n_abins; /* BINNED policy: time-of-day bins, deadline bins, average-duration bins */
+  const int32_t *dbin_edges;    /* [n_dbins - 1] ascending: the deadline feature due - t falls in the first bin i with value < edge[i] */
+  const int32_t *abin_edges;    /* [n_abins - 1] ascending, same rule for the mean remaining duration over the configuration's slices */
 } orc_params_t;
 
 typedef struct { int32_t arr; uint32_t cls; int32_t dur7; int32_t due; } orc_job_in_t;
@@ -120,6 +130,27 @@ int orc_rollout(const orc_params_t *p, uint64_t seed, uint32_t env_id, uint32_t 
                 orc_epoch_rec_t *recs_out, orc_totals_t *totals_out,
                 orc_event_t *trace_buf, uint32_t trace_cap, uint32_t *n_trace_out,
                 float *states_out, uint8_t *actions_out, float *rewards_out);
+
+/* orc_rollout with the round-2 outputs.  policy BINNED: table = the shared [n_configs][n_tbins][B][B][B] u8 table,
+ * B = 1 + n_dbins * n_abins.  return_out: the discounted return sum_k gamma^k r_k, accumulated in fp32 as
+ * G = fmaf(d, r_k, G); d = d * gamma (d starts at 1), or NULL.  util_out: [8] seconds spent with U = 0..7 busy compute
+ * units over the day and the drain (Fig. 6), or NULL. */
+int orc_rollout_ex(const orc_params_t *p, uint64_t seed, uint32_t env_id, uint32_t episode, uint8_t algo, uint8_t cfg0,
+                   int policy, const uint8_t *table, const orc_qnet_t *q, float epsilon,
+                   const orc_job_in_t *jobs, uint32_t n_jobs,
+                   orc_epoch_rec_t *recs_out, orc_totals_t *totals_out,
+                   orc_event_t *trace_buf, uint32_t trace_cap, uint32_t *n_trace_out,
+                   float *states_out, uint8_t *actions_out, float *rewards_out,
+                   float *return_out, int32_t *util_out);
+/* index of the environment's present state in the BINNED policy's table (configuration, time, deadline
+ * and average duration of the first m = 3 jobs, binned) */
+uint32_t orc_env_binned_index(const orc_env_t *e);
+void orc_env_util_hist(const orc_env_t *e, int32_t out[8]);
+
+/* ET metric: x[i] = energy, y[i] = average tardiness of simulation i, group[i] < n_groups = the
+ * algorithm it belongs to.  a = t / (2 s) with s, t the GLOBAL means of x and y over all n simulations;
+ * et_out[g] = mean over the simulations of group g of (a x + y) / (a + 1).  Returns a. */
+double orc_et_reduce(const double *x, const double *y, const uint32_t *group, uint32_t n, uint32_t n_groups, double *et_out);
 
 /* Q-network forward, fp32, one fmaf per term in ascending k; argmax lowest index on ties. */
 void orc_q_eval(const orc_qnet_t *q, const float *state, uint32_t B, float *q_out, uint8_t *argmax_out);

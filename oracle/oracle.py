@@ -46,6 +46,10 @@ class _Params(C.Structure):
         ("crit_laxity_s", C.c_int32), ("crit_max", C.c_uint32),
         ("w_energy", C.c_float), ("w_tardy", C.c_float),
         ("decide_on_events", C.c_uint32),
+        ("speed_nomig", C.c_void_p), ("p_idle_nomig_mw", C.c_int32), ("p_busy_nomig_mw", C.c_int32),
+        ("repart_all_down", C.c_uint32), ("gamma", C.c_float),
+        ("n_tbins", C.c_uint32), ("n_dbins", C.c_uint32), ("n_abins", C.c_uint32),
+        ("dbin_edges", C.c_void_p), ("abin_edges", C.c_void_p),
     ]
 
 
@@ -83,6 +87,13 @@ def lib():
         _lib.orc_rollout.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint8, C.c_uint8, C.c_int,
                                      C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        _lib.orc_rollout_ex.restype = C.c_int
+        _lib.orc_rollout_ex.argtypes = _lib.orc_rollout.argtypes + [C.c_void_p, C.c_void_p]
+        _lib.orc_env_binned_index.restype = C.c_uint32
+        _lib.orc_env_binned_index.argtypes = [C.c_void_p]
+        _lib.orc_env_util_hist.argtypes = [C.c_void_p, C.c_void_p]
+        _lib.orc_et_reduce.restype = C.c_double
+        _lib.orc_et_reduce.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p]
         _lib.orc_q_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]
         _lib.orc_q_eval_f64.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
         _lib.orc_philox4x32_10.argtypes = [C.c_uint32] * 6 + [C.c_void_p]
@@ -117,6 +128,12 @@ class ParamsHolder:
         s.crit_laxity_s, s.crit_max = sp.crit_laxity_s, sp.crit_max
         s.w_energy, s.w_tardy = sp.w_energy, sp.w_tardy
         s.decide_on_events = int(getattr(sp, "decide_on_events", 0))
+        self._keep2 = (sp.speed_nomig, sp.dbin_edges, sp.abin_edges)
+        s.speed_nomig = _ptr(sp.speed_nomig)
+        s.p_idle_nomig_mw, s.p_busy_nomig_mw = int(sp.p_idle_nomig_mw), int(sp.p_busy_nomig_mw)
+        s.repart_all_down, s.gamma = int(sp.repart_all_down), float(sp.gamma)
+        s.n_tbins, s.n_dbins, s.n_abins = int(sp.n_tbins), int(sp.n_dbins), int(sp.n_abins)
+        s.dbin_edges, s.abin_edges = _ptr(sp.dbin_edges), _ptr(sp.abin_edges)
         self.c = s
 
     @property
@@ -168,7 +185,7 @@ def make_jobs(rows) -> np.ndarray:
 
 
 class RolloutResult:
-    __slots__ = ("recs", "totals", "trace", "states", "actions", "rewards")
+    __slots__ = ("recs", "totals", "trace", "states", "actions", "rewards", "ret", "util")
 
 
 def rollout(sp, seed, env_id, *, episode=0, algo=1, cfg0=0, policy=0, table=None, qnet=None, epsilon=0.0,
@@ -186,11 +203,14 @@ def rollout(sp, seed, env_id, *, episode=0, algo=1, cfg0=0, policy=0, table=None
     tb = None if table is None else np.ascontiguousarray(table, dtype=np.uint8)
     qh = None if qnet is None else (qnet if isinstance(qnet, QNetHolder) else QNetHolder(qnet))
     jb = None if jobs is None else np.ascontiguousarray(jobs, dtype=JOB_IN_DTYPE)
-    rc = lib().orc_rollout(ph.ref, seed, env_id, episode, algo, cfg0, policy, _ptr(tb), qh.ref if qh else None,
-                           epsilon, _ptr(jb), 0 if jb is None else len(jb), _ptr(recs), _ptr(totals), _ptr(trace),
-                           trace_cap, _ptr(ntr), _ptr(states), _ptr(actions), _ptr(rewards))
+    ret = np.zeros(1, dtype=np.float32)
+    util = np.zeros(8, dtype=np.int32)
+    rc = lib().orc_rollout_ex(ph.ref, seed, env_id, episode, algo, cfg0, policy, _ptr(tb), qh.ref if qh else None,
+                              epsilon, _ptr(jb), 0 if jb is None else len(jb), _ptr(recs), _ptr(totals), _ptr(trace),
+                              trace_cap, _ptr(ntr), _ptr(states), _ptr(actions), _ptr(rewards), _ptr(ret), _ptr(util))
     assert rc == 0
     r = RolloutResult()
+    r.ret, r.util = float(ret[0]), util
     r.recs, r.totals = recs, totals[0]
     if trace is not None:
         assert ntr[0] <= trace_cap, "trace buffer too small: %d events" % ntr[0]
@@ -248,6 +268,14 @@ class Env:
     def n_sys(self):
         return int(lib().orc_env_n_sys(self.h))
 
+    def binned_index(self):
+        return int(lib().orc_env_binned_index(self.h))
+
+    def util_hist(self):
+        u = np.zeros(8, dtype=np.int32)
+        lib().orc_env_util_hist(self.h, _ptr(u))
+        return u
+
     def trace(self):
         n = int(self.totals()["n_events"])
         assert n <= len(self.trace_buf)
@@ -269,3 +297,12 @@ def q_eval_f64(qnet, states):
     q = np.zeros((x.shape[0], qh.n_actions), dtype=np.float64)
     lib().orc_q_eval_f64(qh.ref, _ptr(x), x.shape[0], _ptr(q))
     return q
+
+
+def et_reduce(x, y, group, n_groups):
+    """ET per group and the global scaling factor a."""
+    x = np.ascontiguousarray(x, dtype=np.float64); y = np.ascontiguousarray(y, dtype=np.float64)
+    g = np.ascontiguousarray(group, dtype=np.uint32)
+    et = np.zeros(n_groups, dtype=np.float64)
+    a = lib().orc_et_reduce(_ptr(x), _ptr(y), _ptr(g), len(x), n_groups, _ptr(et))
+    return et, float(a)

@@ -230,17 +230,17 @@ struct EnvT {
   }
   __device__ __forceinline__ uint2 queue_top_km() { return SK(q_head); }
   __device__ __forceinline__ uint2 queue_top_rd() { return SR(q_head); }
+  __device__ __forceinline__ void queue_refill(const uint4 e) {               // e = gtab[g_head], the smallest of the global part: it moves up into the freed slot
+    g_head = (g_head + 1u) & (a.ring_cap - 1u);
+    q_ng--;
+    const uint32_t p = s_phys(q_ns);
+    SK(p) = make_uint2(e.x, e.y); SR(p) = make_uint2(e.z, e.w);
+    q_ns++;
+  }
   __device__ __forceinline__ void queue_pop() {                              // removes the first record
     q_head = q_head + 1 == S ? 0 : q_head + 1;
     q_ns--; n_wait--;
-    if (q_ng) {                                                              // the smallest of the global part moves up
-      const uint4 e = gtab[g_head];
-      g_head = (g_head + 1u) & (a.ring_cap - 1u);
-      q_ng--;
-      const uint32_t p = s_phys(q_ns);
-      SK(p) = make_uint2(e.x, e.y); SR(p) = make_uint2(e.z, e.w);
-      q_ns++;
-    }
+    if (q_ng) queue_refill(gtab[g_head]);
   }
   // after every key changed (LLF / LALF at a repartition): insertion sort over the logical order
   __device__ __forceinline__ void queue_resort() {
@@ -460,6 +460,8 @@ struct EnvT {
     uint32_t rmask = busy_mask;                     // running jobs not picked yet
     uint32_t keep = 0, nb = 0; int K = 0, nd = MIG_INF, u = 0, pd = 0;
     uint32_t ro = run_order | 0xF0000000u, new_order = 0xFFFFFFFFu;
+    uint4 gh = make_uint4(0u, 0u, 0u, 0u); bool gh_valid = q_ng != 0u;      // the global part's head, requested before the pick that may need it
+    if (gh_valid) gh = gtab[g_head];
     while (avail != 0u) {
       // --- next job in (key, id) order: the first of the unpicked running jobs, or the front of the queue
       uint2 bkm = make_uint2(0x7FFFFFFFu, 0xFFFFFFFFu); int bp = -1;
@@ -479,7 +481,19 @@ struct EnvT {
         if (bp < 0 || before(wk, bkm)) { bkm = wk; bp = 7; }
       }
       if (bp < 0) break;                                                  // nobody left
-      if (bp == 7) { rdv = queue_top_rd(); queue_pop(); } else { rdv = R2(T2_SLRD + bp); rmask &= ~(1u << bp); ro >>= 4; }
+      {                                   // take the record from the queue's front or from the slice table: selects, not a branch
+        const bool take_q = bp == 7;
+        rdv = r2[(take_q ? T2_RING + 2 * (int)q_head + 1 : T2_SLRD + bp) * NT];      // one load, selected row
+        const uint32_t qh1 = q_head + 1u == S ? 0u : q_head + 1u;
+        q_head = take_q ? qh1 : q_head;
+        q_ns -= take_q ? 1u : 0u; n_wait -= take_q ? 1u : 0u;
+        rmask &= take_q ? 0xFFFFFFFFu : ~(1u << bp);
+        ro = take_q ? ro : ro >> 4;
+        if (take_q && q_ng) {                                             // the smallest of the global part moves up
+          if (gh_valid) queue_refill(gh); else queue_refill(gtab[g_head]);
+          gh_valid = false;
+        }
+      }
       const int rem = (int)rdv.x, slack = (int)rdv.y - t;
       const uint32_t cls = m_cls(bkm.y);
       // --- slice choice: one composite key per rule, (r, rank) is unique per slice

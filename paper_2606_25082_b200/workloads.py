@@ -34,7 +34,7 @@ N_THR_BINS = 1440                  # one acceptance threshold per minute of the 
 
 ALGO_EDF_FS, ALGO_EDF_SS, ALGO_LLF, ALGO_LALF, ALGO_EDF_SS_R = 0, 1, 2, 3, 4
 ALGO_NAMES = ("EDF-FS", "EDF-SS", "LLF", "LALF", "EDF-SS-R")     # EDF-SS-R: restricted preemption
-POLICY_STATIC, POLICY_TABLE, POLICY_DQN = 0, 1, 2
+POLICY_STATIC, POLICY_TABLE, POLICY_DQN, POLICY_BINNED = 0, 1, 2, 3   # BINNED: table over the binned 2+2m state
 
 # PAPER.md:L75-88 (Fig. 1): (size, start slot) per slice; config ids here are 0-based (paper id - 1).
 FIG1_CONFIGS = (
@@ -164,7 +164,17 @@ class SimParams:
     w_energy: float = 0.5
     w_tardy: float = 0.5
     env_offset: int = 0
-    decide_on_events: int = 0    # TABLE policy: also decide after every tick with an arrival or a completion
+    decide_on_events: int = 0    # TABLE / BINNED policy: also decide after every tick with an arrival or a completion
+    # round-2 extensions (readings #29-#32); None / 0 = off
+    speed_nomig: "np.ndarray | None" = None   # [n_classes] u32: work units / s on the whole GPU with MIG disabled (size code 8)
+    p_idle_nomig_mw: int = 0
+    p_busy_nomig_mw: int = 0
+    repart_all_down: int = 0     # 1: a repartition takes the whole GPU down for repart_downtime_s
+    gamma: float = 1.0           # discount of the return
+    n_tbins: int = 0             # BINNED policy: time-of-day bins
+    dbin_edges: "np.ndarray | None" = None    # [n_dbins - 1] i32 ascending edges of the deadline feature due - t (seconds)
+    abin_edges: "np.ndarray | None" = None    # [n_abins - 1] i32 ascending edges of the mean remaining duration (seconds)
+    util_hist: int = 0           # 1: keep the time spent per utilisation level (Fig. 6); CUDA side only (the oracle always does)
 
     @property
     def n_classes(self) -> int:
@@ -173,6 +183,19 @@ class SimParams:
     @property
     def n_configs(self) -> int:
         return int(self.size_at_slot.shape[0])
+
+    @property
+    def n_dbins(self) -> int:
+        return 0 if self.dbin_edges is None else int(len(self.dbin_edges)) + 1
+
+    @property
+    def n_abins(self) -> int:
+        return 0 if self.abin_edges is None else int(len(self.abin_edges)) + 1
+
+    @property
+    def binned_codes(self) -> int:
+        """B = 1 + n_dbins * n_abins job codes per position (0 = no job); the BINNED table has n_configs * n_tbins * B^3 entries."""
+        return 1 + self.n_dbins * self.n_abins
 
     def normalised(self) -> "SimParams":
         """Same values with the exact dtypes/contiguity both sides marshal from."""
@@ -187,6 +210,9 @@ class SimParams:
             curve_mw=np.ascontiguousarray(self.curve_mw, dtype=np.int32),
             p_idle_mw=np.ascontiguousarray(self.p_idle_mw, dtype=np.int32),
             p_busy_mw=np.ascontiguousarray(self.p_busy_mw, dtype=np.int32),
+            speed_nomig=None if self.speed_nomig is None else np.ascontiguousarray(self.speed_nomig, dtype=np.uint32),
+            dbin_edges=None if self.dbin_edges is None else np.ascontiguousarray(self.dbin_edges, dtype=np.int32),
+            abin_edges=None if self.abin_edges is None else np.ascontiguousarray(self.abin_edges, dtype=np.int32),
         )
 
 

@@ -36,12 +36,18 @@ def replay(sp, cfg0, trace, *, jobs_in=None, truncated=False):
     n_preempt = n_start = 0
     last_completion_t = 0
 
+    def speed_on(cls, size):           # size code 8: the whole GPU with MIG disabled (reading #29)
+        return int(sp.speed_nomig[cls]) if size == 8 else int(sp.speed[cls][SIZE_IDX[size]])
+
     def power():
-        u = sum(s["size"] for s in slices.values() if s["job"] is not None)
+        u = sum(min(s["size"], 7) for s in slices.values() if s["job"] is not None)
         _chk(u <= 7, "busy units exceed 7")
         p = int(sp.curve_mw[u])
         for s in slices.values():
-            p += int(sp.p_busy_mw[SIZE_IDX[s["size"]]] if s["job"] is not None else sp.p_idle_mw[SIZE_IDX[s["size"]]])
+            if s["size"] == 8:
+                p += int(sp.p_busy_nomig_mw if s["job"] is not None else sp.p_idle_nomig_mw)
+            else:
+                p += int(sp.p_busy_mw[SIZE_IDX[s["size"]]] if s["job"] is not None else sp.p_idle_mw[SIZE_IDX[s["size"]]])
         return p, u
 
     def advance(t_to):
@@ -59,7 +65,7 @@ def replay(sp, cfg0, trace, *, jobs_in=None, truncated=False):
         for s in slices.values():
             if s["job"] is not None:
                 j = jobs[s["job"]]
-                j["done"] += (t_to - t_prev) * int(sp.speed[j["cls"]][SIZE_IDX[s["size"]]])
+                j["done"] += (t_to - t_prev) * speed_on(j["cls"], s["size"])
         t_prev = t_to
 
     def rec_index(t):
@@ -112,10 +118,10 @@ def replay(sp, cfg0, trace, *, jobs_in=None, truncated=False):
         elif ty == EV_COMPLETE:
             j = jobs.get(job)
             _chk(j is not None and j["slot"] == slot and slices[slot]["job"] == job, "COMPLETE of a job not on that slice")
-            v = int(sp.speed[j["cls"]][SIZE_IDX[slices[slot]["size"]]])
+            v = speed_on(j["cls"], slices[slot]["size"])
             _chk(j["work"] <= j["done"] < j["work"] + v, "work conservation: done=%d work=%d v=%d" % (j["done"], j["work"], v))
             _chk(value == max(t - j["due"], 0), "tardiness value")
-            vmax = max(int(x) for x in sp.speed[j["cls"]])
+            vmax = max([int(x) for x in sp.speed[j["cls"]]] + ([int(sp.speed_nomig[j["cls"]])] if getattr(sp, "speed_nomig", None) is not None else []))
             _chk(t >= j["arr"] + -(-j["work"] // vmax), "finished faster than on the fastest slice")
             tard[k] += value
             slices[slot]["job"] = None
@@ -141,7 +147,7 @@ def replay(sp, cfg0, trace, *, jobs_in=None, truncated=False):
                 g = int(size_at[new][p])
                 if not g:
                     continue
-                if p in slices and slices[p]["size"] == g:
+                if p in slices and slices[p]["size"] == g and not getattr(sp, "repart_all_down", 0):
                     newsl[p] = slices[p]
                 else:
                     newsl[p] = {"size": g, "down": sp.repart_downtime_s > 0, "job": None}
