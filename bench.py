@@ -222,6 +222,7 @@ def run_ours(args):
     # ---- per-kernel durations: a second, short region with the library's own event pairs around every launch -------
     sim.set_profiling(True)
     n_prof = max(1, min(args.steps, 3))
+    last_episode = args.warmup + args.steps + n_prof - 1                            # the day `recs` / `totals` hold afterwards
     for k in range(n_prof):
         sim.reset(args.warmup + args.steps + k, d_algo, d_cfg0)
         sim.kernel_times()                                                         # (drops the reset launch)
@@ -260,12 +261,12 @@ def run_ours(args):
     step_api = None
     if rank == 0 and not args.no_step_api:
         acts = [recs[k, :, 52].contiguous() for k in range(sp.n_epochs)]             # byte 52 of a record = cfg
-        totals_roll = totals.clone()                                                  # of the last timed rollout
+        totals_roll = totals.clone()                                                  # of the last rollout (episode last_episode)
         state, reward = sim.alloc_state(), torch.zeros(n_envs, dtype=torch.float32, device="cuda")
         rec1, drain1 = torch.zeros((n_envs, 64), dtype=torch.uint8, device="cuda"), torch.zeros((n_envs, 64), dtype=torch.uint8, device="cuda")
         s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         for it in range(2):                                                           # first day: warm-up
-            sim.reset(args.warmup + args.steps - 1, d_algo, d_cfg0, state_out=state)
+            sim.reset(last_episode, d_algo, d_cfg0, state_out=state)
             s0.record(stream)
             for k in range(sp.n_epochs):
                 sim.step(acts[k], state_out=state, reward_out=reward, rec_out=rec1, drain_rec_out=drain1)

@@ -58,7 +58,15 @@ enum { MIG_ALGO_EDF_FS = 0, MIG_ALGO_EDF_SS = 1, MIG_ALGO_LLF = 2, MIG_ALGO_LALF
         * free slice, else wait (reading #26) */
        MIG_ALGO_EDF_SS_R = 4 };
 /* repartitioning policy of mig_sim_rollout */
-enum { MIG_POLICY_STATIC = 0, MIG_POLICY_TABLE = 1, MIG_POLICY_DQN = 2 };
+enum { MIG_POLICY_STATIC = 0, MIG_POLICY_TABLE = 1, MIG_POLICY_DQN = 2,
+       /* a table over the paper's binned state ("2+2m different features: the current MIG configuration,
+        * time, and the deadlines and average duration of the first m jobs ... binned", m = 3), shared by all environments;
+        * DESIGN.md reading #31 */
+       MIG_POLICY_BINNED = 3 };
+/* slice size code of the whole GPU with MIG DISABLED (the paper's first benchmark; "6% performance
+ * improvement for linear jobs ... compared to a 7g.40gb slice"): allowed at slot 0 as a configuration's only slice when
+ * speed_nomig is given; 7 compute units, its own speed column and power entries (reading #29) */
+#define MIG_SIZE_NOMIG 8
 /* per-environment status bits */
 #define MIG_ST_TRUNCATED 1u  /* t_limit_s reached with jobs still in the system */
 #define MIG_ST_BAD_ACTION 2u /* an action >= n_configs was treated as "stay" */
@@ -98,6 +106,20 @@ typedef struct {
                                  * moment) after every tick of the day in which a job arrived or completed; a different
                                  * configuration is a repartition at that tick ("re-partitioning can happen when a
                                  * job arrives or is completed"; reading #27).  Ignored by mig_sim_step. */
+  /* ---- extensions; all 0 / NULL = off.  Implemented by the thread-per-environment kernel
+   * (mig_sim_set_tile(s, 1), the default): with any of them in use the warp-tile kernels are refused (MIG_EINVAL). */
+  const uint32_t *speed_nomig;  /* [n_classes] work units per second on the whole GPU with MIG disabled (size code 8), or NULL */
+  int32_t p_idle_nomig_mw;      /* idle / busy power of the MIG-disabled GPU */
+  int32_t p_busy_nomig_mw;
+  uint32_t repart_all_down;     /* 1: a repartition takes the WHOLE GPU down for repart_downtime_s: every running job is requeued,
+                                 * every slice of the new configuration comes up at t + downtime (reading #30) */
+  float gamma;                  /* discount of the return G = sum_k gamma^k r_k over the decision epochs ("discounted
+                                 * rewards over time"): fp32, G = fmaf(d, r_k, G); d = d * gamma; read back by mig_sim_aux */
+  uint32_t n_tbins;             /* BINNED policy: time-of-day bins, bin = min(t, day_s - 1) * n_tbins / day_s; 1..255 */
+  uint32_t n_dbins, n_abins;    /* BINNED policy: deadline bins and average-duration bins, 1..8 each */
+  const int32_t *dbin_edges;    /* [n_dbins - 1] ascending; the deadline feature due - t is in the first bin i with value < edge[i] */
+  const int32_t *abin_edges;    /* [n_abins - 1] ascending; same rule for the mean remaining duration over the configuration's slices */
+  uint32_t util_hist;           /* 1: keep the seconds spent at each utilisation level (Fig. 6); mig_sim_aux */
 } mig_params_t;
 
 /* One record per env per epoch (index n_epochs = the drain).  64 bytes. */
@@ -141,7 +163,7 @@ const char *mig_last_error(void);
 const char *mig_version(void);
 
 /* Creates a simulator of n_envs environments on the current CUDA device.  Validates every table (sizes in
- * {0,1,2,3,4,7}, slices inside 7 slots and not overlapping, speed >= 1, monotone quantiles, cap in 1..1024, all
+ * {0,1,2,3,4,7} or 8 = MIG disabled, slices inside 7 slots and not overlapping, speed >= 1, monotone quantiles, cap in 1..1024, all
  * derived quantities inside int32) -> MIG_EINVAL with a message.  seed is the Philox key. */
 int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n_envs, uint64_t seed);
 int mig_sim_destroy(mig_sim_t *s);
@@ -162,12 +184,30 @@ int mig_sim_step(mig_sim_t *s, const uint8_t *action, float *state_out, float *r
  *   STATIC: stay on the current configuration.   TABLE: table dev[n_envs][n_epochs][4] u8, action =
  *   table[env][k][bucket], bucket by jobs in system (0 | <8 | <64 | else).   DQN: q + epsilon (eps-greedy from
  *   Philox stream 2), one Q forward per epoch over the state batch (scratch owned by the handle).
+ *   BINNED: table dev[n_configs][n_tbins][B][B][B] u8, B = 1 + n_dbins * n_abins, ONE table for all environments, indexed
+ *   by (configuration, time bin, code of the 1st, 2nd, 3rd job in (due, id) order over all jobs in system); a job's code is
+ *   0 if there is no such job, else 1 + dbin * n_abins + abin.  With decide_on_events it is looked up after every tick with
+ *   an arrival or a completion as well.  Thread-per-environment kernel only.
  * recs_out: dev[n_epochs+1][n_envs] or NULL.  totals_out: dev[n_envs] or NULL. */
 int mig_sim_rollout(mig_sim_t *s, int policy, const uint8_t *table, const mig_qnet_t *q, float epsilon,
                     mig_epoch_rec_t *recs_out, mig_totals_t *totals_out, void *stream);
 
 /* Per-env totals so far: dev[n_envs]. */
 int mig_sim_totals(mig_sim_t *s, mig_totals_t *totals_out, void *stream);
+
+/* Auxiliary per-env results so far (thread-per-environment kernel; MIG_ESTATE on the warp tiles), each NULL or dev:
+ *   return_out dev[n_envs] fp32: the discounted return over the epochs done (params.gamma);
+ *   util_s_out dev[n_envs][8] int32: seconds spent with U = 0..7 busy compute units over the day and the drain
+ *   (Fig. 6; needs params.util_hist = 1, MIG_ESTATE otherwise). */
+int mig_sim_aux(mig_sim_t *s, float *return_out, int32_t *util_s_out, void *stream);
+
+/* ET metric, HOST arrays, double: x[i] = energy and y[i] = average tardiness of simulation i,
+ * group[i] < n_groups the algorithm / policy it belongs to.  a = t / (2 s) with s, t the means of x and y over ALL n
+ * simulations ("global mean ... across the simulations of all the experiments"); et_out[g] = mean over group g of
+ * (a x_i + y_i) / (a + 1) (0 for an empty group).  a_out may be NULL.  MIG_EINVAL if n = 0, a group id is out of range
+ * or the mean energy is 0. */
+int mig_et_reduce(const double *x, const double *y, const uint32_t *group, uint32_t n, uint32_t n_groups, double *et_out,
+                  double *a_out);
 
 /* End-to-end convenience with HOST buffers: copies algo/cfg0/table (host[n_envs], host[n_envs][n_epochs][4] or NULL)
  * to the device, reset(episode) + rollout, copies totals (host[n_envs]) and records (host[n_epochs+1][n_envs] or
@@ -186,7 +226,7 @@ int mig_qnet_destroy(mig_qnet_t *q);
 int mig_q_eval(const mig_qnet_t *q, const float *state, uint32_t B, float *q_out, uint8_t *argmax_out, void *stream);
 
 /* Debug / parity: re-runs ONE env for a whole day from the last reset's (episode, algo, cfg0), recording every event.
- * policy STATIC or TABLE (table as in rollout), or actions != NULL: dev[n_epochs] explicit action sequence.
+ * policy STATIC, TABLE or BINNED (table as in rollout), or actions != NULL: dev[n_epochs] explicit action sequence.
  * buf dev[cap_events]; n_out dev[1] = number of events emitted (may exceed cap_events; only the first are stored);
  * totals_out dev[1] or NULL.  Does not touch the handle's per-env state. */
 int mig_sim_debug_trace(mig_sim_t *s, uint32_t env, int policy, const uint8_t *table, const uint8_t *actions,

@@ -14,7 +14,7 @@ from . import _build
 from .workloads import STATE_DIM, QNetWeights, SimParams
 
 MIG_OK, MIG_EINVAL, MIG_ENOMEM, MIG_ECUDA, MIG_ESTATE = 0, -1, -2, -3, -4
-POLICY_STATIC, POLICY_TABLE, POLICY_DQN = 0, 1, 2
+POLICY_STATIC, POLICY_TABLE, POLICY_DQN, POLICY_BINNED = 0, 1, 2, 3
 
 EVENT_DTYPE = np.dtype([("t", "<i4"), ("type", "u1"), ("slot", "u1"), ("aux", "<u2"), ("job", "<u4"), ("value", "<i4")])
 REC_DTYPE = np.dtype([
@@ -35,7 +35,7 @@ EXPORTS = (
     "mig_sim_rollout", "mig_sim_totals", "mig_sim_rollout_host", "mig_qnet_create", "mig_qnet_destroy", "mig_q_eval",
     "mig_sim_debug_trace", "mig_sim_debug_set_jobs", "mig_debug_div_magic", "mig_sim_launch_count", "mig_sim_set_tile",
     "mig_sim_get_tile", "mig_sim_set_arrival_buffer", "mig_sim_get_arrival_buffer", "mig_sim_set_envs_per_warp",
-    "mig_sim_kernel_name", "mig_sim_set_profiling", "mig_sim_kernel_times")
+    "mig_sim_kernel_name", "mig_sim_set_profiling", "mig_sim_kernel_times", "mig_sim_aux", "mig_et_reduce")
 
 
 class MigError(RuntimeError):
@@ -56,6 +56,10 @@ class _Params(C.Structure):
         ("repart_downtime_s", C.c_int32), ("repart_energy_mj", C.c_int64),
         ("crit_laxity_s", C.c_int32), ("crit_max", C.c_uint32),
         ("w_energy", C.c_float), ("w_tardy", C.c_float), ("env_base", C.c_uint32), ("decide_on_events", C.c_uint32),
+        ("speed_nomig", C.c_void_p), ("p_idle_nomig_mw", C.c_int32), ("p_busy_nomig_mw", C.c_int32),
+        ("repart_all_down", C.c_uint32), ("gamma", C.c_float),
+        ("n_tbins", C.c_uint32), ("n_dbins", C.c_uint32), ("n_abins", C.c_uint32),
+        ("dbin_edges", C.c_void_p), ("abin_edges", C.c_void_p), ("util_hist", C.c_uint32),
     ]
 
 
@@ -96,6 +100,8 @@ def lib():
         L.mig_sim_kernel_times.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_uint32)]
         L.mig_sim_get_arrival_buffer.argtypes = [vp]
         L.mig_sim_get_arrival_buffer.restype = C.c_uint32
+        L.mig_sim_aux.argtypes = [vp, vp, vp, vp]
+        L.mig_et_reduce.argtypes = [vp, vp, vp, u32, u32, vp, vp]
         _lib = L
     return _lib
 
@@ -152,6 +158,13 @@ def _fill_params(sp: SimParams) -> tuple[_Params, tuple]:
     s.crit_laxity_s, s.crit_max = sp.crit_laxity_s, sp.crit_max
     s.w_energy, s.w_tardy, s.env_base = sp.w_energy, sp.w_tardy, sp.env_offset
     s.decide_on_events = int(sp.decide_on_events)
+    keep = keep + (sp.speed_nomig, sp.dbin_edges, sp.abin_edges)
+    s.speed_nomig = _hp(sp.speed_nomig)
+    s.p_idle_nomig_mw, s.p_busy_nomig_mw = int(sp.p_idle_nomig_mw), int(sp.p_busy_nomig_mw)
+    s.repart_all_down, s.gamma = int(sp.repart_all_down), float(sp.gamma)
+    s.n_tbins, s.n_dbins, s.n_abins = int(sp.n_tbins), int(sp.n_dbins), int(sp.n_abins)
+    s.dbin_edges, s.abin_edges = _hp(sp.dbin_edges), _hp(sp.abin_edges)
+    s.util_hist = int(sp.util_hist)
     return s, keep
 
 
@@ -246,10 +259,16 @@ class MigSim:
     def rollout(self, policy: int, table=None, qnet: QNet | None = None, epsilon: float = 0.0, recs_out=None,
                 totals_out=None, stream=None):
         n = self.n_envs
-        _check(lib().mig_sim_rollout(self.h, policy, _dp(table, torch.uint8, n * self.n_epochs * 4),
+        tb = self.sp.n_configs * self.sp.n_tbins * self.sp.binned_codes ** 3 if policy == POLICY_BINNED else n * self.n_epochs * 4
+        _check(lib().mig_sim_rollout(self.h, policy, _dp(table, torch.uint8, tb),
                                      qnet.h if qnet is not None else None, float(epsilon),
                                      _dp(recs_out, torch.uint8, (self.n_epochs + 1) * n * 64),
                                      _dp(totals_out, torch.uint8, n * 80), _stream(stream)))
+
+    def aux(self, return_out=None, util_s_out=None, stream=None):
+        """mig_sim_aux: discounted return dev[n_envs] fp32 and / or seconds per utilisation level dev[n_envs][8] int32."""
+        _check(lib().mig_sim_aux(self.h, _dp(return_out, torch.float32, self.n_envs * 4), _dp(util_s_out, torch.int32, self.n_envs * 32),
+                                 _stream(stream)))
 
     def totals(self, totals_out, stream=None):
         _check(lib().mig_sim_totals(self.h, _dp(totals_out, torch.uint8, self.n_envs * 80), _stream(stream)))
@@ -263,7 +282,8 @@ class MigSim:
         if recs_out is not None:
             assert recs_out.dtype == REC_DTYPE and recs_out.size == n * (self.n_epochs + 1) and recs_out.flags.c_contiguous
         if table is not None:
-            assert table.dtype == np.uint8 and table.size == n * self.n_epochs * 4 and table.flags.c_contiguous
+            want = self.sp.n_configs * self.sp.n_tbins * self.sp.binned_codes ** 3 if policy == POLICY_BINNED else n * self.n_epochs * 4
+            assert table.dtype == np.uint8 and table.size == want and table.flags.c_contiguous
         _check(lib().mig_sim_rollout_host(self.h, episode, _hp(algo), _hp(cfg0), policy, _hp(table),
                                           qnet.h if qnet is not None else None, float(epsilon), _hp(recs_out), _hp(totals_out)))
 
@@ -312,3 +332,13 @@ def recs_to_numpy(t: torch.Tensor) -> np.ndarray:
 
 def totals_to_numpy(t: torch.Tensor) -> np.ndarray:
     return t.cpu().numpy().view(TOTALS_DTYPE).reshape(t.shape[:-1])
+
+
+def et_reduce(x, y, group, n_groups: int):
+    """mig_et_reduce: ET per group and the global scaling factor a; host arrays."""
+    x = np.ascontiguousarray(x, dtype=np.float64); y = np.ascontiguousarray(y, dtype=np.float64)
+    g = np.ascontiguousarray(group, dtype=np.uint32)
+    et = np.zeros(n_groups, dtype=np.float64)
+    a = C.c_double()
+    _check(lib().mig_et_reduce(_hp(x), _hp(y), _hp(g), len(x), n_groups, _hp(et), C.byref(a)))
+    return et, a.value

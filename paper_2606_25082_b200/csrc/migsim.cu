@@ -90,6 +90,12 @@ extern "C" int mig_debug_div_magic(uint32_t v, uint32_t *m, uint32_t *sh) {
 
 // ------------------------------------------------------------------------------------------------ create
 static int size_index(int g) { return g == 1 ? 0 : g == 2 ? 1 : g == 3 ? 2 : g == 4 ? 3 : g == 7 ? 4 : -1; }
+constexpr int kPolicyExplicit = 4;   // internal: the launch's actions come from SimArgs::actions
+
+// true if the parameter set needs what only the thread-per-environment kernel implements (readings #29-#32)
+static bool uses_extensions(const mig_params_t &p) {
+  return p.speed_nomig || p.repart_all_down || p.util_hist || p.n_tbins || p.n_dbins || p.n_abins;
+}
 
 static int build_tables(const mig_params_t *p, DevTables *t) {
   memset(t, 0, sizeof(*t));
@@ -115,12 +121,33 @@ static int build_tables(const mig_params_t *p, DevTables *t) {
   static const int SIZES[5] = {1, 2, 3, 4, 7};
   for (int i = 0; i < 8; ++i) t->curve[i] = p->curve_mw[i];
   for (int i = 0; i < 5; ++i) { t->p_idle[SIZES[i]] = p->p_idle_mw[i]; t->p_busy[SIZES[i]] = p->p_busy_mw[i]; }
+  if (p->speed_nomig) {                                        // the MIG-disabled GPU (reading #29)
+    if (p->p_idle_nomig_mw < 0 || p->p_idle_nomig_mw > (1 << 27) || p->p_busy_nomig_mw < 0 || p->p_busy_nomig_mw > (1 << 27))
+      return fail(MIG_EINVAL, "create: p_idle_nomig_mw / p_busy_nomig_mw out of [0, 2^27]");
+    t->p_idle[MIG_SIZE_NOMIG] = p->p_idle_nomig_mw; t->p_busy[MIG_SIZE_NOMIG] = p->p_busy_nomig_mw;
+  }
+  if (!(p->gamma >= 0.0f) || p->gamma > 1.0f) return fail(MIG_EINVAL, "create: gamma must be in [0, 1]");
+  if (p->n_tbins || p->n_dbins || p->n_abins) {                // BINNED policy (reading #31)
+    if (p->n_tbins < 1 || p->n_tbins > 255) return fail(MIG_EINVAL, "create: n_tbins %u not in 1..255", p->n_tbins);
+    if (p->n_dbins < 1 || p->n_dbins > 8 || p->n_abins < 1 || p->n_abins > 8) return fail(MIG_EINVAL, "create: n_dbins / n_abins not in 1..8");
+    if ((p->n_dbins > 1 && !p->dbin_edges) || (p->n_abins > 1 && !p->abin_edges)) return fail(MIG_EINVAL, "create: bin edges are NULL");
+    if (p->day_s < 1) return fail(MIG_EINVAL, "create: the BINNED policy needs day_s >= 1");
+    for (int i = 0; i < 8; ++i) { t->dbin_edges[i] = 0x7FFFFFFF; t->abin_edges[i] = 0x7FFFFFFF; }
+    for (uint32_t i = 0; i + 1 < p->n_dbins; ++i) { if (i && p->dbin_edges[i] < p->dbin_edges[i - 1]) return fail(MIG_EINVAL, "create: dbin_edges not ascending"); t->dbin_edges[i] = p->dbin_edges[i]; }
+    for (uint32_t i = 0; i + 1 < p->n_abins; ++i) { if (i && p->abin_edges[i] < p->abin_edges[i - 1]) return fail(MIG_EINVAL, "create: abin_edges not ascending"); t->abin_edges[i] = p->abin_edges[i]; }
+  }
   for (uint32_t c = 0; c < p->n_configs; ++c) {
     uint32_t pack = 0; int covered_to = 0, n = 0;
     for (int s = 0; s < MIG_SLOTS; ++s) {
       int g = p->size_at_slot[c * 7 + s];
       if (!g) continue;
-      if (size_index(g) < 0) return fail(MIG_EINVAL, "create: config %u slot %d: slice size %d not in {1,2,3,4,7}", c, s, g);
+      if (g == MIG_SIZE_NOMIG) {                               // MIG disabled: the whole GPU, alone, at slot 0
+        if (!p->speed_nomig) return fail(MIG_EINVAL, "create: config %u uses size code 8 (MIG disabled) but speed_nomig is NULL", c);
+        if (s != 0 || n) return fail(MIG_EINVAL, "create: config %u: the MIG-disabled GPU must be the only slice, at slot 0", c);
+        covered_to = MIG_SLOTS; pack |= (uint32_t)g << (4 * s); ++n;
+        continue;
+      }
+      if (size_index(g) < 0) return fail(MIG_EINVAL, "create: config %u slot %d: slice size %d not in {1,2,3,4,7} (or 8 = MIG disabled)", c, s, g);
       if (s < covered_to) return fail(MIG_EINVAL, "create: config %u: slices overlap at slot %d", c, s);
       if (s + g > MIG_SLOTS) return fail(MIG_EINVAL, "create: config %u: slice at slot %d exceeds 7 slots", c, s);
       covered_to = s + g; pack |= (uint32_t)g << (4 * s); ++n;
@@ -151,6 +178,13 @@ static int build_tables(const mig_params_t *p, DevTables *t) {
       uint32_t m, sh; mig_debug_div_magic(v, &m, &sh);
       t->speed[c * 5 + i] = make_uint4(v, m, sh, 0);
     }
+    if (p->speed_nomig) {
+      uint32_t v = p->speed_nomig[c];
+      if (v < 1 || v > (1u << 24)) return fail(MIG_EINVAL, "create: speed_nomig[%u] = %u not in 1..2^24", c, v);
+      vmin = v < vmin ? v : vmin; vmax = v > vmax ? v : vmax;
+      uint32_t m, sh; mig_debug_div_magic(v, &m, &sh);
+      t->speed_nomig[c] = make_uint4(v, m, sh, 0);
+    } else t->speed_nomig[c] = t->speed[c * 5 + 4];
     unsigned long long work_max = (unsigned long long)q[64] * p->speed[c * 5 + 4];
     if (work_max + vmax >= (1ull << 31)) return fail(MIG_EINVAL, "create: class %u: max work %llu + max speed exceeds int32", c, work_max);
     if ((work_max + vmin - 1) / vmin >= (1ull << 28)) return fail(MIG_EINVAL, "create: class %u: longest duration exceeds 2^28 s", c);
@@ -187,6 +221,9 @@ static const void *kernel_ptr(int tile, bool evd = false) {
 // shared-memory footprint and resident grid for `tile` lanes per environment (1 = one thread per environment)
 static int configure_tile(mig_sim *s, int tile) {
   if (tile != 1 && tile != 8 && tile != 16 && tile != 32) return fail(MIG_EINVAL, "set_tile: lanes per environment must be 1, 8, 16 or 32 (got %d)", tile);
+  if (tile != 1 && uses_extensions(s->p))
+    return fail(MIG_EINVAL, "set_tile: this parameter set uses an extension (MIG-disabled GPU, whole-GPU repartition, utilisation levels, binned policy) "
+                            "that only the thread-per-environment kernel implements (lanes per environment = 1)");
   const uint32_t cap4 = (s->p.cap + 3u) & ~3u, cap8 = (s->p.cap + 7u) & ~7u;
   uint32_t entries; size_t bytes; int threads;
   if (tile == 1) {
@@ -267,7 +304,8 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
   mig_sim *s = new (std::nothrow) mig_sim();
   if (!s) return fail(MIG_ENOMEM, "create: host allocation failed");
   s->p = *p;
-  s->p.speed = nullptr; s->p.dur7_q = nullptr; s->p.class_cum = nullptr; s->p.slack_q10 = nullptr; s->p.size_at_slot = nullptr; s->p.accept_thr = nullptr;
+  s->p.speed = nullptr; s->p.dur7_q = nullptr; s->p.class_cum = nullptr; s->p.slack_q10 = nullptr; s->p.size_at_slot = nullptr; s->p.accept_thr = nullptr; s->p.dbin_edges = nullptr; s->p.abin_edges = nullptr;
+  if (p->speed_nomig) s->p.speed_nomig = reinterpret_cast<const uint32_t *>(1);   // (only "is it in use" is kept)
   s->n_envs = n_envs; s->seed = seed;
   cudaDeviceProp prop;
   if (cudaGetDevice(&s->device) != cudaSuccess || cudaGetDeviceProperties(&prop, s->device) != cudaSuccess) { delete s; return fail(MIG_ECUDA, "create: cannot query the device"); }
@@ -369,6 +407,8 @@ static void base_args(const mig_sim *s, SimArgs &a) {
   a.algo = s->d_algo; a.cfg0 = s->d_cfg0;
   a.script = s->n_script ? s->d_script : nullptr; a.n_script = s->n_script;
   a.rec_stride = s->n_envs;
+  a.all_down = p.repart_all_down != 0; a.util_hist = p.util_hist != 0; a.gamma = p.gamma;
+  a.n_tbins = p.n_tbins; a.n_dbins = p.n_dbins; a.n_abins = p.n_abins;
 }
 
 // Environments per warp of the thread-per-env kernel: the smallest power of two that keeps the launch one resident wave
@@ -448,7 +488,7 @@ extern "C" int mig_sim_step(mig_sim_t *s, const uint8_t *action, float *state_ou
   if (s->epoch < 0) return fail(MIG_ESTATE, "step: reset has not been called");
   if (s->epoch >= s->p.n_epochs) return fail(MIG_ESTATE, "step: the day is over (%d epochs done); call reset", s->epoch);
   SimArgs a; base_args(s, a);
-  a.save = 1; a.n_steps = 1; a.policy = 3;
+  a.save = 1; a.n_steps = 1; a.policy = kPolicyExplicit;
   a.actions = action; a.act_stride_env = 1; a.act_stride_k = 0;
   a.state_out = state_out; a.reward_out = reward_out; a.energy_out = energy_mj_out; a.tard_out = tardiness_s_out;
   a.recs = rec_out; a.rec_k0 = s->epoch; a.drain_rec = drain_rec_out;
@@ -477,14 +517,16 @@ extern "C" int mig_sim_rollout(mig_sim_t *s, int policy, const uint8_t *table, c
   if (!s) return fail(MIG_EINVAL, "rollout: NULL handle");
   if (s->epoch < 0) return fail(MIG_ESTATE, "rollout: reset has not been called");
   if (s->epoch >= s->p.n_epochs) return fail(MIG_ESTATE, "rollout: the day is over; call reset");
-  if (policy != MIG_POLICY_STATIC && policy != MIG_POLICY_TABLE && policy != MIG_POLICY_DQN) return fail(MIG_EINVAL, "rollout: unknown policy %d", policy);
-  if (policy == MIG_POLICY_TABLE && !table) return fail(MIG_EINVAL, "rollout: TABLE policy needs a table");
+  if (policy != MIG_POLICY_STATIC && policy != MIG_POLICY_TABLE && policy != MIG_POLICY_DQN && policy != MIG_POLICY_BINNED) return fail(MIG_EINVAL, "rollout: unknown policy %d", policy);
+  if ((policy == MIG_POLICY_TABLE || policy == MIG_POLICY_BINNED) && !table) return fail(MIG_EINVAL, "rollout: TABLE / BINNED policy needs a table");
+  if (policy == MIG_POLICY_BINNED && (!s->p.n_tbins || s->tile != 1)) return fail(MIG_EINVAL, "rollout: the BINNED policy needs n_tbins / n_dbins / n_abins at create and the thread-per-environment kernel");
   cudaStream_t st = (cudaStream_t)stream;
   const int ne = s->p.n_epochs;
   if (policy != MIG_POLICY_DQN) {
     SimArgs a; base_args(s, a);
-    a.save = 1; a.n_steps = ne - s->epoch; a.policy = policy; a.table = table;
-    a.ev_decide = policy == MIG_POLICY_TABLE && s->p.decide_on_events;
+    a.save = 1; a.n_steps = ne - s->epoch; a.policy = policy;
+    if (policy == MIG_POLICY_BINNED) a.bin_table = table; else a.table = table;
+    a.ev_decide = (policy == MIG_POLICY_TABLE || policy == MIG_POLICY_BINNED) && s->p.decide_on_events;
     a.recs = recs_out; a.rec_k0 = 0; a.drain_rec = recs_out ? recs_out + (size_t)ne * s->n_envs : nullptr;
     a.totals = totals_out;
     int rc = launch_sim<false>(s, a, st);
@@ -512,7 +554,7 @@ extern "C" int mig_sim_rollout(mig_sim_t *s, int policy, const uint8_t *table, c
     if (rc) return rc;
     s->launches++;
     SimArgs a; base_args(s, a);
-    a.save = 1; a.n_steps = 1; a.policy = 3;
+    a.save = 1; a.n_steps = 1; a.policy = kPolicyExplicit;
     a.actions = s->d_action; a.act_stride_env = 1; a.act_stride_k = 0;
     a.state_out = s->d_state;
     a.recs = recs_out; a.rec_k0 = 0; a.drain_rec = recs_out ? recs_out + (size_t)ne * s->n_envs : nullptr;
@@ -532,6 +574,33 @@ extern "C" int mig_sim_totals(mig_sim_t *s, mig_totals_t *totals_out, void *stre
   return launch_sim<false>(s, a, (cudaStream_t)stream);
 }
 
+extern "C" int mig_sim_aux(mig_sim_t *s, float *return_out, int32_t *util_s_out, void *stream) {
+  if (!s) return fail(MIG_EINVAL, "aux: NULL handle");
+  if (s->epoch < 0) return fail(MIG_ESTATE, "aux: reset has not been called");
+  if (s->tile != 1) return fail(MIG_ESTATE, "aux: the discounted return and the utilisation levels are kept by the thread-per-environment kernel only");
+  if (util_s_out && !s->p.util_hist) return fail(MIG_ESTATE, "aux: params.util_hist was 0 at create: the utilisation levels were not kept");
+  if (!return_out && !util_s_out) return MIG_OK;
+  aux_kernel<<<(s->n_envs + 255) / 256, 256, 0, (cudaStream_t)stream>>>(s->d_hdr, s->n_envs, return_out, util_s_out);
+  CU(cudaGetLastError());
+  s->launches++;
+  return MIG_OK;
+}
+
+// ET: host reduction in double; a = t / (2 s) from the GLOBAL means
+extern "C" int mig_et_reduce(const double *x, const double *y, const uint32_t *group, uint32_t n, uint32_t n_groups, double *et_out, double *a_out) {
+  if (!x || !y || !group || !et_out || n == 0 || n_groups == 0) return fail(MIG_EINVAL, "et_reduce: NULL argument or n = 0");
+  double sx = 0.0, sy = 0.0;
+  for (uint32_t i = 0; i < n; ++i) { if (group[i] >= n_groups) return fail(MIG_EINVAL, "et_reduce: group[%u] = %u out of range", i, group[i]); sx += x[i]; sy += y[i]; }
+  const double smean = sx / n, tmean = sy / n;
+  if (!(smean > 0.0)) return fail(MIG_EINVAL, "et_reduce: the mean energy must be positive");
+  const double a = tmean / (2.0 * smean);
+  std::vector<double> acc(n_groups, 0.0); std::vector<uint32_t> cnt(n_groups, 0);
+  for (uint32_t i = 0; i < n; ++i) { acc[group[i]] += (a * x[i] + y[i]) / (a + 1.0); cnt[group[i]]++; }
+  for (uint32_t g = 0; g < n_groups; ++g) et_out[g] = cnt[g] ? acc[g] / cnt[g] : 0.0;
+  if (a_out) *a_out = a;
+  return MIG_OK;
+}
+
 extern "C" int mig_sim_rollout_host(mig_sim_t *s, uint32_t episode, const uint8_t *algo, const uint8_t *cfg0, int policy,
                                     const uint8_t *table, const mig_qnet_t *q, float epsilon, mig_epoch_rec_t *recs_out,
                                     mig_totals_t *totals_out) {
@@ -539,9 +608,10 @@ extern "C" int mig_sim_rollout_host(mig_sim_t *s, uint32_t episode, const uint8_
   const size_t n = s->n_envs, ne = (size_t)s->p.n_epochs;
   if (!s->d_totals) { if (cudaMalloc((void **)&s->d_totals, n * sizeof(mig_totals_t)) != cudaSuccess) { cudaGetLastError(); return fail(MIG_ENOMEM, "rollout_host: cudaMalloc failed"); } }
   if (recs_out && !s->d_recs) { if (cudaMalloc((void **)&s->d_recs, n * (ne + 1) * sizeof(mig_epoch_rec_t)) != cudaSuccess) { cudaGetLastError(); return fail(MIG_ENOMEM, "rollout_host: cudaMalloc failed"); } }
-  if (policy == MIG_POLICY_TABLE) {
-    if (!table) return fail(MIG_EINVAL, "rollout_host: TABLE policy needs a table");
-    size_t tb = n * ne * 4;
+  if (policy == MIG_POLICY_TABLE || policy == MIG_POLICY_BINNED) {
+    if (!table) return fail(MIG_EINVAL, "rollout_host: TABLE / BINNED policy needs a table");
+    const size_t Bc = 1 + (size_t)s->p.n_dbins * s->p.n_abins;
+    size_t tb = policy == MIG_POLICY_TABLE ? n * ne * 4 : (size_t)s->p.n_configs * s->p.n_tbins * Bc * Bc * Bc;
     if (s->table_bytes < tb) { cudaFree(s->d_table); s->d_table = nullptr; if (cudaMalloc((void **)&s->d_table, tb) != cudaSuccess) { cudaGetLastError(); s->table_bytes = 0; return fail(MIG_ENOMEM, "rollout_host: cudaMalloc failed"); } s->table_bytes = tb; }
     CU(cudaMemcpyAsync(s->d_table, table, tb, cudaMemcpyHostToDevice, 0));
   }
@@ -606,13 +676,18 @@ extern "C" int mig_sim_debug_trace(mig_sim_t *s, uint32_t env, int policy, const
   if (!s || !n_out) return fail(MIG_EINVAL, "debug_trace: NULL argument");
   if (s->epoch < 0) return fail(MIG_ESTATE, "debug_trace: reset has not been called");
   if (env >= s->n_envs) return fail(MIG_EINVAL, "debug_trace: env %u out of range", env);
-  if (!actions && policy != MIG_POLICY_STATIC && policy != MIG_POLICY_TABLE) return fail(MIG_EINVAL, "debug_trace: policy must be STATIC or TABLE, or pass actions");
-  if (!actions && policy == MIG_POLICY_TABLE && !table) return fail(MIG_EINVAL, "debug_trace: TABLE policy needs a table");
+  if (!actions && policy != MIG_POLICY_STATIC && policy != MIG_POLICY_TABLE && policy != MIG_POLICY_BINNED) return fail(MIG_EINVAL, "debug_trace: policy must be STATIC, TABLE or BINNED, or pass actions");
+  if (!actions && policy != MIG_POLICY_STATIC && !table) return fail(MIG_EINVAL, "debug_trace: TABLE / BINNED policy needs a table");
+  if (!actions && policy == MIG_POLICY_BINNED && (!s->p.n_tbins || s->tile != 1)) return fail(MIG_EINVAL, "debug_trace: the BINNED policy needs n_tbins / n_dbins / n_abins at create and the thread-per-environment kernel");
   SimArgs a; base_args(s, a);
   a.n_envs = 1; a.env_first = env; a.tab_override = s->d_dbgtab; a.hdr_override = s->d_dbghdr;
   a.from_init = 1; a.save = 0; a.n_steps = s->p.n_epochs;
-  if (actions) { a.policy = 3; a.actions = actions; a.act_stride_env = 0; a.act_stride_k = 1; }
-  else { a.policy = policy; a.table = table; a.ev_decide = policy == MIG_POLICY_TABLE && s->p.decide_on_events; }
+  if (actions) { a.policy = kPolicyExplicit; a.actions = actions; a.act_stride_env = 0; a.act_stride_k = 1; }
+  else {
+    a.policy = policy;
+    if (policy == MIG_POLICY_BINNED) a.bin_table = table; else a.table = table;
+    a.ev_decide = policy != MIG_POLICY_STATIC && s->p.decide_on_events;
+  }
   a.trace = buf; a.trace_cap = buf ? cap_events : 0; a.trace_n = n_out; a.totals = totals_out;
   return launch_sim<true>(s, a, (cudaStream_t)stream);
 }
@@ -634,6 +709,7 @@ extern "C" int mig_sim_debug_set_jobs(mig_sim_t *s, const mig_job_t *jobs, uint3
     if (j.dur7 < 1 || j.dur7 > (1 << 24)) return fail(MIG_EINVAL, "debug_set_jobs: job %u: dur7 %d not in 1..2^24", i, j.dur7);
     uint32_t vmin = 0xFFFFFFFFu, vmax = 0;
     for (int k = 0; k < 5; ++k) { uint32_t v = host[0].speed[j.cls * 5 + k].x; vmin = v < vmin ? v : vmin; vmax = v > vmax ? v : vmax; }
+    { uint32_t v = host[0].speed_nomig[j.cls].x; vmin = v < vmin ? v : vmin; vmax = v > vmax ? v : vmax; }
     unsigned long long work = (unsigned long long)j.dur7 * host[0].speed[j.cls * 5 + 4].x;
     if (work + vmax >= (1ull << 31) || (work + vmin - 1) / vmin >= (1ull << 28))
       return fail(MIG_EINVAL, "debug_set_jobs: job %u: work %llu out of the int32 / 2^28 s range", i, work);

@@ -26,7 +26,10 @@ struct DevTables {
   int32_t cfg_pidle[MIG_MAX_CONFIGS];       // sum of p_idle over the configuration's slices
   uint32_t thr[MIG_THR_BINS];
   uint32_t logT[257];                        // round(2^24 log2(1 + i/256))
-  int32_t curve[8], p_idle[8], p_busy[8];    // p_idle/p_busy indexed by SIZE (0..7), not by size index
+  int32_t curve[8], p_idle[12], p_busy[12];  // p_idle/p_busy indexed by SIZE (0..8; 8 = MIG disabled), not by size index
+  // extensions (thread-per-environment kernel only)
+  uint4 speed_nomig[MIG_MAX_CLASSES];        // {v, magic, shift, 0} on the whole GPU with MIG disabled (size code 8)
+  int32_t dbin_edges[8], abin_edges[8];      // BINNED policy: bin edges, padded with INT32_MAX
 };
 
 // Kernel arguments (by value, constant bank).
@@ -57,6 +60,12 @@ struct SimArgs {
   const uint8_t *table;                              // [n_envs][n_epochs][4]
   int ev_decide;                                     // TABLE policy: look the table up again after every tick with an arrival or a completion
   const uint8_t *actions; uint32_t act_stride_env, act_stride_k;   // action = actions[env * se + (k - k_first) * sk]
+  // extensions (thread-per-environment kernel only; readings #29-#32)
+  const uint8_t *bin_table;                          // BINNED policy: [n_configs][n_tbins][B][B][B], one table for all envs
+  uint32_t n_tbins, n_dbins, n_abins;
+  int all_down;                                      // a repartition takes the whole GPU down
+  int util_hist;                                     // keep the seconds per utilisation level in the env's header
+  float gamma;                                       // discount of the return kept in the env's header
   const mig_job_t *script; uint32_t n_script;
   const uint2 *arr; uint32_t arr_cap;                // thread-per-env kernel: arrival lists [n_envs][arr_cap] of 8-byte records (gen_kernel.cuh), or NULL
   // outputs (NULL = skip)

@@ -40,15 +40,24 @@ enum { T1_V = 0 /* 7: speed of the running job */, T1_STGDUE = 7 /* 7 */, T1_CNT
 // saved per-env header of this kernel (kHeaderWords words); the running totals H1_TOT / H1_CNT live here all the time
 enum { H1_T = 0, H1_PK, H1_NSYS, H1_NWAIT, H1_HLO, H1_HHI, H1_GK, H1_GT_LO, H1_GT_HI, H1_GDONE, H1_NACC, H1_ISCRIPT,
        H1_DROPS, H1_MASKS /* busy | down << 8 */, H1_ORDER, H1_QHEAD, H1_QNS, H1_GHEAD, H1_QNG, H1_TOT = 20 /* 6 */, H1_LOOKV = 26, H1_LOOKTICK, H1_LOOKCLS, H1_LOOKWORK,
-       H1_LOOKDUE, H1_LOOKID, H1_ACOUNT = 32, H1_AMORE, H1_AID0 /* written by gen_arrivals_kernel */, H1_CNT = 48 /* 10 */ };
+       H1_LOOKDUE, H1_LOOKID, H1_ACOUNT = 32, H1_AMORE, H1_AID0 /* written by gen_arrivals_kernel */,
+       H1_RET = 36 /* discounted return so far, fp32 bits */, H1_DISC /* gamma^k, fp32 bits */, H1_UTIL = 40 /* 8: seconds per utilisation level */,
+       H1_CNT = 48 /* 10 */ };
 static_assert((int)H1_PK == (int)HG_PK && (int)H1_GK == (int)HG_GK && (int)H1_NACC == (int)HG_NACC && (int)H1_ACOUNT == (int)HG_ACOUNT && (int)H1_AID0 == (int)HG_AID0, "header layout shared with gen_kernel.cuh");
 
+constexpr int kSpeedCols = 6;    // speed columns of this kernel's table: 1g, 2g, 3g, 4g, 7g, MIG disabled (size code 8)
 struct HotTablesT {              // per CTA, shared memory
-  HotTables h;
+  uint4 speed[MIG_MAX_CLASSES * kSpeedCols];   // {v, magic, shift, 0}
+  uint32_t cfg_pack[MIG_MAX_CONFIGS];     // nibble p: size of the slice starting at slot p
   uint32_t cfg_rank[MIG_MAX_CONFIGS];     // nibble p: rank of the slice starting at slot p in (size, slot) order (reading #4)
   uint32_t cfg_slot_of[MIG_MAX_CONFIGS];  // nibble r: start slot of the slice of rank r
   int32_t cfg_pidle[MIG_MAX_CONFIGS];     // sum of p_idle over the slices of the configuration
+  int32_t curve[8];
+  int32_t pdiff[12];                      // p_busy - p_idle by slice size (0..8)
 };
+// column of a slice size: 1, 2, 3, 4, 7, 8 -> 0..5;   compute units of a slice: the MIG-disabled GPU (8) has 7
+__device__ __forceinline__ int sidx6_of(int size) { return size >= 7 ? size - 3 : size - 1; }
+__device__ __forceinline__ int units_of(int size) { return min(size, 7); }
 
 __host__ __device__ constexpr size_t thread_smem_bytes(uint32_t smem_entries, int nt) {
   return ((sizeof(HotTablesT) + 127) & ~(size_t)127) + (size_t)nt * ((T2_RING + 2 * (size_t)smem_entries) * 8 + T1_WORDS * 4 + 32);   // + a 32-byte landing slot: four arrival records
@@ -276,7 +285,7 @@ struct EnvT {
 
   // ------------------------------------------------------------------ model
   __device__ __forceinline__ int size_at(int p) const { return (cfg_sizes >> (4 * p)) & 15; }
-  __device__ __forceinline__ const uint4 &speed_of(uint32_t cls, int size) const { return hot.h.speed[cls * 5 + sidx_of(size)]; }
+  __device__ __forceinline__ const uint4 &speed_of(uint32_t cls, int size) const { return hot.speed[cls * kSpeedCols + sidx6_of(size)]; }
 
   // remaining duration against the configuration: fastest slice (LLF) or floor of the mean over all
   // slices of cfg, up or down (LALF; also the state vector's "average duration", L210)
@@ -295,7 +304,7 @@ struct EnvT {
   }
 
   __device__ __forceinline__ void set_cfg_tables(int c) {
-    cfg = c; cfg_sizes = hot.h.cfg_pack[c]; cfg_rank = hot.cfg_rank[c];
+    cfg = c; cfg_sizes = hot.cfg_pack[c]; cfg_rank = hot.cfg_rank[c];
     uint32_t m = 0;
 #pragma unroll
     for (int p = 0; p < kSlots; ++p) m |= ((cfg_sizes >> (4 * p)) & 15u) ? (1u << p) : 0u;
@@ -307,9 +316,9 @@ struct EnvT {
     int u = 0, pd = 0;
     for (uint32_t m = busy_mask; m; m &= m - 1) {
       const int g = size_at(__ffs((int)m) - 1);
-      u += g; pd += hot.h.p_busy[g] - hot.h.p_idle[g];
+      u += units_of(g); pd += hot.pdiff[g];
     }
-    U = u; P = hot.cfg_pidle[cfg] + pd + hot.h.curve[u & 7];
+    U = u; P = hot.cfg_pidle[cfg] + pd + hot.curve[u & 7];
   }
 
   // ------------------------------------------------------------------ arrivals (R2-R5)
@@ -336,7 +345,7 @@ struct EnvT {
   __device__ __forceinline__ void set_look(uint32_t tick, uint32_t cls, uint32_t dur7, uint32_t slack) {
     unsigned long long rel = ((unsigned long long)dur7 * slack) >> 10;
     if (rel < 1) rel = 1;
-    look_tick = (int)tick; look_cls = cls; look_work = (int)(dur7 * hot.h.speed[cls * 5 + 4].x);
+    look_tick = (int)tick; look_cls = cls; look_work = (int)(dur7 * hot.speed[cls * kSpeedCols + 4].x);
     look_due = (int)((long long)tick + (long long)rel);
     look_valid = 1;
   }
@@ -348,7 +357,7 @@ struct EnvT {
       if (i_script < a.n_script) {
         const mig_job_t s = a.script[i_script];
         look_valid = 1; look_tick = s.arr; look_cls = s.cls; look_due = s.due;
-        look_work = (int)((uint32_t)s.dur7 * hot.h.speed[s.cls * 5 + 4].x);
+        look_work = (int)((uint32_t)s.dur7 * hot.speed[s.cls * kSpeedCols + 4].x);
         look_id = i_script; n_accepted++; i_script++;
       }
       return;
@@ -511,7 +520,7 @@ struct EnvT {
       const int s = (int)((hot.cfg_slot_of[cfg] >> (4 * rk)) & 7u);
       const int g = size_at(s);
       avail &= ~(1u << s);
-      nb |= 1u << s; nd = min(nd, t + (pick >> 3)); u += g; pd += hot.h.p_busy[g] - hot.h.p_idle[g];
+      nb |= 1u << s; nd = min(nd, t + (pick >> 3)); u += units_of(g); pd += hot.pdiff[g];
       const bool moved = bp != s;
       if (!moved) keep |= 1u << s;
       R2(T2_STG + K) = make_uint2((bkm.y & ~15u) | (uint32_t)s | (moved ? 8u : 0u), rdv.x);
@@ -547,7 +556,7 @@ struct EnvT {
     }
     if (n_start) count(C_START, (uint32_t)n_start);
     busy_mask = nb; next_done = nd; run_order = new_order;
-    U = u; P = hot.cfg_pidle[cfg] + pd + hot.h.curve[u & 7];
+    U = u; P = hot.cfg_pidle[cfg] + pd + hot.curve[u & 7];
     compute_next_crit();
   }
 
@@ -560,6 +569,7 @@ struct EnvT {
     const int dt = tn - t;
     e_ep += (long long)P * dt;
     busy_ep += (long long)U * dt;
+    if (a.util_hist && dt) hdr[H1_UTIL + U] += (uint32_t)dt;          // time at this utilisation level (Fig. 6)
     t = tn;
     uint32_t done = 0;
     if (dt)
@@ -628,8 +638,12 @@ struct EnvT {
     // event-driven decision (reading #27): after a tick of the day with an arrival or a
     // completion the tabulated policy is looked up with the load bucket of this moment
     if (EVD && a.ev_decide && job_event && !in_drain) {
-      const uint32_t b = n_sys == 0 ? 0u : (n_sys < 8 ? 1u : (n_sys < 64 ? 2u : 3u));
-      const uint32_t action = a.table[((size_t)env_l * a.n_epochs + epoch) * 4 + b];
+      uint32_t action;
+      if (a.policy == MIG_POLICY_BINNED) action = a.bin_table[binned_index()];      // the paper's binned 2+2m state (L210)
+      else {
+        const uint32_t b = n_sys == 0 ? 0u : (n_sys < 8 ? 1u : (n_sys < 64 ? 2u : 3u));
+        action = a.table[((size_t)env_l * a.n_epochs + epoch) * 4 + b];
+      }
       if (action >= a.n_configs) status |= MIG_ST_BAD_ACTION;
       else if ((int)action != cfg) { repartition(action); return; }   // (it reschedules)
     }
@@ -645,10 +659,11 @@ struct EnvT {
   }
   // action is a valid configuration other than the current one; ends with ONE reschedule
   __device__ __forceinline__ void repartition(uint32_t action) {
-    const uint32_t newsizes = hot.h.cfg_pack[action];
+    const uint32_t newsizes = hot.cfg_pack[action];
     uint32_t changed = 0;                                     // slots whose (start, size) differs between the two rows
 #pragma unroll
     for (int p = 0; p < kSlots; ++p) changed |= (((cfg_sizes ^ newsizes) >> (4 * p)) & 15u) ? (1u << p) : 0u;
+    if (a.all_down) changed = 0x7Fu;                          // the whole GPU goes down (reading #30)
     const uint32_t pm = busy_mask & changed;                  // jobs on destroyed slices go back to waiting
     if (pm) {
       count(C_PREEMPT, __popc(pm));
@@ -741,7 +756,7 @@ struct EnvT {
     for (uint32_t m = slice_mask; m; m &= m - 1) {
       const int p = __ffs((int)m) - 1, g = size_at(p);
       const float occ = ((down_mask >> p) & 1u) ? 0.5f : (((busy_mask >> p) & 1u) ? 1.0f : 0.0f);
-      for (int q = 0; q < g; ++q) out[16 + p + q] = occ;        // slots covered by this slice
+      for (int q = 0; q < units_of(g); ++q) out[16 + p + q] = occ;   // slots covered by this slice
       out[23 + p] = (float)g * 0.125f;
     }
     out[30 + (t / 3600) % 24] = 1.0f;
@@ -751,21 +766,54 @@ struct EnvT {
     out[63] = 1.0f;
     int pk = (int)0x80000000; uint32_t pid = 0;
     for (int m = 0; m < 3 && (uint32_t)m < n_sys; ++m) {        // first m = 3 jobs in (due, id) order
-      int bk = MIG_INF; uint32_t bid = 0xFFFFFFFFu; uint2 bkm = make_uint2(0u, 0u), brd = bkm;
-      for (uint32_t j = 0; j < 7u + n_wait; ++j) {
-        uint2 km, rdv;
-        if (!job_at(j, km, rdv)) continue;
-        const int due = (int)rdv.y; const uint32_t id = m_id(km.y);
-        const bool beyond = due > pk || (due == pk && id > pid);
-        const bool better = due < bk || (due == bk && id < bid);
-        if (beyond && better) { bk = due; bid = id; bkm = km; brd = rdv; }
-      }
+      uint2 bkm, brd;
+      next_by_due(pk, pid, bkm, brd);
       const int d = max(-32768, min(32767, (int)brd.y - t));
       const int mean = min(rd_cfg((int)brd.x, m_cls(bkm.y), true), 32767);
       out[56 + m] = (float)d * (1.0f / 4096.0f);
       out[59 + m] = (float)mean * (1.0f / 4096.0f);
-      pk = bk; pid = bid;
     }
+  }
+  // the job that follows (pk, pid) in (due, id) order over all jobs in system (running and waiting); advances (pk, pid)
+  __device__ __forceinline__ void next_by_due(int &pk, uint32_t &pid, uint2 &bkm, uint2 &brd) {
+    int bk = MIG_INF; uint32_t bid = 0xFFFFFFFFu; bkm = make_uint2(0u, 0u); brd = bkm;
+    for (uint32_t j = 0; j < 7u + n_wait; ++j) {
+      uint2 km, rdv;
+      if (!job_at(j, km, rdv)) continue;
+      const int due = (int)rdv.y; const uint32_t id = m_id(km.y);
+      const bool beyond = due > pk || (due == pk && id > pid);
+      const bool better = due < bk || (due == bk && id < bid);
+      if (beyond && better) { bk = due; bid = id; bkm = km; brd = rdv; }
+    }
+    pk = bk; pid = bid;
+  }
+
+  // ------------------------------------------------------------------ binned state (reading #31)
+  // index of the present state in the BINNED policy's table: configuration, time bin, and for each of the first m = 3 jobs
+  // in (due, id) order the code 0 (no such job) or 1 + dbin * n_abins + abin of its deadline (due - t) and its mean
+  // remaining duration over the slices of the configuration
+  static __device__ __forceinline__ uint32_t bin_of(int v, const int32_t *edges, uint32_t n_bins) {
+    uint32_t b = 0;
+    while (b + 1u < n_bins && v >= __ldg(&edges[b])) ++b;
+    return b;
+  }
+  __device__ __forceinline__ uint32_t binned_index() {
+    const uint32_t B = 1u + a.n_dbins * a.n_abins;
+    const uint32_t tc = (uint32_t)min(t, a.day_s - 1);
+    uint32_t idx = (uint32_t)cfg * a.n_tbins + (tc * a.n_tbins) / (uint32_t)a.day_s;
+    int pk = (int)0x80000000; uint32_t pid = 0;
+    for (uint32_t m = 0; m < 3u; ++m) {
+      uint32_t code = 0;
+      if (m < n_sys) {
+        uint2 bkm, brd;
+        next_by_due(pk, pid, bkm, brd);
+        const uint32_t db = bin_of((int)brd.y - t, a.tab->dbin_edges, a.n_dbins);
+        const uint32_t ab = bin_of(rd_cfg((int)brd.x, m_cls(bkm.y), true), a.tab->abin_edges, a.n_abins);
+        code = 1u + db * a.n_abins + ab;
+      }
+      idx = idx * B + code;
+    }
+    return idx;
   }
 
   // ------------------------------------------------------------------ init / load / save
@@ -781,7 +829,8 @@ struct EnvT {
     g_k = 0; g_T = 0; g_done = 0; n_accepted = 0; a_count = 0; a_more = 1; a_id0 = 0;
     look_valid = 0; look_tick = 0; look_work = 0; look_due = 0; look_cls = 0; look_id = 0;
     n_trace = 0; i_script = 0;
-    for (int w = H1_DROPS; w < kHeaderWords; ++w) hdr[w] = 0u;      // running totals, drops
+    for (int w = H1_DROPS; w < kHeaderWords; ++w) hdr[w] = 0u;      // running totals, drops, return, utilisation levels
+    hdr[H1_DISC] = __float_as_uint(1.0f);
   }
   __device__ __forceinline__ void init_rows() {
     begin_span();
@@ -853,6 +902,8 @@ struct EnvT {
         if (a.policy == MIG_POLICY_TABLE) {                                         // load bucket
           const uint32_t b = n_sys == 0 ? 0u : (n_sys < 8 ? 1u : (n_sys < 64 ? 2u : 3u));
           action = a.table[((size_t)env * a.n_epochs + epoch) * 4 + b];
+        } else if (a.policy == MIG_POLICY_BINNED) {                                 // binned 2+2m state
+          action = a.bin_table[binned_index()];
         } else if (a.actions) {
           action = a.actions[(size_t)li * a.act_stride_env + (size_t)s * a.act_stride_k];
         }
@@ -877,8 +928,13 @@ struct EnvT {
       epoch++;
       if (a.energy_out) a.energy_out[out_i] = dE;
       if (a.tard_out) a.tard_out[out_i] = dT;
-      if (a.reward_out)                                       // two fp32 products, one add, negate; no contraction
-        a.reward_out[out_i] = -__fadd_rn(__fmul_rn(a.w_energy, __ll2float_rn(dE)), __fmul_rn(a.w_tardy, __ll2float_rn(dT)));
+      {                                                       // reward: two fp32 products, one add, negate; no contraction
+        const float r = -__fadd_rn(__fmul_rn(a.w_energy, __ll2float_rn(dE)), __fmul_rn(a.w_tardy, __ll2float_rn(dT)));
+        if (a.reward_out) a.reward_out[out_i] = r;
+        const float d = __uint_as_float(hdr[H1_DISC]);          // discounted return (reading #32)
+        hdr[H1_RET] = __float_as_uint(__fmaf_rn(d, r, __uint_as_float(hdr[H1_RET])));
+        hdr[H1_DISC] = __float_as_uint(__fmul_rn(d, a.gamma));
+      }
       ++s;
       if (--steps_left == 0 || epoch >= a.n_epochs) break;
       fresh = true;
@@ -892,11 +948,15 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   HotTablesT &hot = *reinterpret_cast<HotTablesT *>(smem_raw);
   {
     const DevTables *tb = a.tab;
-    for (int i = threadIdx.x; i < MIG_MAX_CLASSES * 5; i += NT) hot.h.speed[i] = tb->speed[i];
-    for (int i = threadIdx.x; i < MIG_MAX_CONFIGS; i += NT) {
-      hot.h.cfg_pack[i] = tb->cfg_pack[i]; hot.cfg_rank[i] = tb->cfg_rank[i]; hot.cfg_slot_of[i] = tb->cfg_slot_of[i]; hot.cfg_pidle[i] = tb->cfg_pidle[i];
+    for (int i = threadIdx.x; i < MIG_MAX_CLASSES * kSpeedCols; i += NT) {
+      const int c = i / kSpeedCols, k = i - c * kSpeedCols;
+      hot.speed[i] = k < 5 ? tb->speed[c * 5 + k] : tb->speed_nomig[c];
     }
-    if (threadIdx.x < 8) { hot.h.curve[threadIdx.x] = tb->curve[threadIdx.x]; hot.h.p_idle[threadIdx.x] = tb->p_idle[threadIdx.x]; hot.h.p_busy[threadIdx.x] = tb->p_busy[threadIdx.x]; }
+    for (int i = threadIdx.x; i < MIG_MAX_CONFIGS; i += NT) {
+      hot.cfg_pack[i] = tb->cfg_pack[i]; hot.cfg_rank[i] = tb->cfg_rank[i]; hot.cfg_slot_of[i] = tb->cfg_slot_of[i]; hot.cfg_pidle[i] = tb->cfg_pidle[i];
+    }
+    if (threadIdx.x < 8) hot.curve[threadIdx.x] = tb->curve[threadIdx.x];
+    if (threadIdx.x < 12) hot.pdiff[threadIdx.x] = tb->p_busy[threadIdx.x] - tb->p_idle[threadIdx.x];
   }
   unsigned char *base = smem_raw + ((sizeof(HotTablesT) + 127) & ~(size_t)127);
   __syncthreads();
@@ -926,6 +986,19 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   if (a.totals) e.store_totals(a.totals + (TRACE ? 0u : env));   // totals so far (hash and t are live values)
   if (a.save) e.save();
   if (TRACE && a.trace_n) *a.trace_n = e.n_trace;
+}
+
+// per-env auxiliary results out of the saved headers: the discounted return and the seconds per utilisation level
+__global__ void aux_kernel(const uint32_t *hdr, uint32_t n_envs, float *ret_out, int32_t *util_out) {
+  const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n_envs) return;
+  const uint32_t *h = hdr + (size_t)e * kHeaderWords;
+  if (ret_out) ret_out[e] = __uint_as_float(h[H1_RET]);
+  if (util_out) {
+    int4 *o = reinterpret_cast<int4 *>(util_out + (size_t)e * 8);
+    o[0] = make_int4((int)h[H1_UTIL], (int)h[H1_UTIL + 1], (int)h[H1_UTIL + 2], (int)h[H1_UTIL + 3]);
+    o[1] = make_int4((int)h[H1_UTIL + 4], (int)h[H1_UTIL + 5], (int)h[H1_UTIL + 6], (int)h[H1_UTIL + 7]);
+  }
 }
 
 }  // namespace migsim

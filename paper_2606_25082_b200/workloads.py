@@ -381,6 +381,73 @@ def config_c5(n_envs: int = 65536) -> Workload:
                     POLICY_TABLE, table=_c5_table(n_envs), mean_jobs_per_day=8000)
 
 
+# --------------------------------------------------------------------------- the paper's benchmark policies and sweeps
+# (SURVEY 8(f) #4).  Input recipes only: tables, no arithmetic of the method.
+NOMIG_CONFIG = ((8, 0),)             # size code 8 = the whole GPU with MIG disabled (reading #29)
+PAPER_STATIC_CFG, PAPER_DAY_CFG, PAPER_NIGHT_CFG = 2, 5, 1     # 0-based ids of the paper's configurations 3, 6 and 2 (L230)
+
+
+def speed_nomig_of(speeds) -> np.ndarray:
+    """Speed on the MIG-disabled GPU per class: "6% performance improvement for linear jobs ... compared to a 7g.40gb slice"
+    (PAPER.md:L230): round(1.06 v_7g) for the linear family, v_7g for every other (the paper names linear jobs only)."""
+    lin = speed_linear()
+    return np.array([int(round(1.06 * s[4])) if list(s) == lin else int(s[4]) for s in speeds], dtype=np.uint32)
+
+
+def benchmark_params(jobs_per_day=2000.0, amplitude=0.6, inference_frac=0.8, **kw) -> SimParams:
+    """The C3/C4 class mix (6 elasticity families x short "inference-like" / long "training-like")
+    with the 12 configurations of Fig. 1 plus the MIG-disabled GPU as a 13th (id 12), the paper's 4 s repartition
+    penalty for the whole GPU (L214), the discount of its reward model and the utilisation levels of Fig. 6."""
+    fams = (speed_linear(), speed_sublinear(0.5), speed_sublinear(0.7), speed_sublinear(0.9), speed_capped(2), speed_capped(4))
+    speeds, durs, w = [], [], []
+    for f in fams:
+        speeds.append(f); durs.append(dur_uniform(2, 20)); w.append(inference_frac)
+        speeds.append(f); durs.append(dur_uniform(30, 150)); w.append(1.0 - inference_frac)
+    args = dict(cap=256, repart_downtime_s=4, repart_energy_mj=0)
+    args.update(kw)
+    p = make_params(speeds, durs, w, jobs_per_day=jobs_per_day, amplitude=amplitude, configs=FIG1_CONFIGS + (NOMIG_CONFIG,), **args)
+    curve, p_idle, p_busy = default_power()
+    return dataclasses.replace(p, speed_nomig=speed_nomig_of(speeds), p_idle_nomig_mw=p_idle[4], p_busy_nomig_mw=p_busy[4],
+                               repart_all_down=1, gamma=0.99, util_hist=1)
+
+
+def day_night_table(n_envs: int) -> np.ndarray:
+    """PAPER.md:L230: "Configuration 6 for day-time, defined as 5:00-17:00, and Configuration 2 for night-time"."""
+    t = np.empty((24, 4), dtype=np.uint8)
+    for h in range(24):
+        t[h] = PAPER_DAY_CFG if 5 <= h < 17 else PAPER_NIGHT_CFG
+    return np.broadcast_to(t, (n_envs, 24, 4)).copy()
+
+
+def config_benchmark(kind: str, n_envs: int = 1024, algo: int = ALGO_EDF_SS_R, **kw) -> Workload:
+    """The paper's three benchmark policies (L230) on one parameter set: "nomig" (full GPU, MIG disabled), "static"
+    (configuration 3), "daynight" (configuration 6 from 5:00 to 17:00, configuration 2 otherwise).  The dynamic policy is
+    C4 (DQN) / the BINNED policy.  algo defaults to EDF-SS with restricted preemption, which the paper's repartitioning
+    experiments run on (L198-204)."""
+    p = benchmark_params(**kw)
+    a = np.full(n_envs, algo, np.uint8)
+    if kind == "nomig":
+        return Workload("nomig", p, n_envs, 11, a, np.full(n_envs, 12, np.uint8), POLICY_STATIC, mean_jobs_per_day=2000)
+    if kind == "static":
+        return Workload("static", p, n_envs, 11, a, np.full(n_envs, PAPER_STATIC_CFG, np.uint8), POLICY_STATIC, mean_jobs_per_day=2000)
+    if kind == "daynight":
+        return Workload("daynight", p, n_envs, 11, a, np.full(n_envs, PAPER_NIGHT_CFG, np.uint8), POLICY_TABLE,
+                        table=day_night_table(n_envs), mean_jobs_per_day=2000)
+    raise ValueError(kind)
+
+
+# The sweeps of Figs. 7-10 are parameter files: the arrival rates 0.1 / 0.5 / 0.75 of L240 relative to the default 0.5,
+# the 20 % / 80 % inference split of L242.
+SWEEP_RATE_SCALE = {"0.1": 0.2, "0.5": 1.0, "0.75": 1.5}
+SWEEP_INFERENCE = {"20": 0.2, "80": 0.8}
+
+
+def binned_defaults(p: SimParams) -> SimParams:
+    """Bin edges of the BINNED policy's state (PAPER.md:L210 gives none; reading #31): 24 hourly time bins,
+    deadline bins overdue | within 10 min | later, average-duration bins < 30 s | < 300 s | longer."""
+    return dataclasses.replace(p, n_tbins=24, dbin_edges=np.array([0, 600], dtype=np.int32), abin_edges=np.array([30, 300], dtype=np.int32))
+
+
 CONFIGS = {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4, "C5": config_c5}
 
 
