@@ -6,6 +6,7 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "mig_oracle.c")
+SRCS = [SRC, os.path.join(HERE, "dqn_oracle.c")]
 HDR = os.path.join(HERE, "mig_oracle.h")
 LIB = os.path.join(HERE, "libmigoracle.so")
 
@@ -15,10 +16,10 @@ CFLAGS = ["-O2", "-std=c99", "-fPIC", "-shared", "-Wall", "-Wextra", "-ffp-contr
 
 def build(force: bool = False) -> str:
     if (not force and os.path.exists(LIB)
-            and os.path.getmtime(LIB) >= max(os.path.getmtime(SRC), os.path.getmtime(HDR))):
+            and os.path.getmtime(LIB) >= max([os.path.getmtime(f) for f in SRCS] + [os.path.getmtime(HDR)])):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    subprocess.run(["gcc", *CFLAGS, SRC, "-o", tmp, "-lm"], check=True, cwd=HERE)
+    subprocess.run(["gcc", *CFLAGS, *SRCS, "-o", tmp, "-lm"], check=True, cwd=HERE)
     os.replace(tmp, LIB)
     return LIB
 

@@ -15,6 +15,7 @@
  */
 #ifndef MIG_ORACLE_H_
 #define MIG_ORACLE_H_
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -156,6 +157,23 @@ double orc_et_reduce(const double *x, const double *y, const uint32_t *group, ui
 void orc_q_eval(const orc_qnet_t *q, const float *state, uint32_t B, float *q_out, uint8_t *argmax_out);
 /* the same network in double precision with plain a*b+c (for the 1e-4 relative bound) */
 void orc_q_eval_f64(const orc_qnet_t *q, const float *state, uint32_t B, double *q_out);
+
+/* --- DQN training step (dqn_oracle.c; readings #33-#36), double precision ----------------- */
+typedef struct orc_dqn orc_dqn_t;
+size_t orc_dqn_n_params(uint32_t hidden, uint32_t n_actions);    /* flat order: W1 [64][H], b1, W2 [H][H], b2, W3 [H][A], b3 */
+orc_dqn_t *orc_dqn_create(const orc_qnet_t *init, double gamma, double lr);   /* online = target = init */
+void orc_dqn_destroy(orc_dqn_t *d);
+void orc_dqn_sync_target(orc_dqn_t *d);                           /* target <- online */
+void orc_dqn_get(const orc_dqn_t *d, int which, double *flat);    /* which: 0 online, 1 target */
+void orc_dqn_set(orc_dqn_t *d, int which, const double *flat);
+void orc_dqn_q(const orc_dqn_t *d, int which, const float *s, uint32_t B, double *q_out);
+/* L = 1/(2B) sum_b (Q(s_b, a_b) - (r_b + gamma (1 - done_b) max_a' Q_target(s'_b, a')))^2 and dL/d(online parameters) */
+double orc_dqn_loss_grad(const orc_dqn_t *d, const float *s, const uint8_t *a, const float *r, const float *s2,
+                         const uint8_t *done, uint32_t B, double *grad);
+double orc_dqn_train_step(orc_dqn_t *d, const float *s, const uint8_t *a, const float *r, const float *s2,
+                          const uint8_t *done, uint32_t B);       /* online -= lr * grad; returns the loss before the step */
+/* replay sampling: idx_b = (word 0 of Philox(counter (b, 3, step, 0), key seed) * size) >> 32 */
+void orc_replay_sample(uint64_t seed, uint32_t step, uint32_t size, uint32_t B, uint32_t *idx_out);
 
 #ifdef __cplusplus
 }

@@ -94,6 +94,20 @@ def lib():
         _lib.orc_env_util_hist.argtypes = [C.c_void_p, C.c_void_p]
         _lib.orc_et_reduce.restype = C.c_double
         _lib.orc_et_reduce.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p]
+        _lib.orc_dqn_n_params.restype = C.c_size_t
+        _lib.orc_dqn_n_params.argtypes = [C.c_uint32, C.c_uint32]
+        _lib.orc_dqn_create.restype = C.c_void_p
+        _lib.orc_dqn_create.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        _lib.orc_dqn_destroy.argtypes = [C.c_void_p]
+        _lib.orc_dqn_sync_target.argtypes = [C.c_void_p]
+        _lib.orc_dqn_get.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        _lib.orc_dqn_set.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        _lib.orc_dqn_q.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_uint32, C.c_void_p]
+        _lib.orc_dqn_loss_grad.restype = C.c_double
+        _lib.orc_dqn_loss_grad.argtypes = [C.c_void_p] * 6 + [C.c_uint32, C.c_void_p]
+        _lib.orc_dqn_train_step.restype = C.c_double
+        _lib.orc_dqn_train_step.argtypes = [C.c_void_p] * 6 + [C.c_uint32]
+        _lib.orc_replay_sample.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p]
         _lib.orc_q_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]
         _lib.orc_q_eval_f64.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
         _lib.orc_philox4x32_10.argtypes = [C.c_uint32] * 6 + [C.c_void_p]
@@ -306,3 +320,72 @@ def et_reduce(x, y, group, n_groups):
     et = np.zeros(n_groups, dtype=np.float64)
     a = lib().orc_et_reduce(_ptr(x), _ptr(y), _ptr(g), len(x), n_groups, _ptr(et))
     return et, float(a)
+
+
+class Dqn:
+    """The DQN training oracle (dqn_oracle.c): online + frozen target network in double precision, squared TD error, SGD."""
+
+    def __init__(self, qnet, gamma: float, lr: float):
+        qh = qnet if isinstance(qnet, QNetHolder) else QNetHolder(qnet)
+        self.H, self.A = int(qh.c.hidden), int(qh.c.n_actions)
+        self.n = int(lib().orc_dqn_n_params(self.H, self.A))
+        self.h = lib().orc_dqn_create(qh.ref, float(gamma), float(lr))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            lib().orc_dqn_destroy(self.h)
+            self.h = None
+
+    @staticmethod
+    def _batch(s, a, r, s2, done):
+        s = np.ascontiguousarray(s, dtype=np.float32).reshape(-1, STATE_DIM)
+        s2 = np.ascontiguousarray(s2, dtype=np.float32).reshape(-1, STATE_DIM)
+        a = np.ascontiguousarray(a, dtype=np.uint8); r = np.ascontiguousarray(r, dtype=np.float32)
+        done = np.zeros(len(a), np.uint8) if done is None else np.ascontiguousarray(done, dtype=np.uint8)
+        assert len(s) == len(s2) == len(a) == len(r) == len(done)
+        return s, a, r, s2, done
+
+    def params(self, which=0) -> np.ndarray:
+        out = np.zeros(self.n, dtype=np.float64)
+        lib().orc_dqn_get(self.h, which, _ptr(out))
+        return out
+
+    def set_params(self, flat, which=0):
+        f = np.ascontiguousarray(flat, dtype=np.float64)
+        assert f.size == self.n
+        lib().orc_dqn_set(self.h, which, _ptr(f))
+
+    def split(self, flat):
+        """flat -> (W1 [64][H], b1, W2 [H][H], b2, W3 [H][A], b3)"""
+        H, A = self.H, self.A
+        sz = [STATE_DIM * H, H, H * H, H, H * A, A]
+        sh = [(STATE_DIM, H), (H,), (H, H), (H,), (H, A), (A,)]
+        out, o = [], 0
+        for n, shp in zip(sz, sh):
+            out.append(np.asarray(flat[o:o + n]).reshape(shp)); o += n
+        return out
+
+    def q(self, s, which=0) -> np.ndarray:
+        s = np.ascontiguousarray(s, dtype=np.float32).reshape(-1, STATE_DIM)
+        out = np.zeros((len(s), self.A), dtype=np.float64)
+        lib().orc_dqn_q(self.h, which, _ptr(s), len(s), _ptr(out))
+        return out
+
+    def loss_grad(self, s, a, r, s2, done=None, want_grad=True):
+        s, a, r, s2, done = self._batch(s, a, r, s2, done)
+        g = np.zeros(self.n, dtype=np.float64) if want_grad else None
+        loss = lib().orc_dqn_loss_grad(self.h, _ptr(s), _ptr(a), _ptr(r), _ptr(s2), _ptr(done), len(a), _ptr(g))
+        return float(loss), g
+
+    def train_step(self, s, a, r, s2, done=None) -> float:
+        s, a, r, s2, done = self._batch(s, a, r, s2, done)
+        return float(lib().orc_dqn_train_step(self.h, _ptr(s), _ptr(a), _ptr(r), _ptr(s2), _ptr(done), len(a)))
+
+    def sync_target(self):
+        lib().orc_dqn_sync_target(self.h)
+
+
+def replay_sample(seed: int, step: int, size: int, B: int) -> np.ndarray:
+    idx = np.zeros(B, dtype=np.uint32)
+    lib().orc_replay_sample(seed, step, size, B, _ptr(idx))
+    return idx
