@@ -225,6 +225,46 @@ int mig_qnet_destroy(mig_qnet_t *q);
 /* state dev[B][64] -> q_out dev[B][n_actions] (or NULL), argmax_out dev[B] u8 lowest index on ties (or NULL). */
 int mig_q_eval(const mig_qnet_t *q, const float *state, uint32_t B, float *q_out, uint8_t *argmax_out, void *stream);
 
+/* ---- DQN training ("Deep Q-Learning, incorporating an epsilon-greedy exploration-exploitation
+ * strategy and an experience replay buffer [21]", L214 "discounted rewards"; the paper gives no loss, optimiser or
+ * hyper-parameter: DESIGN.md readings #33-#36).  One handle = the online network, a frozen target network (both start as
+ * the given weights), a replay ring of `replay_capacity` transitions (s[64], a, r, s'[64], done) in device memory, and the
+ * buffers of one training batch.  One training step on a batch of `batch` transitions:
+ *     y_b = r_b + gamma (1 - done_b) max_a' Q_target(s'_b, a');   L = 1/(2 batch) sum_b (Q(s_b, a_b) - y_b)^2;
+ *     theta <- theta - lr dL/dtheta            (plain squared TD error, plain SGD; the target network is not touched)
+ * All matrix products (forward of both networks, backward through the activations, weight gradients) run on the tensor
+ * cores as 3 x TF32 (hi/lo split of both operands, fp32 accumulation in TMEM): fp32-accurate, NOT bit-reproducible
+ * against a CPU.  This is the training path; the forward that DRIVES a simulated trace stays mig_q_eval (fixed-order FFMA).
+ * Tolerance against a double-precision evaluation of the same step: 1e-4 relative (tests/test_gpu_dqn.py).
+ * hidden: 128 or 256; n_actions <= 16; batch: a multiple of 128.  Host weight arrays as in mig_qnet_create, copied. */
+typedef struct mig_dqn mig_dqn_t;
+int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1, const float *W2, const float *b2, const float *W3,
+                   const float *b3, uint32_t hidden, uint32_t n_actions, uint32_t replay_capacity, uint32_t batch,
+                   float gamma, float lr, uint64_t seed);
+int mig_dqn_destroy(mig_dqn_t *d);
+/* Appends n transitions (dev arrays: s, s2 [n][64] fp32, a [n] u8, r [n] fp32, done [n] u8 or NULL = all 0) to the ring:
+ * transition i lands in slot (head + i) mod capacity; when the ring is full the oldest are overwritten.  Typically fed
+ * straight from mig_sim_step's state_out / reward_out and the actions given to it.  Asynchronous on `stream`. */
+int mig_replay_push(mig_dqn_t *d, const float *s, const uint8_t *a, const float *r, const float *s2, const uint8_t *done,
+                    uint32_t n, void *stream);
+uint32_t mig_replay_size(const mig_dqn_t *d);
+/* One training step on `batch` transitions sampled uniformly with replacement from the ring: index_b = (w * size) >> 32
+ * with w = word 0 of Philox4x32-10(counter (b, 3, step, 0), key = seed) ("stream 3", reading #36).  loss_out: dev[1], the
+ * loss before the step, or NULL.  MIG_ESTATE if the ring is empty.  Asynchronous on `stream`. */
+int mig_dqn_train_step(mig_dqn_t *d, uint32_t step, float *loss_out, void *stream);
+/* The same on an explicit batch: dev arrays of exactly `batch` rows (done may be NULL). */
+int mig_dqn_train_on(mig_dqn_t *d, const float *s, const uint8_t *a, const float *r, const float *s2, const uint8_t *done,
+                     float *loss_out, void *stream);
+/* target <- online (device to device, asynchronous). */
+int mig_dqn_sync_target(mig_dqn_t *d, void *stream);
+/* Q-values of the online (which = 0) or target (1) network through the tensor-core path: state dev[n][64], n <= batch,
+ * q_out dev[n][n_actions].  Within 1e-4 relative of mig_q_eval's. */
+int mig_dqn_q(mig_dqn_t *d, int which, const float *state, uint32_t n, float *q_out, void *stream);
+/* Copies the weights of the online (0) or target (1) network to HOST arrays shaped as in mig_qnet_create; synchronises. */
+int mig_dqn_get_weights(mig_dqn_t *d, int which, float *W1, float *b1, float *W2, float *b2, float *W3, float *b3);
+/* Kernel launches issued through this handle so far. */
+uint64_t mig_dqn_launch_count(const mig_dqn_t *d);
+
 /* Debug / parity: re-runs ONE env for a whole day from the last reset's (episode, algo, cfg0), recording every event.
  * policy STATIC, TABLE or BINNED (table as in rollout), or actions != NULL: dev[n_epochs] explicit action sequence.
  * buf dev[cap_events]; n_out dev[1] = number of events emitted (may exceed cap_events; only the first are stored);

@@ -8,7 +8,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmigsim.so")
-SOURCES = ["migsim.cu"]
+SOURCES = ["migsim.cu", "dqn.cu"]
 
 
 def _deps() -> list[str]:

@@ -35,7 +35,9 @@ EXPORTS = (
     "mig_sim_rollout", "mig_sim_totals", "mig_sim_rollout_host", "mig_qnet_create", "mig_qnet_destroy", "mig_q_eval",
     "mig_sim_debug_trace", "mig_sim_debug_set_jobs", "mig_debug_div_magic", "mig_sim_launch_count", "mig_sim_set_tile",
     "mig_sim_get_tile", "mig_sim_set_arrival_buffer", "mig_sim_get_arrival_buffer", "mig_sim_set_envs_per_warp",
-    "mig_sim_kernel_name", "mig_sim_set_profiling", "mig_sim_kernel_times", "mig_sim_aux", "mig_et_reduce")
+    "mig_sim_kernel_name", "mig_sim_set_profiling", "mig_sim_kernel_times", "mig_sim_aux", "mig_et_reduce",
+    "mig_dqn_create", "mig_dqn_destroy", "mig_replay_push", "mig_replay_size", "mig_dqn_train_step", "mig_dqn_train_on",
+    "mig_dqn_sync_target", "mig_dqn_q", "mig_dqn_get_weights", "mig_dqn_launch_count")
 
 
 class MigError(RuntimeError):
@@ -102,6 +104,18 @@ def lib():
         L.mig_sim_get_arrival_buffer.restype = C.c_uint32
         L.mig_sim_aux.argtypes = [vp, vp, vp, vp]
         L.mig_et_reduce.argtypes = [vp, vp, vp, u32, u32, vp, vp]
+        L.mig_dqn_create.argtypes = [C.POINTER(vp), vp, vp, vp, vp, vp, vp, u32, u32, u32, u32, f32, f32, u64]
+        L.mig_dqn_destroy.argtypes = [vp]
+        L.mig_replay_push.argtypes = [vp, vp, vp, vp, vp, vp, u32, vp]
+        L.mig_replay_size.argtypes = [vp]
+        L.mig_replay_size.restype = u32
+        L.mig_dqn_train_step.argtypes = [vp, u32, vp, vp]
+        L.mig_dqn_train_on.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+        L.mig_dqn_sync_target.argtypes = [vp, vp]
+        L.mig_dqn_q.argtypes = [vp, i32, vp, u32, vp, vp]
+        L.mig_dqn_get_weights.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
+        L.mig_dqn_launch_count.argtypes = [vp]
+        L.mig_dqn_launch_count.restype = u64
         _lib = L
     return _lib
 
@@ -189,6 +203,61 @@ class QNet:
         self.h = None
 
     __del__ = close
+
+
+class Dqn:
+    """mig_dqn_* / mig_replay_*: DQN training on the tensor cores (online + frozen target network, replay ring on the device)."""
+
+    def __init__(self, qw: QNetWeights, replay_capacity: int, batch: int, gamma: float, lr: float, seed: int):
+        if not torch.cuda.is_available():
+            raise MigError(MIG_ECUDA, "no CUDA device: the training step has no CPU fallback")
+        arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in (qw.W1, qw.b1, qw.W2, qw.b2, qw.W3, qw.b3)]
+        self.hidden, self.n_actions, self.batch = int(arrs[0].shape[1]), int(arrs[4].shape[1]), int(batch)
+        self.h = C.c_void_p()
+        _check(lib().mig_dqn_create(C.byref(self.h), *[_hp(a) for a in arrs], self.hidden, self.n_actions, int(replay_capacity),
+                                    self.batch, float(gamma), float(lr), int(seed)))
+
+    def close(self):
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.mig_dqn_destroy(self.h)
+        self.h = None
+
+    __del__ = close
+
+    def push(self, s, a, r, s2, done=None, stream=None):
+        n = a.numel()
+        _check(lib().mig_replay_push(self.h, _dp(s, torch.float32, n * STATE_DIM * 4), _dp(a, torch.uint8, n), _dp(r, torch.float32, n * 4),
+                                     _dp(s2, torch.float32, n * STATE_DIM * 4), _dp(done, torch.uint8, n), n, _stream(stream)))
+
+    def replay_size(self) -> int:
+        return int(lib().mig_replay_size(self.h))
+
+    def train_step(self, step: int, loss_out=None, stream=None):
+        _check(lib().mig_dqn_train_step(self.h, int(step), _dp(loss_out, torch.float32, 4), _stream(stream)))
+
+    def train_on(self, s, a, r, s2, done=None, loss_out=None, stream=None):
+        B = self.batch
+        _check(lib().mig_dqn_train_on(self.h, _dp(s, torch.float32, B * STATE_DIM * 4), _dp(a, torch.uint8, B), _dp(r, torch.float32, B * 4),
+                                      _dp(s2, torch.float32, B * STATE_DIM * 4), _dp(done, torch.uint8, B), _dp(loss_out, torch.float32, 4),
+                                      _stream(stream)))
+
+    def sync_target(self, stream=None):
+        _check(lib().mig_dqn_sync_target(self.h, _stream(stream)))
+
+    def q(self, state: torch.Tensor, which: int = 0, q_out=None, stream=None):
+        n = state.numel() // STATE_DIM
+        q_out = torch.empty((n, self.n_actions), dtype=torch.float32, device="cuda") if q_out is None else q_out
+        _check(lib().mig_dqn_q(self.h, int(which), _dp(state, torch.float32), n, _dp(q_out, torch.float32, n * self.n_actions * 4), _stream(stream)))
+        return q_out
+
+    def weights(self, which: int = 0) -> QNetWeights:
+        H, A = self.hidden, self.n_actions
+        arrs = [np.zeros(sh, dtype=np.float32) for sh in ((STATE_DIM, H), (H,), (H, H), (H,), (H, A), (A,))]
+        _check(lib().mig_dqn_get_weights(self.h, int(which), *[_hp(a) for a in arrs]))
+        return QNetWeights(*arrs)
+
+    def launch_count(self) -> int:
+        return int(lib().mig_dqn_launch_count(self.h))
 
 
 # lanes per environment passed to mig_sim_set_tile by MigSim() when its `tile` argument is 0 (0 = the library's choice)

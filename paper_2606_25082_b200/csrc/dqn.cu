@@ -1,0 +1,313 @@
+// dqn.cu -- host side of the DQN training step of libmigsim.so (include/migsim.h: mig_dqn_*, mig_replay_*): replay buffer in
+// device memory, one training step = sample -> forward (online on s, frozen target on s') -> TD error -> backward -> SGD.
+// Every matrix product runs on the tensor cores through gemm_tf32x3_kernel (dqn_gemm.cuh: tcgen05.mma kind::tf32, TMA,
+// TMEM accumulators); the rest is the handful of small kernels in dqn_train.cuh.  PAPER.md:L208, L214; #33-#36.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "dqn_gemm.cuh"
+#include "dqn_train.cuh"
+#include "sim_common.h"
+
+using namespace migsim;
+
+#define CUD(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return mig_fail(MIG_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); } while (0)
+
+namespace {
+
+struct Net {            // one network: master weights in the caller's layout [in][out] + the transposed copies the products read
+  float *W1, *W1t, *b1, *W2, *W2t, *b2, *W3, *W3t, *b3;      // W1 [64][H], W1t [H][64], W2 [H][H], W2t [H][H], W3 [H][16], W3t [16][H]
+};
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void *p = nullptr; cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+// K-major operand [rows][inner] fp32 with leading dimension ld (elements): boxes of 32 floats (one 128-byte swizzled row) x box_rows
+int make_map(CUtensorMap *m, const float *ptr, uint64_t inner, uint64_t rows, uint64_t ld, uint32_t box_rows) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return mig_fail(MIG_ECUDA, "dqn: cuTensorMapEncodeTiled is not available from this driver");
+  cuuint64_t dims[2] = {inner, rows}, strides[1] = {ld * sizeof(float)};
+  cuuint32_t box[2] = {(cuuint32_t)kGemmBK, box_rows}, es[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float *>(ptr), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return mig_fail(MIG_ECUDA, "dqn: cuTensorMapEncodeTiled failed (%d) for a [%llu][%llu] operand", (int)r, (unsigned long long)rows, (unsigned long long)inner);
+  return MIG_OK;
+}
+
+}  // namespace
+
+struct mig_dqn {   // (mig_dqn_t of include/migsim.h)
+  uint32_t H = 0, A = 0, B = 0, cap = 0, splits = 1;
+  float gamma = 0.0f, lr = 0.0f; uint64_t seed = 0;
+  int device = 0;
+  uint64_t launches = 0, gemm_launches = 0;
+  std::vector<void *> allocs;
+  Net net[2];                                              // [0] online, [1] target
+  // replay ring
+  float *rS = nullptr, *rS2 = nullptr, *rR = nullptr; uint8_t *rA = nullptr, *rD = nullptr;
+  uint32_t head = 0, size = 0;
+  // batch and activations
+  float *X, *X2, *Xt, *H1, *H1t, *H2, *H2t, *Q, *T1, *T2, *Qt, *dQ, *dQt, *dZ2, *dZ2t, *dZ1t, *r, *lossrow, *pW1, *pW2, *pW3, *loss;
+  uint8_t *a, *done;
+  // tensor maps: A operands and B operands of the twelve products
+  CUtensorMap mX, mH1, mH2, mX2, mT1, mT2, mdQ, mdZ2, mH2t, mH1t, mXt;                          // A side (box 128 rows)
+  CUtensorMap mW1t[2], mW2t[2], mW3t[2], mW3, mW2, mdQt, mdZ2t, mdZ1t;                          // B side
+};
+
+static int dalloc(mig_dqn *d, void **p, size_t bytes) {
+  if (cudaMalloc(p, bytes) != cudaSuccess) { cudaGetLastError(); return mig_fail(MIG_ENOMEM, "dqn: cudaMalloc of %zu bytes failed", bytes); }
+  d->allocs.push_back(*p);
+  return cudaMemset(*p, 0, bytes) == cudaSuccess ? MIG_OK : mig_fail(MIG_ECUDA, "dqn: cudaMemset failed");
+}
+#define DA(ptr, count) do { int rc_ = dalloc(d, (void **)&(ptr), (size_t)(count) * sizeof(*(ptr))); if (rc_) { mig_dqn_destroy(d); return rc_; } } while (0)
+
+template <int BN>
+static int launch_gemm(mig_dqn *d, const CUtensorMap &ma, const CUtensorMap &mb, const GemmArgs &g, uint32_t splits, cudaStream_t st) {
+  static bool attr_done[8] = {false, false, false, false, false, false, false, false};
+  if (d->device >= 0 && d->device < 8 && !attr_done[d->device]) {
+    CUD(cudaFuncSetAttribute(gemm_tf32x3_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<BN>::kBytes));
+    attr_done[d->device] = true;
+  }
+  dim3 grid((g.M + kGemmBM - 1) / kGemmBM, g.N / BN, splits);
+  gemm_tf32x3_kernel<BN><<<grid, kGemmThreads, GemmSmem<BN>::kBytes, st>>>(ma, mb, g);
+  CUD(cudaGetLastError());
+  d->launches++; d->gemm_launches++;
+  return MIG_OK;
+}
+
+static GemmArgs gargs(uint32_t M, uint32_t N, uint32_t K) {
+  GemmArgs g; memset(&g, 0, sizeof(g));
+  g.M = M; g.N = N; g.K = K; g.k_blocks = (K + kGemmBK - 1) / kGemmBK;
+  return g;
+}
+
+extern "C" int mig_dqn_destroy(mig_dqn_t *d) {
+  if (!d) return MIG_OK;
+  cudaDeviceSynchronize();
+  for (void *p : d->allocs) cudaFree(p);
+  cudaGetLastError();
+  delete d;
+  return MIG_OK;
+}
+
+extern "C" int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1, const float *W2, const float *b2, const float *W3,
+                              const float *b3, uint32_t hidden, uint32_t n_actions, uint32_t replay_capacity, uint32_t batch,
+                              float gamma, float lr, uint64_t seed) {
+  if (!out || !W1 || !b1 || !W2 || !b2 || !W3 || !b3) return mig_fail(MIG_EINVAL, "dqn_create: NULL argument");
+  *out = nullptr;
+  if (hidden != 128 && hidden != 256) return mig_fail(MIG_EINVAL, "dqn_create: hidden %u must be 128 or 256 (tiles of 128 output columns)", hidden);
+  if (n_actions < 1 || n_actions > MIG_MAX_CONFIGS) return mig_fail(MIG_EINVAL, "dqn_create: n_actions %u not in 1..16", n_actions);
+  if (batch < 128 || batch % 128 || batch > (1u << 20)) return mig_fail(MIG_EINVAL, "dqn_create: batch %u must be a multiple of 128 in 128..2^20", batch);
+  if (replay_capacity < 1 || replay_capacity > (1u << 26)) return mig_fail(MIG_EINVAL, "dqn_create: replay_capacity %u not in 1..2^26", replay_capacity);
+  if (!(gamma >= 0.0f) || gamma > 1.0f || !(lr >= 0.0f)) return mig_fail(MIG_EINVAL, "dqn_create: gamma must be in [0, 1], lr >= 0");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return mig_fail(MIG_ECUDA, "dqn_create: no CUDA device; there is no CPU fallback"); }
+  mig_dqn *d = new (std::nothrow) mig_dqn();
+  if (!d) return mig_fail(MIG_ENOMEM, "dqn_create: host allocation failed");
+  cudaGetDevice(&d->device);
+  const uint32_t H = hidden, A = n_actions, B = batch, P = kDqnApad;
+  d->H = H; d->A = A; d->B = B; d->cap = replay_capacity; d->gamma = gamma; d->lr = lr; d->seed = seed;
+  d->splits = B / 128 < 32 ? B / 128 : 32;                  // split-K of the weight-gradient products: >= 4 k-blocks per split
+  while ((B / kGemmBK) % d->splits) d->splits--;
+  for (int k = 0; k < 2; ++k) {
+    Net &n = d->net[k];
+    DA(n.W1, 64 * H); DA(n.W1t, H * 64); DA(n.b1, H); DA(n.W2, H * H); DA(n.W2t, H * H); DA(n.b2, H); DA(n.W3, H * P); DA(n.W3t, P * H); DA(n.b3, P);
+  }
+  DA(d->rS, (size_t)d->cap * 64); DA(d->rS2, (size_t)d->cap * 64); DA(d->rR, d->cap); DA(d->rA, d->cap); DA(d->rD, d->cap);
+  DA(d->X, (size_t)B * 64); DA(d->X2, (size_t)B * 64); DA(d->Xt, (size_t)64 * B);
+  DA(d->H1, (size_t)B * H); DA(d->H1t, (size_t)H * B); DA(d->H2, (size_t)B * H); DA(d->H2t, (size_t)H * B); DA(d->Q, (size_t)B * P);
+  DA(d->T1, (size_t)B * H); DA(d->T2, (size_t)B * H); DA(d->Qt, (size_t)B * P);
+  DA(d->dQ, (size_t)B * P); DA(d->dQt, (size_t)P * B); DA(d->dZ2, (size_t)B * H); DA(d->dZ2t, (size_t)H * B); DA(d->dZ1t, (size_t)H * B);
+  DA(d->r, B); DA(d->a, B); DA(d->done, B); DA(d->lossrow, B); DA(d->loss, 1);
+  DA(d->pW1, (size_t)d->splits * 64 * H); DA(d->pW2, (size_t)d->splits * H * H); DA(d->pW3, (size_t)d->splits * H * P);
+  // weights: master copies, padded action columns are zero; the transposed copies follow
+  auto up = [&](float *dst, const float *src, size_t rows, size_t cols, size_t ld) {
+    return cudaMemcpy2D(dst, ld * sizeof(float), src, cols * sizeof(float), cols * sizeof(float), rows, cudaMemcpyHostToDevice) == cudaSuccess;
+  };
+  bool ok = true;
+  for (int k = 0; k < 2 && ok; ++k) {
+    Net &n = d->net[k];
+    ok = up(n.W1, W1, 64, H, H) && up(n.b1, b1, 1, H, H) && up(n.W2, W2, H, H, H) && up(n.b2, b2, 1, H, H) && up(n.W3, W3, H, A, P) && up(n.b3, b3, 1, A, P);
+    if (!ok) break;
+    dqn_transpose_kernel<<<(64 * H + 255) / 256, 256>>>(n.W1, n.W1t, 64, H, H, 64);
+    dqn_transpose_kernel<<<(H * H + 255) / 256, 256>>>(n.W2, n.W2t, H, H, H, H);
+    dqn_transpose_kernel<<<(H * P + 255) / 256, 256>>>(n.W3, n.W3t, H, P, P, H);
+  }
+  if (!ok || cudaDeviceSynchronize() != cudaSuccess) { mig_dqn_destroy(d); return mig_fail(MIG_ECUDA, "dqn_create: weight upload failed: %s", cudaGetErrorString(cudaGetLastError())); }
+  int rc = MIG_OK;
+#define MAP(m, ptr, inner, rows, ld, box) if (!rc) rc = make_map(&d->m, ptr, inner, rows, ld, box)
+  MAP(mX, d->X, 64, B, 64, 128); MAP(mH1, d->H1, H, B, H, 128); MAP(mH2, d->H2, H, B, H, 128);
+  MAP(mX2, d->X2, 64, B, 64, 128); MAP(mT1, d->T1, H, B, H, 128); MAP(mT2, d->T2, H, B, H, 128);
+  MAP(mdQ, d->dQ, P, B, P, 128); MAP(mdZ2, d->dZ2, H, B, H, 128);
+  MAP(mH2t, d->H2t, B, H, B, 128); MAP(mH1t, d->H1t, B, H, B, 128); MAP(mXt, d->Xt, B, 64, B, 128);
+  for (int k = 0; k < 2; ++k) { MAP(mW1t[k], d->net[k].W1t, 64, H, 64, 128); MAP(mW2t[k], d->net[k].W2t, H, H, H, 128); MAP(mW3t[k], d->net[k].W3t, H, P, H, P); }
+  MAP(mW3, d->net[0].W3, P, H, P, 128); MAP(mW2, d->net[0].W2, H, H, H, 128);
+  MAP(mdQt, d->dQt, B, P, B, P); MAP(mdZ2t, d->dZ2t, B, H, B, 128); MAP(mdZ1t, d->dZ1t, B, H, B, 128);
+#undef MAP
+  if (rc) { mig_dqn_destroy(d); return rc; }
+  *out = d;
+  return MIG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ forward
+// h1 = relu(b1 + x W1), h2 = relu(b2 + h1 W2), q = b3 + h2 W3 for the B rows of X (online: which = 0, into H1 / H2 / Q with
+// the transposed copies the backward pass needs) or of X2 (target: which = 1, into T1 / T2 / Qt)
+static int forward(mig_dqn *d, int which, cudaStream_t st) {
+  const uint32_t H = d->H, B = d->B, P = kDqnApad;
+  const Net &n = d->net[which];
+  int rc;
+  GemmArgs g = gargs(B, H, 64);
+  g.epi = EPI_BIAS | EPI_RELU; g.bias = n.b1; g.out = which ? d->T1 : d->H1; g.ldo = H;
+  if (!which) { g.out_t = d->H1t; g.ldt = B; }
+  if ((rc = launch_gemm<128>(d, which ? d->mX2 : d->mX, d->mW1t[which], g, 1, st))) return rc;
+  g = gargs(B, H, H);
+  g.epi = EPI_BIAS | EPI_RELU; g.bias = n.b2; g.out = which ? d->T2 : d->H2; g.ldo = H;
+  if (!which) { g.out_t = d->H2t; g.ldt = B; }
+  if ((rc = launch_gemm<128>(d, which ? d->mT1 : d->mH1, d->mW2t[which], g, 1, st))) return rc;
+  g = gargs(B, P, H);
+  g.epi = EPI_BIAS; g.bias = n.b3; g.out = which ? d->Qt : d->Q; g.ldo = P;
+  return launch_gemm<kDqnApad>(d, which ? d->mT2 : d->mH2, d->mW3t[which], g, 1, st);
+}
+
+extern "C" int mig_dqn_q(mig_dqn_t *d, int which, const float *state, uint32_t n, float *q_out, void *stream) {
+  if (!d || !state || !q_out) return mig_fail(MIG_EINVAL, "dqn_q: NULL argument");
+  if (n < 1 || n > d->B) return mig_fail(MIG_EINVAL, "dqn_q: n = %u not in 1..batch (%u)", n, d->B);
+  cudaStream_t st = (cudaStream_t)stream;
+  float *X = which ? d->X2 : d->X;
+  CUD(cudaMemcpyAsync(X, state, (size_t)n * MIG_STATE_DIM * sizeof(float), cudaMemcpyDeviceToDevice, st));
+  if (n < d->B) CUD(cudaMemsetAsync(X + (size_t)n * MIG_STATE_DIM, 0, (size_t)(d->B - n) * MIG_STATE_DIM * sizeof(float), st));
+  int rc = forward(d, which ? 1 : 0, st);
+  if (rc) return rc;
+  CUD(cudaMemcpy2DAsync(q_out, d->A * sizeof(float), which ? d->Qt : d->Q, kDqnApad * sizeof(float), d->A * sizeof(float), n, cudaMemcpyDeviceToDevice, st));
+  return MIG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ one training step
+static int train_on_batch(mig_dqn *d, float *loss_out, cudaStream_t st) {
+  const uint32_t H = d->H, B = d->B, P = kDqnApad, S = d->splits;
+  int rc;
+  if ((rc = forward(d, 0, st)) || (rc = forward(d, 1, st))) return rc;
+  dqn_td_kernel<<<(B + 255) / 256, 256, 0, st>>>(d->Q, d->Qt, d->a, d->r, d->done, B, d->A, d->gamma, d->dQ, d->dQt, d->lossrow);
+  CUD(cudaGetLastError()); d->launches++;
+  // backward through the activations: dZ2 = (dQ W3^T) . [H2 > 0], dZ1 = (dZ2 W2^T) . [H1 > 0]
+  GemmArgs g = gargs(B, H, P);
+  g.epi = EPI_MASK; g.mask = d->H2; g.ldm = H; g.out = d->dZ2; g.ldo = H; g.out_t = d->dZ2t; g.ldt = B;
+  if ((rc = launch_gemm<128>(d, d->mdQ, d->mW3, g, 1, st))) return rc;
+  g = gargs(B, H, H);
+  g.epi = EPI_MASK; g.mask = d->H1; g.ldm = H; g.out_t = d->dZ1t; g.ldt = B;
+  if ((rc = launch_gemm<128>(d, d->mdZ2, d->mW2, g, 1, st))) return rc;
+  // weight gradients, split over the batch dimension: dW3 = H2^T dQ, dW2 = H1^T dZ2, dW1 = X^T dZ1
+  const uint32_t kps = B / S;                                  // batch rows per split
+  g = gargs(H, P, kps); g.out = d->pW3; g.ldo = P; g.out_split_stride = (size_t)H * P;
+  if ((rc = launch_gemm<kDqnApad>(d, d->mH2t, d->mdQt, g, S, st))) return rc;
+  g = gargs(H, H, kps); g.out = d->pW2; g.ldo = H; g.out_split_stride = (size_t)H * H;
+  if ((rc = launch_gemm<128>(d, d->mH1t, d->mdZ2t, g, S, st))) return rc;
+  g = gargs(64, H, kps); g.out = d->pW1; g.ldo = H; g.out_split_stride = (size_t)64 * H;
+  if ((rc = launch_gemm<128>(d, d->mXt, d->mdZ1t, g, S, st))) return rc;
+  // SGD on the online network (the transposed copies follow), bias gradients = row sums of the transposed dZ, the loss
+  Net &n = d->net[0];
+  UpdateArgs u; memset(&u, 0, sizeof(u));
+  u.lr = d->lr; u.B = B; u.n_splits = S;
+  u.W = n.W3; u.Wt = n.W3t; u.rows = H; u.cols = P; u.ldw = P; u.ldt = H; u.partial = d->pW3; u.split_stride = (size_t)H * P; u.ldp = P;
+  u.bias = n.b3; u.dZt = d->dQt; u.n_bias = P; u.lossrow = d->lossrow; u.loss_out = loss_out ? loss_out : d->loss;
+  dqn_update_kernel<<<u.rows + u.n_bias + 1, 256, 0, st>>>(u);
+  u.loss_out = nullptr; u.lossrow = nullptr;
+  u.W = n.W2; u.Wt = n.W2t; u.rows = H; u.cols = H; u.ldw = H; u.ldt = H; u.partial = d->pW2; u.split_stride = (size_t)H * H; u.ldp = H;
+  u.bias = n.b2; u.dZt = d->dZ2t; u.n_bias = H;
+  dqn_update_kernel<<<u.rows + u.n_bias, 256, 0, st>>>(u);
+  u.W = n.W1; u.Wt = n.W1t; u.rows = 64; u.cols = H; u.ldw = H; u.ldt = 64; u.partial = d->pW1; u.split_stride = (size_t)64 * H; u.ldp = H;
+  u.bias = n.b1; u.dZt = d->dZ1t; u.n_bias = H;
+  dqn_update_kernel<<<u.rows + u.n_bias, 256, 0, st>>>(u);
+  CUD(cudaGetLastError()); d->launches += 3;
+  return MIG_OK;
+}
+
+static int gather(mig_dqn *d, const float *S, const uint8_t *A, const float *R, const float *S2, const uint8_t *D, uint32_t size, uint32_t step,
+                  int identity, cudaStream_t st) {
+  GatherArgs g; memset(&g, 0, sizeof(g));
+  g.S = S; g.S2 = S2; g.A = A; g.R = R; g.D = D; g.X = d->X; g.X2 = d->X2; g.Xt = d->Xt; g.a = d->a; g.r = d->r; g.done = d->done;
+  g.B = d->B; g.size = size; g.step = step; g.k0 = (uint32_t)d->seed; g.k1 = (uint32_t)(d->seed >> 32); g.identity = identity;
+  dqn_gather_kernel<<<(d->B + 31) / 32, 256, 0, st>>>(g);
+  CUD(cudaGetLastError()); d->launches++;
+  return MIG_OK;
+}
+
+extern "C" int mig_dqn_train_step(mig_dqn_t *d, uint32_t step, float *loss_out, void *stream) {
+  if (!d) return mig_fail(MIG_EINVAL, "dqn_train_step: NULL handle");
+  if (d->size == 0) return mig_fail(MIG_ESTATE, "dqn_train_step: the replay buffer is empty");
+  int rc = gather(d, d->rS, d->rA, d->rR, d->rS2, d->rD, d->size, step, 0, (cudaStream_t)stream);
+  return rc ? rc : train_on_batch(d, loss_out, (cudaStream_t)stream);
+}
+
+extern "C" int mig_dqn_train_on(mig_dqn_t *d, const float *s, const uint8_t *a, const float *r, const float *s2, const uint8_t *done,
+                                float *loss_out, void *stream) {
+  if (!d || !s || !a || !r || !s2) return mig_fail(MIG_EINVAL, "dqn_train_on: NULL argument");
+  int rc = gather(d, s, a, r, s2, done, d->B, 0, 1, (cudaStream_t)stream);
+  return rc ? rc : train_on_batch(d, loss_out, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------------------------------------ replay buffer, target, weights
+extern "C" int mig_replay_push(mig_dqn_t *d, const float *s, const uint8_t *a, const float *r, const float *s2, const uint8_t *done,
+                               uint32_t n, void *stream) {
+  if (!d || !s || !a || !r || !s2) return mig_fail(MIG_EINVAL, "replay_push: NULL argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  uint32_t off = 0;
+  if (n > d->cap) { off = n - d->cap; n = d->cap; d->head = (uint32_t)(((uint64_t)d->head + off) % d->cap); }   // only the last cap transitions survive
+  while (n) {                                                // transition i lands in slot (head + i) mod capacity
+    const uint32_t run = n < d->cap - d->head ? n : d->cap - d->head, h = d->head;
+    CUD(cudaMemcpyAsync(d->rS + (size_t)h * 64, s + (size_t)off * 64, (size_t)run * 64 * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    CUD(cudaMemcpyAsync(d->rS2 + (size_t)h * 64, s2 + (size_t)off * 64, (size_t)run * 64 * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    CUD(cudaMemcpyAsync(d->rR + h, r + off, (size_t)run * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    CUD(cudaMemcpyAsync(d->rA + h, a + off, run, cudaMemcpyDeviceToDevice, st));
+    if (done) CUD(cudaMemcpyAsync(d->rD + h, done + off, run, cudaMemcpyDeviceToDevice, st));
+    else CUD(cudaMemsetAsync(d->rD + h, 0, run, st));
+    d->head = (h + run) % d->cap; d->size = d->size + run > d->cap ? d->cap : d->size + run;
+    off += run; n -= run;
+  }
+  return MIG_OK;
+}
+
+extern "C" uint32_t mig_replay_size(const mig_dqn_t *d) { return d ? d->size : 0; }
+extern "C" uint64_t mig_dqn_launch_count(const mig_dqn_t *d) { return d ? d->launches : 0; }
+
+extern "C" int mig_dqn_sync_target(mig_dqn_t *d, void *stream) {
+  if (!d) return mig_fail(MIG_EINVAL, "dqn_sync_target: NULL handle");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t H = d->H, P = kDqnApad;
+  const Net &o = d->net[0]; Net &t = d->net[1];
+  const struct { float *dst; const float *src; size_t n; } cp[9] = {
+      {t.W1, o.W1, 64 * H}, {t.W1t, o.W1t, H * 64}, {t.b1, o.b1, H}, {t.W2, o.W2, H * H}, {t.W2t, o.W2t, H * H}, {t.b2, o.b2, H},
+      {t.W3, o.W3, H * P}, {t.W3t, o.W3t, P * H}, {t.b3, o.b3, P}};
+  for (const auto &c : cp) CUD(cudaMemcpyAsync(c.dst, c.src, c.n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+  return MIG_OK;
+}
+
+extern "C" int mig_dqn_get_weights(mig_dqn_t *d, int which, float *W1, float *b1, float *W2, float *b2, float *W3, float *b3) {
+  if (!d || !W1 || !b1 || !W2 || !b2 || !W3 || !b3) return mig_fail(MIG_EINVAL, "dqn_get_weights: NULL argument");
+  CUD(cudaDeviceSynchronize());
+  const Net &n = d->net[which ? 1 : 0];
+  const size_t H = d->H, A = d->A, P = kDqnApad;
+  CUD(cudaMemcpy(W1, n.W1, 64 * H * sizeof(float), cudaMemcpyDeviceToHost));
+  CUD(cudaMemcpy(b1, n.b1, H * sizeof(float), cudaMemcpyDeviceToHost));
+  CUD(cudaMemcpy(W2, n.W2, H * H * sizeof(float), cudaMemcpyDeviceToHost));
+  CUD(cudaMemcpy(b2, n.b2, H * sizeof(float), cudaMemcpyDeviceToHost));
+  CUD(cudaMemcpy2D(W3, A * sizeof(float), n.W3, P * sizeof(float), A * sizeof(float), H, cudaMemcpyDeviceToHost));
+  CUD(cudaMemcpy(b3, n.b3, A * sizeof(float), cudaMemcpyDeviceToHost));
+  return MIG_OK;
+}

@@ -1,0 +1,142 @@
+// dqn_train.cuh -- the small kernels around the tensor-core products of the DQN training step (dqn_gemm.cuh): replay
+// sampling + gather (+ the transposed copy of the batch), the TD error, bias gradients, the SGD update that also keeps the
+// transposed copies of the weights.  PAPER.md:L208, L214; readings #33-#36.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/migsim.h"
+#include "philox.cuh"
+
+namespace migsim {
+
+constexpr int kDqnApad = 16;            // the action dimension is padded to 16 columns (UMMA N = 16)
+
+// ---------------------------------------------------------------------------------------------- sampling + gather
+// Block = 32 batch rows.  idx_b = (w * size) >> 32 with w = word 0 of Philox(counter (b, 3, step, 0), key seed): stream 3
+// (reading #36); with `identity` the batch is rows 0..B-1 of the given arrays.  Writes X[B][64], X2[B][64], the transposed
+// copy Xt[64][B] (through shared memory: both the reads and the writes are coalesced), a, r, done.
+struct GatherArgs {
+  const float *S, *S2; const uint8_t *A; const float *R; const uint8_t *D;     // the replay buffer (or an explicit batch)
+  float *X, *X2, *Xt; uint8_t *a; float *r; uint8_t *done;
+  uint32_t B, size, step, k0, k1; int identity;
+};
+__global__ void __launch_bounds__(256) dqn_gather_kernel(const GatherArgs g) {
+  __shared__ float tile[32][MIG_STATE_DIM + 1];
+  __shared__ uint32_t idx[32];
+  const uint32_t b0 = blockIdx.x * 32u;
+  if (threadIdx.x < 32) {
+    const uint32_t b = b0 + threadIdx.x;
+    uint32_t i = b;
+    if (!g.identity) i = __umulhi(philox4x32_10(b, 3u, g.step, 0u, g.k0, g.k1).x, g.size);
+    idx[threadIdx.x] = i;
+    if (b < g.B) { g.a[b] = g.A[i]; g.r[b] = g.R[i]; g.done[b] = g.D ? g.D[i] : (uint8_t)0; }
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < 32 * MIG_STATE_DIM; e += 256) {
+    const int row = e / MIG_STATE_DIM, k = e % MIG_STATE_DIM;
+    const uint32_t b = b0 + row;
+    if (b >= g.B) continue;
+    const float v = g.S[(size_t)idx[row] * MIG_STATE_DIM + k];
+    tile[row][k] = v;
+    g.X[(size_t)b * MIG_STATE_DIM + k] = v;
+    g.X2[(size_t)b * MIG_STATE_DIM + k] = g.S2[(size_t)idx[row] * MIG_STATE_DIM + k];
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < 32 * MIG_STATE_DIM; e += 256) {
+    const int k = e / 32, row = e % 32;
+    if (b0 + row < g.B) g.Xt[(size_t)k * g.B + b0 + row] = tile[row][k];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- TD error
+// y_b = r_b + gamma (1 - done_b) max_a' Q_target(s'_b, a');  delta_b = Q(s_b, a_b) - y_b;  dL/dQ[b][j] = (j == a_b) delta_b / B;
+// lossrow[b] = delta_b^2 / (2B).  dQ is written row-major [B][16] and transposed [16][B].
+__global__ void __launch_bounds__(256) dqn_td_kernel(const float *Q, const float *Qt, const uint8_t *a, const float *r, const uint8_t *done,
+                                                     uint32_t B, uint32_t n_actions, float gamma, float *dQ, float *dQt, float *lossrow) {
+  const uint32_t b = blockIdx.x * 256u + threadIdx.x;
+  if (b >= B) return;
+  const float4 *q4 = reinterpret_cast<const float4 *>(Q + (size_t)b * kDqnApad), *t4 = reinterpret_cast<const float4 *>(Qt + (size_t)b * kDqnApad);
+  float q[kDqnApad], t[kDqnApad];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float4 x = q4[i], y = t4[i];
+    q[4 * i] = x.x; q[4 * i + 1] = x.y; q[4 * i + 2] = x.z; q[4 * i + 3] = x.w;
+    t[4 * i] = y.x; t[4 * i + 1] = y.y; t[4 * i + 2] = y.z; t[4 * i + 3] = y.w;
+  }
+  float mx = t[0];
+  for (uint32_t j = 1; j < n_actions; ++j) mx = fmaxf(mx, t[j]);
+  const uint32_t ab = a[b];
+  float qa = 0.0f;
+#pragma unroll
+  for (int j = 0; j < kDqnApad; ++j) qa = (uint32_t)j == ab ? q[j] : qa;
+  const float y = done[b] ? r[b] : fmaf(gamma, mx, r[b]);
+  const float delta = qa - y, gq = delta / (float)B;
+  lossrow[b] = delta * delta / (2.0f * (float)B);
+  float4 *o4 = reinterpret_cast<float4 *>(dQ + (size_t)b * kDqnApad);
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+    o4[i] = make_float4(4 * i == (int)ab ? gq : 0.0f, 4 * i + 1 == (int)ab ? gq : 0.0f, 4 * i + 2 == (int)ab ? gq : 0.0f, 4 * i + 3 == (int)ab ? gq : 0.0f);
+#pragma unroll
+  for (int j = 0; j < kDqnApad; ++j) dQt[(size_t)j * B + b] = (uint32_t)j == ab ? gq : 0.0f;
+}
+
+// ---------------------------------------------------------------------------------------------- SGD update
+// One block per row `i` of a weight matrix W [rows][cols] (cols <= 256): W[i][:] -= lr * sum_z partial[z][i][:], in the fixed
+// order z = 0, 1, ...; the transposed copy Wt[cols][ldt] is kept in step.  Blocks beyond `rows` update the bias: bias[o] -= lr *
+// sum_b dZt[o][b] (one block per output o, a fixed-order tree over the batch), block `rows + n_bias` sums the loss.
+struct UpdateArgs {
+  float *W, *Wt; uint32_t rows, cols, ldw, ldt;            // W [rows][ldw] (first `cols` columns live), Wt [cols][ldt]
+  const float *partial; uint32_t n_splits; size_t split_stride; uint32_t ldp;   // partial [z][rows][ldp]
+  float *bias; const float *dZt; uint32_t n_bias, B;       // bias [n_bias], dZt [n_bias][B]
+  float lr;
+  const float *lossrow; float *loss_out;                   // (only the launch that passes them sums the loss)
+};
+__device__ __forceinline__ float block_sum_256(float v, float *red) {
+#pragma unroll
+  for (int d = 16; d; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  float s = 0.0f;
+  if (threadIdx.x == 0) for (int w = 0; w < 8; ++w) s += red[w];
+  __syncthreads();
+  return s;                                                 // valid in thread 0
+}
+__global__ void __launch_bounds__(256) dqn_update_kernel(const UpdateArgs u) {
+  __shared__ float red[8];
+  const uint32_t blk = blockIdx.x;
+  if (blk < u.rows) {
+    for (uint32_t c = threadIdx.x; c < u.cols; c += 256) {
+      float g = 0.0f;
+      for (uint32_t z = 0; z < u.n_splits; ++z) g += u.partial[z * u.split_stride + (size_t)blk * u.ldp + c];
+      const float w = u.W[(size_t)blk * u.ldw + c] - u.lr * g;
+      u.W[(size_t)blk * u.ldw + c] = w;
+      u.Wt[(size_t)c * u.ldt + blk] = w;
+    }
+    return;
+  }
+  if (blk < u.rows + u.n_bias) {
+    const uint32_t o = blk - u.rows;
+    float acc = 0.0f;
+    for (uint32_t b = threadIdx.x; b < u.B; b += 256) acc += u.dZt[(size_t)o * u.B + b];
+    const float s = block_sum_256(acc, red);
+    if (threadIdx.x == 0) u.bias[o] -= u.lr * s;
+    return;
+  }
+  if (u.loss_out) {
+    float acc = 0.0f;
+    for (uint32_t b = threadIdx.x; b < u.B; b += 256) acc += u.lossrow[b];
+    const float s = block_sum_256(acc, red);
+    if (threadIdx.x == 0) *u.loss_out = s;
+  }
+}
+
+// Wt[c][r] = W[r][c] for a small matrix (initialisation and target sync)
+__global__ void dqn_transpose_kernel(const float *W, float *Wt, uint32_t rows, uint32_t cols, uint32_t ldw, uint32_t ldt) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= rows * cols) return;
+  const uint32_t r = i / cols, c = i % cols;
+  Wt[(size_t)c * ldt + r] = W[(size_t)r * ldw + c];
+}
+
+}  // namespace migsim

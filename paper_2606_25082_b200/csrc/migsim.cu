@@ -22,6 +22,11 @@ static int fail(int code, const char *fmt, ...) {
   va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof(g_err), fmt, ap); va_end(ap);
   return code;
 }
+// the same for the other translation units of the library (dqn.cu)
+int mig_fail(int code, const char *fmt, ...) {
+  va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof(g_err), fmt, ap); va_end(ap);
+  return code;
+}
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(MIG_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); } while (0)
 
 extern "C" const char *mig_last_error(void) { return g_err; }

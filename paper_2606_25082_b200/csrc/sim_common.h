@@ -5,6 +5,9 @@
 
 #include "../../include/migsim.h"
 
+// sets mig_last_error()'s message and returns `code` (defined in migsim.cu; shared by the library's translation units)
+int mig_fail(int code, const char *fmt, ...);
+
 namespace migsim {
 
 constexpr int kSlots = MIG_SLOTS;
