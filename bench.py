@@ -157,7 +157,7 @@ def run_ours(args):
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local)
-    if world > 1:
+    if world > 1 or os.environ.get("BENCH_FORCE_DIST") == "1":        # (the flag: a one-rank NCCL group, so that the N > 1 plumbing runs on one GPU)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     from paper_2606_25082_b200 import binding as B
     from paper_2606_25082_b200 import workloads as W
@@ -178,7 +178,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
 
     def barrier():
-        if world > 1:
+        if dist.is_initialized():
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -330,15 +330,116 @@ def run_ours(args):
             "metric": "job_events_per_s", "value": ev_total / t_s, "unit": "job-events/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
             "config": {"workload": args.workload, "n_envs_per_gpu": n_envs, "n_envs_total": n_envs * world, "policy": ["static", "table", "dqn"][wl.policy], "algo": W.ALGO_NAMES[int(wl.algo[0])] if len(set(wl.algo.tolist())) == 1 else "mixed", "lanes_per_env": sim.get_tile(),
-                       "job_events_per_step": ev_total / args.steps, "l2": "flushed between iterations (256 MiB write)", "parallelism": "env-range sharding, no data-path collective"},
+                       "job_events_per_step": ev_total / args.steps, "l2": "flushed between iterations (256 MiB write)", "parallelism": "env-range sharding, no data-path collective",
+                       "dist": ("nccl, world %d" % dist.get_world_size()) if dist.is_initialized() else None},
             "day_episodes_per_s": n_envs * world * args.steps / t_s,
             "e2e": {"value": e2e_ev / e2e_t, "unit": "job-events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
             "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "step_api": step_api,
         }
         print(json.dumps(line))
     sim.close()
-    if world > 1:
+    if dist.is_initialized():
         dist.destroy_process_group()
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ DQN training step (secondary)
+DQN_FLOP_PER_TRANSITION = 647168.0   # algorithmic, H = 256, A = 12: forward of two networks 4 (64H + H^2 + HA), backward through the
+                                     # activations 2 (HA + H^2), weight gradients 2 (HA + H^2 + 64H); the 3 x TF32 split is NOT counted
+
+
+def _dqn_oracle_sample(n):
+    from oracle import oracle as O
+    from paper_2606_25082_b200 import workloads as W
+    net = W.make_qnet(1003, 12, 256)
+    rng = np.random.default_rng(0)
+    o = O.Dqn(net, 0.9, 0.01)
+    s, s2 = rng.normal(0, 1, (n, 64)).astype(np.float32), rng.normal(0, 1, (n, 64)).astype(np.float32)
+    a, r = rng.integers(0, 12, n).astype(np.uint8), rng.normal(0, 1, n).astype(np.float32)
+    t0 = time.perf_counter()
+    o.train_step(s, a, r, s2, None)
+    return time.perf_counter() - t0
+
+
+def run_dqn(args):
+    """`--workload DQN`: one step = one mig_dqn_train_step on a batch of --envs transitions (default 32768) sampled from a
+    replay ring of 24 x 8192 transitions (one C4 day): sample + forward of the online and the target network + TD error +
+    backward + SGD, all products on the tensor cores (3 x TF32).  SURVEY 8(f) #2; a secondary line, not the headline."""
+    import torch
+    from paper_2606_25082_b200 import binding as B
+    from paper_2606_25082_b200 import workloads as W
+    if args.impl == "reference":
+        n = 512
+        dt = [_dqn_oracle_sample(n) for _ in range(max(1, args.steps))]
+        v = n * len(dt) / sum(dt)
+        print(json.dumps({"impl": "reference", "metric": "dqn_transitions_per_s", "value": v, "unit": "transitions/s", "n_gpus": args.gpus, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": 1e3 * sum(dt) / len(dt), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                          "data": "synthetic", "config": {"workload": "DQN", "batch": n}, "cpu_baseline": {"value": v, "unit": "transitions/s", "cores": 1, "kind": "oracle",
+                          "sample": "one training step on %d transitions" % n}, "e2e": {"value": v, "unit": "transitions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+        return 0
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    peaks, peak_src = _peaks()
+    batch = args.envs if args.envs and args.envs % 128 == 0 else 32768
+    cap = 24 * 8192
+    net = W.make_qnet(1003, 12, 256)
+    d = B.Dqn(net, cap, batch, 0.9, 1e-3, 1003)
+    g = torch.Generator(device="cuda"); g.manual_seed(0)
+    S, S2 = torch.randn((cap, 64), device="cuda", generator=g), torch.randn((cap, 64), device="cuda", generator=g)
+    A = torch.randint(0, 12, (cap,), device="cuda", dtype=torch.uint8, generator=g); R = torch.randn(cap, device="cuda", generator=g)
+    d.push(S, A, R, S2)
+    loss = torch.zeros(1, dtype=torch.float32, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+    for w in range(max(3, args.warmup)):
+        d.train_step(w, loss_out=loss); flush.fill_(w & 0xFF)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    pairs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    l0 = d.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for k in range(args.steps):
+        pairs[k][0].record(stream)
+        d.train_step(100 + k, loss_out=loss)
+        pairs[k][1].record(stream)
+        flush.fill_(k & 0xFF)                                                          # L2 flush between iterations
+    e1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    launches = d.launch_count() - l0
+    step_ms = statistics.mean(a.elapsed_time(b) for a, b in pairs)
+    wall_s = e0.elapsed_time(e1) / 1e3
+    # end to end: the batch comes from pinned HOST buffers, the loss goes back to the host, every step
+    hs, hs2 = torch.randn((batch, 64)).pin_memory(), torch.randn((batch, 64)).pin_memory()
+    ha, hr = torch.randint(0, 12, (batch,), dtype=torch.uint8).pin_memory(), torch.randn(batch).pin_memory()
+    ds, ds2, da, dr = (torch.empty_like(x, device="cuda") for x in (hs, hs2, ha, hr))
+    n_e2e = max(1, min(args.steps, 5))
+    torch.cuda.synchronize(); t0 = time.perf_counter()
+    for k in range(n_e2e):
+        ds.copy_(hs, non_blocking=True); ds2.copy_(hs2, non_blocking=True); da.copy_(ha, non_blocking=True); dr.copy_(hr, non_blocking=True)
+        d.train_on(ds, da, dr, ds2, None, loss_out=loss)
+        float(loss.item())
+    e2e_s = time.perf_counter() - t0
+    h2d = hs.numel() * 4 * 2 + ha.numel() + hr.numel() * 4
+    tf32_peak = float(peaks.get("bf16_tflops", peaks.get("bf16_tflops_burst", 1685.8))) / 2.0      # the guide's nominal ratio TF32 : BF16 = 1 : 2
+    achieved = DQN_FLOP_PER_TRANSITION * batch / (step_ms / 1e3) / 1e12
+    cpu = None
+    if not args.no_cpu_baseline:
+        n = 512
+        dt = _dqn_oracle_sample(n)
+        cpu = {"value": n / dt, "unit": "transitions/s", "cores": 1, "kind": "oracle", "sample": "one double-precision training step on %d transitions (%.2f s)" % (n, dt)}
+    line = {"metric": "dqn_transitions_per_s", "value": batch * args.steps / wall_s, "unit": "transitions/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * wall_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "tf32x3 (fp32 in, fp32 accumulate)",
+            "data": "synthetic", "config": {"workload": "DQN", "batch": batch, "replay": cap, "net": "64-256-256-12", "l2": "flushed between iterations (256 MiB write)"},
+            "train_steps_per_s": 1e3 / step_ms, "e2e": {"value": batch * n_e2e / e2e_s, "unit": "transitions/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": 4, "steps": n_e2e},
+            "gpu_launches": launches, "clocks": clocks,
+            "roofline": {"bound": "tensor", "achieved": achieved, "peak": tf32_peak, "unit": "TFLOP/s", "frac": achieved / tf32_peak, "traffic": None,
+                         "kernel": "gemm_tf32x3_kernel<128>", "step_ms": step_ms, "flop_per_transition_algorithmic": DQN_FLOP_PER_TRANSITION,
+                         "issued_over_algorithmic": 3.0, "peak_source": "%s bf16 dense / 2 (TF32 : BF16 = 1 : 2, B200_PROFILING.md)" % peak_src},
+            "cpu_baseline": cpu}
+    print(json.dumps(line))
+    d.close()
     return 0
 
 
@@ -347,7 +448,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5", "DQN"])
     ap.add_argument("--envs", type=int, default=0, help="environments per GPU (default: the workload's BASELINE size)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -357,6 +458,8 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
+    if args.workload == "DQN":
+        return run_dqn(args)
     if not args.envs:
         args.envs = {"C1": 1, "C2": 1024, "C3": 4096, "C4": 8192, "C5": 65536}[args.workload]
     global _ALGO_OVERRIDE

@@ -463,7 +463,7 @@ def reduce_over_ranks(seconds: float, units: int, device="cpu") -> tuple[float, 
     on any initialised torch.distributed backend (NCCL with a CUDA device, gloo on CPU); a no-op without one."""
     import torch
     import torch.distributed as dist
-    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+    if not (dist.is_available() and dist.is_initialized()):
         return float(seconds), int(units)
     t = torch.tensor([seconds], dtype=torch.float64, device=device)
     n = torch.tensor([units], dtype=torch.int64, device=device)
