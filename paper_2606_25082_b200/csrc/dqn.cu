@@ -55,7 +55,7 @@ int make_map(CUtensorMap *m, const float *ptr, uint64_t inner, uint64_t rows, ui
 struct mig_dqn {   // (mig_dqn_t of include/migsim.h)
   uint32_t H = 0, A = 0, B = 0, cap = 0, splits = 1;
   float gamma = 0.0f, lr = 0.0f; uint64_t seed = 0;
-  int device = 0;
+  int device = 0, n_sm = 148;
   uint64_t launches = 0, gemm_launches = 0;
   std::vector<void *> allocs;
   Net net[2];                                              // [0] online, [1] target
@@ -84,8 +84,10 @@ static int launch_gemm(mig_dqn *d, const CUtensorMap &ma, const CUtensorMap &mb,
     CUD(cudaFuncSetAttribute(gemm_tf32x3_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<BN>::kBytes));
     attr_done[d->device] = true;
   }
-  dim3 grid((g.M + kGemmBM - 1) / kGemmBM, g.N / BN, splits);
-  gemm_tf32x3_kernel<BN><<<grid, kGemmThreads, GemmSmem<BN>::kBytes, st>>>(ma, mb, g);
+  GemmArgs ga = g; ga.splits = splits;
+  const uint32_t n_tiles = ((g.M + kGemmBM - 1) / kGemmBM) * (g.N / BN) * splits;
+  const uint32_t grid = n_tiles < (uint32_t)d->n_sm ? n_tiles : (uint32_t)d->n_sm;          // persistent: one CTA per SM walks the tiles
+  gemm_tf32x3_kernel<BN><<<grid, kGemmThreads, GemmSmem<BN>::kBytes, st>>>(ma, mb, ga);
   CUD(cudaGetLastError());
   d->launches++; d->gemm_launches++;
   return MIG_OK;
@@ -121,6 +123,7 @@ extern "C" int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1,
   mig_dqn *d = new (std::nothrow) mig_dqn();
   if (!d) return mig_fail(MIG_ENOMEM, "dqn_create: host allocation failed");
   cudaGetDevice(&d->device);
+  cudaDeviceGetAttribute(&d->n_sm, cudaDevAttrMultiProcessorCount, d->device);
   const uint32_t H = hidden, A = n_actions, B = batch, P = kDqnApad;
   d->H = H; d->A = A; d->B = B; d->cap = replay_capacity; d->gamma = gamma; d->lr = lr; d->seed = seed;
   d->splits = B / 128 < 32 ? B / 128 : 32;                  // split-K of the weight-gradient products: >= 4 k-blocks per split

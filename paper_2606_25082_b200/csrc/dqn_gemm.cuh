@@ -8,9 +8,10 @@
 //   warp 0      TMA producer: cp.async.bulk.tensor loads of a 128 x 32 tile of A and a BN x 32 tile of B per stage (one
 //               128-byte swizzled row = 32 floats of k), completion on an mbarrier; it also owns the TMEM allocation;
 //   warps 2..5  split the landed tiles in place (hi over the TMA'd data, lo into a second buffer at the SAME offsets, so
-//               the 128-byte swizzle never has to be decoded), fence.proxy.async, arrive; after the K loop they are the
-//               epilogue: tcgen05.ld of the accumulator (each warp its own 32 TMEM lanes = 32 rows), bias / ReLU / ReLU-mask,
+//               the 128-byte swizzle never has to be decoded), fence.proxy.async, arrive;
+//   warps 6..9  epilogue: tcgen05.ld of the accumulator (each warp its own 32 TMEM lanes = 32 rows), bias / ReLU / ReLU-mask,
 //               row-major store and / or TRANSPOSED store (32 lanes = 32 consecutive m: coalesced), or a split-K partial;
+//               TMEM holds TWO accumulators, so this overlaps the products of the CTA's next tile (persistent kernel);
 //   warp 1      one elected lane issues 3 x 4 tcgen05.mma.kind::tf32 per stage (UMMA K = 8 floats = 32 bytes; the shared-
 //               memory descriptor advances by 32 bytes inside the swizzled row), accumulator in TMEM (BN columns x 128
 //               lanes), tcgen05.commit frees the stage / publishes the accumulator.
@@ -25,13 +26,14 @@ namespace migsim {
 
 constexpr int kGemmBM = 128;           // rows of C per CTA = TMEM lanes
 constexpr int kGemmBK = 32;            // floats of k per stage: one 128-byte swizzled row
-constexpr int kGemmThreads = 192;      // 6 warps: TMA, MMA, 4 x split / epilogue
+constexpr int kGemmThreads = 320;      // 10 warps: TMA, MMA, 4 x hi/lo split, 4 x epilogue
 
 enum { EPI_BIAS = 1, EPI_RELU = 2, EPI_MASK = 4 /* multiply by (mask[m][n] > 0) */ };
 
 struct GemmArgs {
   uint32_t M, N, K;                    // C is M x N; K = the contraction length of ONE split
   uint32_t k_blocks;                   // K / 32 per split (the last block may run past K: TMA fills zeros)
+  uint32_t splits;                     // split-K factor (1 = none)
   float *out; uint32_t ldo;            // row-major result (or NULL); split z writes at out + z * out_split_stride
   float *out_t; uint32_t ldt;          // transposed result out_t[n][m] (or NULL)
   size_t out_split_stride;             // elements between the partials of consecutive splits (0 without split-K)
@@ -85,16 +87,31 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, float v[8]) {
   for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
 }
 
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float v[16]) {
+  uint32_t r[16];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]),
+                 "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]) : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+
 template <int BN> struct GemmSmem {
   static constexpr int kStageA = kGemmBM * kGemmBK * 4;        // 16 KB
   static constexpr int kStageB = BN * kGemmBK * 4;
   static constexpr int kStage = 2 * (kStageA + kStageB);      // hi + lo of both operands
   static constexpr int kStages = (200 * 1024) / kStage >= 4 ? 4 : (200 * 1024) / kStage;
   static constexpr int kBytes = kStages * kStage + 1024 /* alignment slack */ + 256 /* barriers, tmem address */;
-  static constexpr int kTmemCols = BN < 32 ? 32 : BN;
+  static constexpr int kAccCols = BN < 32 ? 32 : BN;         // TMEM columns of one accumulator
+  static constexpr int kTmemCols = 2 * kAccCols;             // two accumulators: the epilogue of tile i overlaps the products of tile i + 1
 };
 
 // ---------------------------------------------------------------------------------------------- the kernel
+// PERSISTENT: gridDim.x CTAs (one per SM) walk the tiles t = blockIdx.x, + gridDim.x, ... of the tiles_m x tiles_n x splits
+// grid (n fastest: consecutive tiles share their rows of A in L2).  The shared-memory ring and its mbarrier phases run
+// straight through the tile boundaries, so the producer is already loading tile i + 1 while tile i's last stages are
+// multiplied and its accumulator is drained.
 template <int BN>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b, const GemmArgs g) {
@@ -103,16 +120,15 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
   unsigned char *base = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(gemm_smem_raw) + 1023) & ~(uintptr_t)1023);
   unsigned char *tiles = base;
   uint64_t *bars = reinterpret_cast<uint64_t *>(base + S::kStages * S::kStage);
-  uint64_t *full = bars, *split = bars + S::kStages, *empty = bars + 2 * S::kStages, *acc_full = bars + 3 * S::kStages;
-  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(acc_full + 1);
+  uint64_t *full = bars, *split = bars + S::kStages, *empty = bars + 2 * S::kStages, *acc_full = bars + 3 * S::kStages, *acc_empty = acc_full + 2;
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(acc_empty + 2);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t m0 = blockIdx.x * kGemmBM, n0 = blockIdx.y * BN, z = blockIdx.z;
-  const int k_first = (int)(z * g.k_blocks * kGemmBK);
+  const uint32_t tiles_n = g.N / BN, tiles_mn = ((g.M + kGemmBM - 1) / kGemmBM) * tiles_n, n_tiles = tiles_mn * g.splits;
 
   if (warp == 0) {
     if (lane == 0) {
       for (int s = 0; s < S::kStages; ++s) { mbar_init(&full[s], 1); mbar_init(&split[s], 128); mbar_init(&empty[s], 1); }
-      mbar_init(acc_full, 1);
+      for (int s = 0; s < 2; ++s) { mbar_init(&acc_full[s], 1); mbar_init(&acc_empty[s], 128); }
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncwarp();
@@ -127,104 +143,130 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
   if (warp == 0) {
     // ===== TMA producer
     if (lane == 0) {
-      for (uint32_t kb = 0; kb < g.k_blocks; ++kb) {
-        const int s = kb % S::kStages; const uint32_t round = kb / S::kStages;
-        if (round) mbar_wait(&empty[s], (round - 1) & 1u);
-        unsigned char *st = tiles + s * S::kStage;
-        mbar_expect_tx(&full[s], S::kStageA + S::kStageB);
-        tma_load_2d(st, &map_a, &full[s], k_first + (int)kb * kGemmBK, (int)m0);
-        tma_load_2d(st + 2 * S::kStageA, &map_b, &full[s], k_first + (int)kb * kGemmBK, (int)n0);
+      uint32_t it = 0;                                         // k-blocks issued so far, over all tiles of this CTA
+      for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const uint32_t z = tile / tiles_mn, mn = tile - z * tiles_mn, m0 = (mn / tiles_n) * kGemmBM, n0 = (mn % tiles_n) * BN;
+        const int k_first = (int)(z * g.k_blocks * kGemmBK);
+        for (uint32_t kb = 0; kb < g.k_blocks; ++kb, ++it) {
+          const int s = it % S::kStages; const uint32_t round = it / S::kStages;
+          if (round) mbar_wait(&empty[s], (round - 1) & 1u);
+          unsigned char *st = tiles + s * S::kStage;
+          mbar_expect_tx(&full[s], S::kStageA + S::kStageB);
+          tma_load_2d(st, &map_a, &full[s], k_first + (int)kb * kGemmBK, (int)m0);
+          tma_load_2d(st + 2 * S::kStageA, &map_b, &full[s], k_first + (int)kb * kGemmBK, (int)n0);
+        }
       }
     }
   } else if (warp == 1) {
     // ===== MMA issuer
     const uint32_t idesc = umma_idesc_tf32(kGemmBM, BN);
-    for (uint32_t kb = 0; kb < g.k_blocks; ++kb) {
-      const int s = kb % S::kStages; const uint32_t round = kb / S::kStages;
-      mbar_wait(&split[s], round & 1u);
+    uint32_t it = 0, ti = 0;
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++ti) {
+      const uint32_t as = ti & 1u, around = ti >> 1;          // accumulator stage and how often it has been used
+      if (around) mbar_wait(&acc_empty[as], (around - 1) & 1u);      // the epilogue has drained this accumulator
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      if (lane == 0) {                                         // ONE thread issues every MMA of the tile: they execute in its issue order
-        const uint32_t a_hi = smem_u32(tiles + s * S::kStage), a_lo = a_hi + S::kStageA, b_hi = a_hi + 2 * S::kStageA, b_lo = b_hi + S::kStageB;
+      const uint32_t acc = tmem + as * (uint32_t)S::kAccCols;
+      for (uint32_t kb = 0; kb < g.k_blocks; ++kb, ++it) {
+        const int s = it % S::kStages; const uint32_t round = it / S::kStages;
+        mbar_wait(&split[s], round & 1u);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (lane == 0) {                                       // ONE thread issues every MMA: they execute in its issue order
+          const uint32_t a_hi = smem_u32(tiles + s * S::kStage), a_lo = a_hi + S::kStageA, b_hi = a_hi + 2 * S::kStageA, b_lo = b_hi + S::kStageB;
 #pragma unroll
-        for (int k = 0; k < kGemmBK / 8; ++k) {                // UMMA K = 8 floats = 32 bytes inside the swizzled row
-          const uint32_t o = (uint32_t)k * 32u;
-          umma_tf32(tmem, umma_desc_k_sw128(a_lo + o), umma_desc_k_sw128(b_hi + o), idesc, (kb | (uint32_t)k) != 0u);
-          umma_tf32(tmem, umma_desc_k_sw128(a_hi + o), umma_desc_k_sw128(b_lo + o), idesc, 1u);
-          umma_tf32(tmem, umma_desc_k_sw128(a_hi + o), umma_desc_k_sw128(b_hi + o), idesc, 1u);
+          for (int k = 0; k < kGemmBK / 8; ++k) {              // UMMA K = 8 floats = 32 bytes inside the swizzled row
+            const uint32_t o = (uint32_t)k * 32u;
+            umma_tf32(acc, umma_desc_k_sw128(a_lo + o), umma_desc_k_sw128(b_hi + o), idesc, (kb | (uint32_t)k) != 0u);
+            umma_tf32(acc, umma_desc_k_sw128(a_hi + o), umma_desc_k_sw128(b_lo + o), idesc, 1u);
+            umma_tf32(acc, umma_desc_k_sw128(a_hi + o), umma_desc_k_sw128(b_hi + o), idesc, 1u);
+          }
+          umma_commit(&empty[s]);                              // (implies tcgen05.fence::before_thread_sync)
+          if (kb + 1 == g.k_blocks) umma_commit(&acc_full[as]);
         }
-        umma_commit(&empty[s]);                                // (implies tcgen05.fence::before_thread_sync)
-        if (kb + 1 == g.k_blocks) umma_commit(acc_full);
+        __syncwarp();
       }
-      __syncwarp();
+    }
+  } else if (warp < 6) {
+    // ===== hi / lo split of every landed stage, in place
+    const int t = threadIdx.x - 64;                            // 0..127
+    uint32_t it = 0;
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      for (uint32_t kb = 0; kb < g.k_blocks; ++kb, ++it) {
+        const int s = it % S::kStages; const uint32_t round = it / S::kStages;
+        mbar_wait(&full[s], round & 1u);
+        unsigned char *st = tiles + s * S::kStage;
+        float4 *a_hi = reinterpret_cast<float4 *>(st), *a_lo = reinterpret_cast<float4 *>(st + S::kStageA);
+        float4 *b_hi = reinterpret_cast<float4 *>(st + 2 * S::kStageA), *b_lo = reinterpret_cast<float4 *>(st + 2 * S::kStageA + S::kStageB);
+#pragma unroll 4
+        for (int i = t; i < S::kStageA / 16; i += 128) {
+          const float4 x = a_hi[i];
+          float4 h, l;
+          h.x = __uint_as_float(__float_as_uint(x.x) & 0xFFFFE000u); l.x = x.x - h.x;
+          h.y = __uint_as_float(__float_as_uint(x.y) & 0xFFFFE000u); l.y = x.y - h.y;
+          h.z = __uint_as_float(__float_as_uint(x.z) & 0xFFFFE000u); l.z = x.z - h.z;
+          h.w = __uint_as_float(__float_as_uint(x.w) & 0xFFFFE000u); l.w = x.w - h.w;
+          a_hi[i] = h; a_lo[i] = l;
+        }
+#pragma unroll 4
+        for (int i = t; i < S::kStageB / 16; i += 128) {
+          const float4 x = b_hi[i];
+          float4 h, l;
+          h.x = __uint_as_float(__float_as_uint(x.x) & 0xFFFFE000u); l.x = x.x - h.x;
+          h.y = __uint_as_float(__float_as_uint(x.y) & 0xFFFFE000u); l.y = x.y - h.y;
+          h.z = __uint_as_float(__float_as_uint(x.z) & 0xFFFFE000u); l.z = x.z - h.z;
+          h.w = __uint_as_float(__float_as_uint(x.w) & 0xFFFFE000u); l.w = x.w - h.w;
+          b_hi[i] = h; b_lo[i] = l;
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
+        mbar_arrive(&split[s]);
+      }
     }
   } else {
-    // ===== split (per stage), then epilogue
-    const int t = threadIdx.x - 64;                            // 0..127
-    for (uint32_t kb = 0; kb < g.k_blocks; ++kb) {
-      const int s = kb % S::kStages; const uint32_t round = kb / S::kStages;
-      mbar_wait(&full[s], round & 1u);
-      unsigned char *st = tiles + s * S::kStage;
-      float4 *a_hi = reinterpret_cast<float4 *>(st), *a_lo = reinterpret_cast<float4 *>(st + S::kStageA);
-      float4 *b_hi = reinterpret_cast<float4 *>(st + 2 * S::kStageA), *b_lo = reinterpret_cast<float4 *>(st + 2 * S::kStageA + S::kStageB);
-#pragma unroll 4
-      for (int i = t; i < S::kStageA / 16; i += 128) {
-        const float4 x = a_hi[i];
-        float4 h, l;
-        h.x = __uint_as_float(__float_as_uint(x.x) & 0xFFFFE000u); l.x = x.x - h.x;
-        h.y = __uint_as_float(__float_as_uint(x.y) & 0xFFFFE000u); l.y = x.y - h.y;
-        h.z = __uint_as_float(__float_as_uint(x.z) & 0xFFFFE000u); l.z = x.z - h.z;
-        h.w = __uint_as_float(__float_as_uint(x.w) & 0xFFFFE000u); l.w = x.w - h.w;
-        a_hi[i] = h; a_lo[i] = l;
-      }
-#pragma unroll 4
-      for (int i = t; i < S::kStageB / 16; i += 128) {
-        const float4 x = b_hi[i];
-        float4 h, l;
-        h.x = __uint_as_float(__float_as_uint(x.x) & 0xFFFFE000u); l.x = x.x - h.x;
-        h.y = __uint_as_float(__float_as_uint(x.y) & 0xFFFFE000u); l.y = x.y - h.y;
-        h.z = __uint_as_float(__float_as_uint(x.z) & 0xFFFFE000u); l.z = x.z - h.z;
-        h.w = __uint_as_float(__float_as_uint(x.w) & 0xFFFFE000u); l.w = x.w - h.w;
-        b_hi[i] = h; b_lo[i] = l;
-      }
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
-      mbar_arrive(&split[s]);
-    }
-    mbar_wait(acc_full, 0);
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const uint32_t q = (uint32_t)warp & 3u;                    // a warp reads the TMEM lanes 32 (warp % 4) .. + 31
-    const uint32_t m = m0 + q * 32u + (uint32_t)lane;
-    float *orow = g.out ? g.out + (size_t)z * g.out_split_stride + (size_t)m * g.ldo + n0 : nullptr;
-    const float *mrow = (g.epi & EPI_MASK) ? g.mask + (size_t)m * g.ldm + n0 : nullptr;
+    // ===== epilogue (warps 6..9: warp % 4 = 2, 3, 0, 1 -> each its own 32 TMEM lanes)
+    const uint32_t q = (uint32_t)warp & 3u;
+    uint32_t ti = 0;
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++ti) {
+      const uint32_t z = tile / tiles_mn, mn = tile - z * tiles_mn, m0 = (mn / tiles_n) * kGemmBM, n0 = (mn % tiles_n) * BN;
+      const uint32_t as = ti & 1u, around = ti >> 1;
+      mbar_wait(&acc_full[as], around & 1u);
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      const uint32_t m = m0 + q * 32u + (uint32_t)lane;
+      const uint32_t trow = tmem + as * (uint32_t)S::kAccCols + ((q * 32u) << 16);
+      float *orow = g.out ? g.out + (size_t)z * g.out_split_stride + (size_t)m * g.ldo + n0 : nullptr;
+      const float *mrow = (g.epi & EPI_MASK) ? g.mask + (size_t)m * g.ldm + n0 : nullptr;
 #pragma unroll 1
-    for (int c = 0; c < BN; c += 8) {
-      float v[8];
-      tmem_ld8(tmem + ((q * 32u) << 16) + (uint32_t)c, v);
-      if (g.epi & EPI_BIAS) {
+      for (int c = 0; c < BN; c += 16) {
+        float v[16];
+        tmem_ld16(trow + (uint32_t)c, v);
+        if (g.epi & EPI_BIAS) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) v[j] += __ldg(&g.bias[n0 + c + j]);
-      }
-      if (g.epi & EPI_RELU) {
-#pragma unroll
-        for (int j = 0; j < 8; ++j) v[j] = fmaxf(v[j], 0.0f);
-      }
-      if (mrow) {
-        const float4 k0 = *reinterpret_cast<const float4 *>(mrow + c), k1 = *reinterpret_cast<const float4 *>(mrow + c + 4);
-        const float kk[8] = {k0.x, k0.y, k0.z, k0.w, k1.x, k1.y, k1.z, k1.w};
-#pragma unroll
-        for (int j = 0; j < 8; ++j) v[j] = kk[j] > 0.0f ? v[j] : 0.0f;
-      }
-      if (m < g.M) {
-        if (orow) {
-          *reinterpret_cast<float4 *>(orow + c) = make_float4(v[0], v[1], v[2], v[3]);
-          *reinterpret_cast<float4 *>(orow + c + 4) = make_float4(v[4], v[5], v[6], v[7]);
+          for (int j = 0; j < 16; ++j) v[j] += __ldg(&g.bias[n0 + c + j]);
         }
-        if (g.out_t) {
+        if (g.epi & EPI_RELU) {
 #pragma unroll
-          for (int j = 0; j < 8; ++j) g.out_t[(size_t)(n0 + c + j) * g.ldt + m] = v[j];
+          for (int j = 0; j < 16; ++j) v[j] = fmaxf(v[j], 0.0f);
+        }
+        if (mrow && m < g.M) {
+#pragma unroll
+          for (int j4 = 0; j4 < 4; ++j4) {
+            const float4 k4 = *reinterpret_cast<const float4 *>(mrow + c + 4 * j4);
+            v[4 * j4] = k4.x > 0.0f ? v[4 * j4] : 0.0f; v[4 * j4 + 1] = k4.y > 0.0f ? v[4 * j4 + 1] : 0.0f;
+            v[4 * j4 + 2] = k4.z > 0.0f ? v[4 * j4 + 2] : 0.0f; v[4 * j4 + 3] = k4.w > 0.0f ? v[4 * j4 + 3] : 0.0f;
+          }
+        }
+        if (m < g.M) {
+          if (orow) {
+#pragma unroll
+            for (int j4 = 0; j4 < 4; ++j4) *reinterpret_cast<float4 *>(orow + c + 4 * j4) = make_float4(v[4 * j4], v[4 * j4 + 1], v[4 * j4 + 2], v[4 * j4 + 3]);
+          }
+          if (g.out_t) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) g.out_t[(size_t)(n0 + c + j) * g.ldt + m] = v[j];
+          }
         }
       }
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+      mbar_arrive(&acc_empty[as]);                             // this accumulator may be overwritten
     }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   }
   __syncthreads();
   if (warp == 0) {

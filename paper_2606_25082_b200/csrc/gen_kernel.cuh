@@ -76,6 +76,9 @@ __device__ __forceinline__ uint32_t class_of(uint32_t w, const uint32_t *cum) {
   return c;
 }
 
+
+
+
 __global__ void __launch_bounds__(kGenWarps * 32) gen_arrivals_kernel(const GenArgs a) {
   __shared__ GenSmem sm;
   {
@@ -102,16 +105,28 @@ __global__ void __launch_bounds__(kGenWarps * 32) gen_arrivals_kernel(const GenA
   if (epoch < a.n_epochs && !done) {
     const unsigned long long horizon = (unsigned long long)(min(epoch + a.n_steps, a.n_epochs) * a.epoch_s);
     const uint32_t lt = (1u << lane) - 1u;
+    // a gap is at most 32 gap_scale (E24 <= 32 << 24): with gap_scale < 2^22 the sum of a pass of 32 is < 2^32
+    const bool narrow = a.gap_scale < (1ull << 22);
     for (;;) {                                                    // every condition below is warp-uniform
       if (nacc >= limit) break;
       if (count >= a.arr_cap) { more = 1; break; }
       const uint32_t kl = k + lane;
       const uint4 w = philox4x32_10(kl, 0u, env_g, a.episode, a.k0, a.k1);       // stream 0: gap, accept, class, slack
       unsigned long long gap = ((unsigned long long)neglog2_q24_tab(w.x, sm.logT) * a.gap_scale) >> 24;
+      if (narrow) {                                               // 32 gaps of < 2^27 each: the prefix sum fits 32 bits (kernel-uniform branch)
+        uint32_t g32 = (uint32_t)gap;
 #pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {                          // inclusive prefix sum of the gaps, 64-bit integer
-        const unsigned long long o = __shfl_up_sync(0xffffffffu, gap, d);
-        if (lane >= (uint32_t)d) gap += o;
+        for (int d = 1; d < 32; d <<= 1) {
+          const uint32_t o = __shfl_up_sync(0xffffffffu, g32, d);
+          if (lane >= (uint32_t)d) g32 += o;
+        }
+        gap = g32;
+      } else {
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {                        // inclusive prefix sum of the gaps, 64-bit integer
+          const unsigned long long o = __shfl_up_sync(0xffffffffu, gap, d);
+          if (lane >= (uint32_t)d) gap += o;
+        }
       }
       const unsigned long long Tl = T + gap, tick = Tl >> 16;
       const bool in_day = tick < (unsigned long long)a.day_s;     // arrivals stop at the end of the day

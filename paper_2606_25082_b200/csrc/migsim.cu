@@ -52,7 +52,7 @@ struct mig_sim {
   uint32_t envs_per_warp = 0;   // thread-per-env kernel: 0 = chosen per launch so that the batch is one resident wave
   DevTables *d_tab = nullptr;
   uint32_t *d_hdr = nullptr; uint4 *d_jobtab = nullptr; uint4 *d_dbgtab = nullptr; uint32_t *d_dbghdr = nullptr;
-  unsigned int *d_counter = nullptr;
+  unsigned int *d_counter = nullptr; uint32_t *d_algo_mask = nullptr;
   uint8_t *d_algo = nullptr, *d_cfg0 = nullptr;      // copies of the last reset's arrays (debug_trace re-runs from them)
   float *d_state = nullptr; uint8_t *d_action = nullptr;   // scratch of the DQN rollout
   uint8_t *d_table = nullptr; size_t table_bytes = 0;      // staging of rollout_host
@@ -335,7 +335,7 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
   ALLOC(s->d_jobtab, n * (s->ring_cap + kThreadTabExtra) * sizeof(uint4));
   ALLOC(s->d_dbgtab, (size_t)(s->ring_cap + kThreadTabExtra) * sizeof(uint4));
   ALLOC(s->d_dbghdr, kHeaderWords * 4);
-  ALLOC(s->d_counter, sizeof(unsigned int));
+  ALLOC(s->d_counter, sizeof(unsigned int)); ALLOC(s->d_algo_mask, sizeof(uint32_t));
   ALLOC(s->d_algo, n); ALLOC(s->d_cfg0, n);
   ALLOC(s->d_state, n * MIG_STATE_DIM * sizeof(float));
   ALLOC(s->d_action, n);
@@ -353,7 +353,7 @@ extern "C" int mig_sim_create(mig_sim_t **out, const mig_params_t *p, uint32_t n
 extern "C" int mig_sim_destroy(mig_sim_t *s) {
   if (!s) return MIG_OK;
   cudaDeviceSynchronize();
-  cudaFree(s->d_tab); cudaFree(s->d_hdr); cudaFree(s->d_jobtab); cudaFree(s->d_dbgtab); cudaFree(s->d_dbghdr); cudaFree(s->d_counter);
+  cudaFree(s->d_tab); cudaFree(s->d_hdr); cudaFree(s->d_jobtab); cudaFree(s->d_dbgtab); cudaFree(s->d_dbghdr); cudaFree(s->d_counter); cudaFree(s->d_algo_mask);
   cudaFree(s->d_algo); cudaFree(s->d_cfg0); cudaFree(s->d_state); cudaFree(s->d_action); cudaFree(s->d_table);
   cudaFree(s->d_recs); cudaFree(s->d_totals); cudaFree(s->d_script); cudaFree(s->d_arr);
   for (auto &sp : s->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
@@ -409,7 +409,7 @@ static void base_args(const mig_sim *s, SimArgs &a) {
   a.downtime_s = p.repart_downtime_s; a.repart_energy = p.repart_energy_mj;
   a.theta = p.crit_laxity_s; a.crit_max = p.crit_max;
   a.w_energy = p.w_energy; a.w_tardy = p.w_tardy;
-  a.algo = s->d_algo; a.cfg0 = s->d_cfg0;
+  a.algo = s->d_algo; a.cfg0 = s->d_cfg0; a.algo_mask = s->d_algo_mask;
   a.script = s->n_script ? s->d_script : nullptr; a.n_script = s->n_script;
   a.rec_stride = s->n_envs;
   a.all_down = p.repart_all_down != 0; a.util_hist = p.util_hist != 0; a.gamma = p.gamma;
@@ -428,6 +428,9 @@ static uint32_t auto_envs_per_warp(const mig_sim *s, uint32_t n_envs) {
 
 template <bool TRACE>
 static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
+  int devnow = 0;
+  CU(cudaGetDevice(&devnow));
+  if (devnow != s->device) return fail(MIG_ESTATE, "the simulator lives on device %d but device %d is current: its pointers are not valid here", s->device, devnow);
   if (s->tile == 1) {                                     // one thread per environment, one CTA per 64 environments
     SimArgs b = a;
     // arrivals of this launch's horizon: drawn by the generator kernel into the per-environment lists, on the same stream,
@@ -479,6 +482,7 @@ extern "C" int mig_sim_reset(mig_sim_t *s, uint32_t episode, const uint8_t *algo
   CU(cudaMemcpyAsync(s->d_algo, algo, s->n_envs, cudaMemcpyDeviceToDevice, st));
   CU(cudaMemcpyAsync(s->d_cfg0, cfg0, s->n_envs, cudaMemcpyDeviceToDevice, st));
   s->episode = episode;
+  CU(cudaMemsetAsync(s->d_algo_mask, 0, sizeof(uint32_t), st));     // (the init launch collects the batch's algorithms)
   SimArgs a; base_args(s, a);
   a.from_init = 1; a.save = 1; a.n_steps = 0; a.state_out = state_out;
   int rc = launch_sim<false>(s, a, st);
@@ -506,10 +510,13 @@ extern "C" int mig_sim_step(mig_sim_t *s, const uint8_t *action, float *state_ou
 static int launch_qnet(const mig_qnet *q, QArgs &qa, cudaStream_t st) {
   qa.W1 = q->W1; qa.b1 = q->b1; qa.W2 = q->W2; qa.b2 = q->b2; qa.W3 = q->W3; qa.b3 = q->b3; qa.H = q->H; qa.A = q->A;
   size_t smem = (size_t)(MIG_STATE_DIM + 2 * q->H + q->A) * kQRows * sizeof(float) + (size_t)kQStages * kQChunk * q->H * sizeof(float);
-  static thread_local size_t attr_set = 0;
-  if (smem > 48 * 1024 && attr_set < smem) {
+  static size_t attr_set[64] = {0};            // per DEVICE: the opt-in to > 48 KB of dynamic shared memory is a per-device function attribute
+  int devnow = 0;
+  CU(cudaGetDevice(&devnow));
+  if (devnow != q->device) return fail(MIG_ESTATE, "q_eval: the Q-network lives on device %d but device %d is current", q->device, devnow);
+  if (smem > 48 * 1024 && (devnow < 0 || devnow >= 64 || attr_set[devnow] < smem)) {
     CU(cudaFuncSetAttribute(qnet_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set = smem;
+    if (devnow >= 0 && devnow < 64) attr_set[devnow] = smem;
   }
   uint32_t blocks = (qa.B + kQRows - 1) / kQRows;
   qnet_kernel<<<blocks, q->H / kQCols * (kQRows / kQRpt), smem, st>>>(qa);

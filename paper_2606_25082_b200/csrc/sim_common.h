@@ -60,6 +60,7 @@ struct SimArgs {
   int n_steps;          // epochs to run in this launch
   int policy;           // 0 static, 1 table, 3 explicit actions
   const uint8_t *algo, *cfg0;                        // from_init
+  uint32_t *algo_mask;                               // thread-per-env kernel: bit i = some environment runs algorithm i (set by the reset launch)
   const uint8_t *table;                              // [n_envs][n_epochs][4]
   int ev_decide;                                     // TABLE policy: look the table up again after every tick with an arrival or a completion
   const uint8_t *actions; uint32_t act_stride_env, act_stride_k;   // action = actions[env * se + (k - k_first) * sk]

@@ -93,7 +93,10 @@ static __device__ __noinline__ InlineDraw draw_next_arrival(const DevTables *tb,
   return d;
 }
 
-template <int NT, bool TRACE, bool EVD>     // EVD: event-driven decisions of the tabulated policy compiled in (reading #27)
+// EVD: event-driven decisions of the tabulated policy compiled in (reading #27).  EDF: every environment of the batch runs
+// EDF-FS or EDF-SS (the kernel reads the handle's algorithm mask): laxity keys, critical-laxity events and the restricted-
+// preemption pass are compiled out of this instantiation -- the same results from a shorter instruction stream.
+template <int NT, bool TRACE, bool EVD, bool EDF>
 struct EnvT {
   // ------------------------------------------------------------------ environment state
   const SimArgs &a;
@@ -297,7 +300,7 @@ struct EnvT {
     }
     return mean ? sum / n : best;
   }
-  __device__ __forceinline__ bool is_lax() const { return (algo & ~1) == MIG_ALGO_LLF; }      // LLF or LALF
+  __device__ __forceinline__ bool is_lax() const { return !EDF && (algo & ~1) == MIG_ALGO_LLF; }      // LLF or LALF
   __device__ __forceinline__ int skey_of(int due, int rem, uint32_t cls) const {
     if (!is_lax()) return due;                                  // EDF: deadline
     return due - rd_cfg(rem, cls, algo == MIG_ALGO_LALF);                 // laxity + t (t is common to all jobs)
@@ -353,7 +356,7 @@ struct EnvT {
   // advance the look-ahead to the next accepted arrival (or none)
   __device__ __forceinline__ void gen_next() {
     look_valid = 0;
-    if (a.script) {                                                           // scripted arrivals (tests), kernel-uniform branch
+    if (a.script) {                                      // scripted arrivals (tests), kernel-uniform branch
       if (i_script < a.n_script) {
         const mig_job_t s = a.script[i_script];
         look_valid = 1; look_tick = s.arr; look_cls = s.cls; look_due = s.due;
@@ -458,7 +461,7 @@ struct EnvT {
   // Every job in the system is re-evaluated: in (key, id) order, while an up slice is left, each job picks a slice by its
   // rule.  The order is produced by merging the running jobs (slice table) with the front of the waiting queue.
   __device__ __forceinline__ void reschedule() {
-    if (algo == MIG_ALGO_EDF_SS_R) { reschedule_restricted(); return; }
+    if (!EDF && algo == MIG_ALGO_EDF_SS_R) { reschedule_restricted(); return; }
     if (is_lax())                       // the keys of running jobs move with their remaining work
       for (uint32_t m = busy_mask; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
@@ -591,7 +594,7 @@ struct EnvT {
       n_sys--;
       happened = true;
     }
-    if (next_up == t) {                                               // (ii) slices coming up, ascending slot
+    if (next_up == t) {                                     // (ii) slices coming up, ascending slot
       int nu = MIG_INF;
       for (uint32_t m = down_mask; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
@@ -616,7 +619,7 @@ struct EnvT {
       happened = true; job_event = true;
       gen_next();
     }
-    if (next_crit == t) {                                             // (iv) critical laxity, ascending id
+    if (!EDF && next_crit == t) {                                     // (iv) critical laxity, ascending id
       int last_id = -1;
       for (;;) {
         uint32_t bid = 0xFFFFFFFFu, bi = 0; uint2 bkm = make_uint2(0u, 0u);
@@ -820,6 +823,10 @@ struct EnvT {
   __device__ __forceinline__ void init_regs(uint32_t env_local) {
     algo = a.algo[env_local]; t = 0; epoch = 0; status = 0; n_sys = 0; n_wait = 0;
     if (algo > MIG_ALGO_EDF_SS_R) { algo = MIG_ALGO_EDF_FS; status |= MIG_ST_BAD_ALGO; }   // reading #28
+    if (a.algo_mask) {                                        // which algorithms this batch runs (picks the kernel body of later launches)
+      const uint32_t act = __activemask(), m = __reduce_or_sync(act, 1u << algo);
+      if ((threadIdx.x & 31u) == (uint32_t)(__ffs((int)act) - 1)) atomicOr(a.algo_mask, m);
+    }
     q_head = 0; q_ns = 0; g_head = 0; q_ng = 0;
     h_lo = 0x84222325u; h_hi = 0xcbf29ce4u;                   // FNV-1a-64 offset basis
     uint32_t c0 = a.cfg0[env_local];
@@ -896,7 +903,7 @@ struct EnvT {
     in_drain = false;
     long long dE = 0, dT = 0;
     for (int s = 0;;) {
-      if (fresh) {                                            // ---- the next decision epoch begins
+      if (fresh) {                                  // ---- the next decision epoch begins
         fresh = false; drain = false; in_drain = false; dE = 0; dT = 0;
         uint32_t action = (uint32_t)cfg;                                            // STATIC: stay
         if (a.policy == MIG_POLICY_TABLE) {                                         // load bucket
@@ -942,6 +949,31 @@ struct EnvT {
   }
 };
 
+template <int NT, bool TRACE, bool EVD, bool EDF>
+__device__ __forceinline__ void thread_body(const SimArgs &a, const HotTablesT &hot, unsigned char *base, uint32_t li) {
+  uint2 *r2 = reinterpret_cast<uint2 *>(base) + threadIdx.x;
+  uint32_t *r1 = reinterpret_cast<uint32_t *>(base + (size_t)NT * (T2_RING + 2 * (size_t)a.smem_entries) * 8) + threadIdx.x;
+  EnvT<NT, TRACE, EVD, EDF> e(a, hot, r2, r1);
+  e.land = reinterpret_cast<uint4 *>(base + (size_t)NT * ((T2_RING + 2 * (size_t)a.smem_entries) * 8 + T1_WORDS * 4)) + threadIdx.x;
+  const uint32_t env = a.env_first + li;
+  e.env_g = a.env_base + env; e.env_l = env; e.in_drain = false;
+  e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * (a.ring_cap + kThreadTabExtra);
+  e.hdr = a.hdr_override ? a.hdr_override : a.hdr + (size_t)env * kHeaderWords;
+  e.arr = (a.arr && !a.script) ? a.arr + (size_t)env * a.arr_cap : nullptr;   // (the host launches gen_arrivals_kernel first)
+  e.a_head = 0;
+  if (a.from_init) { e.init_regs(env); e.init_rows(); } else { e.load_regs(); e.load_rows(); }
+  if (a.n_steps > 0 && e.epoch < a.n_epochs) {
+    if (e.arr && e.a_count) e.fetch_block(0);
+    if (!e.look_valid) e.gen_next();                            // prime the look-ahead (one may be carried over from the last launch)
+  }
+  e.run(li, env);
+  if (a.state_out) e.observe(a.state_out + (size_t)(TRACE ? 0u : env) * MIG_STATE_DIM);
+  if (a.totals) e.store_totals(a.totals + (TRACE ? 0u : env));   // totals so far (hash and t are live values)
+  if (a.save) e.save();
+  if (TRACE && a.trace_n) *a.trace_n = e.n_trace;
+}
+
+
 template <int NT, bool TRACE, bool EVD>
 __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -966,26 +998,10 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   const uint32_t li = (blockIdx.x * (NT / 32) + (threadIdx.x >> 5)) * a.envs_per_warp + lane;   // index inside this launch's env range
   const bool alive = lane < a.envs_per_warp && li < a.n_envs;
   if (!alive) return;
-  uint2 *r2 = reinterpret_cast<uint2 *>(base) + threadIdx.x;
-  uint32_t *r1 = reinterpret_cast<uint32_t *>(base + (size_t)NT * (T2_RING + 2 * (size_t)a.smem_entries) * 8) + threadIdx.x;
-  EnvT<NT, TRACE, EVD> e(a, hot, r2, r1);
-  e.land = reinterpret_cast<uint4 *>(base + (size_t)NT * ((T2_RING + 2 * (size_t)a.smem_entries) * 8 + T1_WORDS * 4)) + threadIdx.x;
-  const uint32_t env = a.env_first + li;
-  e.env_g = a.env_base + env; e.env_l = env; e.in_drain = false;
-  e.gtab = a.tab_override ? a.tab_override : a.jobtab + (size_t)env * (a.ring_cap + kThreadTabExtra);
-  e.hdr = a.hdr_override ? a.hdr_override : a.hdr + (size_t)env * kHeaderWords;
-  e.arr = (a.arr && !a.script) ? a.arr + (size_t)env * a.arr_cap : nullptr;   // (the host launches gen_arrivals_kernel first)
-  e.a_head = 0;
-  if (a.from_init) { e.init_regs(env); e.init_rows(); } else { e.load_regs(); e.load_rows(); }
-  if (a.n_steps > 0 && e.epoch < a.n_epochs) {
-    if (e.arr && e.a_count) e.fetch_block(0);
-    if (!e.look_valid) e.gen_next();                            // prime the look-ahead (one may be carried over from the last launch)
-  }
-  e.run(li, env);
-  if (a.state_out) e.observe(a.state_out + (size_t)(TRACE ? 0u : env) * MIG_STATE_DIM);
-  if (a.totals) e.store_totals(a.totals + (TRACE ? 0u : env));   // totals so far (hash and t are live values)
-  if (a.save) e.save();
-  if (TRACE && a.trace_n) *a.trace_n = e.n_trace;
+  // every environment of the batch on EDF-FS / EDF-SS (bits 0, 1 of the mask that the reset launch collected): the short body
+  const bool edf_only = !a.from_init && a.algo_mask && (__ldg(a.algo_mask) & ~3u) == 0u;
+  if (edf_only) thread_body<NT, TRACE, EVD, true>(a, hot, base, li);
+  else thread_body<NT, TRACE, EVD, false>(a, hot, base, li);
 }
 
 // per-env auxiliary results out of the saved headers: the discounted return and the seconds per utilisation level
