@@ -3,12 +3,15 @@
 //
 // The arrival process does not depend on the schedule, so a launch's arrivals can all be drawn before
 // it simulates -- and drawing them is embarrassingly parallel over thinning CANDIDATES, where the event loop is serial:
-//   * ONE WARP PER ENVIRONMENT, 32 candidates per pass: lane l draws candidate k + l (Philox stream 0: gap, accept,
-//     class, slack), the integer -log2 turns w_gap into a Q16 gap, a 64-bit inclusive warp scan (SHFL.UP) plus the
-//     running sum gives every candidate its arrival tick -- integer addition is associative, so this IS the oracle's
-//     sequential accumulation;
-//   * Lewis-Shedler thinning against the per-minute threshold table; ballot + popc compact the accepted candidates;
-//   * only accepted candidates draw Philox stream 1 (duration) and look their class / duration / slack up;
+//   * ONE WARP PER ENVIRONMENT, 128 candidates per pass: lane l draws the four consecutive candidates k + 4 l + j (Philox
+//     stream 0: gap, accept, class, slack; four independent chains per lane), the integer -log2 turns w_gap into a Q16
+//     gap, the lane sums its own four, ONE warp scan (SHFL.UP; 32-bit when 128 gaps fit, else 64-bit) plus the running
+//     sum gives every candidate its arrival tick -- integer addition is associative, so this IS the oracle's sequential
+//     accumulation;
+//   * Lewis-Shedler thinning against the per-minute threshold table; a warp scan of the per-lane counts compacts the
+//     accepted candidates into a per-warp shared-memory buffer in list order;
+//   * the attribute pass runs over that buffer 32 at a time with every lane busy: only accepted candidates draw Philox
+//     stream 1 (duration) and look their class / duration / slack up;
 //   * each accepted job becomes ONE 8-BYTE record {dur7 | class | slack, tick} appended to the environment's list; the
 //     32 lanes of a pass write neighbouring records (coalesced).  The event loop recomputes work = dur7 * v7[class] and
 //     due = tick + max(1, dur7 * slack >> 10) when it takes the record (two multiplies) -- half the bytes of a
@@ -43,7 +46,12 @@ struct GenArgs {
   uint32_t job_limit;
 };
 
+constexpr int kGenRun = 4;       // consecutive candidates per lane and pass: 128 per warp pass, four independent Philox chains per lane
+static_assert(kGenRun <= 4, "the per-lane flag word holds three nibbles");
+struct GenPend { uint32_t k, tick, wz, ww; };   // an accepted candidate waiting for its attributes: index, arrival tick, class word, slack word
+
 struct GenSmem {
+  GenPend pend[kGenWarps][32 * kGenRun];
   uint32_t thr[MIG_THR_BINS];
   int32_t dur7_q[MIG_MAX_CLASSES * 65];
   uint32_t class_cum[MIG_MAX_CLASSES];      // padded with 0xFFFFFFFF beyond n_classes
@@ -79,7 +87,7 @@ __device__ __forceinline__ uint32_t class_of(uint32_t w, const uint32_t *cum) {
 
 
 
-__global__ void __launch_bounds__(kGenWarps * 32) gen_arrivals_kernel(const GenArgs a) {
+__global__ void __launch_bounds__(kGenWarps * 32, 3) gen_arrivals_kernel(const GenArgs a) {
   __shared__ GenSmem sm;
   {
     const DevTables *tb = a.tab;
@@ -104,54 +112,101 @@ __global__ void __launch_bounds__(kGenWarps * 32) gen_arrivals_kernel(const GenA
   uint32_t count = 0, more = 0;
   if (epoch < a.n_epochs && !done) {
     const unsigned long long horizon = (unsigned long long)(min(epoch + a.n_steps, a.n_epochs) * a.epoch_s);
-    const uint32_t lt = (1u << lane) - 1u;
-    // a gap is at most 32 gap_scale (E24 <= 32 << 24): with gap_scale < 2^22 the sum of a pass of 32 is < 2^32
-    const bool narrow = a.gap_scale < (1ull << 22);
+    // a gap is at most 32 gap_scale (E24 <= 32 << 24): with gap_scale < 2^20 the sum of a pass of 128 is < 2^32
+    const bool narrow = a.gap_scale < (1ull << 20);
+    GenPend *pend = sm.pend[threadIdx.x >> 5];                    // this warp's accepted candidates of the pass
     for (;;) {                                                    // every condition below is warp-uniform
       if (nacc >= limit) break;
       if (count >= a.arr_cap) { more = 1; break; }
-      const uint32_t kl = k + lane;
-      const uint4 w = philox4x32_10(kl, 0u, env_g, a.episode, a.k0, a.k1);       // stream 0: gap, accept, class, slack
-      unsigned long long gap = ((unsigned long long)neglog2_q24_tab(w.x, sm.logT) * a.gap_scale) >> 24;
-      if (narrow) {                                               // 32 gaps of < 2^27 each: the prefix sum fits 32 bits (kernel-uniform branch)
-        uint32_t g32 = (uint32_t)gap;
+      // ---- lane l draws the kGenRun consecutive candidates k + kGenRun l + j (Philox stream 0: gap, accept, class, slack)
+      const uint32_t kb = k + lane * kGenRun;
+      uint32_t wy[kGenRun], wz[kGenRun], ww[kGenRun];
+      unsigned long long s[kGenRun];                              // inclusive sums of the lane's own gaps
+      unsigned long long run = 0;
+#pragma unroll
+      for (int j = 0; j < kGenRun; ++j) {
+        const uint4 w = philox4x32_10(kb + (uint32_t)j, 0u, env_g, a.episode, a.k0, a.k1);
+        run += ((unsigned long long)neglog2_q24_tab(w.x, sm.logT) * a.gap_scale) >> 24;
+        s[j] = run; wy[j] = w.y; wz[j] = w.z; ww[j] = w.w;
+      }
+      // ---- exclusive warp scan of the lane totals (integer: the same sums as the oracle's sequential accumulation)
+      unsigned long long incl;
+      if (narrow) {
+        uint32_t g32 = (uint32_t)run;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
           const uint32_t o = __shfl_up_sync(0xffffffffu, g32, d);
           if (lane >= (uint32_t)d) g32 += o;
         }
-        gap = g32;
+        incl = g32;
       } else {
+        incl = run;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {                        // inclusive prefix sum of the gaps, 64-bit integer
-          const unsigned long long o = __shfl_up_sync(0xffffffffu, gap, d);
-          if (lane >= (uint32_t)d) gap += o;
+        for (int d = 1; d < 32; d <<= 1) {
+          const unsigned long long o = __shfl_up_sync(0xffffffffu, incl, d);
+          if (lane >= (uint32_t)d) incl += o;
         }
       }
-      const unsigned long long Tl = T + gap, tick = Tl >> 16;
-      const bool in_day = tick < (unsigned long long)a.day_s;     // arrivals stop at the end of the day
-      const bool ok = in_day && tick <= horizon;
-      const bool acc0 = ok && w.y <= sm.thr[(uint32_t)tick / 60u];               // Lewis-Shedler thinning
-      const uint32_t accm = __ballot_sync(0xffffffffu, acc0);
-      const uint32_t before = __popc(accm & lt);                  // accepted among the earlier candidates of this pass
+      const unsigned long long base = T + (incl - run);
+      // ---- thinning (Lewis-Shedler) per candidate; flags: bit j = inside the day, bit 4 + j = also inside the horizon, bit 8 + j = accepted
+      uint32_t tick[kGenRun], fl = 0, n_acc_l = 0;
+#pragma unroll
+      for (int j = 0; j < kGenRun; ++j) {
+        const unsigned long long tk = (base + s[j]) >> 16;
+        const bool in_day = tk < (unsigned long long)a.day_s;     // arrivals stop at the end of the day
+        const bool ok = in_day && tk <= horizon;
+        tick[j] = (uint32_t)tk;
+        const bool acc = ok && wy[j] <= sm.thr[(ok ? (uint32_t)tk : 0u) / 60u];
+        fl |= (in_day ? 1u : 0u) << j | (ok ? 1u : 0u) << (4 + j) | (acc ? 1u : 0u) << (8 + j);
+        n_acc_l += acc ? 1u : 0u;
+      }
+      uint32_t before = n_acc_l;                                  // accepted among the EARLIER candidates of the pass (lane-major order)
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t o = __shfl_up_sync(0xffffffffu, before, d);
+        if (lane >= (uint32_t)d) before += o;
+      }
+      before -= n_acc_l;
+      // ---- commit a prefix of the pass: inside the horizon and room left in the list (ticks and `before` are monotone)
       const uint32_t room = min(a.arr_cap - count, limit - nacc);
-      const bool commit = ok && before < room;                    // a prefix of the pass: ticks and `before` are monotone
-      const uint32_t cm = __ballot_sync(0xffffffffu, commit);
-      const int nc = __popc(cm);
-      if (acc0 && commit) {                                       // job attributes (R5)
-        const uint32_t c = class_of(w.z, sm.class_cum);
-        const uint4 wd = philox4x32_10(kl, 1u, env_g, a.episode, a.k0, a.k1);    // stream 1: duration
+      uint32_t nc_l = 0, na_l = 0, b = before;
+#pragma unroll
+      for (int j = 0; j < kGenRun; ++j) {
+        const bool commit = ((fl >> (4 + j)) & 1u) && b < room;
+        const bool acc = (fl >> (8 + j)) & 1u;
+        nc_l += commit ? 1u : 0u;
+        if (commit && acc) {                                      // park it for the attribute pass, in list order
+          pend[b] = GenPend{kb + (uint32_t)j, tick[j], wz[j], ww[j]};
+          ++na_l;
+        }
+        b += acc ? 1u : 0u;
+      }
+      const uint32_t nc = __reduce_add_sync(0xffffffffu, nc_l), na = __reduce_add_sync(0xffffffffu, na_l);
+      __syncwarp();
+      // ---- job attributes (R5) of the accepted candidates, 32 per trip with every lane busy: class, Philox stream 1
+      // (duration), slack; one coalesced 8-byte record each
+      for (uint32_t i = lane; i < na; i += 32u) {
+        const GenPend e = pend[i];
+        const uint32_t c = class_of(e.wz, sm.class_cum);
+        const uint4 wd = philox4x32_10(e.k, 1u, env_g, a.episode, a.k0, a.k1);
         const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
         const int q0 = sm.dur7_q[c * 65 + qi], q1 = sm.dur7_q[c * 65 + qi + 1];
         const int dur7 = q0 + (int)(((long long)(q1 - q0) * (long long)f) >> 10);
-        const uint32_t slack = sm.slack_lo[c] + __umulhi(w.w, sm.slack_span[c]);
-        __stcg(&out[count + before], pack_arrival((uint32_t)tick, c, (uint32_t)dur7, slack));   // streamed past L1
+        const uint32_t slack = sm.slack_lo[c] + __umulhi(e.ww, sm.slack_span[c]);
+        __stcg(&out[count + i], pack_arrival(e.tick, c, (uint32_t)dur7, slack));   // streamed past L1
       }
-      const uint32_t na = __popc(accm & cm);
+      __syncwarp();
       count += na; nacc += na;
-      if (nc) { T = __shfl_sync(0xffffffffu, Tl, nc - 1); k += (uint32_t)nc; }
-      if (nc < 32) {                                              // the first uncommitted candidate says why we stop
-        const bool s_in_day = __shfl_sync(0xffffffffu, (int)in_day, nc) != 0, s_ok = __shfl_sync(0xffffffffu, (int)ok, nc) != 0;
+      if (nc) {                                                   // the generator moves past the committed candidates
+        const uint32_t lc = (nc - 1u) / kGenRun, jc = (nc - 1u) % kGenRun;
+        unsigned long long tl = base + s[0];
+#pragma unroll
+        for (int j = 1; j < kGenRun; ++j) tl = jc == (uint32_t)j ? base + s[j] : tl;
+        T = __shfl_sync(0xffffffffu, tl, (int)lc); k += nc;
+      }
+      if (nc < 32u * kGenRun) {                                   // the first uncommitted candidate says why we stop
+        const uint32_t f1 = __shfl_sync(0xffffffffu, fl, (int)(nc / kGenRun)), j1 = nc % kGenRun;
+        const bool s_in_day = (f1 >> j1) & 1u, s_ok = (f1 >> (4 + j1)) & 1u;
         if (!s_in_day) done = 1;                                  // end of the day
         else if (s_ok && nacc < limit) more = 1;                  // inside the horizon: the list is full
         break;
