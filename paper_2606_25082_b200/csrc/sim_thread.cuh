@@ -314,6 +314,16 @@ struct EnvT {
     slice_mask = m;
   }
 
+  // run_order without the entry of slot p (a job left its slice): the zero-nibble trick on order ^ pppppppp finds it -- the
+  // LOWEST flagged nibble is exact, slots are unique in the list and the 0xF end markers never match p <= 6
+  static __device__ __forceinline__ uint32_t drop_slot(uint32_t order, int p) {
+    const uint32_t x = order ^ (0x11111111u * (uint32_t)p);
+    const uint32_t z = (x - 0x11111111u) & ~x & 0x88888888u;
+    if (!z) return order;
+    const uint32_t sh = (uint32_t)(__ffs((int)z) - 1) & ~3u, lo = (1u << sh) - 1u;
+    return (order & lo) | ((order >> 4) & ~lo) | 0xF0000000u;
+  }
+
   // power and busy units from the slice table (a down slice counts idle)
   __device__ __forceinline__ void update_power() {
     int u = 0, pd = 0;
@@ -477,22 +487,26 @@ struct EnvT {
     while (avail != 0u) {
       // --- next job in (key, id) order: the first of the unpicked running jobs, or the front of the queue
       uint2 bkm = make_uint2(0x7FFFFFFFu, 0xFFFFFFFFu); int bp = -1;
-      if (!is_lax()) {                    // EDF keys are static: the running jobs are still in last time's order
-        while ((ro & 15u) != 15u && !((rmask >> (ro & 15u)) & 1u)) ro >>= 4;
-        if ((ro & 15u) != 15u) { bp = (int)(ro & 15u); bkm = R2(T2_SLKM + bp); }
+      if (!is_lax()) {                    // EDF keys are static: run_order lists exactly the running jobs, still in key order
+        const uint32_t rs = ro & 15u;     // (15: none left); both candidate keys are loaded, the choice is two selects
+        const uint2 rkm = R2(T2_SLKM + (int)(rs & 7u)), wk = queue_top_km();      // (valid rows even when there is no such job)
+        const bool has_r = rs != 15u, has_w = n_wait != 0u;
+        if (!has_r && !has_w) break;                                      // nobody left
+        const bool from_q = has_w && (!has_r || before(wk, rkm));
+        bkm = from_q ? wk : rkm; bp = from_q ? 7 : (int)rs;
       } else {
         for (uint32_t m = rmask; m; m &= m - 1) {
           const int p = __ffs((int)m) - 1;
           const uint2 km = R2(T2_SLKM + p);
           if (bp < 0 || before(km, bkm)) { bkm = km; bp = p; }
         }
+        if (n_wait) {
+          const uint2 wk = queue_top_km();
+          if (bp < 0 || before(wk, bkm)) { bkm = wk; bp = 7; }
+        }
+        if (bp < 0) break;                                                // nobody left
       }
       uint2 rdv;
-      if (n_wait) {
-        const uint2 wk = queue_top_km();
-        if (bp < 0 || before(wk, bkm)) { bkm = wk; bp = 7; }
-      }
-      if (bp < 0) break;                                                  // nobody left
       {                                   // take the record from the queue's front or from the slice table: selects, not a branch
         const bool take_q = bp == 7;
         rdv = r2[(take_q ? T2_RING + 2 * (int)q_head + 1 : T2_SLRD + bp) * NT];      // one load, selected row
@@ -591,6 +605,7 @@ struct EnvT {
       count(C_COMPLETED, 1u);
       if (tard > 0) count(C_TARDY, 1u);
       busy_mask &= ~(1u << p);
+      run_order = drop_slot(run_order, p);
       n_sys--;
       happened = true;
     }
@@ -679,6 +694,10 @@ struct EnvT {
         queue_push_front(R2(T2_SLKM + p), R2(T2_SLRD + p));
       }
       busy_mask &= ~pm;
+      uint32_t o = 0xFFFFFFFFu; int k = 0;                    // run_order keeps the jobs that stay, in their order
+      for (uint32_t ro = run_order | 0xF0000000u; (ro & 15u) != 15u; ro >>= 4)
+        if ((busy_mask >> (ro & 15u)) & 1u) { o = (o & ~(15u << (4 * k))) | ((ro & 15u) << (4 * k)); ++k; }
+      run_order = o;
     }
     const int old = cfg;
     set_cfg_tables((int)action);
