@@ -481,6 +481,7 @@ struct EnvT {
     uint32_t avail = slice_mask & ~down_mask;       // every UP slice, occupied or not
     uint32_t rmask = busy_mask;                     // running jobs not picked yet
     uint32_t keep = 0, nb = 0; int K = 0, nd = MIG_INF, u = 0, pd = 0;
+    uint32_t moved_mask = 0;
     uint32_t ro = run_order | 0xF0000000u, new_order = 0xFFFFFFFFu;
     uint4 gh = make_uint4(0u, 0u, 0u, 0u); bool gh_valid = q_ng != 0u;      // the global part's head, requested before the pick that may need it
     if (gh_valid) gh = gtab[g_head];
@@ -540,6 +541,7 @@ struct EnvT {
       nb |= 1u << s; nd = min(nd, t + (pick >> 3)); u += units_of(g); pd += hot.pdiff[g];
       const bool moved = bp != s;
       if (!moved) keep |= 1u << s;
+      moved_mask |= (moved ? 1u : 0u) << K;
       R2(T2_STG + K) = make_uint2((bkm.y & ~15u) | (uint32_t)s | (moved ? 8u : 0u), rdv.x);
       R1(T1_STGDUE + K) = rdv.y;
       new_order = (new_order & ~(15u << (4 * K))) | ((uint32_t)s << (4 * K));
@@ -558,18 +560,16 @@ struct EnvT {
         queue_push_front(R2(T2_SLKM + p), R2(T2_SLRD + p));
       }
     }
-    int n_start = 0;
-    for (int k = 0; k < K; ++k) {
+    const int n_start = __popc(moved_mask);
+    for (uint32_t mm = moved_mask; mm; mm &= mm - 1) {                    // only the picks that changed slice: no test inside the loop
+      const int k = __ffs((int)mm) - 1;
       const uint2 st = R2(T2_STG + k);
-      if (st.x & 8u) {
-        const int s = (int)(st.x & 7u), g = size_at(s);
-        const uint32_t meta = st.x & ~15u, due = R1(T1_STGDUE + k);
-        emit(MIG_EV_START, s, (uint32_t)g, m_id(meta), (int)st.y);
-        R2(T2_SLKM + s) = make_uint2(due, meta);                          // EDF key = due; LLF / LALF keys are refreshed on use
-        R2(T2_SLRD + s) = make_uint2(st.y, due);
-        R1(T1_V + s) = speed_of(m_cls(meta), g).x;
-        ++n_start;
-      }
+      const int s = (int)(st.x & 7u), g = size_at(s);
+      const uint32_t meta = st.x & ~15u, due = R1(T1_STGDUE + k);
+      emit(MIG_EV_START, s, (uint32_t)g, m_id(meta), (int)st.y);
+      R2(T2_SLKM + s) = make_uint2(due, meta);
+      R2(T2_SLRD + s) = make_uint2(st.y, due);
+      R1(T1_V + s) = speed_of(m_cls(meta), g).x;
     }
     if (n_start) count(C_START, (uint32_t)n_start);
     busy_mask = nb; next_done = nd; run_order = new_order;
