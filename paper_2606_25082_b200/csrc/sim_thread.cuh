@@ -94,8 +94,9 @@ static __device__ __noinline__ InlineDraw draw_next_arrival(const DevTables *tb,
 }
 
 // EVD: event-driven decisions of the tabulated policy compiled in (reading #27).  EDF: every environment of the batch runs
-// EDF-FS or EDF-SS (the kernel reads the handle's algorithm mask): laxity keys, critical-laxity events and the restricted-
-// preemption pass are compiled out of this instantiation -- the same results from a shorter instruction stream.
+// a deadline-keyed algorithm -- EDF-FS, EDF-SS or EDF-SS with restricted preemption (the kernel reads the handle's algorithm
+// mask): laxity keys and critical-laxity events are compiled out of this instantiation -- the same results from a shorter
+// instruction stream.
 template <int NT, bool TRACE, bool EVD, bool EDF>
 struct EnvT {
   // ------------------------------------------------------------------ environment state
@@ -471,7 +472,7 @@ struct EnvT {
   // Every job in the system is re-evaluated: in (key, id) order, while an up slice is left, each job picks a slice by its
   // rule.  The order is produced by merging the running jobs (slice table) with the front of the waiting queue.
   __device__ __forceinline__ void reschedule() {
-    if (!EDF && algo == MIG_ALGO_EDF_SS_R) { reschedule_restricted(); return; }
+    if (algo == MIG_ALGO_EDF_SS_R) { reschedule_restricted(); return; }
     if (is_lax())                       // the keys of running jobs move with their remaining work
       for (uint32_t m = busy_mask; m; m &= m - 1) {
         const int p = __ffs((int)m) - 1;
@@ -1017,8 +1018,9 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   const uint32_t li = (blockIdx.x * (NT / 32) + (threadIdx.x >> 5)) * a.envs_per_warp + lane;   // index inside this launch's env range
   const bool alive = lane < a.envs_per_warp && li < a.n_envs;
   if (!alive) return;
-  // every environment of the batch on EDF-FS / EDF-SS (bits 0, 1 of the mask that the reset launch collected): the short body
-  const bool edf_only = !a.from_init && a.algo_mask && (__ldg(a.algo_mask) & ~3u) == 0u;
+  // every environment of the batch on EDF-FS / EDF-SS / restricted EDF-SS (bits 0, 1, 4 of the mask that the reset launch
+  // collected): the short body
+  const bool edf_only = !a.from_init && a.algo_mask && (__ldg(a.algo_mask) & ~0x13u) == 0u;
   if (edf_only) thread_body<NT, TRACE, EVD, true>(a, hot, base, li);
   else thread_body<NT, TRACE, EVD, false>(a, hot, base, li);
 }
