@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -56,7 +57,8 @@ struct mig_dqn {   // (mig_dqn_t of include/migsim.h)
   uint32_t H = 0, A = 0, B = 0, cap = 0, splits = 1;
   float gamma = 0.0f, lr = 0.0f; uint64_t seed = 0;
   int device = 0, n_sm = 148;
-  uint64_t launches = 0, gemm_launches = 0;
+  uint64_t launches = 0, gemm_launches = 0, kernels_per_step = 0, gemms_per_step = 0;
+  bool use_graph = true; cudaGraphExec_t graph_exec = nullptr;
   std::vector<void *> allocs;
   Net net[2];                                              // [0] online, [1] target
   // replay ring
@@ -79,11 +81,6 @@ static int dalloc(mig_dqn *d, void **p, size_t bytes) {
 
 template <int BN>
 static int launch_gemm(mig_dqn *d, const CUtensorMap &ma, const CUtensorMap &mb, const GemmArgs &g, uint32_t splits, cudaStream_t st) {
-  static bool attr_done[8] = {false, false, false, false, false, false, false, false};
-  if (d->device >= 0 && d->device < 8 && !attr_done[d->device]) {
-    CUD(cudaFuncSetAttribute(gemm_tf32x3_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<BN>::kBytes));
-    attr_done[d->device] = true;
-  }
   GemmArgs ga = g; ga.splits = splits;
   const uint32_t n_tiles = ((g.M + kGemmBM - 1) / kGemmBM) * (g.N / BN) * splits;
   const uint32_t grid = n_tiles < (uint32_t)d->n_sm ? n_tiles : (uint32_t)d->n_sm;          // persistent: one CTA per SM walks the tiles
@@ -102,6 +99,7 @@ static GemmArgs gargs(uint32_t M, uint32_t N, uint32_t K) {
 extern "C" int mig_dqn_destroy(mig_dqn_t *d) {
   if (!d) return MIG_OK;
   cudaDeviceSynchronize();
+  if (d->graph_exec) cudaGraphExecDestroy(d->graph_exec);
   for (void *p : d->allocs) cudaFree(p);
   cudaGetLastError();
   delete d;
@@ -123,6 +121,7 @@ extern "C" int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1,
   mig_dqn *d = new (std::nothrow) mig_dqn();
   if (!d) return mig_fail(MIG_ENOMEM, "dqn_create: host allocation failed");
   cudaGetDevice(&d->device);
+  { const char *ng = getenv("MIG_DQN_NO_GRAPH"); d->use_graph = !(ng && ng[0] == '1'); }
   cudaDeviceGetAttribute(&d->n_sm, cudaDevAttrMultiProcessorCount, d->device);
   const uint32_t H = hidden, A = n_actions, B = batch, P = kDqnApad;
   d->H = H; d->A = A; d->B = B; d->cap = replay_capacity; d->gamma = gamma; d->lr = lr; d->seed = seed;
@@ -154,6 +153,10 @@ extern "C" int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1,
   }
   if (!ok || cudaDeviceSynchronize() != cudaSuccess) { mig_dqn_destroy(d); return mig_fail(MIG_ECUDA, "dqn_create: weight upload failed: %s", cudaGetErrorString(cudaGetLastError())); }
   int rc = MIG_OK;
+  if (cudaFuncSetAttribute(gemm_tf32x3_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<128>::kBytes) != cudaSuccess ||
+      cudaFuncSetAttribute(gemm_tf32x3_kernel<kDqnApad>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<kDqnApad>::kBytes) != cudaSuccess) {
+    mig_dqn_destroy(d); return mig_fail(MIG_ECUDA, "dqn_create: %d bytes of shared memory per CTA refused (%s)", GemmSmem<128>::kBytes, cudaGetErrorString(cudaGetLastError()));
+  }
 #define MAP(m, ptr, inner, rows, ld, box) if (!rc) rc = make_map(&d->m, ptr, inner, rows, ld, box)
   MAP(mX, d->X, 64, B, 64, 128); MAP(mH1, d->H1, H, B, H, 128); MAP(mH2, d->H2, H, B, H, 128);
   MAP(mX2, d->X2, 64, B, 64, 128); MAP(mT1, d->T1, H, B, H, 128); MAP(mT2, d->T2, H, B, H, 128);
@@ -188,8 +191,15 @@ static int forward(mig_dqn *d, int which, cudaStream_t st) {
   return launch_gemm<kDqnApad>(d, which ? d->mT2 : d->mH2, d->mW3t[which], g, 1, st);
 }
 
+static int on_device(const mig_dqn *d) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != d->device) return mig_fail(MIG_ESTATE, "dqn: the handle lives on device %d but device %d is current", d->device, dev);
+  return MIG_OK;
+}
+
 extern "C" int mig_dqn_q(mig_dqn_t *d, int which, const float *state, uint32_t n, float *q_out, void *stream) {
   if (!d || !state || !q_out) return mig_fail(MIG_EINVAL, "dqn_q: NULL argument");
+  if (int rcd = on_device(d)) return rcd;
   if (n < 1 || n > d->B) return mig_fail(MIG_EINVAL, "dqn_q: n = %u not in 1..batch (%u)", n, d->B);
   cudaStream_t st = (cudaStream_t)stream;
   float *X = which ? d->X2 : d->X;
@@ -202,7 +212,9 @@ extern "C" int mig_dqn_q(mig_dqn_t *d, int which, const float *state, uint32_t n
 }
 
 // ------------------------------------------------------------------------------------------------ one training step
-static int train_on_batch(mig_dqn *d, float *loss_out, cudaStream_t st) {
+// forward of both networks, TD error, backward, SGD on the batch that the gather kernel left in X / X2 / a / r / done:
+// fifteen launches, always with the same arguments (the loss lands in d->loss)
+static int train_kernels(mig_dqn *d, cudaStream_t st) {
   const uint32_t H = d->H, B = d->B, P = kDqnApad, S = d->splits;
   int rc;
   if ((rc = forward(d, 0, st)) || (rc = forward(d, 1, st))) return rc;
@@ -228,7 +240,7 @@ static int train_on_batch(mig_dqn *d, float *loss_out, cudaStream_t st) {
   UpdateArgs u; memset(&u, 0, sizeof(u));
   u.lr = d->lr; u.B = B; u.n_splits = S;
   u.W = n.W3; u.Wt = n.W3t; u.rows = H; u.cols = P; u.ldw = P; u.ldt = H; u.partial = d->pW3; u.split_stride = (size_t)H * P; u.ldp = P;
-  u.bias = n.b3; u.dZt = d->dQt; u.n_bias = P; u.lossrow = d->lossrow; u.loss_out = loss_out ? loss_out : d->loss;
+  u.bias = n.b3; u.dZt = d->dQt; u.n_bias = P; u.lossrow = d->lossrow; u.loss_out = d->loss;
   dqn_update_kernel<<<u.rows + u.n_bias + 1, 256, 0, st>>>(u);
   u.loss_out = nullptr; u.lossrow = nullptr;
   u.W = n.W2; u.Wt = n.W2t; u.rows = H; u.cols = H; u.ldw = H; u.ldt = H; u.partial = d->pW2; u.split_stride = (size_t)H * H; u.ldp = H;
@@ -239,6 +251,37 @@ static int train_on_batch(mig_dqn *d, float *loss_out, cudaStream_t st) {
   dqn_update_kernel<<<u.rows + u.n_bias, 256, 0, st>>>(u);
   CUD(cudaGetLastError()); d->launches += 3;
   return MIG_OK;
+}
+
+// The fifteen launches are captured ONCE into a CUDA graph (their arguments never change) and replayed with one
+// cudaGraphLaunch per step: at batch 8192 the step is launch-bound without it.  MIG_DQN_NO_GRAPH=1 in the environment
+// launches the kernels one by one instead (profiling by kernel name).
+static int train_on_batch(mig_dqn *d, float *loss_out, cudaStream_t st) {
+  int rc = MIG_OK;
+  if (!d->use_graph) rc = train_kernels(d, st);
+  else {
+    if (!d->graph_exec) {
+      cudaStream_t cs = nullptr; cudaGraph_t g = nullptr;
+      CUD(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+      const uint64_t l0 = d->launches, g0 = d->gemm_launches;
+      cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+      if (e == cudaSuccess) {
+        rc = train_kernels(d, cs);
+        e = cudaStreamEndCapture(cs, &g);
+        if (e == cudaSuccess && !rc) e = cudaGraphInstantiate(&d->graph_exec, g, 0);
+      }
+      if (g) cudaGraphDestroy(g);
+      cudaStreamDestroy(cs);
+      d->kernels_per_step = d->launches - l0; d->gemms_per_step = d->gemm_launches - g0;
+      d->launches = l0; d->gemm_launches = g0;                 // (capturing launched nothing)
+      if (rc) return rc;
+      if (e != cudaSuccess) { d->graph_exec = nullptr; return mig_fail(MIG_ECUDA, "dqn: capturing the training step into a CUDA graph failed: %s", cudaGetErrorString(e)); }
+    }
+    CUD(cudaGraphLaunch(d->graph_exec, st));
+    d->launches += d->kernels_per_step; d->gemm_launches += d->gemms_per_step;     // kernels executed, one graph launch
+  }
+  if (!rc && loss_out) CUD(cudaMemcpyAsync(loss_out, d->loss, sizeof(float), cudaMemcpyDeviceToDevice, st));
+  return rc;
 }
 
 static int gather(mig_dqn *d, const float *S, const uint8_t *A, const float *R, const float *S2, const uint8_t *D, uint32_t size, uint32_t step,
@@ -254,6 +297,7 @@ static int gather(mig_dqn *d, const float *S, const uint8_t *A, const float *R, 
 extern "C" int mig_dqn_train_step(mig_dqn_t *d, uint32_t step, float *loss_out, void *stream) {
   if (!d) return mig_fail(MIG_EINVAL, "dqn_train_step: NULL handle");
   if (d->size == 0) return mig_fail(MIG_ESTATE, "dqn_train_step: the replay buffer is empty");
+  if (int rcd = on_device(d)) return rcd;
   int rc = gather(d, d->rS, d->rA, d->rR, d->rS2, d->rD, d->size, step, 0, (cudaStream_t)stream);
   return rc ? rc : train_on_batch(d, loss_out, (cudaStream_t)stream);
 }
@@ -261,6 +305,7 @@ extern "C" int mig_dqn_train_step(mig_dqn_t *d, uint32_t step, float *loss_out, 
 extern "C" int mig_dqn_train_on(mig_dqn_t *d, const float *s, const uint8_t *a, const float *r, const float *s2, const uint8_t *done,
                                 float *loss_out, void *stream) {
   if (!d || !s || !a || !r || !s2) return mig_fail(MIG_EINVAL, "dqn_train_on: NULL argument");
+  if (int rcd = on_device(d)) return rcd;
   int rc = gather(d, s, a, r, s2, done, d->B, 0, 1, (cudaStream_t)stream);
   return rc ? rc : train_on_batch(d, loss_out, (cudaStream_t)stream);
 }
