@@ -311,6 +311,33 @@ def test_env_base_sharding_is_placement_invariant():
         sim.close()
 
 
+def test_both_kernel_bodies_give_the_same_days():
+    # The thread-per-environment kernel has two bodies: one with the laxity algorithms compiled out, taken when the whole
+    # batch runs deadline-keyed algorithms (EDF-FS, EDF-SS, restricted EDF-SS), and the generic one.  The same 96 envs are
+    # run alone (short body) and next to one LLF env (generic body); the step API and the rollout are both exercised.
+    if B.DEFAULT_TILE not in (0, 1):
+        pytest.skip("thread-per-environment kernel only")
+    n = 96
+    wl = W.config_c3(n + 1)
+    algo = np.concatenate([np.array([0, 1, 4] * (n // 3), np.uint8), [2]]).astype(np.uint8)      # the last env runs LLF
+    out = []
+    for m in (n, n + 1):
+        sim = B.MigSim(wl.params, m, wl.seed)
+        recs, tot = sim.alloc_recs(), sim.alloc_totals()
+        sim.reset(0, dev(algo[:m]), dev(wl.cfg0[:m]))
+        acts = [dev(wl.table[:m, k, 0].copy()) for k in range(3)]
+        for k in range(3):                                     # three epochs through mig_sim_step, the rest through the rollout
+            sim.step(acts[k])
+        sim.rollout(wl.policy, table=dev(wl.table[:m]), recs_out=recs, totals_out=tot)
+        torch.cuda.synchronize()
+        out.append((B.recs_to_numpy(recs)[3:, :n].copy(), B.totals_to_numpy(tot)[:n].copy()))
+        sim.close()
+    assert out[0][1].tobytes() == out[1][1].tobytes() and out[0][0].tobytes() == out[1][0].tobytes()
+    for e in (0, 1, 2, 50):
+        r = O.rollout(wl.params, wl.seed, e, algo=int(algo[e]), cfg0=int(wl.cfg0[e]), policy=wl.policy, table=wl.table[e])
+        assert out[0][1][e].tobytes() == r.totals.tobytes()
+
+
 def _oracle_custom(args):
     sp, seed, e, algo, cfg0, table = args
     r = O.rollout(sp, seed, e, algo=algo, cfg0=cfg0, policy=W.POLICY_TABLE, table=table, trace_cap=400000, want_states=True)
