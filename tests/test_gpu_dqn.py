@@ -65,7 +65,7 @@ def test_tensor_core_forward_matches_double(hidden, n, A):
     d.close(); qn.close()
 
 
-@pytest.mark.parametrize("hidden,batch,A,steps", [(256, 128, 12, 3), (256, 1024, 12, 4), (128, 512, 7, 3), (256, 8192, 12, 2)])
+@pytest.mark.parametrize("hidden,batch,A,steps", [(256, 128, 12, 3), (256, 1024, 12, 4), (128, 512, 7, 3), (256, 8192, 12, 2), (256, 4224, 12, 2), (128, 896, 16, 2)])
 def test_training_steps_match_the_oracle(hidden, batch, A, steps):
     net = W.make_qnet(31, n_actions=A, hidden=hidden)
     gamma, lr = 0.9, 0.05
