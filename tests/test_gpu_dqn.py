@@ -177,3 +177,15 @@ def test_boundary_errors():
     with pytest.raises(B.MigError):
         d.q(torch.zeros((256, 64), dtype=torch.float32, device="cuda"))               # more rows than the batch
     d.close()
+
+
+def test_training_loop_runs_end_to_end():
+    # paper_2606_25082_b200/dqn_loop.py: simulated days -> replay ring -> tensor-core training -> the next day's decisions
+    import dataclasses
+    from paper_2606_25082_b200 import dqn_loop
+    sp = dataclasses.replace(W.benchmark_params(jobs_per_day=600.0), w_energy=1e-9, w_tardy=1e-5, util_hist=0)
+    net0 = W.make_qnet(77, n_actions=sp.n_configs, hidden=128)
+    net1, hist = dqn_loop.train(sp, net0, 256, 2, batch=1024, steps_per_epoch=1, lr=0.01)
+    assert len(hist) == 2 and all(np.isfinite(list(h.values())).all() for h in hist)
+    assert hist[0]["repartitions"] > 1 and hist[0]["energy_mj"] > 0
+    assert np.abs(flat(net1) - flat(net0)).max() > 1e-5
