@@ -106,8 +106,7 @@ typedef struct {
                                  * moment) after every tick of the day in which a job arrived or completed; a different
                                  * configuration is a repartition at that tick ("re-partitioning can happen when a
                                  * job arrives or is completed"; reading #27).  Ignored by mig_sim_step. */
-  /* ---- extensions; all 0 / NULL = off.  Implemented by the thread-per-environment kernel
-   * (mig_sim_set_tile(s, 1), the default): with any of them in use the warp-tile kernels are refused (MIG_EINVAL). */
+  /* ---- extensions; all 0 / NULL = off.  Implemented by both kernel families (mig_sim_set_tile). */
   const uint32_t *speed_nomig;  /* [n_classes] work units per second on the whole GPU with MIG disabled (size code 8), or NULL */
   int32_t p_idle_nomig_mw;      /* idle / busy power of the MIG-disabled GPU */
   int32_t p_busy_nomig_mw;

@@ -97,11 +97,6 @@ extern "C" int mig_debug_div_magic(uint32_t v, uint32_t *m, uint32_t *sh) {
 static int size_index(int g) { return g == 1 ? 0 : g == 2 ? 1 : g == 3 ? 2 : g == 4 ? 3 : g == 7 ? 4 : -1; }
 constexpr int kPolicyExplicit = 4;   // internal: the launch's actions come from SimArgs::actions
 
-// true if the parameter set needs what only the thread-per-environment kernel implements (readings #29-#32)
-static bool uses_extensions(const mig_params_t &p) {
-  return p.speed_nomig || p.repart_all_down || p.util_hist || p.n_tbins || p.n_dbins || p.n_abins;
-}
-
 static int build_tables(const mig_params_t *p, DevTables *t) {
   memset(t, 0, sizeof(*t));
   if (!p->speed || !p->dur7_q || !p->class_cum || !p->slack_q10 || !p->size_at_slot || !p->accept_thr)
@@ -226,9 +221,6 @@ static const void *kernel_ptr(int tile, bool evd = false) {
 // shared-memory footprint and resident grid for `tile` lanes per environment (1 = one thread per environment)
 static int configure_tile(mig_sim *s, int tile) {
   if (tile != 1 && tile != 8 && tile != 16 && tile != 32) return fail(MIG_EINVAL, "set_tile: lanes per environment must be 1, 8, 16 or 32 (got %d)", tile);
-  if (tile != 1 && uses_extensions(s->p))
-    return fail(MIG_EINVAL, "set_tile: this parameter set uses an extension (MIG-disabled GPU, whole-GPU repartition, utilisation levels, binned policy) "
-                            "that only the thread-per-environment kernel implements (lanes per environment = 1)");
   const uint32_t cap4 = (s->p.cap + 3u) & ~3u, cap8 = (s->p.cap + 7u) & ~7u;
   uint32_t entries; size_t bytes; int threads;
   if (tile == 1) {
@@ -531,7 +523,7 @@ extern "C" int mig_sim_rollout(mig_sim_t *s, int policy, const uint8_t *table, c
   if (s->epoch >= s->p.n_epochs) return fail(MIG_ESTATE, "rollout: the day is over; call reset");
   if (policy != MIG_POLICY_STATIC && policy != MIG_POLICY_TABLE && policy != MIG_POLICY_DQN && policy != MIG_POLICY_BINNED) return fail(MIG_EINVAL, "rollout: unknown policy %d", policy);
   if ((policy == MIG_POLICY_TABLE || policy == MIG_POLICY_BINNED) && !table) return fail(MIG_EINVAL, "rollout: TABLE / BINNED policy needs a table");
-  if (policy == MIG_POLICY_BINNED && (!s->p.n_tbins || s->tile != 1)) return fail(MIG_EINVAL, "rollout: the BINNED policy needs n_tbins / n_dbins / n_abins at create and the thread-per-environment kernel");
+  if (policy == MIG_POLICY_BINNED && !s->p.n_tbins) return fail(MIG_EINVAL, "rollout: the BINNED policy needs n_tbins / n_dbins / n_abins at create");
   cudaStream_t st = (cudaStream_t)stream;
   const int ne = s->p.n_epochs;
   if (policy != MIG_POLICY_DQN) {
@@ -589,10 +581,9 @@ extern "C" int mig_sim_totals(mig_sim_t *s, mig_totals_t *totals_out, void *stre
 extern "C" int mig_sim_aux(mig_sim_t *s, float *return_out, int32_t *util_s_out, void *stream) {
   if (!s) return fail(MIG_EINVAL, "aux: NULL handle");
   if (s->epoch < 0) return fail(MIG_ESTATE, "aux: reset has not been called");
-  if (s->tile != 1) return fail(MIG_ESTATE, "aux: the discounted return and the utilisation levels are kept by the thread-per-environment kernel only");
   if (util_s_out && !s->p.util_hist) return fail(MIG_ESTATE, "aux: params.util_hist was 0 at create: the utilisation levels were not kept");
   if (!return_out && !util_s_out) return MIG_OK;
-  aux_kernel<<<(s->n_envs + 255) / 256, 256, 0, (cudaStream_t)stream>>>(s->d_hdr, s->n_envs, return_out, util_s_out);
+  aux_kernel<<<(s->n_envs + 255) / 256, 256, 0, (cudaStream_t)stream>>>(s->d_hdr, s->n_envs, s->tile != 1, return_out, util_s_out);
   CU(cudaGetLastError());
   s->launches++;
   return MIG_OK;
@@ -690,7 +681,7 @@ extern "C" int mig_sim_debug_trace(mig_sim_t *s, uint32_t env, int policy, const
   if (env >= s->n_envs) return fail(MIG_EINVAL, "debug_trace: env %u out of range", env);
   if (!actions && policy != MIG_POLICY_STATIC && policy != MIG_POLICY_TABLE && policy != MIG_POLICY_BINNED) return fail(MIG_EINVAL, "debug_trace: policy must be STATIC, TABLE or BINNED, or pass actions");
   if (!actions && policy != MIG_POLICY_STATIC && !table) return fail(MIG_EINVAL, "debug_trace: TABLE / BINNED policy needs a table");
-  if (!actions && policy == MIG_POLICY_BINNED && (!s->p.n_tbins || s->tile != 1)) return fail(MIG_EINVAL, "debug_trace: the BINNED policy needs n_tbins / n_dbins / n_abins at create and the thread-per-environment kernel");
+  if (!actions && policy == MIG_POLICY_BINNED && !s->p.n_tbins) return fail(MIG_EINVAL, "debug_trace: the BINNED policy needs n_tbins / n_dbins / n_abins at create");
   SimArgs a; base_args(s, a);
   a.n_envs = 1; a.env_first = env; a.tab_override = s->d_dbgtab; a.hdr_override = s->d_dbghdr;
   a.from_init = 1; a.save = 0; a.n_steps = s->p.n_epochs;

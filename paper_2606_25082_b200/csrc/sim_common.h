@@ -30,7 +30,7 @@ struct DevTables {
   uint32_t thr[MIG_THR_BINS];
   uint32_t logT[257];                        // round(2^24 log2(1 + i/256))
   int32_t curve[8], p_idle[12], p_busy[12];  // p_idle/p_busy indexed by SIZE (0..8; 8 = MIG disabled), not by size index
-  // extensions (thread-per-environment kernel only)
+  // extensions (readings #29, #31)
   uint4 speed_nomig[MIG_MAX_CLASSES];        // {v, magic, shift, 0} on the whole GPU with MIG disabled (size code 8)
   int32_t dbin_edges[8], abin_edges[8];      // BINNED policy: bin edges, padded with INT32_MAX
 };
@@ -58,13 +58,13 @@ struct SimArgs {
   int from_init;        // 1: initialise from algo/cfg0 (reset), 0: load the saved state
   int save;             // 1: write the state back
   int n_steps;          // epochs to run in this launch
-  int policy;           // 0 static, 1 table, 3 explicit actions
+  int policy;           // MIG_POLICY_STATIC / TABLE / BINNED, or explicit actions (a.actions)
   const uint8_t *algo, *cfg0;                        // from_init
   uint32_t *algo_mask;                               // thread-per-env kernel: bit i = some environment runs algorithm i (set by the reset launch)
   const uint8_t *table;                              // [n_envs][n_epochs][4]
   int ev_decide;                                     // TABLE policy: look the table up again after every tick with an arrival or a completion
   const uint8_t *actions; uint32_t act_stride_env, act_stride_k;   // action = actions[env * se + (k - k_first) * sk]
-  // extensions (thread-per-environment kernel only; readings #29-#32)
+  // extensions (readings #29-#32)
   const uint8_t *bin_table;                          // BINNED policy: [n_configs][n_tbins][B][B][B], one table for all envs
   uint32_t n_tbins, n_dbins, n_abins;
   int all_down;                                      // a repartition takes the whole GPU down

@@ -37,12 +37,16 @@ enum { WS_STAGE = 0, WS_CNT = 64, WS_TOT = 74 /* 3 x u64 */, WS_TBASE = 80 /* u6
 // saved per-env header (kHeaderWords words, a.hdr): word indices
 enum { H_UPAT = 0 /* 7 */, H_T = 7, H_PK, H_NSYS, H_HLO, H_HHI, H_GKBASE, H_TBASE_LO, H_TBASE_HI, H_GPENDING, H_NACC, H_GDONE,
        H_ISCRIPT, H_DROPS, H_TOT /* 6 */, H_LOOKV = 26, H_LOOKTICK, H_LOOKCLS, H_LOOKWORK, H_LOOKDUE, H_LOOKID,
-       H_SLICE = 32 /* 7 */, H_GK = 39, H_GT_LO, H_GT_HI, H_CNT = 48 /* 10 */ };
+       H_SLICE = 32 /* 7 */, H_GK = 39, H_GT_LO, H_GT_HI, H_UTIL_HI = 42 /* 2: utilisation levels 6, 7 */,
+       H_RET = 44 /* discounted return so far, fp32 bits */, H_DISC /* gamma^k, fp32 bits */, H_CNT = 48 /* 10 */,
+       H_UTIL_LO = 58 /* 6: seconds at utilisation levels 0..5 */ };
+__host__ __device__ constexpr int tile_util_word(int level) { return level < 6 ? H_UTIL_LO + level : H_UTIL_HI + level - 6; }
 
 struct HotTables {               // per CTA, shared memory
   uint4 speed[MIG_MAX_CLASSES * 5];
+  uint4 speed_nomig[MIG_MAX_CLASSES];   // size code 8: the whole GPU with MIG disabled (reading #29)
   uint32_t cfg_pack[MIG_MAX_CONFIGS];
-  int32_t curve[8], p_idle[8], p_busy[8];
+  int32_t curve[8], p_idle[12], p_busy[12];
 };
 
 __host__ __device__ constexpr size_t tile_smem_bytes(uint32_t smem_entries) {
@@ -51,6 +55,7 @@ __host__ __device__ constexpr size_t tile_smem_bytes(uint32_t smem_entries) {
 }
 
 __device__ __forceinline__ int sidx_of(int size) { return size == 7 ? 4 : size - 1; }   // 1,2,3,4,7 -> 0..4
+__device__ __forceinline__ int tile_units_of(int size) { return min(size, 7); }         // compute units: size code 8 is the whole GPU
 
 // ceil(rem / v) for 0 < rem, rem + v - 1 < 2^31, by the precomputed magic number of v (exact; see mig_debug_div_magic)
 __device__ __forceinline__ int rd_magic(int rem, uint4 sp) {
@@ -130,7 +135,9 @@ struct Env {
   uint32_t g_kbase;                                                      // base candidate index of the CURRENT batch
   int look_valid, look_tick, look_work, look_due; uint32_t look_cls, look_id;
   uint32_t n_trace, i_script;
+  float ret_acc, disc;     // discounted return so far and gamma^epoch (reading #32)
   // per lane
+  uint32_t util_acc;       // tile lane u < 8: seconds spent with u compute units busy
   uint32_t cntA, cntB;     // counters of the current record span (see C_*)
   int g_tick, g_work, g_due; uint32_t g_cls;                             // this lane's candidate of the current batch
   int sl_size, sl_down, sl_upat, sl_pos, sl_rank;                        // slice starting at slot `gl` (gl < 7)
@@ -191,7 +198,10 @@ struct Env {
 
   // ------------------------------------------------------------------ model
   __device__ __forceinline__ int size_at(int p) const { return (cfg_sizes >> (4 * (p & 7))) & 15; }
-  __device__ __forceinline__ int rd(int rem, uint32_t cls, int size) const { return rd_magic(rem, hot.speed[cls * 5 + sidx_of(size)]); }
+  __device__ __forceinline__ const uint4 &speed_of(uint32_t cls, int size) const {
+    return size == MIG_SIZE_NOMIG ? hot.speed_nomig[cls] : hot.speed[cls * 5 + sidx_of(size)];
+  }
+  __device__ __forceinline__ int rd(int rem, uint32_t cls, int size) const { return rd_magic(rem, speed_of(cls, size)); }
 
   // remaining duration against the configuration: fastest slice (LLF) or floor of the mean over all
   // slices of cfg, up or down (LALF; also the state vector's "average duration", L210).  Per-lane loop.
@@ -213,7 +223,7 @@ struct Env {
   __device__ __forceinline__ void update_power(bool pred) {
     bool busy = sl_pos >= 0;
     int c = sl_size ? (busy ? hot.p_busy[sl_size] : hot.p_idle[sl_size]) : 0;
-    int u = busy ? sl_size : 0;
+    int u = busy ? tile_units_of(sl_size) : 0;
     int Un = T::tadd(u);
     int Pn = T::tadd(c) + hot.curve[Un & 7];
     if (pred) { U = Un; P = Pn; }
@@ -369,7 +379,7 @@ struct Env {
       const uint32_t cls = (km.y >> 20) & 15u, id = km.y & kIdMask;
       const int rem = (int)rdv.x, due = (int)rdv.y;
       int r = MIG_INF >> 3;
-      if (open && up) r = rd_magic(rem, hot.speed[cls * 5 + sidx_of(sl_size)]);
+      if (open && up) r = rd_magic(rem, speed_of(cls, sl_size));
       const bool on_time = r <= due - t;
       const bool is_free = open && up && sl_pos < 0;
       const bool later = open && up && sl_pos >= 0 && (rj_due > due || (rj_due == due && rj_id > id));
@@ -392,7 +402,7 @@ struct Env {
       if (st && gl == s) {
         *entry_word(b, 1) = (km.y & ~(7u << 28)) | ((uint32_t)(s + 1) << 28);
         sl_pos = (int)b; rj_id = id; rj_rem = rem; rj_due = due;
-        rj_v = hot.speed[cls * 5 + sidx_of(sl_size)].x;
+        rj_v = speed_of(cls, sl_size).x;
         rj_ctime = t + r;
       }
       __syncwarp();
@@ -449,7 +459,7 @@ struct Env {
       // --- slice choice by the slice lanes: one composite key per rule, (r, rank) unique per lane
       const bool mine = act && ((avail >> gl) & 1u);
       int r = MIG_INF >> 3;
-      if (mine) r = rd_magic((int)rdv.x, hot.speed[cls * 5 + sidx_of(sl_size)]);
+      if (mine) r = rd_magic((int)rdv.x, speed_of(cls, sl_size));
       const int fs = mine ? ((r << 3) | sl_rank) : MIG_INF;                                    // fastest; ties -> smaller size, lower slot (reading #4)
       const int ss = (mine && r <= (int)rdv.y - t) ? ((r << 3) | (7 - sl_rank)) : -1;          // slowest that meets the deadline; same ties
       const int fsb = T::tmin(fs), ssb = T::tmax(ss);
@@ -493,7 +503,7 @@ struct Env {
       sl_pos = new_pos;
       if (new_pos >= 0) {
         rj_id = new_id; rj_rem = new_rem; rj_due = new_due;
-        rj_v = hot.speed[new_cls * 5 + sidx_of(sl_size)].x;
+        rj_v = speed_of(new_cls, sl_size).x;
         rj_ctime = t + new_r;
       }
     }
@@ -529,6 +539,7 @@ struct Env {
       const int dt = running ? tn - t : 0;
       e_ep += (long long)P * dt;
       busy_ep += (long long)U * dt;
+      if (a.util_hist && gl == U) util_acc += (uint32_t)dt;     // time at this utilisation level (Fig. 6)
       if (sl_pos >= 0 && dt) { rj_rem -= dt * (int)rj_v; *entry_word((uint32_t)sl_pos, 2) = (uint32_t)rj_rem; }
       t += dt;
       __syncwarp();
@@ -610,7 +621,9 @@ struct Env {
       if (a.ev_decide && !drain) {                            // event-driven decision (reading #27)
         const bool dec = running && job_event;
         uint32_t action = (uint32_t)cfg;
-        if (dec) {
+        if (a.policy == MIG_POLICY_BINNED) {                  // the paper's binned 2+2m state (L210); every lane takes part
+          if (MIG_ANY(dec)) { const uint32_t bi = binned_index(); if (dec) action = a.bin_table[bi]; }
+        } else if (dec) {
           const uint32_t b = n_sys == 0 ? 0u : (n_sys < 8 ? 1u : (n_sys < 64 ? 2u : 3u));
           action = a.table[((size_t)env_l * a.n_epochs + epoch) * 4 + b];
         }
@@ -637,7 +650,8 @@ struct Env {
   __device__ __forceinline__ void repartition(const bool rp, uint32_t action) {
     const uint32_t newsizes = hot.cfg_pack[action & (MIG_MAX_CONFIGS - 1)];
     const int mynew = gl < kSlots ? (int)((newsizes >> (4 * gl)) & 15u) : 0;
-    const bool destroyed = rp && sl_size && sl_size != mynew;
+    const bool redo = sl_size != mynew || (a.all_down && (sl_size || mynew));   // the whole GPU goes down (reading #30)
+    const bool destroyed = rp && sl_size && redo;
     uint32_t pm = T::tballot(destroyed && sl_pos >= 0, gshift);
     count<C_PREEMPT>(__popc(pm));
     while (MIG_ANY(pm != 0u)) {                               // jobs on destroyed slices go back to waiting
@@ -647,7 +661,7 @@ struct Env {
       pm &= pm - 1;
     }
     if (destroyed && sl_pos >= 0) { *entry_word((uint32_t)sl_pos, 1) &= ~(7u << 28); sl_pos = -1; }
-    if (rp && sl_size != mynew) {                             // same (start, size) in both rows keeps job and up_at
+    if (rp && redo) {                                         // same (start, size) in both rows keeps job and up_at
       sl_size = mynew; sl_pos = -1; sl_down = 0; sl_upat = 0;
       if (mynew && a.downtime_s > 0) { sl_down = 1; sl_upat = t + a.downtime_s; }
     }
@@ -741,7 +755,7 @@ struct Env {
     const uint32_t n_run = __popc(T::tballot(sl_pos >= 0, gshift));
     if (gl < kSlots) {
       const float occ = sl_down ? 0.5f : (sl_pos >= 0 ? 1.0f : 0.0f);
-      for (int q = 0; q < sl_size; ++q) st[16 + gl + q] = __float_as_uint(occ);        // slots covered by this slice
+      for (int q = 0; q < tile_units_of(sl_size); ++q) st[16 + gl + q] = __float_as_uint(occ);        // slots covered by this slice
       st[23 + gl] = __float_as_uint((float)sl_size * 0.125f);
     }
     if (gl == 7 % G) {
@@ -755,30 +769,67 @@ struct Env {
 #pragma unroll 1
     for (int m = 0; m < 3; ++m) {                               // first m = 3 jobs in (due, id) order
       const bool act = (uint32_t)m < n_sys;
-      int bk = MIG_INF; uint32_t bid = 0xFFFFFFFFu; int bi = -1;
-      if (act)
-        for (uint32_t i = gl; i < n_sys; i += G) {
-          int due = (int)ld_rd(i).y; uint32_t id = ld_km(i).y & kIdMask;
-          bool beyond = due > pk || (due == pk && id > pid);
-          bool better = due < bk || (due == bk && id < bid);
-          if (beyond && better) { bk = due; bid = id; bi = (int)i; }
-        }
-      const int mk = T::tmin(bk);
-      const uint32_t mid = T::tminu((bi >= 0 && bk == mk) ? bid : 0xFFFFFFFFu);
-      const int wl = __ffs((int)T::tballot(bi >= 0 && bk == mk && bid == mid, gshift)) - 1;
-      const uint32_t b = (uint32_t)T::tshfl(bi, wl);
+      const uint32_t b = next_by_due(act, pk, pid);
       if (act) {
         uint2 km = ld_km(b), rdv = ld_rd(b);
         int d = max(-32768, min(32767, (int)rdv.y - t));
         int mean = min(rd_cfg((int)rdv.x, (km.y >> 20) & 15u, true), 32767);
         if (gl == 0) { st[56 + m] = __float_as_uint((float)d * (1.0f / 4096.0f)); st[59 + m] = __float_as_uint((float)mean * (1.0f / 4096.0f)); }
-        pk = mk; pid = mid;
       }
     }
     __syncwarp();
     if (alive)
       for (int w = gl; w < MIG_STATE_DIM; w += G) out[w] = __uint_as_float(st[w]);
     __syncwarp();
+  }
+  // tiles with act: entry index of the job that follows (pk, pid) in (due, id) order over all jobs in system (running and
+  // waiting); advances (pk, pid).  One tile argmin; every lane of the warp executes it.
+  __device__ __forceinline__ uint32_t next_by_due(bool act, int &pk, uint32_t &pid) {
+    int bk = MIG_INF; uint32_t bid = 0xFFFFFFFFu; int bi = -1;
+    if (act)
+      for (uint32_t i = gl; i < n_sys; i += G) {
+        int due = (int)ld_rd(i).y; uint32_t id = ld_km(i).y & kIdMask;
+        bool beyond = due > pk || (due == pk && id > pid);
+        bool better = due < bk || (due == bk && id < bid);
+        if (beyond && better) { bk = due; bid = id; bi = (int)i; }
+      }
+    const int mk = T::tmin(bk);
+    const uint32_t mid = T::tminu((bi >= 0 && bk == mk) ? bid : 0xFFFFFFFFu);
+    const int wl = __ffs((int)T::tballot(bi >= 0 && bk == mk && bid == mid, gshift)) - 1;
+    const uint32_t b = (uint32_t)T::tshfl(bi, wl);
+    if (act) { pk = mk; pid = mid; }
+    return b;
+  }
+
+  // ------------------------------------------------------------------ binned state (reading #31)
+  // index of the present state in the BINNED policy's table: configuration, time bin, and for each of the first m = 3 jobs
+  // in (due, id) order the code 0 (no such job) or 1 + dbin * n_abins + abin of its deadline (due - t) and its mean
+  // remaining duration over the slices of the configuration.  Tile-uniform; every lane of the warp executes it.
+  static __device__ __forceinline__ uint32_t bin_of(int v, const int32_t *edges, uint32_t n_bins) {
+    uint32_t b = 0;
+    while (b + 1u < n_bins && v >= __ldg(&edges[b])) ++b;
+    return b;
+  }
+  __device__ __forceinline__ uint32_t binned_index() {
+    const uint32_t B = 1u + a.n_dbins * a.n_abins;
+    const uint32_t tc = (uint32_t)min(t, a.day_s - 1);
+    uint32_t idx = (uint32_t)cfg * a.n_tbins + (tc * a.n_tbins) / (uint32_t)a.day_s;
+    int pk = (int)0x80000000; uint32_t pid = 0;
+    __syncwarp();
+#pragma unroll 1
+    for (uint32_t m = 0; m < 3u; ++m) {
+      const bool act = m < n_sys;
+      const uint32_t b = next_by_due(act, pk, pid);
+      uint32_t code = 0;
+      if (act) {
+        const uint2 km = ld_km(b), rdv = ld_rd(b);
+        const uint32_t db = bin_of((int)rdv.y - t, a.tab->dbin_edges, a.n_dbins);
+        const uint32_t ab = bin_of(rd_cfg((int)rdv.x, (km.y >> 20) & 15u, true), a.tab->abin_edges, a.n_abins);
+        code = 1u + db * a.n_abins + ab;
+      }
+      idx = idx * B + code;
+    }
+    return idx;
   }
 
   // ------------------------------------------------------------------ init / load / save
@@ -806,6 +857,7 @@ struct Env {
     g_k = 0; g_T = 0; g_pending = 0; n_accepted = 0; g_done = 0; g_kbase = 0;
     look_valid = 0; look_tick = 0; look_work = 0; look_due = 0; look_cls = 0; look_id = 0;
     next_crit = MIG_INF; n_trace = 0; i_script = 0; P = 0; U = 0;
+    util_acc = 0; ret_acc = 0.0f; disc = 1.0f;
     __syncwarp();
     for (int w = gl; w < WS_WORDS; w += G) ws[w] = 0;
     __syncwarp();
@@ -829,9 +881,11 @@ struct Env {
       st[H_LOOKV] = (uint32_t)look_valid; st[H_LOOKTICK] = (uint32_t)look_tick; st[H_LOOKCLS] = look_cls;
       st[H_LOOKWORK] = (uint32_t)look_work; st[H_LOOKDUE] = (uint32_t)look_due; st[H_LOOKID] = look_id;
       st[H_GK] = g_k; st[H_GT_LO] = (uint32_t)g_T; st[H_GT_HI] = (uint32_t)(g_T >> 32);
+      st[H_RET] = __float_as_uint(ret_acc); st[H_DISC] = __float_as_uint(disc);
 #pragma unroll
       for (int i = 0; i < C_COUNT; ++i) st[H_CNT + i] = ws[WS_CNT + i];
     }
+    if (gl < 8) st[tile_util_word(gl)] = util_acc;
     if (gl < kSlots) {
       st[H_UPAT + gl] = (uint32_t)sl_upat;
       st[H_SLICE + gl] = (uint32_t)sl_size | ((uint32_t)sl_down << 8) | ((uint32_t)(sl_pos + 1) << 16);
@@ -869,6 +923,8 @@ struct Env {
     look_valid = (int)st[H_LOOKV]; look_tick = (int)st[H_LOOKTICK]; look_cls = st[H_LOOKCLS];
     look_work = (int)st[H_LOOKWORK]; look_due = (int)st[H_LOOKDUE]; look_id = st[H_LOOKID];
     const uint32_t gk = st[H_GK];
+    ret_acc = __uint_as_float(st[H_RET]); disc = __uint_as_float(st[H_DISC]);
+    util_acc = gl < 8 ? st[tile_util_word(gl)] : 0u;
     const unsigned long long gT = (unsigned long long)st[H_GT_LO] | ((unsigned long long)st[H_GT_HI] << 32);
     cfg_sizes = hot.cfg_pack[cfg & (MIG_MAX_CONFIGS - 1)];
     sl_size = 0; sl_down = 0; sl_upat = 0; sl_pos = -1;
@@ -898,7 +954,7 @@ struct Env {
     if (gl == 0) { ws[WS_TBASE] = tb_lo; ws[WS_TBASE + 1] = tb_hi; }
     if (sl_pos >= 0) {                                       // running job: t + ceil(rem / v) never drifts
       uint2 km = ld_km((uint32_t)sl_pos), rdv = ld_rd((uint32_t)sl_pos);
-      uint4 sp = hot.speed[((km.y >> 20) & 15u) * 5 + sidx_of(sl_size)];
+      uint4 sp = speed_of((km.y >> 20) & 15u, sl_size);
       rj_id = km.y & kIdMask; rj_rem = (int)rdv.x; rj_due = (int)rdv.y; rj_v = sp.x;
       rj_ctime = t + rd_magic(rj_rem, sp);
     }
@@ -927,12 +983,15 @@ struct Env {
       close_record(a.drain_rec ? a.drain_rec + env_local : nullptr);
     }
     epoch = k + 1;
+    // reward: two fp32 products, one add, negate; no contraction
+    const float r = -__fadd_rn(__fmul_rn(a.w_energy, __ll2float_rn(dE)), __fmul_rn(a.w_tardy, __ll2float_rn(dT)));
     if (alive && gl == 0) {
       if (a.energy_out) a.energy_out[env_local] = dE;
       if (a.tard_out) a.tard_out[env_local] = dT;
-      if (a.reward_out)                                       // two fp32 products, one add, negate; no contraction
-        a.reward_out[env_local] = -__fadd_rn(__fmul_rn(a.w_energy, __ll2float_rn(dE)), __fmul_rn(a.w_tardy, __ll2float_rn(dT)));
+      if (a.reward_out) a.reward_out[env_local] = r;
     }
+    ret_acc = __fmaf_rn(disc, r, ret_acc);                    // discounted return (reading #32)
+    disc = __fmul_rn(disc, a.gamma);
   }
 };
 
@@ -946,7 +1005,9 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) sim_kernel(const SimArgs
     const DevTables *tb = a.tab;
     for (int i = threadIdx.x; i < MIG_MAX_CLASSES * 5; i += blockDim.x) hot.speed[i] = tb->speed[i];
     for (int i = threadIdx.x; i < MIG_MAX_CONFIGS; i += blockDim.x) hot.cfg_pack[i] = tb->cfg_pack[i];
-    if (threadIdx.x < 8) { hot.curve[threadIdx.x] = tb->curve[threadIdx.x]; hot.p_idle[threadIdx.x] = tb->p_idle[threadIdx.x]; hot.p_busy[threadIdx.x] = tb->p_busy[threadIdx.x]; }
+    for (int i = threadIdx.x; i < MIG_MAX_CLASSES; i += blockDim.x) hot.speed_nomig[i] = tb->speed_nomig[i];
+    if (threadIdx.x < 8) hot.curve[threadIdx.x] = tb->curve[threadIdx.x];
+    if (threadIdx.x < 12) { hot.p_idle[threadIdx.x] = tb->p_idle[threadIdx.x]; hot.p_busy[threadIdx.x] = tb->p_busy[threadIdx.x]; }
   }
   __syncthreads();
   const size_t per_tile = tile_smem_bytes(a.smem_entries);
@@ -971,6 +1032,8 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 4) sim_kernel(const SimArgs
       if (a.policy == MIG_POLICY_TABLE) {                                           // load bucket
         uint32_t b = e.n_sys == 0 ? 0u : (e.n_sys < 8 ? 1u : (e.n_sys < 64 ? 2u : 3u));
         action = a.table[((size_t)env * a.n_epochs + e.epoch) * 4 + b];
+      } else if (a.policy == MIG_POLICY_BINNED) {                                   // binned 2+2m state
+        action = a.bin_table[e.binned_index()];
       } else if (a.actions) {
         action = a.actions[(size_t)(e.alive ? li : 0u) * a.act_stride_env + (size_t)s * a.act_stride_k];
       }

@@ -1026,15 +1026,19 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
 }
 
 // per-env auxiliary results out of the saved headers: the discounted return and the seconds per utilisation level
-__global__ void aux_kernel(const uint32_t *hdr, uint32_t n_envs, float *ret_out, int32_t *util_out) {
+// (`tiled`: the header was written by the warp-tile kernels, whose layout differs)
+__global__ void aux_kernel(const uint32_t *hdr, uint32_t n_envs, int tiled, float *ret_out, int32_t *util_out) {
   const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= n_envs) return;
   const uint32_t *h = hdr + (size_t)e * kHeaderWords;
-  if (ret_out) ret_out[e] = __uint_as_float(h[H1_RET]);
+  if (ret_out) ret_out[e] = __uint_as_float(h[tiled ? (int)H_RET : (int)H1_RET]);
   if (util_out) {
+    int v[8];
+#pragma unroll
+    for (int l = 0; l < 8; ++l) v[l] = (int)h[tiled ? tile_util_word(l) : H1_UTIL + l];
     int4 *o = reinterpret_cast<int4 *>(util_out + (size_t)e * 8);
-    o[0] = make_int4((int)h[H1_UTIL], (int)h[H1_UTIL + 1], (int)h[H1_UTIL + 2], (int)h[H1_UTIL + 3]);
-    o[1] = make_int4((int)h[H1_UTIL + 4], (int)h[H1_UTIL + 5], (int)h[H1_UTIL + 6], (int)h[H1_UTIL + 7]);
+    o[0] = make_int4(v[0], v[1], v[2], v[3]);
+    o[1] = make_int4(v[4], v[5], v[6], v[7]);
   }
 }
 

@@ -1,8 +1,8 @@
 """GPU parity of the extensions (readings #29-#32): the CUDA path (through the C ABI) vs the
 oracle, bit for bit -- the MIG-disabled GPU as a configuration, the whole-GPU repartition penalty, the time per utilisation
 level, the discounted return, the BINNED policy (hourly and event-driven), the paper's benchmark policies (No-MIG, static
-configuration 3, day / night), the ET reduction.  These run on the thread-per-environment kernel (the library default);
-the warp-tile kernels refuse parameter sets that use them (tested).
+configuration 3, day / night), the ET reduction.  Every test runs on both kernel families: one thread per environment (the
+library default) and warp tiles of 8, 16 and 32 lanes per environment (mig_sim_set_tile).
 """
 import dataclasses
 
@@ -22,13 +22,15 @@ G1 = golden("handworked.json")
 B = None
 
 
-@pytest.fixture(scope="module", autouse=True)
-def _binding():
+@pytest.fixture(scope="module", autouse=True, params=[1, 8, 16, 32], ids=["thread", "tile8", "tile16", "tile32"])
+def _binding(request):
     global B
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
     from paper_2606_25082_b200 import binding
     B = binding
+    B.DEFAULT_TILE = request.param
     yield
+    B.DEFAULT_TILE = 0
 
 
 def dev(a):
@@ -200,9 +202,7 @@ def test_step_api_keeps_return_and_levels():
 def test_boundary_errors_of_the_extensions():
     sp = W.benchmark_params()
     sim = B.MigSim(sp, 4, 1)
-    with pytest.raises(B.MigError) as ei:
-        sim.set_tile(8)                                       # the warp tiles do not implement the extensions
-    assert ei.value.code == B.MIG_EINVAL
+    assert sim.get_tile() == B.DEFAULT_TILE
     with pytest.raises(B.MigError):
         sim.rollout(W.POLICY_BINNED, table=dev(np.zeros(16, np.uint8)))      # (reset not called / no bins)
     sim.close()
