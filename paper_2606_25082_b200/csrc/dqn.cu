@@ -21,9 +21,10 @@ using namespace migsim;
 
 namespace {
 
-struct Net {            // one network: master weights in the caller's layout [in][out] + the transposed copies the products read
-  float *W1, *W1t, *b1, *W2, *W2t, *b2, *W3, *W3t, *b3;      // W1 [64][H], W1t [H][64], W2 [H][H], W2t [H][H], W3 [H][16], W3t [16][H]
-};
+struct Net {            // one network: master weights in the caller's layout [in][out] + the copies the products read, kept split
+  float *W1, *W1t, *b1, *W2, *W2t, *b2, *W3, *W3t, *b3;      // W1 [64][H], W1t [2 H][64], W2 [H][H], W2t [2 H][H], W3 [H][16], W3t [2 x 16][H]
+  float *W2s, *W3s;                                          // W2s [2 H][H], W3s [2 H][16]: untransposed, for the backward products
+};                                                           // (split: TF32 high parts in the first half of the rows, remainders in the second)
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -54,7 +55,7 @@ int make_map(CUtensorMap *m, const float *ptr, uint64_t inner, uint64_t rows, ui
 }  // namespace
 
 struct mig_dqn {   // (mig_dqn_t of include/migsim.h)
-  uint32_t H = 0, A = 0, B = 0, cap = 0, splits = 1;
+  uint32_t H = 0, A = 0, B = 0, cap = 0, splits = 1, bn_h = 128;   // bn_h: tile width of the products with N = H
   float gamma = 0.0f, lr = 0.0f; uint64_t seed = 0;
   int device = 0, n_sm = 148;
   uint64_t launches = 0, gemm_launches = 0, kernels_per_step = 0, gemms_per_step = 0;
@@ -88,6 +89,12 @@ static int launch_gemm(mig_dqn *d, const CUtensorMap &ma, const CUtensorMap &mb,
   CUD(cudaGetLastError());
   d->launches++; d->gemm_launches++;
   return MIG_OK;
+}
+
+// the products whose N is the hidden width: one 128 x 256 tile per row block when the width allows it (a quarter less
+// shared-memory traffic per flop than two 128 x 128 tiles: the A tile is split and read once for twice the columns)
+static int launch_gemm_h(mig_dqn *d, const CUtensorMap &ma, const CUtensorMap &mb, const GemmArgs &g, uint32_t splits, cudaStream_t st) {
+  return d->bn_h == 256 ? launch_gemm<256>(d, ma, mb, g, splits, st) : launch_gemm<128>(d, ma, mb, g, splits, st);
 }
 
 static GemmArgs gargs(uint32_t M, uint32_t N, uint32_t K) {
@@ -125,11 +132,15 @@ extern "C" int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1,
   cudaDeviceGetAttribute(&d->n_sm, cudaDevAttrMultiProcessorCount, d->device);
   const uint32_t H = hidden, A = n_actions, B = batch, P = kDqnApad;
   d->H = H; d->A = A; d->B = B; d->cap = replay_capacity; d->gamma = gamma; d->lr = lr; d->seed = seed;
+  // 128 x 256 tiles once there are enough row blocks to keep every SM busy with them (measured: 0.402 -> 0.396 ms per step at
+  // batch 32768, 1.29 -> 1.24 at 131072; at 8192 the 64 wide tiles leave SMs idle: 0.163 -> 0.207); MIG_DQN_BN=128 / 256 overrides
+  { const char *e = getenv("MIG_DQN_BN"); const int f = e ? atoi(e) : 0; d->bn_h = (H == 256 && (f == 256 || (f != 128 && B >= 32768u))) ? 256 : 128; }
   d->splits = B / 128 < 32 ? B / 128 : 32;                  // split-K of the weight-gradient products: >= 4 k-blocks per split
   while ((B / kGemmBK) % d->splits) d->splits--;
   for (int k = 0; k < 2; ++k) {
     Net &n = d->net[k];
-    DA(n.W1, 64 * H); DA(n.W1t, H * 64); DA(n.b1, H); DA(n.W2, H * H); DA(n.W2t, H * H); DA(n.b2, H); DA(n.W3, H * P); DA(n.W3t, P * H); DA(n.b3, P);
+    DA(n.W1, 64 * H); DA(n.W1t, 2 * H * 64); DA(n.b1, H); DA(n.W2, H * H); DA(n.W2t, 2 * H * H); DA(n.b2, H); DA(n.W3, H * P); DA(n.W3t, 2 * P * H); DA(n.b3, P);
+    DA(n.W2s, 2 * H * H); DA(n.W3s, 2 * H * P);
   }
   DA(d->rS, (size_t)d->cap * 64); DA(d->rS2, (size_t)d->cap * 64); DA(d->rR, d->cap); DA(d->rA, d->cap); DA(d->rD, d->cap);
   DA(d->X, (size_t)B * 64); DA(d->X2, (size_t)B * 64); DA(d->Xt, (size_t)64 * B);
@@ -147,13 +158,14 @@ extern "C" int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1,
     Net &n = d->net[k];
     ok = up(n.W1, W1, 64, H, H) && up(n.b1, b1, 1, H, H) && up(n.W2, W2, H, H, H) && up(n.b2, b2, 1, H, H) && up(n.W3, W3, H, A, P) && up(n.b3, b3, 1, A, P);
     if (!ok) break;
-    dqn_transpose_kernel<<<(64 * H + 255) / 256, 256>>>(n.W1, n.W1t, 64, H, H, 64);
-    dqn_transpose_kernel<<<(H * H + 255) / 256, 256>>>(n.W2, n.W2t, H, H, H, H);
-    dqn_transpose_kernel<<<(H * P + 255) / 256, 256>>>(n.W3, n.W3t, H, P, P, H);
+    dqn_split_kernel<<<(64 * H + 255) / 256, 256>>>(n.W1, n.W1t, nullptr, 64, H, H, 64);
+    dqn_split_kernel<<<(H * H + 255) / 256, 256>>>(n.W2, n.W2t, n.W2s, H, H, H, H);
+    dqn_split_kernel<<<(H * P + 255) / 256, 256>>>(n.W3, n.W3t, n.W3s, H, P, P, H);
   }
   if (!ok || cudaDeviceSynchronize() != cudaSuccess) { mig_dqn_destroy(d); return mig_fail(MIG_ECUDA, "dqn_create: weight upload failed: %s", cudaGetErrorString(cudaGetLastError())); }
   int rc = MIG_OK;
   if (cudaFuncSetAttribute(gemm_tf32x3_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<128>::kBytes) != cudaSuccess ||
+      cudaFuncSetAttribute(gemm_tf32x3_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<256>::kBytes) != cudaSuccess ||
       cudaFuncSetAttribute(gemm_tf32x3_kernel<kDqnApad>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<kDqnApad>::kBytes) != cudaSuccess) {
     mig_dqn_destroy(d); return mig_fail(MIG_ECUDA, "dqn_create: %d bytes of shared memory per CTA refused (%s)", GemmSmem<128>::kBytes, cudaGetErrorString(cudaGetLastError()));
   }
@@ -162,8 +174,9 @@ extern "C" int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1,
   MAP(mX2, d->X2, 64, B, 64, 128); MAP(mT1, d->T1, H, B, H, 128); MAP(mT2, d->T2, H, B, H, 128);
   MAP(mdQ, d->dQ, P, B, P, 128); MAP(mdZ2, d->dZ2, H, B, H, 128);
   MAP(mH2t, d->H2t, B, H, B, 128); MAP(mH1t, d->H1t, B, H, B, 128); MAP(mXt, d->Xt, B, 64, B, 128);
-  for (int k = 0; k < 2; ++k) { MAP(mW1t[k], d->net[k].W1t, 64, H, 64, 128); MAP(mW2t[k], d->net[k].W2t, H, H, H, 128); MAP(mW3t[k], d->net[k].W3t, H, P, H, P); }
-  MAP(mW3, d->net[0].W3, P, H, P, 128); MAP(mW2, d->net[0].W2, H, H, H, 128);
+  const uint32_t bn = d->bn_h;
+  for (int k = 0; k < 2; ++k) { MAP(mW1t[k], d->net[k].W1t, 64, 2 * H, 64, bn); MAP(mW2t[k], d->net[k].W2t, H, 2 * H, H, bn); MAP(mW3t[k], d->net[k].W3t, H, 2 * P, H, P); }
+  MAP(mW3, d->net[0].W3s, P, 2 * H, P, bn); MAP(mW2, d->net[0].W2s, H, 2 * H, H, bn);
   MAP(mdQt, d->dQt, B, P, B, P); MAP(mdZ2t, d->dZ2t, B, H, B, 128); MAP(mdZ1t, d->dZ1t, B, H, B, 128);
 #undef MAP
   if (rc) { mig_dqn_destroy(d); return rc; }
@@ -179,15 +192,15 @@ static int forward(mig_dqn *d, int which, cudaStream_t st) {
   const Net &n = d->net[which];
   int rc;
   GemmArgs g = gargs(B, H, 64);
-  g.epi = EPI_BIAS | EPI_RELU; g.bias = n.b1; g.out = which ? d->T1 : d->H1; g.ldo = H;
+  g.epi = EPI_BIAS | EPI_RELU; g.bias = n.b1; g.out = which ? d->T1 : d->H1; g.ldo = H; g.b_lo_row = H;
   if (!which) { g.out_t = d->H1t; g.ldt = B; }
-  if ((rc = launch_gemm<128>(d, which ? d->mX2 : d->mX, d->mW1t[which], g, 1, st))) return rc;
+  if ((rc = launch_gemm_h(d, which ? d->mX2 : d->mX, d->mW1t[which], g, 1, st))) return rc;
   g = gargs(B, H, H);
-  g.epi = EPI_BIAS | EPI_RELU; g.bias = n.b2; g.out = which ? d->T2 : d->H2; g.ldo = H;
+  g.epi = EPI_BIAS | EPI_RELU; g.bias = n.b2; g.out = which ? d->T2 : d->H2; g.ldo = H; g.b_lo_row = H;
   if (!which) { g.out_t = d->H2t; g.ldt = B; }
-  if ((rc = launch_gemm<128>(d, which ? d->mT1 : d->mH1, d->mW2t[which], g, 1, st))) return rc;
+  if ((rc = launch_gemm_h(d, which ? d->mT1 : d->mH1, d->mW2t[which], g, 1, st))) return rc;
   g = gargs(B, P, H);
-  g.epi = EPI_BIAS; g.bias = n.b3; g.out = which ? d->Qt : d->Q; g.ldo = P;
+  g.epi = EPI_BIAS; g.bias = n.b3; g.out = which ? d->Qt : d->Q; g.ldo = P; g.b_lo_row = P;
   return launch_gemm<kDqnApad>(d, which ? d->mT2 : d->mH2, d->mW3t[which], g, 1, st);
 }
 
@@ -222,11 +235,11 @@ static int train_kernels(mig_dqn *d, cudaStream_t st) {
   CUD(cudaGetLastError()); d->launches++;
   // backward through the activations: dZ2 = (dQ W3^T) . [H2 > 0], dZ1 = (dZ2 W2^T) . [H1 > 0]
   GemmArgs g = gargs(B, H, P);
-  g.epi = EPI_MASK; g.mask = d->H2; g.ldm = H; g.out = d->dZ2; g.ldo = H; g.out_t = d->dZ2t; g.ldt = B;
-  if ((rc = launch_gemm<128>(d, d->mdQ, d->mW3, g, 1, st))) return rc;
+  g.epi = EPI_MASK; g.mask = d->H2; g.ldm = H; g.out = d->dZ2; g.ldo = H; g.out_t = d->dZ2t; g.ldt = B; g.b_lo_row = H;
+  if ((rc = launch_gemm_h(d, d->mdQ, d->mW3, g, 1, st))) return rc;
   g = gargs(B, H, H);
-  g.epi = EPI_MASK; g.mask = d->H1; g.ldm = H; g.out_t = d->dZ1t; g.ldt = B;
-  if ((rc = launch_gemm<128>(d, d->mdZ2, d->mW2, g, 1, st))) return rc;
+  g.epi = EPI_MASK; g.mask = d->H1; g.ldm = H; g.out_t = d->dZ1t; g.ldt = B; g.b_lo_row = H;
+  if ((rc = launch_gemm_h(d, d->mdZ2, d->mW2, g, 1, st))) return rc;
   // weight gradients, split over the batch dimension: dW3 = H2^T dQ, dW2 = H1^T dZ2, dW1 = X^T dZ1
   const uint32_t kps = B / S;                                  // batch rows per split
   g = gargs(H, P, kps); g.out = d->pW3; g.ldo = P; g.out_split_stride = (size_t)H * P;
@@ -239,14 +252,14 @@ static int train_kernels(mig_dqn *d, cudaStream_t st) {
   Net &n = d->net[0];
   UpdateArgs u; memset(&u, 0, sizeof(u));
   u.lr = d->lr; u.B = B; u.n_splits = S;
-  u.W = n.W3; u.Wt = n.W3t; u.rows = H; u.cols = P; u.ldw = P; u.ldt = H; u.partial = d->pW3; u.split_stride = (size_t)H * P; u.ldp = P;
+  u.W = n.W3; u.Wt = n.W3t; u.Ws = n.W3s; u.rows = H; u.cols = P; u.ldw = P; u.ldt = H; u.partial = d->pW3; u.split_stride = (size_t)H * P; u.ldp = P;
   u.bias = n.b3; u.dZt = d->dQt; u.n_bias = P; u.lossrow = d->lossrow; u.loss_out = d->loss;
   dqn_update_kernel<<<u.rows + u.n_bias + 1, 256, 0, st>>>(u);
   u.loss_out = nullptr; u.lossrow = nullptr;
-  u.W = n.W2; u.Wt = n.W2t; u.rows = H; u.cols = H; u.ldw = H; u.ldt = H; u.partial = d->pW2; u.split_stride = (size_t)H * H; u.ldp = H;
+  u.W = n.W2; u.Wt = n.W2t; u.Ws = n.W2s; u.rows = H; u.cols = H; u.ldw = H; u.ldt = H; u.partial = d->pW2; u.split_stride = (size_t)H * H; u.ldp = H;
   u.bias = n.b2; u.dZt = d->dZ2t; u.n_bias = H;
   dqn_update_kernel<<<u.rows + u.n_bias, 256, 0, st>>>(u);
-  u.W = n.W1; u.Wt = n.W1t; u.rows = 64; u.cols = H; u.ldw = H; u.ldt = 64; u.partial = d->pW1; u.split_stride = (size_t)64 * H; u.ldp = H;
+  u.W = n.W1; u.Wt = n.W1t; u.Ws = nullptr; u.rows = 64; u.cols = H; u.ldw = H; u.ldt = 64; u.partial = d->pW1; u.split_stride = (size_t)64 * H; u.ldp = H;
   u.bias = n.b1; u.dZt = d->dZ1t; u.n_bias = H;
   dqn_update_kernel<<<u.rows + u.n_bias, 256, 0, st>>>(u);
   CUD(cudaGetLastError()); d->launches += 3;
@@ -339,9 +352,9 @@ extern "C" int mig_dqn_sync_target(mig_dqn_t *d, void *stream) {
   cudaStream_t st = (cudaStream_t)stream;
   const size_t H = d->H, P = kDqnApad;
   const Net &o = d->net[0]; Net &t = d->net[1];
-  const struct { float *dst; const float *src; size_t n; } cp[9] = {
-      {t.W1, o.W1, 64 * H}, {t.W1t, o.W1t, H * 64}, {t.b1, o.b1, H}, {t.W2, o.W2, H * H}, {t.W2t, o.W2t, H * H}, {t.b2, o.b2, H},
-      {t.W3, o.W3, H * P}, {t.W3t, o.W3t, P * H}, {t.b3, o.b3, P}};
+  const struct { float *dst; const float *src; size_t n; } cp[9] = {             // (the target's backward copies are never read)
+      {t.W1, o.W1, 64 * H}, {t.W1t, o.W1t, 2 * H * 64}, {t.b1, o.b1, H}, {t.W2, o.W2, H * H}, {t.W2t, o.W2t, 2 * H * H}, {t.b2, o.b2, H},
+      {t.W3, o.W3, H * P}, {t.W3t, o.W3t, 2 * P * H}, {t.b3, o.b3, P}};
   for (const auto &c : cp) CUD(cudaMemcpyAsync(c.dst, c.src, c.n * sizeof(float), cudaMemcpyDeviceToDevice, st));
   return MIG_OK;
 }

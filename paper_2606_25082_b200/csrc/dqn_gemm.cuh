@@ -40,6 +40,8 @@ struct GemmArgs {
   const float *bias;                   // [N] (EPI_BIAS)
   const float *mask; uint32_t ldm;     // [M][ldm] (EPI_MASK): the forward activation whose ReLU is differentiated
   uint32_t epi;
+  uint32_t b_lo_row;                   // 0: B is fp32 and split here.  > 0: B was written split (TF32 high parts in rows [0, N), the
+                                       // remainders in rows [b_lo_row, b_lo_row + N) of the same map): both tiles are loaded, none is split
 };
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
@@ -151,9 +153,11 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
           const int s = it % S::kStages; const uint32_t round = it / S::kStages;
           if (round) mbar_wait(&empty[s], (round - 1) & 1u);
           unsigned char *st = tiles + s * S::kStage;
-          mbar_expect_tx(&full[s], S::kStageA + S::kStageB);
+          mbar_expect_tx(&full[s], S::kStageA + (g.b_lo_row ? 2 : 1) * S::kStageB);
           tma_load_2d(st, &map_a, &full[s], k_first + (int)kb * kGemmBK, (int)m0);
           tma_load_2d(st + 2 * S::kStageA, &map_b, &full[s], k_first + (int)kb * kGemmBK, (int)n0);
+          if (g.b_lo_row)                                      // B was split when it was written (weights): its low parts are rows of the same map
+            tma_load_2d(st + 2 * S::kStageA + S::kStageB, &map_b, &full[s], k_first + (int)kb * kGemmBK, (int)(g.b_lo_row + n0));
         }
       }
     }
@@ -206,6 +210,7 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
           h.w = __uint_as_float(__float_as_uint(x.w) & 0xFFFFE000u); l.w = x.w - h.w;
           a_hi[i] = h; a_lo[i] = l;
         }
+        if (!g.b_lo_row)
 #pragma unroll 4
         for (int i = t; i < S::kStageB / 16; i += 128) {
           const float4 x = b_hi[i];
@@ -237,9 +242,13 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
       for (int c = 0; c < BN; c += 16) {
         float v[16];
         tmem_ld16(trow + (uint32_t)c, v);
-        if (g.epi & EPI_BIAS) {
+        if (g.epi & EPI_BIAS) {                                // (warp-uniform addresses: four 16-byte loads, not sixteen scalar ones)
+          const float4 *b4 = reinterpret_cast<const float4 *>(g.bias + n0 + c);
 #pragma unroll
-          for (int j = 0; j < 16; ++j) v[j] += __ldg(&g.bias[n0 + c + j]);
+          for (int j4 = 0; j4 < 4; ++j4) {
+            const float4 bb = __ldg(b4 + j4);
+            v[4 * j4] += bb.x; v[4 * j4 + 1] += bb.y; v[4 * j4 + 2] += bb.z; v[4 * j4 + 3] += bb.w;
+          }
         }
         if (g.epi & EPI_RELU) {
 #pragma unroll

@@ -85,8 +85,11 @@ __global__ void __launch_bounds__(256) dqn_td_kernel(const float *Q, const float
 // One block per row `i` of a weight matrix W [rows][cols] (cols <= 256): W[i][:] -= lr * sum_z partial[z][i][:], in the fixed
 // order z = 0, 1, ...; the transposed copy Wt[cols][ldt] is kept in step.  Blocks beyond `rows` update the bias: bias[o] -= lr *
 // sum_b dZt[o][b] (one block per output o, a fixed-order tree over the batch), block `rows + n_bias` sums the loss.
+// The products read the weights as TF32 pairs (dqn_gemm.cuh): the copies are kept SPLIT, high parts first -- Wt [2 cols][ldt]
+// (transposed: rows [0, cols) high, [cols, 2 cols) low) and, where the backward pass reads the matrix untransposed, Ws [2 rows][ldw].
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 struct UpdateArgs {
-  float *W, *Wt; uint32_t rows, cols, ldw, ldt;            // W [rows][ldw] (first `cols` columns live), Wt [cols][ldt]
+  float *W, *Wt, *Ws; uint32_t rows, cols, ldw, ldt;       // W [rows][ldw] (first `cols` columns live), Wt [2 cols][ldt], Ws [2 rows][ldw] or NULL
   const float *partial; uint32_t n_splits; size_t split_stride; uint32_t ldp;   // partial [z][rows][ldp]
   float *bias; const float *dZt; uint32_t n_bias, B;       // bias [n_bias], dZt [n_bias][B]
   float lr;
@@ -111,7 +114,9 @@ __global__ void __launch_bounds__(256) dqn_update_kernel(const UpdateArgs u) {
       for (uint32_t z = 0; z < u.n_splits; ++z) g += u.partial[z * u.split_stride + (size_t)blk * u.ldp + c];
       const float w = u.W[(size_t)blk * u.ldw + c] - u.lr * g;
       u.W[(size_t)blk * u.ldw + c] = w;
-      u.Wt[(size_t)c * u.ldt + blk] = w;
+      const float h = tf32_hi(w), l = w - h;
+      u.Wt[(size_t)c * u.ldt + blk] = h; u.Wt[(size_t)(u.cols + c) * u.ldt + blk] = l;
+      if (u.Ws) { u.Ws[(size_t)blk * u.ldw + c] = h; u.Ws[(size_t)(u.rows + blk) * u.ldw + c] = l; }
     }
     return;
   }
@@ -131,12 +136,14 @@ __global__ void __launch_bounds__(256) dqn_update_kernel(const UpdateArgs u) {
   }
 }
 
-// Wt[c][r] = W[r][c] for a small matrix (initialisation and target sync)
-__global__ void dqn_transpose_kernel(const float *W, float *Wt, uint32_t rows, uint32_t cols, uint32_t ldw, uint32_t ldt) {
+// the split copies of a small matrix W [rows][ldw] (initialisation): Wt [2 cols][ldt] transposed, Ws [2 rows][ldw] (or NULL)
+__global__ void dqn_split_kernel(const float *W, float *Wt, float *Ws, uint32_t rows, uint32_t cols, uint32_t ldw, uint32_t ldt) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= rows * cols) return;
   const uint32_t r = i / cols, c = i % cols;
-  Wt[(size_t)c * ldt + r] = W[(size_t)r * ldw + c];
+  const float w = W[(size_t)r * ldw + c], h = tf32_hi(w), l = w - h;
+  Wt[(size_t)c * ldt + r] = h; Wt[(size_t)(cols + c) * ldt + r] = l;
+  if (Ws) { Ws[(size_t)r * ldw + c] = h; Ws[(size_t)(rows + r) * ldw + c] = l; }
 }
 
 }  // namespace migsim

@@ -96,6 +96,22 @@ def test_training_steps_match_the_oracle(hidden, batch, A, steps):
     d.close()
 
 
+@pytest.mark.parametrize("bn", ["128", "256"])
+def test_both_tile_widths_of_the_hidden_layer_products(bn, monkeypatch):
+    # products with N = 256 run as 128 x 256 tiles from batch 32768 on (MIG_DQN_BN overrides the rule at create): same results
+    monkeypatch.setenv("MIG_DQN_BN", bn)
+    test_training_steps_match_the_oracle(256, 1024, 12, 3)
+    test_tensor_core_forward_matches_double(256, 1000, 12)
+    monkeypatch.delenv("MIG_DQN_BN")
+    net = W.make_qnet(21, n_actions=12, hidden=256)            # the rule itself: a batch of 32768 takes the wide tiles
+    d = B.Dqn(net, 256, 32768, 0.9, 0.01, 1)
+    s = make_batch(23, 32768, 12)[0]
+    q = d.q(dev(s)).cpu().numpy()
+    want = O.Dqn(net, 0.9, 0.01).q(s)
+    assert np.abs(q - want).max() <= TOL * np.abs(want).max()
+    d.close()
+
+
 def test_replay_ring_and_sampling():
     A, batch, cap = 12, 256, 1000
     net = W.make_qnet(51, n_actions=A, hidden=256)
