@@ -170,6 +170,8 @@ def run_ours(args):
         wl.algo[:] = args.algo
     sp = dataclasses.replace(wl.params, env_offset=rank * n_envs)      # Philox keyed by global env id
     sim = B.MigSim(sp, n_envs, wl.seed, tile=args.tile)
+    if args.envs_per_warp:
+        sim.set_envs_per_warp(args.envs_per_warp)
     qnet = B.QNet(wl.qnet) if wl.qnet is not None else None
     d_algo, d_cfg0 = torch.from_numpy(wl.algo).cuda(), torch.from_numpy(wl.cfg0).cuda()
     d_table = None if wl.table is None else torch.from_numpy(wl.table).cuda()
@@ -329,7 +331,7 @@ def run_ours(args):
         line = {
             "metric": "job_events_per_s", "value": ev_total / t_s, "unit": "job-events/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
-            "config": {"workload": args.workload, "n_envs_per_gpu": n_envs, "n_envs_total": n_envs * world, "policy": ["static", "table", "dqn"][wl.policy], "algo": W.ALGO_NAMES[int(wl.algo[0])] if len(set(wl.algo.tolist())) == 1 else "mixed", "lanes_per_env": sim.get_tile(),
+            "config": {"workload": args.workload, "n_envs_per_gpu": n_envs, "n_envs_total": n_envs * world, "policy": ["static", "table", "dqn"][wl.policy], "algo": W.ALGO_NAMES[int(wl.algo[0])] if len(set(wl.algo.tolist())) == 1 else "mixed", "lanes_per_env": sim.get_tile(), "envs_per_warp": args.envs_per_warp or "auto",
                        "job_events_per_step": ev_total / args.steps, "l2": "flushed between iterations (256 MiB write)", "parallelism": "env-range sharding, no data-path collective",
                        "dist": ("nccl, world %d" % dist.get_world_size()) if dist.is_initialized() else None},
             "day_episodes_per_s": n_envs * world * args.steps / t_s,
@@ -435,7 +437,7 @@ def run_dqn(args):
             "train_steps_per_s": 1e3 / step_ms, "e2e": {"value": batch * n_e2e / e2e_s, "unit": "transitions/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": 4, "steps": n_e2e},
             "gpu_launches": launches, "clocks": clocks,
             "roofline": {"bound": "tensor", "achieved": achieved, "peak": tf32_peak, "unit": "TFLOP/s", "frac": achieved / tf32_peak, "traffic": None,
-                         "kernel": "gemm_tf32x3_kernel<128>", "step_ms": step_ms, "flop_per_transition_algorithmic": DQN_FLOP_PER_TRANSITION,
+                         "kernel": "gemm_tf32x3_kernel<BN> (BN = 128, 256 and 16: the twelve products of a step)", "step_ms": step_ms, "flop_per_transition_algorithmic": DQN_FLOP_PER_TRANSITION,
                          "issued_over_algorithmic": 3.0, "peak_source": "%s bf16 dense / 2 (TF32 : BF16 = 1 : 2, B200_PROFILING.md)" % peak_src},
             "cpu_baseline": cpu}
     print(json.dumps(line))
@@ -454,6 +456,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-step-api", action="store_true", help="skip the secondary mig_sim_step measurement")
     ap.add_argument("--algo", type=int, default=-1, choices=[-1, 0, 1, 2, 3, 4], help="override the workload's scheduling algorithm for every env (4 = EDF-SS with restricted preemption); -1 = the workload's own")
+    ap.add_argument("--envs-per-warp", type=int, default=0, choices=[0, 1, 2, 4, 8, 16, 32],
+                    help="thread-per-environment kernel: environments in each warp (0 = the library's choice: one resident wave); a study knob, see profiles/r2_thread.md")
     ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 8, 16, 32], help="lanes per environment (0 = library default = 1: one thread per environment; 8, 16, 32: warp tiles)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
