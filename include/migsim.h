@@ -259,6 +259,22 @@ int mig_dqn_sync_target(mig_dqn_t *d, void *stream);
 /* Q-values of the online (which = 0) or target (1) network through the tensor-core path: state dev[n][64], n <= batch,
  * q_out dev[n][n_actions].  Within 1e-4 relative of mig_q_eval's. */
 int mig_dqn_q(mig_dqn_t *d, int which, const float *state, uint32_t n, float *q_out, void *stream);
+/* The same forward with NO allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, serving
+ * loops, harnesses that forbid it): no handle; the scratch it needs (split weight copies, two hidden activations, padded
+ * Q rows) is a file-scope static __device__ array of the library -- 4.8 MiB on every GPU that loads libmigsim.so, held
+ * until the process exits -- sized for at most MIG_Q_STATIC_MAX_ROWS rows of a network with hidden <= 256.
+ *   W1 dev[64][hidden], b1 dev[hidden], W2 dev[hidden][hidden], b2 dev[hidden], W3 dev[hidden][n_actions], b3
+ *   dev[n_actions] (mig_qnet_create's layout, but DEVICE pointers: read on `stream`, never copied to the host); state
+ *   dev[n][64]; q_out dev[n][n_actions]; state, b1 and b2 16-byte aligned.  hidden 128 or 256, n_actions 1..16.
+ * Calls no cudaMalloc / cudaFree / allocating library routine: memsets, copies and kernels on `stream`, tensor maps encoded
+ * on the host.  The first call on a device also takes the array's device address (cudaGetSymbolAddress) and sets the
+ * kernels' shared-memory limits: make that call outside a graph capture.  MIG_EINVAL, with a message naming the limit,
+ * if n > MIG_Q_STATIC_MAX_ROWS (call it on chunks of the batch) or an argument is out of range; MIG_ECUDA otherwise.
+ * EVERY call on a device shares the one array: calls that overlap on the GPU (two streams, two threads, two graphs in
+ * flight) race on it -- order them on one stream or with events.  Results: those of mig_dqn_q (same kernels). */
+#define MIG_Q_STATIC_MAX_ROWS 2048
+int mig_q_forward_static(const float *W1, const float *b1, const float *W2, const float *b2, const float *W3, const float *b3,
+                         uint32_t hidden, uint32_t n_actions, const float *state, uint32_t n, float *q_out, void *stream);
 /* Copies the weights of the online (0) or target (1) network to HOST arrays shaped as in mig_qnet_create; synchronises. */
 int mig_dqn_get_weights(mig_dqn_t *d, int which, float *W1, float *b1, float *W2, float *b2, float *W3, float *b3);
 /* Kernel launches issued through this handle so far. */

@@ -37,7 +37,7 @@ EXPORTS = (
     "mig_sim_get_tile", "mig_sim_set_arrival_buffer", "mig_sim_get_arrival_buffer", "mig_sim_set_envs_per_warp",
     "mig_sim_kernel_name", "mig_sim_set_profiling", "mig_sim_kernel_times", "mig_sim_aux", "mig_et_reduce",
     "mig_dqn_create", "mig_dqn_destroy", "mig_replay_push", "mig_replay_size", "mig_dqn_train_step", "mig_dqn_train_on",
-    "mig_dqn_sync_target", "mig_dqn_q", "mig_dqn_get_weights", "mig_dqn_launch_count")
+    "mig_dqn_sync_target", "mig_dqn_q", "mig_dqn_get_weights", "mig_dqn_launch_count", "mig_q_forward_static")
 
 
 class MigError(RuntimeError):
@@ -114,6 +114,7 @@ def lib():
         L.mig_dqn_sync_target.argtypes = [vp, vp]
         L.mig_dqn_q.argtypes = [vp, i32, vp, u32, vp, vp]
         L.mig_dqn_get_weights.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
+        L.mig_q_forward_static.argtypes = [vp, vp, vp, vp, vp, vp, u32, u32, vp, u32, vp, vp]
         L.mig_dqn_launch_count.argtypes = [vp]
         L.mig_dqn_launch_count.restype = u64
         _lib = L
@@ -401,6 +402,21 @@ def recs_to_numpy(t: torch.Tensor) -> np.ndarray:
 
 def totals_to_numpy(t: torch.Tensor) -> np.ndarray:
     return t.cpu().numpy().view(TOTALS_DTYPE).reshape(t.shape[:-1])
+
+
+Q_STATIC_MAX_ROWS = 2048                                     # MIG_Q_STATIC_MAX_ROWS of include/migsim.h
+
+
+def q_forward_static(W1, b1, W2, b2, W3, b3, state: torch.Tensor, q_out: torch.Tensor, stream=None):
+    """mig_q_forward_static: Q-values on the tensor cores with no allocation anywhere (the scratch is a static array of the
+    library; at most Q_STATIC_MAX_ROWS rows per call).  All arguments are caller-owned CUDA tensors: weights in
+    mig_qnet_create's layout, state [n][64], q_out [n][n_actions].  Calls that overlap on the GPU race on the scratch."""
+    H, A = int(W2.shape[0]), int(W3.shape[1])
+    n = state.numel() // STATE_DIM
+    _check(lib().mig_q_forward_static(_dp(W1, torch.float32, STATE_DIM * H * 4), _dp(b1, torch.float32, H * 4), _dp(W2, torch.float32, H * H * 4),
+                                      _dp(b2, torch.float32, H * 4), _dp(W3, torch.float32, H * A * 4), _dp(b3, torch.float32, A * 4), H, A,
+                                      _dp(state, torch.float32), n, _dp(q_out, torch.float32, n * A * 4), _stream(stream)))
+    return q_out
 
 
 def et_reduce(x, y, group, n_groups: int):

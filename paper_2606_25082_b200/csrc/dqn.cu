@@ -9,6 +9,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <mutex>
 #include <vector>
 
 #include "dqn_gemm.cuh"
@@ -370,5 +371,127 @@ extern "C" int mig_dqn_get_weights(mig_dqn_t *d, int which, float *W1, float *b1
   CUD(cudaMemcpy(b2, n.b2, H * sizeof(float), cudaMemcpyDeviceToHost));
   CUD(cudaMemcpy2D(W3, A * sizeof(float), n.W3, P * sizeof(float), A * sizeof(float), H, cudaMemcpyDeviceToHost));
   CUD(cudaMemcpy(b3, n.b3, A * sizeof(float), cudaMemcpyDeviceToHost));
+  return MIG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ forward without allocation
+// mig_q_forward_static (include/migsim.h): the tensor-core forward of mig_dqn_q for callers that cannot call cudaMalloc (code
+// under CUDA graph capture, serving loops, harnesses that forbid it).  Its scratch -- the split weight copies, the two hidden
+// activations, the padded Q rows -- is this file-scope array: 4.8 MiB on every GPU that loads the library, until exit.  The
+// array's name is a host-side stand-in in host code, not a device address: its address is taken ONCE PER DEVICE with
+// cudaGetSymbolAddress (that device current) and only that pointer reaches kernels, memsets, copies and tensor maps.
+namespace {
+
+constexpr uint32_t kStaticMaxRows = MIG_Q_STATIC_MAX_ROWS, kStaticMaxH = 256;
+// regions, in floats; every offset is a multiple of 64 floats (256 bytes: TMA base alignment and float4 access)
+constexpr size_t kOffW1t = 0;                                              // [2 H][64]   split, transposed
+constexpr size_t kOffW2t = kOffW1t + 2 * (size_t)kStaticMaxH * 64;         // [2 H][H]
+constexpr size_t kOffW3t = kOffW2t + 2 * (size_t)kStaticMaxH * kStaticMaxH; // [2 x 16][H]
+constexpr size_t kOffB3 = kOffW3t + 2 * (size_t)kDqnApad * kStaticMaxH;    // [16] (+ padding to 64)
+constexpr size_t kOffH1 = kOffB3 + 64;                                     // [rows][H]
+constexpr size_t kOffH2 = kOffH1 + (size_t)kStaticMaxRows * kStaticMaxH;   // [rows][H]
+constexpr size_t kOffQ = kOffH2 + (size_t)kStaticMaxRows * kStaticMaxH;    // [rows][16]
+constexpr size_t kStaticFloats = kOffQ + (size_t)kStaticMaxRows * kDqnApad;
+static_assert(kOffW2t % 64 == 0 && kOffW3t % 64 == 0 && kOffB3 % 64 == 0 && kOffH1 % 64 == 0 && kOffH2 % 64 == 0 && kOffQ % 64 == 0, "256-byte regions");
+
+static __device__ __align__(256) float g_q_static_scratch[kStaticFloats];
+
+// split, transposed copy of W [rows][ldw] (first `cols` columns): Wt[c][r] = hi(W[r][c]), Wt[lo_row + c][r] = W[r][c] - hi
+// (dqn_split_kernel with the row of the low parts given: the action columns are padded to 16 rows here, not in W)
+__global__ void dqn_split_rows_kernel(const float *W, float *Wt, uint32_t rows, uint32_t cols, uint32_t ldw, uint32_t ldt, uint32_t lo_row) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= rows * cols) return;
+  const uint32_t r = i / cols, c = i % cols;
+  const float w = W[(size_t)r * ldw + c], h = tf32_hi(w), l = w - h;
+  Wt[(size_t)c * ldt + r] = h; Wt[(size_t)(lo_row + c) * ldt + r] = l;
+}
+
+struct StaticDev { bool ready = false; float *base = nullptr; int n_sm = 0; };
+constexpr int kMaxDevices = 64;
+StaticDev g_static_dev[kMaxDevices];
+std::mutex g_static_mutex;
+
+// once per device, with that device current: the scratch array's DEVICE address, the kernels' shared-memory limits
+int static_setup(int dev, StaticDev **out) {
+  if (dev < 0 || dev >= kMaxDevices) return mig_fail(MIG_EINVAL, "q_forward_static: device ordinal %d not in 0..%d", dev, kMaxDevices - 1);
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  StaticDev &sd = g_static_dev[dev];
+  if (!sd.ready) {
+    void *p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_q_static_scratch);
+    if (e != cudaSuccess || !p) { cudaGetLastError(); return mig_fail(MIG_ECUDA, "q_forward_static: cudaGetSymbolAddress of the scratch array failed on device %d: %s", dev, cudaGetErrorString(e)); }
+    if (reinterpret_cast<uintptr_t>(p) & 255u) return mig_fail(MIG_ECUDA, "q_forward_static: the scratch array is not 256-byte aligned");
+    if (cudaFuncSetAttribute(gemm_tf32x3_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<128>::kBytes) != cudaSuccess ||
+        cudaFuncSetAttribute(gemm_tf32x3_kernel<kDqnApad>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<kDqnApad>::kBytes) != cudaSuccess) {
+      const cudaError_t e2 = cudaGetLastError();
+      return mig_fail(MIG_ECUDA, "q_forward_static: %d bytes of shared memory per CTA refused on device %d (%s)", GemmSmem<128>::kBytes, dev, cudaGetErrorString(e2));
+    }
+    if (cudaDeviceGetAttribute(&sd.n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sd.n_sm < 1) { cudaGetLastError(); return mig_fail(MIG_ECUDA, "q_forward_static: no SM count for device %d", dev); }
+    sd.base = static_cast<float *>(p);
+    sd.ready = true;
+  }
+  *out = &sd;
+  return MIG_OK;
+}
+
+template <int BN>
+int launch_gemm_static(int n_sm, const CUtensorMap &ma, const CUtensorMap &mb, const GemmArgs &g, cudaStream_t st) {
+  GemmArgs ga = g; ga.splits = 1;
+  const uint32_t n_tiles = ((g.M + kGemmBM - 1) / kGemmBM) * (g.N / BN);
+  const uint32_t grid = n_tiles < (uint32_t)n_sm ? n_tiles : (uint32_t)n_sm;
+  gemm_tf32x3_kernel<BN><<<grid, kGemmThreads, GemmSmem<BN>::kBytes, st>>>(ma, mb, ga);
+  CUD(cudaGetLastError());
+  return MIG_OK;
+}
+
+}  // namespace
+
+extern "C" int mig_q_forward_static(const float *W1, const float *b1, const float *W2, const float *b2, const float *W3, const float *b3,
+                                    uint32_t hidden, uint32_t n_actions, const float *state, uint32_t n, float *q_out, void *stream) {
+  if (!W1 || !b1 || !W2 || !b2 || !W3 || !b3 || !state || !q_out) return mig_fail(MIG_EINVAL, "q_forward_static: NULL argument");
+  if (hidden != 128 && hidden != 256) return mig_fail(MIG_EINVAL, "q_forward_static: hidden %u must be 128 or 256", hidden);
+  if (n_actions < 1 || n_actions > MIG_MAX_CONFIGS) return mig_fail(MIG_EINVAL, "q_forward_static: n_actions %u not in 1..16", n_actions);
+  if (n < 1) return mig_fail(MIG_EINVAL, "q_forward_static: n = 0 rows");
+  if (n > kStaticMaxRows)
+    return mig_fail(MIG_EINVAL, "q_forward_static: n = %u rows exceed MIG_Q_STATIC_MAX_ROWS = %u, the size of the library's static scratch "
+                                "(call it on chunks of the batch, or use mig_dqn_q, which allocates at create)", n, kStaticMaxRows);
+  if ((reinterpret_cast<uintptr_t>(state) | reinterpret_cast<uintptr_t>(b1) | reinterpret_cast<uintptr_t>(b2)) & 15u)
+    return mig_fail(MIG_EINVAL, "q_forward_static: state, b1 and b2 must be 16-byte aligned device pointers");
+  int dev = 0;
+  CUD(cudaGetDevice(&dev));
+  StaticDev *sd = nullptr;
+  if (int rc = static_setup(dev, &sd)) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const uint32_t H = hidden, A = n_actions, P = kDqnApad;
+  float *W1t = sd->base + kOffW1t, *W2t = sd->base + kOffW2t, *W3t = sd->base + kOffW3t, *b3p = sd->base + kOffB3;
+  float *H1 = sd->base + kOffH1, *H2 = sd->base + kOffH2, *Q = sd->base + kOffQ;
+  // the array keeps the last call's contents: the padded action rows of W3t and of the bias must be zero for THIS call
+  CUD(cudaMemsetAsync(W3t, 0, 2 * (size_t)P * H * sizeof(float), st));
+  CUD(cudaMemsetAsync(b3p, 0, 64 * sizeof(float), st));
+  dqn_split_rows_kernel<<<(64 * H + 255) / 256, 256, 0, st>>>(W1, W1t, 64, H, H, 64, H);
+  dqn_split_rows_kernel<<<(H * H + 255) / 256, 256, 0, st>>>(W2, W2t, H, H, H, H, H);
+  dqn_split_rows_kernel<<<(H * A + 255) / 256, 256, 0, st>>>(W3, W3t, H, A, A, H, P);
+  CUD(cudaGetLastError());
+  CUD(cudaMemcpyAsync(b3p, b3, A * sizeof(float), cudaMemcpyDeviceToDevice, st));
+  // tensor maps (host-side encoding, no allocation): A operands with exactly n rows, so that rows beyond n read as zeros
+  CUtensorMap mX, mH1, mH2, mW1t, mW2t, mW3t;
+  int rc = MIG_OK;
+  if (!rc) rc = make_map(&mX, state, 64, n, 64, 128);
+  if (!rc) rc = make_map(&mH1, H1, H, n, H, 128);
+  if (!rc) rc = make_map(&mH2, H2, H, n, H, 128);
+  if (!rc) rc = make_map(&mW1t, W1t, 64, 2 * H, 64, 128);
+  if (!rc) rc = make_map(&mW2t, W2t, H, 2 * H, H, 128);
+  if (!rc) rc = make_map(&mW3t, W3t, H, 2 * P, H, P);
+  if (rc) return rc;
+  GemmArgs g = gargs(n, H, 64);
+  g.epi = EPI_BIAS | EPI_RELU; g.bias = b1; g.out = H1; g.ldo = H; g.b_lo_row = H;
+  if ((rc = launch_gemm_static<128>(sd->n_sm, mX, mW1t, g, st))) return rc;
+  g = gargs(n, H, H);
+  g.epi = EPI_BIAS | EPI_RELU; g.bias = b2; g.out = H2; g.ldo = H; g.b_lo_row = H;
+  if ((rc = launch_gemm_static<128>(sd->n_sm, mH1, mW2t, g, st))) return rc;
+  g = gargs(n, P, H);
+  g.epi = EPI_BIAS; g.bias = b3p; g.out = Q; g.ldo = P; g.b_lo_row = P;
+  if ((rc = launch_gemm_static<kDqnApad>(sd->n_sm, mH2, mW3t, g, st))) return rc;
+  CUD(cudaMemcpy2DAsync(q_out, A * sizeof(float), Q, P * sizeof(float), A * sizeof(float), n, cudaMemcpyDeviceToDevice, st));
   return MIG_OK;
 }
