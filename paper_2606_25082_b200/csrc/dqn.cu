@@ -53,7 +53,24 @@ int make_map(CUtensorMap *m, const float *ptr, uint64_t inner, uint64_t rows, ui
   return MIG_OK;
 }
 
+// MN-major operand: a row-major activation [rows = batch][inner = features] read as the [K][M] side of a product that
+// contracts over the batch: boxes of 32 rows x 32 columns, 128-byte rows swizzled in 32-byte chunks (dqn_gemm.cuh)
+int make_map_mn(CUtensorMap *m, const float *ptr, uint64_t inner, uint64_t rows, uint64_t ld, uint32_t box_inner) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return mig_fail(MIG_ECUDA, "dqn: cuTensorMapEncodeTiled is not available from this driver");
+  cuuint64_t dims[2] = {inner, rows}, strides[1] = {ld * sizeof(float)};
+  cuuint32_t box[2] = {box_inner, (cuuint32_t)kGemmBK}, es[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float *>(ptr), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return mig_fail(MIG_ECUDA, "dqn: cuTensorMapEncodeTiled failed (%d) for an MN-major [%llu][%llu] operand", (int)r, (unsigned long long)rows, (unsigned long long)inner);
+  return MIG_OK;
+}
+
 }  // namespace
+
+constexpr uint32_t kDqLd = 32;         // row pitch of dQ: 16 action columns + 16 zero ones (MN-major tiles are 32 columns wide)
+constexpr uint32_t kBiasChunks = 64;   // row chunks of the bias-gradient column sums
 
 struct mig_dqn {   // (mig_dqn_t of include/migsim.h)
   uint32_t H = 0, A = 0, B = 0, cap = 0, splits = 1, bn_h = 128;   // bn_h: tile width of the products with N = H
@@ -61,6 +78,13 @@ struct mig_dqn {   // (mig_dqn_t of include/migsim.h)
   int device = 0, n_sm = 148;
   uint64_t launches = 0, gemm_launches = 0, kernels_per_step = 0, gemms_per_step = 0;
   bool use_graph = true; cudaGraphExec_t graph_exec = nullptr;
+  // weight gradients from the ROW-MAJOR activations (MN-major tensor-core operands, contraction over the batch rows): no
+  // transposed copy of any [B][H] tensor is written, the bias gradients are column sums.  MIG_DQN_MN=0 in the environment at
+  // create selects the earlier path instead -- every activation also written transposed by the epilogue that produces it,
+  // K-major weight-gradient products over those copies -- kept for A/B timing and run by the tests
+  bool mn = true;
+  float *dZ1 = nullptr, *pb2 = nullptr, *pb1 = nullptr;    // row-major dZ1; partial column sums of dZ2 / dZ1 [kBiasChunks][H]
+  CUtensorMap mH2r, mH1r, mXr, mdQr, mdZ2r, mdZ1r;         // MN-major views of the row-major activations
   std::vector<void *> allocs;
   Net net[2];                                              // [0] online, [1] target
   // replay ring
@@ -81,12 +105,12 @@ static int dalloc(mig_dqn *d, void **p, size_t bytes) {
 }
 #define DA(ptr, count) do { int rc_ = dalloc(d, (void **)&(ptr), (size_t)(count) * sizeof(*(ptr))); if (rc_) { mig_dqn_destroy(d); return rc_; } } while (0)
 
-template <int BN>
+template <int BN, bool MN = false>
 static int launch_gemm(mig_dqn *d, const CUtensorMap &ma, const CUtensorMap &mb, const GemmArgs &g, uint32_t splits, cudaStream_t st) {
   GemmArgs ga = g; ga.splits = splits;
   const uint32_t n_tiles = ((g.M + kGemmBM - 1) / kGemmBM) * (g.N / BN) * splits;
   const uint32_t grid = n_tiles < (uint32_t)d->n_sm ? n_tiles : (uint32_t)d->n_sm;          // persistent: one CTA per SM walks the tiles
-  gemm_tf32x3_kernel<BN><<<grid, kGemmThreads, GemmSmem<BN>::kBytes, st>>>(ma, mb, ga);
+  gemm_tf32x3_kernel<BN, MN><<<grid, kGemmThreads, GemmSmem<BN>::kBytes, st>>>(ma, mb, ga);
   CUD(cudaGetLastError());
   d->launches++; d->gemm_launches++;
   return MIG_OK;
@@ -147,9 +171,12 @@ extern "C" int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1,
   DA(d->X, (size_t)B * 64); DA(d->X2, (size_t)B * 64); DA(d->Xt, (size_t)64 * B);
   DA(d->H1, (size_t)B * H); DA(d->H1t, (size_t)H * B); DA(d->H2, (size_t)B * H); DA(d->H2t, (size_t)H * B); DA(d->Q, (size_t)B * P);
   DA(d->T1, (size_t)B * H); DA(d->T2, (size_t)B * H); DA(d->Qt, (size_t)B * P);
-  DA(d->dQ, (size_t)B * P); DA(d->dQt, (size_t)P * B); DA(d->dZ2, (size_t)B * H); DA(d->dZ2t, (size_t)H * B); DA(d->dZ1t, (size_t)H * B);
+  DA(d->dQ, (size_t)B * kDqLd); DA(d->dQt, (size_t)P * B); DA(d->dZ2, (size_t)B * H); DA(d->dZ2t, (size_t)H * B); DA(d->dZ1t, (size_t)H * B);
+  DA(d->dZ1, (size_t)B * H);
+  DA(d->pb2, (size_t)kBiasChunks * H); DA(d->pb1, (size_t)kBiasChunks * H);
+  { const char *e = getenv("MIG_DQN_MN"); d->mn = !(e && e[0] == '0'); }
   DA(d->r, B); DA(d->a, B); DA(d->done, B); DA(d->lossrow, B); DA(d->loss, 1);
-  DA(d->pW1, (size_t)d->splits * 64 * H); DA(d->pW2, (size_t)d->splits * H * H); DA(d->pW3, (size_t)d->splits * H * P);
+  DA(d->pW1, (size_t)d->splits * 64 * H); DA(d->pW2, (size_t)d->splits * H * H); DA(d->pW3, (size_t)d->splits * H * kDqLd);
   // weights: master copies, padded action columns are zero; the transposed copies follow
   auto up = [&](float *dst, const float *src, size_t rows, size_t cols, size_t ld) {
     return cudaMemcpy2D(dst, ld * sizeof(float), src, cols * sizeof(float), cols * sizeof(float), rows, cudaMemcpyHostToDevice) == cudaSuccess;
@@ -167,19 +194,25 @@ extern "C" int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1,
   int rc = MIG_OK;
   if (cudaFuncSetAttribute(gemm_tf32x3_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<128>::kBytes) != cudaSuccess ||
       cudaFuncSetAttribute(gemm_tf32x3_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<256>::kBytes) != cudaSuccess ||
+      cudaFuncSetAttribute(gemm_tf32x3_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<128>::kBytes) != cudaSuccess ||
+      cudaFuncSetAttribute(gemm_tf32x3_kernel<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<32>::kBytes) != cudaSuccess ||
       cudaFuncSetAttribute(gemm_tf32x3_kernel<kDqnApad>, cudaFuncAttributeMaxDynamicSharedMemorySize, GemmSmem<kDqnApad>::kBytes) != cudaSuccess) {
     mig_dqn_destroy(d); return mig_fail(MIG_ECUDA, "dqn_create: %d bytes of shared memory per CTA refused (%s)", GemmSmem<128>::kBytes, cudaGetErrorString(cudaGetLastError()));
   }
 #define MAP(m, ptr, inner, rows, ld, box) if (!rc) rc = make_map(&d->m, ptr, inner, rows, ld, box)
   MAP(mX, d->X, 64, B, 64, 128); MAP(mH1, d->H1, H, B, H, 128); MAP(mH2, d->H2, H, B, H, 128);
   MAP(mX2, d->X2, 64, B, 64, 128); MAP(mT1, d->T1, H, B, H, 128); MAP(mT2, d->T2, H, B, H, 128);
-  MAP(mdQ, d->dQ, P, B, P, 128); MAP(mdZ2, d->dZ2, H, B, H, 128);
+  MAP(mdQ, d->dQ, P, B, kDqLd, 128); MAP(mdZ2, d->dZ2, H, B, H, 128);
   MAP(mH2t, d->H2t, B, H, B, 128); MAP(mH1t, d->H1t, B, H, B, 128); MAP(mXt, d->Xt, B, 64, B, 128);
   const uint32_t bn = d->bn_h;
   for (int k = 0; k < 2; ++k) { MAP(mW1t[k], d->net[k].W1t, 64, 2 * H, 64, bn); MAP(mW2t[k], d->net[k].W2t, H, 2 * H, H, bn); MAP(mW3t[k], d->net[k].W3t, H, 2 * P, H, P); }
   MAP(mW3, d->net[0].W3s, P, 2 * H, P, bn); MAP(mW2, d->net[0].W2s, H, 2 * H, H, bn);
   MAP(mdQt, d->dQt, B, P, B, P); MAP(mdZ2t, d->dZ2t, B, H, B, 128); MAP(mdZ1t, d->dZ1t, B, H, B, 128);
 #undef MAP
+#define MAPMN(m, ptr, inner, ld, box) if (!rc) rc = make_map_mn(&d->m, ptr, inner, B, ld, box)
+  MAPMN(mH2r, d->H2, H, H, 32); MAPMN(mH1r, d->H1, H, H, 32); MAPMN(mXr, d->X, 64, 64, 32);
+  MAPMN(mdQr, d->dQ, kDqLd, kDqLd, 32); MAPMN(mdZ2r, d->dZ2, H, H, 32); MAPMN(mdZ1r, d->dZ1, H, H, 32);
+#undef MAPMN
   if (rc) { mig_dqn_destroy(d); return rc; }
   *out = d;
   return MIG_OK;
@@ -194,11 +227,11 @@ static int forward(mig_dqn *d, int which, cudaStream_t st) {
   int rc;
   GemmArgs g = gargs(B, H, 64);
   g.epi = EPI_BIAS | EPI_RELU; g.bias = n.b1; g.out = which ? d->T1 : d->H1; g.ldo = H; g.b_lo_row = H;
-  if (!which) { g.out_t = d->H1t; g.ldt = B; }
+  if (!which && !d->mn) { g.out_t = d->H1t; g.ldt = B; }
   if ((rc = launch_gemm_h(d, which ? d->mX2 : d->mX, d->mW1t[which], g, 1, st))) return rc;
   g = gargs(B, H, H);
   g.epi = EPI_BIAS | EPI_RELU; g.bias = n.b2; g.out = which ? d->T2 : d->H2; g.ldo = H; g.b_lo_row = H;
-  if (!which) { g.out_t = d->H2t; g.ldt = B; }
+  if (!which && !d->mn) { g.out_t = d->H2t; g.ldt = B; }
   if ((rc = launch_gemm_h(d, which ? d->mT1 : d->mH1, d->mW2t[which], g, 1, st))) return rc;
   g = gargs(B, P, H);
   g.epi = EPI_BIAS; g.bias = n.b3; g.out = which ? d->Qt : d->Q; g.ldo = P; g.b_lo_row = P;
@@ -227,47 +260,57 @@ extern "C" int mig_dqn_q(mig_dqn_t *d, int which, const float *state, uint32_t n
 
 // ------------------------------------------------------------------------------------------------ one training step
 // forward of both networks, TD error, backward, SGD on the batch that the gather kernel left in X / X2 / a / r / done:
-// fifteen launches, always with the same arguments (the loss lands in d->loss)
+// seventeen launches (fifteen on the MIG_DQN_MN=0 path), always with the same arguments (the loss lands in d->loss)
 static int train_kernels(mig_dqn *d, cudaStream_t st) {
   const uint32_t H = d->H, B = d->B, P = kDqnApad, S = d->splits;
   int rc;
   if ((rc = forward(d, 0, st)) || (rc = forward(d, 1, st))) return rc;
-  dqn_td_kernel<<<(B + 255) / 256, 256, 0, st>>>(d->Q, d->Qt, d->a, d->r, d->done, B, d->A, d->gamma, d->dQ, d->dQt, d->lossrow);
+  dqn_td_kernel<<<(B + 255) / 256, 256, 0, st>>>(d->Q, d->Qt, d->a, d->r, d->done, B, d->A, d->gamma, d->dQ, kDqLd, d->dQt, d->lossrow);
   CUD(cudaGetLastError()); d->launches++;
   // backward through the activations: dZ2 = (dQ W3^T) . [H2 > 0], dZ1 = (dZ2 W2^T) . [H1 > 0]
   GemmArgs g = gargs(B, H, P);
-  g.epi = EPI_MASK; g.mask = d->H2; g.ldm = H; g.out = d->dZ2; g.ldo = H; g.out_t = d->dZ2t; g.ldt = B; g.b_lo_row = H;
+  g.epi = EPI_MASK; g.mask = d->H2; g.ldm = H; g.out = d->dZ2; g.ldo = H; g.b_lo_row = H;
+  if (!d->mn) { g.out_t = d->dZ2t; g.ldt = B; }
   if ((rc = launch_gemm_h(d, d->mdQ, d->mW3, g, 1, st))) return rc;
   g = gargs(B, H, H);
-  g.epi = EPI_MASK; g.mask = d->H1; g.ldm = H; g.out_t = d->dZ1t; g.ldt = B; g.b_lo_row = H;
+  g.epi = EPI_MASK; g.mask = d->H1; g.ldm = H; g.b_lo_row = H;
+  if (d->mn) { g.out = d->dZ1; g.ldo = H; } else { g.out_t = d->dZ1t; g.ldt = B; }
   if ((rc = launch_gemm_h(d, d->mdZ2, d->mW2, g, 1, st))) return rc;
   // weight gradients, split over the batch dimension: dW3 = H2^T dQ, dW2 = H1^T dZ2, dW1 = X^T dZ1
   const uint32_t kps = B / S;                                  // batch rows per split
-  g = gargs(H, P, kps); g.out = d->pW3; g.ldo = P; g.out_split_stride = (size_t)H * P;
-  if ((rc = launch_gemm<kDqnApad>(d, d->mH2t, d->mdQt, g, S, st))) return rc;
+  const uint32_t ld3 = d->mn ? kDqLd : P;                     // (MN-major tiles are 32 columns wide: the partials of dW3 carry 16 zero columns)
+  g = gargs(H, ld3, kps); g.out = d->pW3; g.ldo = ld3; g.out_split_stride = (size_t)H * ld3;
+  if ((rc = d->mn ? launch_gemm<32, true>(d, d->mH2r, d->mdQr, g, S, st) : launch_gemm<kDqnApad>(d, d->mH2t, d->mdQt, g, S, st))) return rc;
   g = gargs(H, H, kps); g.out = d->pW2; g.ldo = H; g.out_split_stride = (size_t)H * H;
-  if ((rc = launch_gemm<128>(d, d->mH1t, d->mdZ2t, g, S, st))) return rc;
+  if ((rc = d->mn ? launch_gemm<128, true>(d, d->mH1r, d->mdZ2r, g, S, st) : launch_gemm<128>(d, d->mH1t, d->mdZ2t, g, S, st))) return rc;
   g = gargs(64, H, kps); g.out = d->pW1; g.ldo = H; g.out_split_stride = (size_t)64 * H;
-  if ((rc = launch_gemm<128>(d, d->mXt, d->mdZ1t, g, S, st))) return rc;
+  if ((rc = d->mn ? launch_gemm<128, true>(d, d->mXr, d->mdZ1r, g, S, st) : launch_gemm<128>(d, d->mXt, d->mdZ1t, g, S, st))) return rc;
+  if (d->mn) {                                                 // bias gradients of the hidden layers: column sums of the row-major dZ
+    dqn_colsum_kernel<<<dim3(H / 32, kBiasChunks), 256, 0, st>>>(d->dZ2, B, H, kBiasChunks, d->pb2);
+    dqn_colsum_kernel<<<dim3(H / 32, kBiasChunks), 256, 0, st>>>(d->dZ1, B, H, kBiasChunks, d->pb1);
+    CUD(cudaGetLastError()); d->launches += 2;
+  }
   // SGD on the online network (the transposed copies follow), bias gradients = row sums of the transposed dZ, the loss
   Net &n = d->net[0];
   UpdateArgs u; memset(&u, 0, sizeof(u));
   u.lr = d->lr; u.B = B; u.n_splits = S;
-  u.W = n.W3; u.Wt = n.W3t; u.Ws = n.W3s; u.rows = H; u.cols = P; u.ldw = P; u.ldt = H; u.partial = d->pW3; u.split_stride = (size_t)H * P; u.ldp = P;
+  u.W = n.W3; u.Wt = n.W3t; u.Ws = n.W3s; u.rows = H; u.cols = P; u.ldw = P; u.ldt = H; u.partial = d->pW3; u.split_stride = (size_t)H * ld3; u.ldp = ld3;
   u.bias = n.b3; u.dZt = d->dQt; u.n_bias = P; u.lossrow = d->lossrow; u.loss_out = d->loss;
   dqn_update_kernel<<<u.rows + u.n_bias + 1, 256, 0, st>>>(u);
   u.loss_out = nullptr; u.lossrow = nullptr;
   u.W = n.W2; u.Wt = n.W2t; u.Ws = n.W2s; u.rows = H; u.cols = H; u.ldw = H; u.ldt = H; u.partial = d->pW2; u.split_stride = (size_t)H * H; u.ldp = H;
   u.bias = n.b2; u.dZt = d->dZ2t; u.n_bias = H;
+  if (d->mn) { u.dZt = nullptr; u.bias_part = d->pb2; u.n_chunks = kBiasChunks; }
   dqn_update_kernel<<<u.rows + u.n_bias, 256, 0, st>>>(u);
   u.W = n.W1; u.Wt = n.W1t; u.Ws = nullptr; u.rows = 64; u.cols = H; u.ldw = H; u.ldt = 64; u.partial = d->pW1; u.split_stride = (size_t)64 * H; u.ldp = H;
   u.bias = n.b1; u.dZt = d->dZ1t; u.n_bias = H;
+  if (d->mn) { u.dZt = nullptr; u.bias_part = d->pb1; u.n_chunks = kBiasChunks; }
   dqn_update_kernel<<<u.rows + u.n_bias, 256, 0, st>>>(u);
   CUD(cudaGetLastError()); d->launches += 3;
   return MIG_OK;
 }
 
-// The fifteen launches are captured ONCE into a CUDA graph (their arguments never change) and replayed with one
+// The seventeen launches are captured ONCE into a CUDA graph (their arguments never change) and replayed with one
 // cudaGraphLaunch per step: at batch 8192 the step is launch-bound without it.  MIG_DQN_NO_GRAPH=1 in the environment
 // launches the kernels one by one instead (profiling by kernel name).
 static int train_on_batch(mig_dqn *d, float *loss_out, cudaStream_t st) {
@@ -301,7 +344,7 @@ static int train_on_batch(mig_dqn *d, float *loss_out, cudaStream_t st) {
 static int gather(mig_dqn *d, const float *S, const uint8_t *A, const float *R, const float *S2, const uint8_t *D, uint32_t size, uint32_t step,
                   int identity, cudaStream_t st) {
   GatherArgs g; memset(&g, 0, sizeof(g));
-  g.S = S; g.S2 = S2; g.A = A; g.R = R; g.D = D; g.X = d->X; g.X2 = d->X2; g.Xt = d->Xt; g.a = d->a; g.r = d->r; g.done = d->done;
+  g.S = S; g.S2 = S2; g.A = A; g.R = R; g.D = D; g.X = d->X; g.X2 = d->X2; g.Xt = d->mn ? nullptr : d->Xt; g.a = d->a; g.r = d->r; g.done = d->done;
   g.B = d->B; g.size = size; g.step = step; g.k0 = (uint32_t)d->seed; g.k1 = (uint32_t)(d->seed >> 32); g.identity = identity;
   dqn_gather_kernel<<<(d->B + 31) / 32, 256, 0, st>>>(g);
   CUD(cudaGetLastError()); d->launches++;

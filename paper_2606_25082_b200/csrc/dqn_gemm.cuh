@@ -15,8 +15,10 @@
 //   warp 1      one elected lane issues 3 x 4 tcgen05.mma.kind::tf32 per stage (UMMA K = 8 floats = 32 bytes; the shared-
 //               memory descriptor advances by 32 bytes inside the swizzled row), accumulator in TMEM (BN columns x 128
 //               lanes), tcgen05.commit frees the stage / publishes the accumulator.
-// Every matrix product of the training step goes through this one kernel; operands that the mathematics wants transposed
-// are written transposed by the epilogue that produces them (dqn_train.cuh), so only the K-major form is ever needed.
+// Every matrix product of the training step goes through this one kernel.  The weight-gradient products contract over the
+// BATCH rows of two row-major activations: they run the MN = true instantiation, which reads both operands MN-major straight
+// from the row-major tensors (no transposed copy of an activation exists).  The epilogue can still write a transposed result
+// (out_t): the K-major weight-gradient path over such copies is kept behind MIG_DQN_MN=0 (dqn.cu) for A/B timing.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -69,9 +71,18 @@ __device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *map, u
 __device__ __forceinline__ uint64_t umma_desc_k_sw128(uint32_t saddr) {
   return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
 }
-// instruction descriptor: D = fp32, A = B = TF32, both K-major, M x N
-__device__ __forceinline__ uint32_t umma_idesc_tf32(uint32_t m, uint32_t n) {
-  return (1u << 4) | (2u << 7) | (2u << 10) | ((n >> 3) << 17) | ((m >> 4) << 24);
+// the same for an MN-major tile (the m / n index contiguous in memory: a row-major [k][m] block, as TMA brings it from a
+// row-major activation [batch][features] when the contraction runs over the batch).  32-bit MN-major operands have ONE
+// shared-memory layout: 128-byte rows of 32 m, swizzled in 32-byte chunks (layout type 1; TMA's SWIZZLE_128B_ATOM_32B), in
+// atoms of 4 k-rows (512 bytes); LBO = bytes between atoms along m / n (the next 32 columns), SBO = bytes between atoms
+// along k.  One UMMA (K = 8) reads two k-atoms = 8 rows = 1024 bytes of every 32-column block.
+__device__ __forceinline__ uint64_t umma_desc_mn_sw128_32b(uint32_t saddr, uint32_t lbo_bytes) {
+  return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(512 >> 4) << 32) | ((uint64_t)1 << 46) |
+         ((uint64_t)1 << 61);
+}
+// instruction descriptor: D = fp32, A = B = TF32, M x N; both operands K-major, or both MN-major (bits 15, 16)
+__device__ __forceinline__ uint32_t umma_idesc_tf32(uint32_t m, uint32_t n, bool mn_major = false) {
+  return (1u << 4) | (2u << 7) | (2u << 10) | ((n >> 3) << 17) | ((m >> 4) << 24) | (mn_major ? (3u << 15) : 0u);
 }
 __device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
   asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
@@ -114,7 +125,11 @@ template <int BN> struct GemmSmem {
 // grid (n fastest: consecutive tiles share their rows of A in L2).  The shared-memory ring and its mbarrier phases run
 // straight through the tile boundaries, so the producer is already loading tile i + 1 while tile i's last stages are
 // multiplied and its accumulator is drained.
-template <int BN>
+// MN = true: C[M][N] = sum_k A[k][m] * B[k][n] -- both operands MN-major (row-major [K][M] and [K][N] in global memory: the
+// weight-gradient products, whose contraction runs over the batch rows of two row-major activations).  A stage then holds
+// 4 blocks [32 k][32 m] of A (4 KB each) and BN / 32 such blocks of B (BN a multiple of 32); everything else (split,
+// accumulators, epilogues) is the same.
+template <int BN, bool MN = false>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b, const GemmArgs g) {
   using S = GemmSmem<BN>;
@@ -154,6 +169,15 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
           if (round) mbar_wait(&empty[s], (round - 1) & 1u);
           unsigned char *st = tiles + s * S::kStage;
           mbar_expect_tx(&full[s], S::kStageA + (g.b_lo_row ? 2 : 1) * S::kStageB);
+          if constexpr (MN) {                                  // boxes of {32 (or 16) columns, 32 batch rows}: coordinates {column, row}
+            const int k0 = k_first + (int)kb * kGemmBK;
+#pragma unroll
+            for (int j = 0; j < kGemmBM / 32; ++j) tma_load_2d(st + j * 4096, &map_a, &full[s], (int)m0 + 32 * j, k0);
+            static_assert(!MN || BN % 32 == 0, "MN-major tiles are blocks of 32 columns");
+#pragma unroll
+            for (int j = 0; j < BN / 32; ++j) tma_load_2d(st + 2 * S::kStageA + j * 4096, &map_b, &full[s], (int)n0 + 32 * j, k0);
+            continue;
+          }
           tma_load_2d(st, &map_a, &full[s], k_first + (int)kb * kGemmBK, (int)m0);
           tma_load_2d(st + 2 * S::kStageA, &map_b, &full[s], k_first + (int)kb * kGemmBK, (int)n0);
           if (g.b_lo_row)                                      // B was split when it was written (weights): its low parts are rows of the same map
@@ -163,7 +187,7 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
     }
   } else if (warp == 1) {
     // ===== MMA issuer
-    const uint32_t idesc = umma_idesc_tf32(kGemmBM, BN);
+    const uint32_t idesc = umma_idesc_tf32(kGemmBM, BN, MN);
     uint32_t it = 0, ti = 0;
     for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++ti) {
       const uint32_t as = ti & 1u, around = ti >> 1;          // accumulator stage and how often it has been used
@@ -176,6 +200,15 @@ gemm_tf32x3_kernel(const __grid_constant__ CUtensorMap map_a, const __grid_const
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         if (lane == 0) {                                       // ONE thread issues every MMA: they execute in its issue order
           const uint32_t a_hi = smem_u32(tiles + s * S::kStage), a_lo = a_hi + S::kStageA, b_hi = a_hi + 2 * S::kStageA, b_lo = b_hi + S::kStageB;
+          if constexpr (MN) {
+#pragma unroll
+            for (int k = 0; k < kGemmBK / 8; ++k) {            // UMMA K = 8 batch rows = 1024 bytes down every 32-column block
+              const uint32_t o = (uint32_t)k * 1024u;
+              umma_tf32(acc, umma_desc_mn_sw128_32b(a_lo + o, 4096), umma_desc_mn_sw128_32b(b_hi + o, 4096), idesc, (kb | (uint32_t)k) != 0u);
+              umma_tf32(acc, umma_desc_mn_sw128_32b(a_hi + o, 4096), umma_desc_mn_sw128_32b(b_lo + o, 4096), idesc, 1u);
+              umma_tf32(acc, umma_desc_mn_sw128_32b(a_hi + o, 4096), umma_desc_mn_sw128_32b(b_hi + o, 4096), idesc, 1u);
+            }
+          } else
 #pragma unroll
           for (int k = 0; k < kGemmBK / 8; ++k) {              // UMMA K = 8 floats = 32 bytes inside the swizzled row
             const uint32_t o = (uint32_t)k * 32u;

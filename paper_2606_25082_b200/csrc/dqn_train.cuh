@@ -14,8 +14,8 @@ constexpr int kDqnApad = 16;            // the action dimension is padded to 16 
 
 // ---------------------------------------------------------------------------------------------- sampling + gather
 // Block = 32 batch rows.  idx_b = (w * size) >> 32 with w = word 0 of Philox(counter (b, 3, step, 0), key seed): stream 3
-// (reading #36); with `identity` the batch is rows 0..B-1 of the given arrays.  Writes X[B][64], X2[B][64], the transposed
-// copy Xt[64][B] (through shared memory: both the reads and the writes are coalesced), a, r, done.
+// (reading #36); with `identity` the batch is rows 0..B-1 of the given arrays.  Writes X[B][64], X2[B][64], a, r, done and,
+// if Xt is not NULL, the transposed copy Xt[64][B] (through shared memory: both the reads and the writes are coalesced).
 struct GatherArgs {
   const float *S, *S2; const uint8_t *A; const float *R; const uint8_t *D;     // the replay buffer (or an explicit batch)
   float *X, *X2, *Xt; uint8_t *a; float *r; uint8_t *done;
@@ -43,6 +43,7 @@ __global__ void __launch_bounds__(256) dqn_gather_kernel(const GatherArgs g) {
     g.X2[(size_t)b * MIG_STATE_DIM + k] = g.S2[(size_t)idx[row] * MIG_STATE_DIM + k];
   }
   __syncthreads();
+  if (!g.Xt) return;                                        // (the transposed copy is only read by the K-major weight-gradient path)
   for (int e = threadIdx.x; e < 32 * MIG_STATE_DIM; e += 256) {
     const int k = e / 32, row = e % 32;
     if (b0 + row < g.B) g.Xt[(size_t)k * g.B + b0 + row] = tile[row][k];
@@ -51,9 +52,10 @@ __global__ void __launch_bounds__(256) dqn_gather_kernel(const GatherArgs g) {
 
 // ---------------------------------------------------------------------------------------------- TD error
 // y_b = r_b + gamma (1 - done_b) max_a' Q_target(s'_b, a');  delta_b = Q(s_b, a_b) - y_b;  dL/dQ[b][j] = (j == a_b) delta_b / B;
-// lossrow[b] = delta_b^2 / (2B).  dQ is written row-major [B][16] and transposed [16][B].
+// lossrow[b] = delta_b^2 / (2B).  dQ is written row-major [B][ldq] (16 live columns; the caller keeps the others zero) and
+// transposed [16][B].
 __global__ void __launch_bounds__(256) dqn_td_kernel(const float *Q, const float *Qt, const uint8_t *a, const float *r, const uint8_t *done,
-                                                     uint32_t B, uint32_t n_actions, float gamma, float *dQ, float *dQt, float *lossrow) {
+                                                     uint32_t B, uint32_t n_actions, float gamma, float *dQ, uint32_t ldq, float *dQt, float *lossrow) {
   const uint32_t b = blockIdx.x * 256u + threadIdx.x;
   if (b >= B) return;
   const float4 *q4 = reinterpret_cast<const float4 *>(Q + (size_t)b * kDqnApad), *t4 = reinterpret_cast<const float4 *>(Qt + (size_t)b * kDqnApad);
@@ -73,7 +75,7 @@ __global__ void __launch_bounds__(256) dqn_td_kernel(const float *Q, const float
   const float y = done[b] ? r[b] : fmaf(gamma, mx, r[b]);
   const float delta = qa - y, gq = delta / (float)B;
   lossrow[b] = delta * delta / (2.0f * (float)B);
-  float4 *o4 = reinterpret_cast<float4 *>(dQ + (size_t)b * kDqnApad);
+  float4 *o4 = reinterpret_cast<float4 *>(dQ + (size_t)b * ldq);
 #pragma unroll
   for (int i = 0; i < 4; ++i)
     o4[i] = make_float4(4 * i == (int)ab ? gq : 0.0f, 4 * i + 1 == (int)ab ? gq : 0.0f, 4 * i + 2 == (int)ab ? gq : 0.0f, 4 * i + 3 == (int)ab ? gq : 0.0f);
@@ -92,6 +94,7 @@ struct UpdateArgs {
   float *W, *Wt, *Ws; uint32_t rows, cols, ldw, ldt;       // W [rows][ldw] (first `cols` columns live), Wt [2 cols][ldt], Ws [2 rows][ldw] or NULL
   const float *partial; uint32_t n_splits; size_t split_stride; uint32_t ldp;   // partial [z][rows][ldp]
   float *bias; const float *dZt; uint32_t n_bias, B;       // bias [n_bias], dZt [n_bias][B]
+  const float *bias_part; uint32_t n_chunks;               // or (dZt == NULL) column sums of the row-major dZ: bias_part [n_chunks][n_bias]
   float lr;
   const float *lossrow; float *loss_out;                   // (only the launch that passes them sums the loss)
 };
@@ -122,6 +125,14 @@ __global__ void __launch_bounds__(256) dqn_update_kernel(const UpdateArgs u) {
   }
   if (blk < u.rows + u.n_bias) {
     const uint32_t o = blk - u.rows;
+    if (u.bias_part) {                                        // partial column sums (dqn_colsum_kernel), added in the fixed order z = 0, 1, ...
+      if (threadIdx.x == 0) {
+        float s = 0.0f;
+        for (uint32_t z = 0; z < u.n_chunks; ++z) s += u.bias_part[(size_t)z * u.n_bias + o];
+        u.bias[o] -= u.lr * s;
+      }
+      return;
+    }
     float acc = 0.0f;
     for (uint32_t b = threadIdx.x; b < u.B; b += 256) acc += u.dZt[(size_t)o * u.B + b];
     const float s = block_sum_256(acc, red);
@@ -133,6 +144,25 @@ __global__ void __launch_bounds__(256) dqn_update_kernel(const UpdateArgs u) {
     for (uint32_t b = threadIdx.x; b < u.B; b += 256) acc += u.lossrow[b];
     const float s = block_sum_256(acc, red);
     if (threadIdx.x == 0) *u.loss_out = s;
+  }
+}
+
+// Partial column sums of a row-major Z [B][H] (the bias gradients when no transposed copy of dZ exists): block (x, z) sums
+// rows [z B / n_chunks, (z + 1) B / n_chunks) of columns [32 x, 32 x + 32) -- a warp reads 128 contiguous bytes of a row, the
+// eight warps of the block take every eighth row, their sums are added in warp order: part[z][col].  Fixed order throughout.
+__global__ void __launch_bounds__(256) dqn_colsum_kernel(const float *Z, uint32_t B, uint32_t H, uint32_t n_chunks, float *part) {
+  __shared__ float red[8][32];
+  const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5, col = blockIdx.x * 32u + lane, z = blockIdx.y;
+  const uint32_t r0 = (uint32_t)(((uint64_t)z * B) / n_chunks), r1 = (uint32_t)(((uint64_t)(z + 1) * B) / n_chunks);
+  float acc = 0.0f;
+  for (uint32_t r = r0 + w; r < r1; r += 8u) acc += Z[(size_t)r * H + col];
+  red[w][lane] = acc;
+  __syncthreads();
+  if (w == 0) {
+    float s = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += red[i][lane];
+    part[(size_t)z * H + col] = s;
   }
 }
 

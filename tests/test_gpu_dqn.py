@@ -112,6 +112,14 @@ def test_both_tile_widths_of_the_hidden_layer_products(bn, monkeypatch):
     d.close()
 
 
+def test_k_major_weight_gradient_path_gives_the_same_step(monkeypatch):
+    # MIG_DQN_MN=0 at create: every activation also written transposed, K-major weight-gradient products over the copies, bias
+    # gradients as row sums (the path before the MN-major operands; kept for A/B timing).  Same oracle, same tolerance.
+    monkeypatch.setenv("MIG_DQN_MN", "0")
+    test_training_steps_match_the_oracle(256, 1024, 12, 3)
+    test_training_steps_match_the_oracle(128, 896, 16, 2)
+
+
 def test_replay_ring_and_sampling():
     A, batch, cap = 12, 256, 1000
     net = W.make_qnet(51, n_actions=A, hidden=256)
