@@ -426,6 +426,13 @@ def run_dqn(args):
     h2d = hs.numel() * 4 * 2 + ha.numel() + hr.numel() * 4
     tf32_peak = float(peaks.get("bf16_tflops", peaks.get("bf16_tflops_burst", 1685.8))) / 2.0      # the guide's nominal ratio TF32 : BF16 = 1 : 2
     achieved = DQN_FLOP_PER_TRANSITION * batch / (step_ms / 1e3) / 1e12
+    from paper_2606_25082_b200 import ncu_summary                   # DRAM bytes of the eleven products of one step, from the committed capture
+    try:
+        with open(NCU_SUMMARY) as f:
+            cap = json.load(f).get("gemm_tf32x3_kernel (the 11 products of one step)|DQN|%d" % batch)
+    except Exception:
+        cap = None
+    traffic = cap.get("dram_bytes") if cap and cap.get("csrc_sha16") == ncu_summary.csrc_sha16() else None
     cpu = None
     if not args.no_cpu_baseline:
         n = 512
@@ -436,8 +443,9 @@ def run_dqn(args):
             "data": "synthetic", "config": {"workload": "DQN", "batch": batch, "replay": cap, "net": "64-256-256-12", "l2": "flushed between iterations (256 MiB write)"},
             "train_steps_per_s": 1e3 / step_ms, "e2e": {"value": batch * n_e2e / e2e_s, "unit": "transitions/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": 4, "steps": n_e2e},
             "gpu_launches": launches, "clocks": clocks,
-            "roofline": {"bound": "tensor", "achieved": achieved, "peak": tf32_peak, "unit": "TFLOP/s", "frac": achieved / tf32_peak, "traffic": None,
-                         "kernel": "gemm_tf32x3_kernel<BN> (BN = 128, 256 and 16: the twelve products of a step)", "step_ms": step_ms, "flop_per_transition_algorithmic": DQN_FLOP_PER_TRANSITION,
+            "roofline": {"bound": "tensor", "achieved": achieved, "peak": tf32_peak, "unit": "TFLOP/s", "frac": achieved / tf32_peak, "traffic": traffic,
+                         "traffic_scope": "DRAM bytes of the eleven tensor-core launches of one step (ncu --set full, profiles/r2_dqn.md); achieved is over all kernels of the step",
+                         "kernel": "gemm_tf32x3_kernel<BN, MN> (the eleven products of a step: 128 x 256, 128 x 128, 128 x 16 tiles, K-major; 128 x 32 and 128 x 128 MN-major)", "step_ms": step_ms, "flop_per_transition_algorithmic": DQN_FLOP_PER_TRANSITION,
                          "issued_over_algorithmic": 3.0, "peak_source": "%s bf16 dense / 2 (TF32 : BF16 = 1 : 2, B200_PROFILING.md)" % peak_src},
             "cpu_baseline": cpu}
     print(json.dumps(line))

@@ -91,13 +91,23 @@ def main():
     ap.add_argument("--n-envs", type=int, required=True)
     ap.add_argument("--out", required=True)
     ap.add_argument("--command", default="", help="the ncu command line that made the capture (recorded verbatim)")
+    ap.add_argument("--sum-first", type=int, default=0, help="instead of one entry per kernel: ONE entry, the sums over the first N launches of the capture")
+    ap.add_argument("--sum-key", default="", help="kernel field of that entry")
     a = ap.parse_args()
     try:
         with open(a.out) as f:
             doc = json.load(f)
     except Exception:
         doc = {}
-    for rec in parse(a.raw_csv):
+    recs = parse(a.raw_csv)
+    if a.sum_first:                                          # e.g. the eleven products of ONE training step
+        part = recs[:a.sum_first]
+        assert len(part) == a.sum_first and a.sum_key, "capture shorter than --sum-first, or no --sum-key"
+        tot = {"kernel": a.sum_key, "launches": a.sum_first, "kernels": [r["kernel"] for r in part]}
+        for k in ("dram_bytes_read", "dram_bytes_write", "duration_ms", "warp_inst_executed"):
+            tot[k] = sum(r.get(k, 0.0) for r in part)
+        recs = [tot]
+    for rec in recs:
         rec.update(workload=a.workload, n_envs=a.n_envs, csrc_sha16=csrc_sha16(), command=a.command)
         if "dram_bytes_read" in rec and "dram_bytes_write" in rec:
             rec["dram_bytes"] = rec["dram_bytes_read"] + rec["dram_bytes_write"]
