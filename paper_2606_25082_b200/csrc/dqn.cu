@@ -93,7 +93,7 @@ struct mig_dqn {   // (mig_dqn_t of include/migsim.h)
   // batch and activations
   float *X, *X2, *Xt, *H1, *H1t, *H2, *H2t, *Q, *T1, *T2, *Qt, *dQ, *dQt, *dZ2, *dZ2t, *dZ1t, *r, *lossrow, *pW1, *pW2, *pW3, *loss;
   uint8_t *a, *done;
-  // tensor maps: A operands and B operands of the twelve products
+  // tensor maps: A operands and B operands of the eleven products
   CUtensorMap mX, mH1, mH2, mX2, mT1, mT2, mdQ, mdZ2, mH2t, mH1t, mXt;                          // A side (box 128 rows)
   CUtensorMap mW1t[2], mW2t[2], mW3t[2], mW3, mW2, mdQt, mdZ2t, mdZ1t;                          // B side
 };
@@ -220,7 +220,7 @@ extern "C" int mig_dqn_create(mig_dqn_t **out, const float *W1, const float *b1,
 
 // ------------------------------------------------------------------------------------------------ forward
 // h1 = relu(b1 + x W1), h2 = relu(b2 + h1 W2), q = b3 + h2 W3 for the B rows of X (online: which = 0, into H1 / H2 / Q with
-// the transposed copies the backward pass needs) or of X2 (target: which = 1, into T1 / T2 / Qt)
+// the transposed copies that the MIG_DQN_MN=0 backward pass needs) or of X2 (target: which = 1, into T1 / T2 / Qt)
 static int forward(mig_dqn *d, int which, cudaStream_t st) {
   const uint32_t H = d->H, B = d->B, P = kDqnApad;
   const Net &n = d->net[which];
@@ -260,7 +260,7 @@ extern "C" int mig_dqn_q(mig_dqn_t *d, int which, const float *state, uint32_t n
 
 // ------------------------------------------------------------------------------------------------ one training step
 // forward of both networks, TD error, backward, SGD on the batch that the gather kernel left in X / X2 / a / r / done:
-// seventeen launches (fifteen on the MIG_DQN_MN=0 path), always with the same arguments (the loss lands in d->loss)
+// fourteen launches (thirteen on the MIG_DQN_MN=0 path), always with the same arguments (the loss lands in d->loss)
 static int train_kernels(mig_dqn *d, cudaStream_t st) {
   const uint32_t H = d->H, B = d->B, P = kDqnApad, S = d->splits;
   int rc;
@@ -286,31 +286,33 @@ static int train_kernels(mig_dqn *d, cudaStream_t st) {
   g = gargs(64, H, kps); g.out = d->pW1; g.ldo = H; g.out_split_stride = (size_t)64 * H;
   if ((rc = d->mn ? launch_gemm<128, true>(d, d->mXr, d->mdZ1r, g, S, st) : launch_gemm<128>(d, d->mXt, d->mdZ1t, g, S, st))) return rc;
   if (d->mn) {                                                 // bias gradients of the hidden layers: column sums of the row-major dZ
-    dqn_colsum_kernel<<<dim3(H / 32, kBiasChunks), 256, 0, st>>>(d->dZ2, B, H, kBiasChunks, d->pb2);
-    dqn_colsum_kernel<<<dim3(H / 32, kBiasChunks), 256, 0, st>>>(d->dZ1, B, H, kBiasChunks, d->pb1);
-    CUD(cudaGetLastError()); d->launches += 2;
+    dqn_colsum_kernel<<<dim3(H / 32, kBiasChunks, 2), 256, 0, st>>>(d->dZ2, d->dZ1, B, H, kBiasChunks, d->pb2, d->pb1);
+    CUD(cudaGetLastError()); d->launches++;
   }
-  // SGD on the online network (the transposed copies follow), bias gradients = row sums of the transposed dZ, the loss
+  // SGD on the online network (the split copies of the weights follow), bias gradients (the partial column sums, or row sums of
+  // the transposed dZ on the MIG_DQN_MN=0 path), the loss: one launch for the three layers
   Net &n = d->net[0];
+  UpdateArgs3 u3; memset(&u3, 0, sizeof(u3));
   UpdateArgs u; memset(&u, 0, sizeof(u));
   u.lr = d->lr; u.B = B; u.n_splits = S;
   u.W = n.W3; u.Wt = n.W3t; u.Ws = n.W3s; u.rows = H; u.cols = P; u.ldw = P; u.ldt = H; u.partial = d->pW3; u.split_stride = (size_t)H * ld3; u.ldp = ld3;
   u.bias = n.b3; u.dZt = d->dQt; u.n_bias = P; u.lossrow = d->lossrow; u.loss_out = d->loss;
-  dqn_update_kernel<<<u.rows + u.n_bias + 1, 256, 0, st>>>(u);
+  u3.l[0] = u; u3.first[0] = 0; u3.first[1] = u.rows + u.n_bias + 1;
   u.loss_out = nullptr; u.lossrow = nullptr;
   u.W = n.W2; u.Wt = n.W2t; u.Ws = n.W2s; u.rows = H; u.cols = H; u.ldw = H; u.ldt = H; u.partial = d->pW2; u.split_stride = (size_t)H * H; u.ldp = H;
   u.bias = n.b2; u.dZt = d->dZ2t; u.n_bias = H;
   if (d->mn) { u.dZt = nullptr; u.bias_part = d->pb2; u.n_chunks = kBiasChunks; }
-  dqn_update_kernel<<<u.rows + u.n_bias, 256, 0, st>>>(u);
+  u3.l[1] = u; u3.first[2] = u3.first[1] + u.rows + u.n_bias;
   u.W = n.W1; u.Wt = n.W1t; u.Ws = nullptr; u.rows = 64; u.cols = H; u.ldw = H; u.ldt = 64; u.partial = d->pW1; u.split_stride = (size_t)64 * H; u.ldp = H;
   u.bias = n.b1; u.dZt = d->dZ1t; u.n_bias = H;
   if (d->mn) { u.dZt = nullptr; u.bias_part = d->pb1; u.n_chunks = kBiasChunks; }
-  dqn_update_kernel<<<u.rows + u.n_bias, 256, 0, st>>>(u);
-  CUD(cudaGetLastError()); d->launches += 3;
+  u3.l[2] = u; u3.first[3] = u3.first[2] + u.rows + u.n_bias;
+  dqn_update_kernel<<<u3.first[3], 256, 0, st>>>(u3);
+  CUD(cudaGetLastError()); d->launches++;
   return MIG_OK;
 }
 
-// The seventeen launches are captured ONCE into a CUDA graph (their arguments never change) and replayed with one
+// The fourteen launches are captured ONCE into a CUDA graph (their arguments never change) and replayed with one
 // cudaGraphLaunch per step: at batch 8192 the step is launch-bound without it.  MIG_DQN_NO_GRAPH=1 in the environment
 // launches the kernels one by one instead (profiling by kernel name).
 static int train_on_batch(mig_dqn *d, float *loss_out, cudaStream_t st) {

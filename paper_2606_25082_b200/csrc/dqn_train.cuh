@@ -108,9 +108,9 @@ __device__ __forceinline__ float block_sum_256(float v, float *red) {
   __syncthreads();
   return s;                                                 // valid in thread 0
 }
-__global__ void __launch_bounds__(256) dqn_update_kernel(const UpdateArgs u) {
-  __shared__ float red[8];
-  const uint32_t blk = blockIdx.x;
+// (one launch updates the three layers: blocks [first[l], first[l + 1]) run layer l's update)
+struct UpdateArgs3 { UpdateArgs l[3]; uint32_t first[4]; };
+__device__ __forceinline__ void dqn_update_block(const UpdateArgs &u, const uint32_t blk, float *red) {
   if (blk < u.rows) {
     for (uint32_t c = threadIdx.x; c < u.cols; c += 256) {
       float g = 0.0f;
@@ -146,12 +146,20 @@ __global__ void __launch_bounds__(256) dqn_update_kernel(const UpdateArgs u) {
     if (threadIdx.x == 0) *u.loss_out = s;
   }
 }
+__global__ void __launch_bounds__(256) dqn_update_kernel(const UpdateArgs3 a) {
+  __shared__ float red[8];
+  const uint32_t b = blockIdx.x;
+  const int l = b >= a.first[2] ? 2 : (b >= a.first[1] ? 1 : 0);   // (block-uniform)
+  dqn_update_block(a.l[l], b - a.first[l], red);
+}
 
 // Partial column sums of a row-major Z [B][H] (the bias gradients when no transposed copy of dZ exists): block (x, z) sums
 // rows [z B / n_chunks, (z + 1) B / n_chunks) of columns [32 x, 32 x + 32) -- a warp reads 128 contiguous bytes of a row, the
 // eight warps of the block take every eighth row, their sums are added in warp order: part[z][col].  Fixed order throughout.
-__global__ void __launch_bounds__(256) dqn_colsum_kernel(const float *Z, uint32_t B, uint32_t H, uint32_t n_chunks, float *part) {
+// blockIdx.z selects the tensor: one launch sums dZ2 (z = 0, into part0) and dZ1 (z = 1, into part1).
+__global__ void __launch_bounds__(256) dqn_colsum_kernel(const float *Z0, const float *Z1, uint32_t B, uint32_t H, uint32_t n_chunks, float *part0, float *part1) {
   __shared__ float red[8][32];
+  const float *Z = blockIdx.z ? Z1 : Z0; float *part = blockIdx.z ? part1 : part0;
   const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5, col = blockIdx.x * 32u + lane, z = blockIdx.y;
   const uint32_t r0 = (uint32_t)(((uint64_t)z * B) / n_chunks), r1 = (uint32_t)(((uint64_t)(z + 1) * B) / n_chunks);
   float acc = 0.0f;
