@@ -172,6 +172,9 @@ def run_ours(args):
     sim = B.MigSim(sp, n_envs, wl.seed, tile=args.tile)
     if args.envs_per_warp:
         sim.set_envs_per_warp(args.envs_per_warp)
+    prefetch = bool(args.prefetch) and args.tile in (0, 1)
+    if prefetch:                                         # the next step's arrival lists are drawn in the tail of this step's event loop
+        sim.set_prefetch(True)
     qnet = B.QNet(wl.qnet) if wl.qnet is not None else None
     d_algo, d_cfg0 = torch.from_numpy(wl.algo).cuda(), torch.from_numpy(wl.cfg0).cuda()
     d_table = None if wl.table is None else torch.from_numpy(wl.table).cuda()
@@ -239,6 +242,32 @@ def run_ours(args):
     sim.set_profiling(False)
     torch.cuda.synchronize()
     per_day_ms = {key: ms_sum[key] / n_prof for key in ms_sum}                      # per day-batch, all launches of that family
+    # ---- the same steps with nothing drawn ahead (mig_sim_set_prefetch off): generator, then event loop, one after the other
+    serial = None
+    if prefetch:
+        sim.set_prefetch(False)
+        n_ser = max(1, min(args.steps, 5))
+        one_step(0)
+        torch.cuda.synchronize()
+        z0, z1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev_ser = torch.zeros(1, dtype=torch.int64, device="cuda")
+        z0.record(stream)
+        for k in range(n_ser):
+            one_step(1 + k)
+            ev_ser += count_events()
+            flush.fill_(k & 0xFF)
+        z1.record(stream)
+        torch.cuda.synchronize()
+        sim.kernel_times()
+        sim.set_profiling(True)
+        sim.reset(last_episode, d_algo, d_cfg0)
+        sim.kernel_times()
+        sim.rollout(wl.policy, table=d_table, qnet=qnet, epsilon=wl.epsilon, recs_out=recs, totals_out=totals)   # (leaves `recs` / `totals` on last_episode)
+        ms_ser, _ = sim.kernel_times()
+        sim.set_profiling(False)
+        serial = {"ms_per_step": z0.elapsed_time(z1) / n_ser, "value": int(ev_ser.item()) / (z0.elapsed_time(z1) / 1e3), "unit": "job-events/s", "steps": n_ser,
+                  "kernels_ms_per_day": dict(ms_ser), "what": "mig_sim_set_prefetch off: every step draws its own arrivals before its event loop starts"}
+        sim.set_prefetch(True)
     # ---- end to end: HOST buffers through the C ABI, copies inside the timed region ---------------------------------
     h_tot = np.zeros(n_envs, dtype=B.TOTALS_DTYPE)
     h_recs = np.zeros((sp.n_epochs + 1, n_envs), dtype=B.REC_DTYPE)
@@ -286,6 +315,10 @@ def run_ours(args):
     peak_gips = props.multi_processor_count * 128 * sm_mhz * 1e6 / 1e9           # G lane-instr/s: SMs x 128 lanes x f_max
     sim_ms = per_day_ms["sim"] if per_day_ms["sim"] > 0 else kern_ms
     alg_sim = ALG_LANE_INSTR["sim"] + (0.0 if per_day_ms["gen"] > 0 else ALG_LANE_INSTR["gen"])   # tiles draw arrivals inside the rollout kernel
+    drawn_in_tail = None
+    if serial and serial["kernels_ms_per_day"].get("gen", 0.0) > 0:                 # the share of the generator's work that the event loop's tail did
+        drawn_in_tail = max(0.0, 1.0 - per_day_ms["gen"] / serial["kernels_ms_per_day"]["gen"])
+        alg_sim += ALG_LANE_INSTR["gen"] * drawn_in_tail
     achieved_gips = alg_sim * ev_per_launch / (sim_ms / 1e3) / 1e9
     path_gips = (ALG_LANE_INSTR["sim"] + ALG_LANE_INSTR["gen"]) * ev_per_launch / (kern_ms / 1e3) / 1e9
     # algorithmic HBM bytes per launch: the outputs the caller asked for + the per-env inputs, nothing else
@@ -304,7 +337,7 @@ def run_ours(args):
                 "peak_source": "%d SMs x 128 lanes x %s sm_max_mhz %.0f" % (props.multi_processor_count, peak_src, sm_mhz),
                 "hot_path": {"frac": path_gips / peak_gips, "achieved": path_gips, "ms": kern_ms, "alg_lane_instr_per_job_event": ALG_LANE_INSTR["sim"] + ALG_LANE_INSTR["gen"],
                              "what": "generator + event loop: the whole mig_sim_rollout call (round 1's definition of frac)"},
-                "kernels_ms_per_day": per_day_ms, "launches_per_day": {key: n_sum[key] / n_prof for key in n_sum},
+                "drawn_in_tail": drawn_in_tail, "kernels_ms_per_day": per_day_ms, "launches_per_day": {key: n_sum[key] / n_prof for key in n_sum},
                 "hbm_algorithmic_bytes_per_launch": alg_bytes, "traffic_over_algorithmic": (traffic / alg_bytes) if traffic else None,
                 "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_frac": alg_bytes / (sim_ms / 1e3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0)),
                 "arrival_list_records_per_env": sim.get_arrival_buffer() if tile == 1 else 0,
@@ -332,11 +365,12 @@ def run_ours(args):
             "metric": "job_events_per_s", "value": ev_total / t_s, "unit": "job-events/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
             "config": {"workload": args.workload, "n_envs_per_gpu": n_envs, "n_envs_total": n_envs * world, "policy": ["static", "table", "dqn"][wl.policy], "algo": W.ALGO_NAMES[int(wl.algo[0])] if len(set(wl.algo.tolist())) == 1 else "mixed", "lanes_per_env": sim.get_tile(), "envs_per_warp": args.envs_per_warp or "auto",
+                       "prefetch": ("on: the arrival lists of step k + 1 are drawn in the tail of step k's event loop; every timed step draws one day of lists and simulates one" if prefetch else "off"),
                        "job_events_per_step": ev_total / args.steps, "l2": "flushed between iterations (256 MiB write)", "parallelism": "env-range sharding, no data-path collective",
                        "dist": ("nccl, world %d" % dist.get_world_size()) if dist.is_initialized() else None},
             "day_episodes_per_s": n_envs * world * args.steps / t_s,
             "e2e": {"value": e2e_ev / e2e_t, "unit": "job-events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e},
-            "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "step_api": step_api,
+            "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "step_api": step_api, "serial": serial,
         }
         print(json.dumps(line))
     sim.close()
@@ -466,6 +500,9 @@ def main():
     ap.add_argument("--algo", type=int, default=-1, choices=[-1, 0, 1, 2, 3, 4], help="override the workload's scheduling algorithm for every env (4 = EDF-SS with restricted preemption); -1 = the workload's own")
     ap.add_argument("--envs-per-warp", type=int, default=0, choices=[0, 1, 2, 4, 8, 16, 32],
                     help="thread-per-environment kernel: environments in each warp (0 = the library's choice: one resident wave); a study knob, see profiles/r2_thread.md")
+    ap.add_argument("--prefetch", type=int, default=1, choices=[0, 1],
+                    help="1 (default): mig_sim_set_prefetch -- the next step's arrival lists are drawn in the tail of this step's event loop (same results; "
+                         "the line's `serial` object is the same measurement with it off); thread-per-environment kernel only")
     ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 8, 16, 32], help="lanes per environment (0 = library default = 1: one thread per environment; 8, 16, 32: warp tiles)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

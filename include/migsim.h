@@ -315,6 +315,17 @@ int mig_sim_set_envs_per_warp(mig_sim_t *s, uint32_t envs_per_warp);
 int mig_sim_set_arrival_buffer(mig_sim_t *s, uint32_t entries_per_env);
 /* Capacity of the arrival lists in use (records per environment); 0 = arrivals are drawn inside the event loop. */
 uint32_t mig_sim_get_arrival_buffer(const mig_sim_t *s);
+/* Thread-per-environment kernel only: draw the NEXT episode's arrivals ahead ("the arrival process does not
+ * depend on the schedule", so a day's arrivals can be drawn before the day before it has ended).  on != 0: after a FULL-DAY
+ * launch of episode e -- mig_sim_rollout straight after mig_sim_reset under a STATIC / TABLE / BINNED policy, 32
+ * environments per warp -- the warps of the event loop that finish their day early draw the arrival lists of episode e + 1
+ * into a second list buffer until the launch's last day ends; the next full-day launch, if its episode IS e + 1, finds them
+ * in place and its generator draws only the environments that were left.  Any other call sequence (another episode,
+ * mig_sim_step, a DQN rollout) simply does not use what was drawn.  Results are identical with the setting on or off
+ * (tested); it costs a second list buffer (n_envs x capacity x 8 bytes; MIG_ENOMEM if that does not fit) and is off by
+ * default.  Synchronises the device.  Allowed between any two calls. */
+int mig_sim_set_prefetch(mig_sim_t *s, int on);
+int mig_sim_get_prefetch(const mig_sim_t *s);
 int mig_sim_get_tile(const mig_sim_t *s);
 /* Number of kernel launches issued through this handle so far (bench.py's gpu_launches). */
 uint64_t mig_sim_launch_count(const mig_sim_t *s);

@@ -37,7 +37,8 @@ EXPORTS = (
     "mig_sim_get_tile", "mig_sim_set_arrival_buffer", "mig_sim_get_arrival_buffer", "mig_sim_set_envs_per_warp",
     "mig_sim_kernel_name", "mig_sim_set_profiling", "mig_sim_kernel_times", "mig_sim_aux", "mig_et_reduce",
     "mig_dqn_create", "mig_dqn_destroy", "mig_replay_push", "mig_replay_size", "mig_dqn_train_step", "mig_dqn_train_on",
-    "mig_dqn_sync_target", "mig_dqn_q", "mig_dqn_get_weights", "mig_dqn_launch_count", "mig_q_forward_static")
+    "mig_dqn_sync_target", "mig_dqn_q", "mig_dqn_get_weights", "mig_dqn_launch_count", "mig_q_forward_static",
+    "mig_sim_set_prefetch", "mig_sim_get_prefetch")
 
 
 class MigError(RuntimeError):
@@ -96,6 +97,8 @@ def lib():
         L.mig_sim_get_tile.argtypes = [vp]
         L.mig_sim_set_arrival_buffer.argtypes = [vp, C.c_uint32]
         L.mig_sim_set_envs_per_warp.argtypes = [vp, C.c_uint32]
+        L.mig_sim_set_prefetch.argtypes = [vp, i32]
+        L.mig_sim_get_prefetch.argtypes = [vp]
         L.mig_sim_kernel_name.argtypes = [vp]
         L.mig_sim_kernel_name.restype = C.c_char_p
         L.mig_sim_set_profiling.argtypes = [vp, i32]
@@ -295,6 +298,12 @@ class MigSim:
 
     def get_arrival_buffer(self) -> int:
         return int(lib().mig_sim_get_arrival_buffer(self.h))
+
+    def set_prefetch(self, on: bool):
+        _check(lib().mig_sim_set_prefetch(self.h, 1 if on else 0))
+
+    def get_prefetch(self) -> bool:
+        return bool(lib().mig_sim_get_prefetch(self.h))
 
     def close(self):
         if getattr(self, "h", None) and _lib is not None:

@@ -35,16 +35,10 @@ constexpr int kGenWarps = 8;     // environments (= warps) per CTA of the genera
 enum { HG_PK = 1 /* epoch in the low byte */, HG_GK = 6, HG_GT_LO, HG_GT_HI, HG_GDONE, HG_NACC,
        HG_ACOUNT = 32 /* records in this launch's list */, HG_AMORE /* the list filled up before the horizon */, HG_AID0 /* job id of record 0 */ };
 
-struct GenArgs {
-  const DevTables *tab;
-  uint32_t *hdr;                       // [n_envs][kHeaderWords]
-  uint2 *arr; uint32_t arr_cap;        // [n_envs][arr_cap] records
-  uint32_t n_envs, env_first;
-  uint32_t k0, k1, episode, env_base;  // Philox key, counter words
-  uint64_t gap_scale;
-  int32_t day_s, epoch_s, n_epochs, n_steps;
-  uint32_t job_limit;
-};
+constexpr int kGenWords = 8;     // generator words of an environment: HG_GK .. HG_NACC (5), HG_ACOUNT .. HG_AID0 (3)
+
+// the tables the generator reads (shared-memory copies in gen_arrivals_kernel, the global originals in the event loop's tail)
+struct GenTabs { const uint32_t *thr; const int32_t *dur7_q; const uint32_t *class_cum, *slack_lo, *slack_span, *logT; };
 
 constexpr int kGenRun = 4;       // consecutive candidates per lane and pass: 128 per warp pass, four independent Philox chains per lane
 static_assert(kGenRun <= 4, "the per-lane flag word holds three nibbles");
@@ -87,37 +81,24 @@ __device__ __forceinline__ uint32_t class_of(uint32_t w, const uint32_t *cum) {
 
 
 
-__global__ void __launch_bounds__(kGenWarps * 32, 3) gen_arrivals_kernel(const GenArgs a) {
-  __shared__ GenSmem sm;
-  {
-    const DevTables *tb = a.tab;
-    for (int i = threadIdx.x; i < MIG_THR_BINS; i += kGenWarps * 32) sm.thr[i] = tb->thr[i];
-    for (int i = threadIdx.x; i < MIG_MAX_CLASSES * 65; i += kGenWarps * 32) sm.dur7_q[i] = tb->dur7_q[i];
-    for (int i = threadIdx.x; i < 257; i += kGenWarps * 32) sm.logT[i] = tb->logT[i];
-    if (threadIdx.x < MIG_MAX_CLASSES) {
-      sm.class_cum[threadIdx.x] = tb->class_cum[threadIdx.x];
-      sm.slack_lo[threadIdx.x] = tb->slack_lo[threadIdx.x]; sm.slack_span[threadIdx.x] = tb->slack_span[threadIdx.x];
-    }
-  }
-  __syncthreads();
-  const uint32_t lane = threadIdx.x & 31u, li = blockIdx.x * kGenWarps + (threadIdx.x >> 5);
-  if (li >= a.n_envs) return;
-  const uint32_t env = a.env_first + li, env_g = a.env_base + env;
-  uint32_t *hdr = a.hdr + (size_t)env * kHeaderWords;
-  uint2 *out = a.arr + (size_t)env * a.arr_cap;
-  const int epoch = (int)(hdr[HG_PK] & 0xFFu);
-  uint32_t k = hdr[HG_GK], done = hdr[HG_GDONE], nacc = hdr[HG_NACC];
-  unsigned long long T = (unsigned long long)hdr[HG_GT_LO] | ((unsigned long long)hdr[HG_GT_HI] << 32);
+// One environment's arrivals from the generator state (epoch, k, done, nacc, T) up to the launch's horizon, by one warp
+// (every condition in the loop is warp-uniform).  `pend(i)`: the warp's buffer of 32 * kGenRun accepted candidates; `pace()` runs
+// before every pass (the event loop's tail yields to the warps that still simulate);
+// o_state[5] receives {k, T lo, T hi, done, nacc}, o_list[3] {records in the list, list filled up, job id of record 0}.
+template <class Pend, class Pace>
+__device__ __forceinline__ void gen_env(const GenArgs &a, const GenTabs &tb, Pend pend, Pace pace, uint32_t lane, uint32_t env_g, uint2 *out,
+                                        int epoch, uint32_t k, uint32_t done, uint32_t nacc, unsigned long long T,
+                                        uint32_t *o_state, uint32_t *o_list) {
   const uint32_t id0 = nacc, limit = a.job_limit ? min(a.job_limit, MIG_MAX_JOBS) : MIG_MAX_JOBS;
   uint32_t count = 0, more = 0;
   if (epoch < a.n_epochs && !done) {
     const unsigned long long horizon = (unsigned long long)(min(epoch + a.n_steps, a.n_epochs) * a.epoch_s);
     // a gap is at most 32 gap_scale (E24 <= 32 << 24): with gap_scale < 2^20 the sum of a pass of 128 is < 2^32
     const bool narrow = a.gap_scale < (1ull << 20);
-    GenPend *pend = sm.pend[threadIdx.x >> 5];                    // this warp's accepted candidates of the pass
     for (;;) {                                                    // every condition below is warp-uniform
       if (nacc >= limit) break;
       if (count >= a.arr_cap) { more = 1; break; }
+      pace();
       // ---- lane l draws the kGenRun consecutive candidates k + kGenRun l + j (Philox stream 0: gap, accept, class, slack)
       const uint32_t kb = k + lane * kGenRun;
       uint32_t wy[kGenRun], wz[kGenRun], ww[kGenRun];
@@ -126,7 +107,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 3) gen_arrivals_kernel(const G
 #pragma unroll
       for (int j = 0; j < kGenRun; ++j) {
         const uint4 w = philox4x32_10(kb + (uint32_t)j, 0u, env_g, a.episode, a.k0, a.k1);
-        run += ((unsigned long long)neglog2_q24_tab(w.x, sm.logT) * a.gap_scale) >> 24;
+        run += ((unsigned long long)neglog2_q24_tab(w.x, tb.logT) * a.gap_scale) >> 24;
         s[j] = run; wy[j] = w.y; wz[j] = w.z; ww[j] = w.w;
       }
       // ---- exclusive warp scan of the lane totals (integer: the same sums as the oracle's sequential accumulation)
@@ -156,7 +137,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 3) gen_arrivals_kernel(const G
         const bool in_day = tk < (unsigned long long)a.day_s;     // arrivals stop at the end of the day
         const bool ok = in_day && tk <= horizon;
         tick[j] = (uint32_t)tk;
-        const bool acc = ok && wy[j] <= sm.thr[(ok ? (uint32_t)tk : 0u) / 60u];
+        const bool acc = ok && wy[j] <= tb.thr[(ok ? (uint32_t)tk : 0u) / 60u];
         fl |= (in_day ? 1u : 0u) << j | (ok ? 1u : 0u) << (4 + j) | (acc ? 1u : 0u) << (8 + j);
         n_acc_l += acc ? 1u : 0u;
       }
@@ -176,7 +157,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 3) gen_arrivals_kernel(const G
         const bool acc = (fl >> (8 + j)) & 1u;
         nc_l += commit ? 1u : 0u;
         if (commit && acc) {                                      // park it for the attribute pass, in list order
-          pend[b] = GenPend{kb + (uint32_t)j, tick[j], wz[j], ww[j]};
+          pend(b) = GenPend{kb + (uint32_t)j, tick[j], wz[j], ww[j]};
           ++na_l;
         }
         b += acc ? 1u : 0u;
@@ -186,13 +167,13 @@ __global__ void __launch_bounds__(kGenWarps * 32, 3) gen_arrivals_kernel(const G
       // ---- job attributes (R5) of the accepted candidates, 32 per trip with every lane busy: class, Philox stream 1
       // (duration), slack; one coalesced 8-byte record each
       for (uint32_t i = lane; i < na; i += 32u) {
-        const GenPend e = pend[i];
-        const uint32_t c = class_of(e.wz, sm.class_cum);
+        const GenPend e = pend(i);
+        const uint32_t c = class_of(e.wz, tb.class_cum);
         const uint4 wd = philox4x32_10(e.k, 1u, env_g, a.episode, a.k0, a.k1);
         const uint32_t qi = wd.x >> 26, f = (wd.x >> 16) & 0x3FFu;
-        const int q0 = sm.dur7_q[c * 65 + qi], q1 = sm.dur7_q[c * 65 + qi + 1];
+        const int q0 = tb.dur7_q[c * 65 + qi], q1 = tb.dur7_q[c * 65 + qi + 1];
         const int dur7 = q0 + (int)(((long long)(q1 - q0) * (long long)f) >> 10);
-        const uint32_t slack = sm.slack_lo[c] + __umulhi(e.ww, sm.slack_span[c]);
+        const uint32_t slack = tb.slack_lo[c] + __umulhi(e.ww, tb.slack_span[c]);
         __stcg(&out[count + i], pack_arrival(e.tick, c, (uint32_t)dur7, slack));   // streamed past L1
       }
       __syncwarp();
@@ -214,9 +195,37 @@ __global__ void __launch_bounds__(kGenWarps * 32, 3) gen_arrivals_kernel(const G
     }
   }
   if (lane == 0) {
-    hdr[HG_GK] = k; hdr[HG_GT_LO] = (uint32_t)T; hdr[HG_GT_HI] = (uint32_t)(T >> 32); hdr[HG_GDONE] = done; hdr[HG_NACC] = nacc;
-    hdr[HG_ACOUNT] = count; hdr[HG_AMORE] = more; hdr[HG_AID0] = id0;
+    o_state[0] = k; o_state[1] = (uint32_t)T; o_state[2] = (uint32_t)(T >> 32); o_state[3] = done; o_state[4] = nacc;
+    o_list[0] = count; o_list[1] = more; o_list[2] = id0;
   }
+}
+
+__global__ void __launch_bounds__(kGenWarps * 32, 3) gen_arrivals_kernel(const GenArgs a) {
+  __shared__ GenSmem sm;
+  const uint32_t lane = threadIdx.x & 31u, li = blockIdx.x * kGenWarps + (threadIdx.x >> 5);
+  const uint32_t env = a.env_first + (li < a.n_envs ? li : 0u);
+  uint32_t *hdr = a.hdr + (size_t)env * kHeaderWords;
+  // drawn ahead (mig_sim_set_prefetch): the eight generator words move into the header, the list is in place
+  const bool ahead = li < a.n_envs && a.pf_flag && a.pf_flag[env] == a.pf_tag;
+  if (ahead && lane < (uint32_t)kGenWords) hdr[lane < 5u ? HG_GK + lane : HG_ACOUNT + (lane - 5u)] = a.pf_words[(size_t)env * kGenWords + lane];
+  if (!__syncthreads_or(li < a.n_envs && !ahead)) return;          // nothing to draw in this CTA
+  {
+    const DevTables *tb = a.tab;
+    for (int i = threadIdx.x; i < MIG_THR_BINS; i += kGenWarps * 32) sm.thr[i] = tb->thr[i];
+    for (int i = threadIdx.x; i < MIG_MAX_CLASSES * 65; i += kGenWarps * 32) sm.dur7_q[i] = tb->dur7_q[i];
+    for (int i = threadIdx.x; i < 257; i += kGenWarps * 32) sm.logT[i] = tb->logT[i];
+    if (threadIdx.x < MIG_MAX_CLASSES) {
+      sm.class_cum[threadIdx.x] = tb->class_cum[threadIdx.x];
+      sm.slack_lo[threadIdx.x] = tb->slack_lo[threadIdx.x]; sm.slack_span[threadIdx.x] = tb->slack_span[threadIdx.x];
+    }
+  }
+  __syncthreads();
+  if (li >= a.n_envs || ahead) return;
+  const GenTabs tb{sm.thr, sm.dur7_q, sm.class_cum, sm.slack_lo, sm.slack_span, sm.logT};
+  GenPend *const mine = sm.pend[threadIdx.x >> 5];                // this warp's accepted candidates of the pass
+  const unsigned long long T = (unsigned long long)hdr[HG_GT_LO] | ((unsigned long long)hdr[HG_GT_HI] << 32);
+  gen_env(a, tb, [mine](uint32_t i) -> GenPend & { return mine[i]; }, [] {}, lane, a.env_base + env, a.arr + (size_t)env * a.arr_cap,
+          (int)(hdr[HG_PK] & 0xFFu), hdr[HG_GK], hdr[HG_GDONE], hdr[HG_NACC], T, hdr + HG_GK, hdr + HG_ACOUNT);
 }
 
 }  // namespace migsim

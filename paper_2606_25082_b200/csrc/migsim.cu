@@ -8,6 +8,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "qnet_device.cuh"
@@ -49,6 +50,11 @@ struct mig_sim {
   uint32_t ring_cap = 1;     // power of two >= cap
   uint2 *d_arr = nullptr; uint32_t arr_cap = 0;      // thread-per-env kernel: arrival lists [n_envs][arr_cap] of 8-byte records (0 = none: arrivals are drawn inside the event loop)
   uint32_t arr_default = 0;  // capacity chosen at create: expected accepted arrivals per day + 8 sigma
+  // mig_sim_set_prefetch: the next episode's lists are drawn in the tail of a full-day launch, into the other list buffer
+  bool pf_on = false, pf_valid = false;
+  uint2 *d_arr_alt = nullptr; uint32_t *d_pf_words = nullptr, *d_pf_flag = nullptr; unsigned int *d_pf_ctr = nullptr;   // ctr: {claim, finished, busy[kPfScheds]}
+  uint32_t pf_pace_ns = 2000;   // measured on C5 (profiles/r2_prefetch.md): 0 / 500 / 2000 / 8000 / 32000 ns -> 72.8 / 72.6 / 72.2 / 72.4 / 72.4 ms per step
+  uint32_t pf_episode = 0, pf_tag = 0;
   uint32_t envs_per_warp = 0;   // thread-per-env kernel: 0 = chosen per launch so that the batch is one resident wave
   DevTables *d_tab = nullptr;
   uint32_t *d_hdr = nullptr; uint4 *d_jobtab = nullptr; uint4 *d_dbgtab = nullptr; uint32_t *d_dbghdr = nullptr;
@@ -267,6 +273,7 @@ extern "C" int mig_sim_set_envs_per_warp(mig_sim_t *s, uint32_t envs_per_warp) {
 static int alloc_arrival_lists(mig_sim *s, uint32_t entries) {
   if (cudaDeviceSynchronize() != cudaSuccess) return fail(MIG_ECUDA, "set_arrival_buffer: %s", cudaGetErrorString(cudaGetLastError()));
   cudaFree(s->d_arr); s->d_arr = nullptr; s->arr_cap = 0;
+  cudaFree(s->d_arr_alt); s->d_arr_alt = nullptr; s->pf_valid = false;
   if (entries == 0) return MIG_OK;
   entries = (entries + 3u) & ~3u;
   const size_t need = (size_t)s->n_envs * entries * sizeof(uint2);
@@ -276,13 +283,46 @@ static int alloc_arrival_lists(mig_sim *s, uint32_t entries) {
                             "(slower, same results) -- choose a capacity that fits with mig_sim_set_arrival_buffer", need, s->n_envs, entries);
   }
   s->arr_cap = entries;
+  if (s->pf_on && cudaMalloc((void **)&s->d_arr_alt, need) != cudaSuccess) {
+    cudaGetLastError(); s->d_arr_alt = nullptr; s->pf_on = false;
+    return fail(MIG_ENOMEM, "arrival lists: cudaMalloc of the second buffer (%zu bytes) failed; drawing ahead is switched off", need);
+  }
   return MIG_OK;
 }
 
+// Drawing ahead (off by default; results are identical either way, tested): after a full-day launch of episode e -- a
+// rollout from reset under a policy that lives on the device, every environment of the handle, 32 per warp -- the warps
+// that finish their day early draw the arrival lists of episode e + 1 into a second list buffer (the arrival process
+// does not depend on the schedule); a following full-day launch of episode e + 1 finds them in place and
+// its generator draws only what was left.  Any other call leaves the drawn lists alone (they stay valid) or, if the episode
+// differs, unused.  Costs a second list buffer (n_envs x capacity x 8 bytes).
+constexpr int kPfScheds = 4 * 1024;     // warp schedulers the pacing counters cover (SM id < 1024)
+extern "C" int mig_sim_set_prefetch(mig_sim_t *s, int on) {
+  if (!s) return fail(MIG_EINVAL, "set_prefetch: NULL handle");
+  if ((on != 0) == s->pf_on) return MIG_OK;
+  if (cudaDeviceSynchronize() != cudaSuccess) return fail(MIG_ECUDA, "set_prefetch: %s", cudaGetErrorString(cudaGetLastError()));
+  s->pf_valid = false;
+  if (!on) { cudaFree(s->d_arr_alt); s->d_arr_alt = nullptr; s->pf_on = false; return MIG_OK; }
+  if (!s->d_arr) return fail(MIG_ESTATE, "set_prefetch: the handle has no arrival lists (mig_sim_set_arrival_buffer(s, 0) was called)");
+  const size_t n = s->n_envs;
+  if (!s->d_pf_words) {
+    if (cudaMalloc((void **)&s->d_pf_words, n * kGenWords * 4) != cudaSuccess || cudaMalloc((void **)&s->d_pf_flag, n * 4) != cudaSuccess ||
+        cudaMalloc((void **)&s->d_pf_ctr, (2 + kPfScheds) * sizeof(unsigned int)) != cudaSuccess || cudaMemset(s->d_pf_flag, 0, n * 4) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(MIG_ENOMEM, "set_prefetch: cudaMalloc failed");
+    }
+  }
+  const size_t need = n * s->arr_cap * sizeof(uint2);
+  if (cudaMalloc((void **)&s->d_arr_alt, need) != cudaSuccess) { cudaGetLastError(); s->d_arr_alt = nullptr; return fail(MIG_ENOMEM, "set_prefetch: cudaMalloc of the second list buffer (%zu bytes) failed", need); }
+  s->pf_on = true;
+  return MIG_OK;
+}
+extern "C" int mig_sim_get_prefetch(const mig_sim_t *s) { return s && s->pf_on ? 1 : 0; }
+
 extern "C" int mig_sim_set_arrival_buffer(mig_sim_t *s, uint32_t entries_per_env) {
   if (!s) return fail(MIG_EINVAL, "set_arrival_buffer: NULL handle");
-  if (entries_per_env > MIG_MAX_JOBS) return fail(MIG_EINVAL, "set_arrival_buffer: more than %u entries per environment", MIG_MAX_JOBS);
   if (entries_per_env == 0xFFFFFFFFu) entries_per_env = s->arr_default;
+  if (entries_per_env > MIG_MAX_JOBS) return fail(MIG_EINVAL, "set_arrival_buffer: more than %u entries per environment", MIG_MAX_JOBS);
   return alloc_arrival_lists(s, entries_per_env);
 }
 
@@ -347,7 +387,7 @@ extern "C" int mig_sim_destroy(mig_sim_t *s) {
   cudaDeviceSynchronize();
   cudaFree(s->d_tab); cudaFree(s->d_hdr); cudaFree(s->d_jobtab); cudaFree(s->d_dbgtab); cudaFree(s->d_dbghdr); cudaFree(s->d_counter); cudaFree(s->d_algo_mask);
   cudaFree(s->d_algo); cudaFree(s->d_cfg0); cudaFree(s->d_state); cudaFree(s->d_action); cudaFree(s->d_table);
-  cudaFree(s->d_recs); cudaFree(s->d_totals); cudaFree(s->d_script); cudaFree(s->d_arr);
+  cudaFree(s->d_recs); cudaFree(s->d_totals); cudaFree(s->d_script); cudaFree(s->d_arr); cudaFree(s->d_arr_alt); cudaFree(s->d_pf_words); cudaFree(s->d_pf_flag); cudaFree(s->d_pf_ctr);
   for (auto &sp : s->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   for (auto e : s->ev_pool) cudaEventDestroy(e);
   cudaGetLastError();
@@ -428,8 +468,16 @@ static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
     // arrivals of this launch's horizon: drawn by the generator kernel into the per-environment lists, on the same stream,
     // before the event loop runs (not for scripted arrivals, nor for the one-env debug trace, which draws its own)
     const bool lists = s->d_arr && a.n_steps > 0 && !a.script && !a.from_init && !a.hdr_override;
+    // a full day of every environment of the handle, straight from reset: the launch whose lists may have been drawn ahead
+    // (mig_sim_set_prefetch) and whose tail draws the next episode's
+    const bool full_day = lists && !TRACE && s->pf_on && s->d_arr_alt && s->epoch == 0 && a.n_steps >= a.n_epochs && a.env_first == 0 && a.n_envs == s->n_envs;
     if (lists) {
       GenArgs g; memset(&g, 0, sizeof(g));
+      if (full_day && s->pf_valid && s->pf_episode == a.episode) {      // drawn ahead: the lists are in the other buffer
+        std::swap(s->d_arr, s->d_arr_alt);
+        g.pf_flag = s->d_pf_flag; g.pf_words = s->d_pf_words; g.pf_tag = s->pf_tag;
+      }
+      if (full_day) s->pf_valid = false;
       g.tab = a.tab; g.hdr = a.hdr; g.arr = s->d_arr; g.arr_cap = s->arr_cap; g.n_envs = a.n_envs; g.env_first = a.env_first;
       g.k0 = a.k0; g.k1 = a.k1; g.episode = a.episode; g.env_base = a.env_base; g.gap_scale = a.gap_scale;
       g.day_s = a.day_s; g.epoch_s = a.epoch_s; g.n_epochs = a.n_epochs; g.n_steps = a.n_steps; g.job_limit = a.job_limit;
@@ -439,6 +487,20 @@ static int launch_sim(mig_sim *s, const SimArgs &a, cudaStream_t st) {
     }
     b.arr = lists ? s->d_arr : nullptr; b.arr_cap = s->arr_cap;
     b.envs_per_warp = s->envs_per_warp ? s->envs_per_warp : auto_envs_per_warp(s, b.n_envs);
+    if (full_day && b.envs_per_warp == 32u && b.n_envs >= 32u) {        // the launch's tail draws episode + 1 into the other buffer
+      CU(cudaMemsetAsync(s->d_pf_ctr, 0, (2 + kPfScheds) * sizeof(unsigned int), st));
+      b.pf_on = 1;
+      PrefetchArgs &pf = b.pf;
+      pf.g.tab = a.tab; pf.g.hdr = nullptr; pf.g.arr = s->d_arr_alt; pf.g.arr_cap = s->arr_cap; pf.g.n_envs = s->n_envs; pf.g.env_first = 0;
+      pf.g.k0 = a.k0; pf.g.k1 = a.k1; pf.g.episode = a.episode + 1u; pf.g.env_base = a.env_base; pf.g.gap_scale = a.gap_scale;
+      pf.g.day_s = a.day_s; pf.g.epoch_s = a.epoch_s; pf.g.n_epochs = a.n_epochs; pf.g.n_steps = a.n_epochs; pf.g.job_limit = a.job_limit;
+      pf.g.pf_flag = nullptr; pf.g.pf_words = nullptr; pf.g.pf_tag = 0;
+      pf.words = s->d_pf_words; pf.flag = s->d_pf_flag; pf.tag = ++s->pf_tag;
+      if (pf.tag == 0) pf.tag = ++s->pf_tag;                            // (0 is the flags' initial value)
+      pf.claim = s->d_pf_ctr; pf.finished = s->d_pf_ctr + 1; pf.n_warps = b.n_envs / 32u;
+      pf.busy = s->d_pf_ctr + 2; pf.pace_ns = s->pf_pace_ns;
+      s->pf_valid = true; s->pf_episode = a.episode + 1u;
+    }
     const uint32_t per_cta = b.envs_per_warp * (kThreadCta / 32);
     const dim3 grid((b.n_envs + per_cta - 1) / per_cta), block(kThreadCta);
     {

@@ -35,6 +35,34 @@ struct DevTables {
   int32_t dbin_edges[8], abin_edges[8];      // BINNED policy: bin edges, padded with INT32_MAX
 };
 
+// Arguments of the arrival generator (gen_kernel.cuh).
+struct GenArgs {
+  const DevTables *tab;
+  uint32_t *hdr;                       // [n_envs][kHeaderWords]
+  uint2 *arr; uint32_t arr_cap;        // [n_envs][arr_cap] records
+  uint32_t n_envs, env_first;
+  uint32_t k0, k1, episode, env_base;  // Philox key, counter words
+  uint64_t gap_scale;
+  int32_t day_s, epoch_s, n_epochs, n_steps;
+  uint32_t job_limit;
+  // lists drawn ahead, in the tail of the previous day's event loop (mig_sim_set_prefetch; sim_thread.cuh: tail_prefetch): an
+  // environment whose flag carries `pf_tag` has its list in `arr` already and its eight generator words in pf_words
+  const uint32_t *pf_flag; const uint32_t *pf_words; uint32_t pf_tag;
+};
+
+// Drawing the NEXT day's arrivals in the tail of this day's event loop (mig_sim_set_prefetch; sim_thread.cuh: tail_prefetch):
+// a warp whose 32 environments have finished their day claims environments one at a time and draws their lists of episode
+// g.episode into g.arr (the handle's other list buffer) until every warp of the launch has finished its day.
+struct PrefetchArgs {
+  GenArgs g;                   // a fresh full day: generator state zero, horizon = the whole day
+  uint32_t *words;             // [n_envs][kGenWords] generator words of the drawn lists
+  uint32_t *flag; uint32_t tag;   // flag[env] = tag once its list and words are written
+  unsigned int *claim;         // next environment to draw
+  unsigned int *finished; uint32_t n_warps;   // warps that have finished their day / warps that will
+  unsigned int *busy;          // [SMs][4]: warps of this launch still inside their day, per warp scheduler (warp slot & 3)
+  uint32_t pace_ns;            // a drawing warp that shares its scheduler with such a warp sleeps this long before every pass
+};
+
 // Kernel arguments (by value, constant bank).
 struct SimArgs {
   const DevTables *tab;
@@ -72,6 +100,7 @@ struct SimArgs {
   float gamma;                                       // discount of the return kept in the env's header
   const mig_job_t *script; uint32_t n_script;
   const uint2 *arr; uint32_t arr_cap;                // thread-per-env kernel: arrival lists [n_envs][arr_cap] of 8-byte records (gen_kernel.cuh), or NULL
+  int pf_on; PrefetchArgs pf;                        // thread-per-env kernel: draw the next day's lists in the launch's tail
   // outputs (NULL = skip)
   float *state_out; float *reward_out; int64_t *energy_out; int64_t *tard_out;
   mig_epoch_rec_t *recs; int32_t rec_k0; mig_epoch_rec_t *drain_rec;   // record of epoch k -> recs[(k - rec_k0) * n_envs_total + env]

@@ -994,6 +994,41 @@ __device__ __forceinline__ void thread_body(const SimArgs &a, const HotTablesT &
 }
 
 
+// The tail of a full-day launch (mig_sim_set_prefetch): a warp whose 32 environments have finished their day draws arrival
+// lists of the NEXT episode, one claimed environment at a time, until every warp of the launch has finished its day -- the
+// idle lanes of a launch whose warps end between 60 and 69 ms do the generator's work of the next step (the arrival
+// process does not depend on the schedule).  What is left is drawn by the next step's gen_arrivals_kernel,
+// which skips the flagged environments.  Not inlined and everything BY VALUE: off the hot path, and the kernel's argument
+// block must not become addressable.  `mine`: this warp's half of the per-thread rows (dead by now), 256 bytes in every
+// 8-byte row = sixteen 16-byte entries; the warp's 128 pending candidates take the first eight rows.
+// index of this warp's scheduler in PrefetchArgs::busy: SM id x 4 + warp slot & 3 (a heuristic: only pacing depends on it)
+static __device__ __forceinline__ uint32_t sched_slot() {
+  uint32_t sm, w;
+  asm volatile("mov.u32 %0, %%smid;\n\tmov.u32 %1, %%warpid;" : "=r"(sm), "=r"(w));
+  return (sm & 1023u) * 4u + (w & 3u);
+}
+
+template <int NT>
+static __device__ __noinline__ void tail_prefetch(const PrefetchArgs pf, unsigned char *mine, uint32_t lane) {
+  unsigned int *const busy = pf.busy + sched_slot();
+  if (lane == 0) { atomicAdd(pf.finished, 1u); atomicSub(busy, 1u); }
+  const uint32_t pace_ns = pf.pace_ns;
+  const DevTables *t = pf.g.tab;
+  const GenTabs tb{t->thr, t->dur7_q, t->class_cum, t->slack_lo, t->slack_span, t->logT};
+  for (;;) {
+    uint32_t w = 0xFFFFFFFFu;
+    if (lane == 0 && *reinterpret_cast<volatile unsigned int *>(pf.finished) < pf.n_warps) w = atomicAdd(pf.claim, 1u);
+    w = __shfl_sync(0xffffffffu, w, 0);
+    if (w >= pf.g.n_envs) break;                                  // every day of the launch is over, or nothing is left to draw
+    uint32_t *o = pf.words + (size_t)w * kGenWords;
+    gen_env(pf.g, tb, [mine](uint32_t i) -> GenPend & { return *reinterpret_cast<GenPend *>(mine + (size_t)(i >> 4) * (NT * 8) + (i & 15u) * 16u); },
+            [busy, pace_ns] { if (pace_ns && *reinterpret_cast<volatile unsigned int *>(busy)) __nanosleep(pace_ns); },
+            lane, pf.g.env_base + w, pf.g.arr + (size_t)w * pf.g.arr_cap, 0, 0u, 0u, 0u, 0ull, o, o + 5);
+    __syncwarp();
+    if (lane == 0) { __threadfence(); pf.flag[w] = pf.tag; }
+  }
+}
+
 template <int NT, bool TRACE, bool EVD>
 __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -1018,11 +1053,17 @@ __global__ void __launch_bounds__(NT, 7) sim_thread_kernel(const SimArgs a) {
   const uint32_t li = (blockIdx.x * (NT / 32) + (threadIdx.x >> 5)) * a.envs_per_warp + lane;   // index inside this launch's env range
   const bool alive = lane < a.envs_per_warp && li < a.n_envs;
   if (!alive) return;
+  const bool tail = a.pf_on && a.envs_per_warp == 32u && li - lane + 31u < a.n_envs;      // a full warp of a full-day launch (warp-uniform)
+  if (!TRACE && tail && lane == 0) atomicAdd(a.pf.busy + sched_slot(), 1u);
   // every environment of the batch on EDF-FS / EDF-SS / restricted EDF-SS (bits 0, 1, 4 of the mask that the reset launch
   // collected): the short body
   const bool edf_only = !a.from_init && a.algo_mask && (__ldg(a.algo_mask) & ~0x13u) == 0u;
   if (edf_only) thread_body<NT, TRACE, EVD, true>(a, hot, base, li);
   else thread_body<NT, TRACE, EVD, false>(a, hot, base, li);
+  if (!TRACE && tail) {
+    __syncwarp();                                               // the warp's 32 days are over: its rows are free
+    tail_prefetch<NT>(a.pf, base + (threadIdx.x >> 5) * 256u, lane);
+  }
 }
 
 // per-env auxiliary results out of the saved headers: the discounted return and the seconds per utilisation level
