@@ -1,10 +1,8 @@
 """mig_sim_set_prefetch (the next episode's arrival lists drawn in the tail of a full-day launch): the days
 are the same with the setting on or off -- records, totals and trace hashes byte for byte -- whatever the call sequence
-(consecutive episodes, an episode that was not drawn ahead, steps in between, a batch whose last warp is partial), and a
-sample of them is checked against the oracle directly.
+(consecutive episodes, an episode that was not drawn ahead, steps in between, a batch whose last warp is partial, BASELINE
+C5 at full size in the launch configuration bench.py times), and a sample of them is checked against the oracle directly.
 """
-import dataclasses
-
 import numpy as np
 import pytest
 import torch
@@ -20,9 +18,8 @@ def dev(a):
 
 
 def _workload(n_envs):
-    """The C5 recipe (heavy load, hourly TABLE policy) with a lighter day so that the oracle's sample is cheap."""
-    wl = W.CONFIGS["C5"](n_envs)
-    return wl
+    """The C5 recipe (heavy load, hourly TABLE policy, queues that spill into the global ring) on a smaller batch."""
+    return W.CONFIGS["C5"](n_envs)
 
 
 def _days(B, wl, n, episodes, prefetch, steps_before=()):
@@ -66,6 +63,39 @@ def test_prefetch_days_are_identical(n):
         for e in (0, 31, 32, n // 2 + 5, n - 1):
             r = O.rollout(ph, wl.seed, e, episode=ep, algo=int(wl.algo[e]), cfg0=int(wl.cfg0[e]), policy=wl.policy, table=wl.table[e])
             assert tot[e].tobytes() == r.totals.tobytes(), "episode %d env %d differs from the oracle" % (ep, e)
+
+
+def test_prefetch_full_size_c5_in_the_bench_configuration():
+    """BASELINE C5 at full size (65 536 env-days, 32 per warp by the library's own choice: the launch bench.py times): three
+    consecutive episodes with drawing ahead on equal the same episodes with it off, every env; a sample against the oracle."""
+    from paper_2606_25082_b200 import binding as B
+    n = 65536
+    wl = W.CONFIGS["C5"](n)
+    d_algo, d_cfg0, d_table = dev(wl.algo), dev(wl.cfg0), dev(wl.table)
+    res = {}
+    for on in (True, False):
+        sim = B.MigSim(wl.params, n, wl.seed)
+        if on:
+            sim.set_prefetch(True)
+        out = []
+        for ep in (0, 1, 2):
+            recs, tot = sim.alloc_recs(), sim.alloc_totals()
+            sim.reset(ep, d_algo, d_cfg0)
+            sim.rollout(wl.policy, table=d_table, recs_out=recs, totals_out=tot)
+            torch.cuda.synchronize()
+            out.append((recs.cpu(), B.totals_to_numpy(tot).copy()))
+            del recs, tot
+        res[on] = out
+        sim.close()
+        del sim
+        torch.cuda.empty_cache()
+    for ep in (0, 1, 2):
+        assert torch.equal(res[True][ep][0], res[False][ep][0]), "records of episode %d differ" % ep
+        assert res[True][ep][1].tobytes() == res[False][ep][1].tobytes(), "totals of episode %d differ" % ep
+    ph = O.ParamsHolder(wl.params)
+    for e in (0, 4095, 32768, 65535):
+        r = O.rollout(ph, wl.seed, e, episode=2, algo=int(wl.algo[e]), cfg0=int(wl.cfg0[e]), policy=wl.policy, table=wl.table[e])
+        assert res[True][2][1][e].tobytes() == r.totals.tobytes(), "episode 2 env %d differs from the oracle" % e
 
 
 def test_prefetch_needs_lists_and_survives_a_new_capacity():
