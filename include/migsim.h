@@ -210,7 +210,10 @@ int mig_et_reduce(const double *x, const double *y, const uint32_t *group, uint3
 
 /* End-to-end convenience with HOST buffers: copies algo/cfg0/table (host[n_envs], host[n_envs][n_epochs][4] or NULL)
  * to the device, reset(episode) + rollout, copies totals (host[n_envs]) and records (host[n_epochs+1][n_envs] or
- * NULL) back, synchronises.  DQN policy allowed (q non-NULL). */
+ * NULL) back, synchronises.  DQN policy allowed (q non-NULL).  A result buffer that lies in pinned, mapped host memory
+ * (cudaHostAlloc / cudaHostRegister over the whole buffer) is written by the kernels directly: its bytes cross the link
+ * while the launch runs and no copy follows; ordinary host memory is filled by a copy after the launch.  Same bytes
+ * either way (tested). */
 int mig_sim_rollout_host(mig_sim_t *s, uint32_t episode, const uint8_t *algo, const uint8_t *cfg0, int policy,
                          const uint8_t *table, const mig_qnet_t *q, float epsilon, mig_epoch_rec_t *recs_out,
                          mig_totals_t *totals_out);

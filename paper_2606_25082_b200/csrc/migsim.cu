@@ -666,13 +666,28 @@ extern "C" int mig_et_reduce(const double *x, const double *y, const uint32_t *g
   return MIG_OK;
 }
 
+// The device's address of a HOST buffer that it can write directly -- pinned and mapped memory (cudaHostAlloc,
+// cudaHostRegister) -- or NULL for ordinary host memory.  First and last byte are looked up: both must be registered.
+static void *mapped_device_ptr(const void *host, size_t bytes) {
+  cudaPointerAttributes lo, hi;
+  if (!host || bytes == 0) return nullptr;
+  if (cudaPointerGetAttributes(&lo, host) != cudaSuccess || cudaPointerGetAttributes(&hi, static_cast<const char *>(host) + bytes - 1) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  if (lo.type != cudaMemoryTypeHost || hi.type != cudaMemoryTypeHost || !lo.devicePointer) return nullptr;
+  return lo.devicePointer;
+}
+
 extern "C" int mig_sim_rollout_host(mig_sim_t *s, uint32_t episode, const uint8_t *algo, const uint8_t *cfg0, int policy,
                                     const uint8_t *table, const mig_qnet_t *q, float epsilon, mig_epoch_rec_t *recs_out,
                                     mig_totals_t *totals_out) {
   if (!s || !algo || !cfg0 || !totals_out) return fail(MIG_EINVAL, "rollout_host: NULL argument");
   const size_t n = s->n_envs, ne = (size_t)s->p.n_epochs;
-  if (!s->d_totals) { if (cudaMalloc((void **)&s->d_totals, n * sizeof(mig_totals_t)) != cudaSuccess) { cudaGetLastError(); return fail(MIG_ENOMEM, "rollout_host: cudaMalloc failed"); } }
-  if (recs_out && !s->d_recs) { if (cudaMalloc((void **)&s->d_recs, n * (ne + 1) * sizeof(mig_epoch_rec_t)) != cudaSuccess) { cudaGetLastError(); return fail(MIG_ENOMEM, "rollout_host: cudaMalloc failed"); } }
+  // result buffers in pinned, mapped host memory are written by the kernels themselves (every record and every totals row
+  // is stored once, 64 and 80 contiguous bytes per environment): the results cross the link while the launch runs and
+  // there is no copy after it; ordinary host memory goes through the handle's device copy
+  mig_totals_t *tot_map = static_cast<mig_totals_t *>(mapped_device_ptr(totals_out, n * sizeof(mig_totals_t)));
+  mig_epoch_rec_t *rec_map = static_cast<mig_epoch_rec_t *>(mapped_device_ptr(recs_out, recs_out ? n * (ne + 1) * sizeof(mig_epoch_rec_t) : 0));
+  if (!tot_map && !s->d_totals) { if (cudaMalloc((void **)&s->d_totals, n * sizeof(mig_totals_t)) != cudaSuccess) { cudaGetLastError(); return fail(MIG_ENOMEM, "rollout_host: cudaMalloc failed"); } }
+  if (recs_out && !rec_map && !s->d_recs) { if (cudaMalloc((void **)&s->d_recs, n * (ne + 1) * sizeof(mig_epoch_rec_t)) != cudaSuccess) { cudaGetLastError(); return fail(MIG_ENOMEM, "rollout_host: cudaMalloc failed"); } }
   if (policy == MIG_POLICY_TABLE || policy == MIG_POLICY_BINNED) {
     if (!table) return fail(MIG_EINVAL, "rollout_host: TABLE / BINNED policy needs a table");
     const size_t Bc = 1 + (size_t)s->p.n_dbins * s->p.n_abins;
@@ -686,10 +701,10 @@ extern "C" int mig_sim_rollout_host(mig_sim_t *s, uint32_t episode, const uint8_
   CU(cudaMemcpyAsync(stage_cfg, cfg0, n, cudaMemcpyHostToDevice, 0));
   int rc = mig_sim_reset(s, episode, stage_algo, stage_cfg, nullptr, nullptr);
   if (rc) return rc;
-  rc = mig_sim_rollout(s, policy, s->d_table, q, epsilon, recs_out ? s->d_recs : nullptr, s->d_totals, nullptr);
+  rc = mig_sim_rollout(s, policy, s->d_table, q, epsilon, recs_out ? (rec_map ? rec_map : s->d_recs) : nullptr, tot_map ? tot_map : s->d_totals, nullptr);
   if (rc) return rc;
-  CU(cudaMemcpyAsync(totals_out, s->d_totals, n * sizeof(mig_totals_t), cudaMemcpyDeviceToHost, 0));
-  if (recs_out) CU(cudaMemcpyAsync(recs_out, s->d_recs, n * (ne + 1) * sizeof(mig_epoch_rec_t), cudaMemcpyDeviceToHost, 0));
+  if (!tot_map) CU(cudaMemcpyAsync(totals_out, s->d_totals, n * sizeof(mig_totals_t), cudaMemcpyDeviceToHost, 0));
+  if (recs_out && !rec_map) CU(cudaMemcpyAsync(recs_out, s->d_recs, n * (ne + 1) * sizeof(mig_epoch_rec_t), cudaMemcpyDeviceToHost, 0));
   CU(cudaStreamSynchronize(0));
   return MIG_OK;
 }

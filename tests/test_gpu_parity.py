@@ -293,6 +293,21 @@ def test_rollout_host_matches_device_rollout():
         recs = np.zeros((25, n), dtype=B.REC_DTYPE)
         sim.rollout_host(0, wl.algo, wl.cfg0, wl.policy, wl.table, q, wl.epsilon, recs, tot)
         assert tot.tobytes() == tot_ref.tobytes() and recs.tobytes() == recs_ref.tobytes()
+        # result buffers in pinned, mapped host memory: the kernels write them directly (no copy after the launch)
+        tot2, recs2 = np.zeros(n, dtype=B.TOTALS_DTYPE), np.zeros((25, n), dtype=B.REC_DTYPE)
+        rt = torch.cuda.cudart()
+        for a in (tot2, recs2):
+            assert int(rt.cudaHostRegister(a.ctypes.data, a.nbytes, 0)) == 0
+        try:
+            sim.rollout_host(0, wl.algo, wl.cfg0, wl.policy, wl.table, q, wl.epsilon, recs2, tot2)
+            assert tot2.tobytes() == tot_ref.tobytes() and recs2.tobytes() == recs_ref.tobytes()
+            recs2[:] = 0                                    # records mapped, totals not
+            tot3 = np.zeros(n, dtype=B.TOTALS_DTYPE)
+            sim.rollout_host(0, wl.algo, wl.cfg0, wl.policy, wl.table, q, wl.epsilon, recs2, tot3)
+            assert tot3.tobytes() == tot_ref.tobytes() and recs2.tobytes() == recs_ref.tobytes()
+        finally:
+            for a in (tot2, recs2):
+                rt.cudaHostUnregister(a.ctypes.data)
         sim.close()
 
 
