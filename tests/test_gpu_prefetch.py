@@ -43,11 +43,13 @@ def _days(B, wl, n, episodes, prefetch, steps_before=()):
     return out
 
 
-@pytest.mark.parametrize("n", [2048, 1000])
-def test_prefetch_days_are_identical(n):
+@pytest.mark.parametrize("n,mixed", [(2048, False), (1000, False), (512, True)], ids=["2048", "1000", "512-all-algorithms"])
+def test_prefetch_days_are_identical(n, mixed):
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
     from paper_2606_25082_b200 import binding as B
     wl = _workload(n)
+    if mixed:                                       # EDF-FS, EDF-SS, LLF, LALF and restricted EDF-SS side by side: the kernel's generic body
+        wl.algo[:] = np.arange(n, dtype=np.uint8) % 5
     # 0, 1, 2: each drawn ahead by the one before; 7: not drawn ahead (what was drawn for 3 is dropped); 8: ahead again;
     # 8 once more: the lists drawn for 9 stay unused; 9 begins with three explicit steps (no full-day launch) and 10 follows
     episodes = [0, 1, 2, 7, 8, 8, 9, 10]
